@@ -1,0 +1,396 @@
+"""Pins for the fp64 CPU oracle (oracle/wd_oracle.cpp): every check here compares the oracle with
+something OTHER than itself -- a closed form, a symmetry, a dense inverse by a library routine, a
+finite difference of the action (BASELINE.json north_star checks (a)-(d)).
+The paper (arxiv/paper_1009_5169) prints no worked numerical example, so no golden value of the
+paper exists; tests/golden/gamma_chiral.txt is the convention table of SURVEY.md Appendix A.
+"""
+import os
+
+import numpy as np
+import pytest
+
+import wd_inputs as wi
+from oracle import wd_oracle as orc
+
+GOLD = os.path.join(os.path.dirname(__file__), "golden")
+
+
+def cview(a):
+    return wi.to_complex(a)
+
+
+def rview(c):
+    return wi.from_complex(c)
+
+
+def inner(a, b):
+    return np.vdot(cview(a).ravel(), cview(b).ravel())
+
+
+def relerr(a, b):
+    return np.linalg.norm((a - b).ravel()) / max(np.linalg.norm(b.ravel()), 1e-300)
+
+
+def read_golden_gamma():
+    tok = {"0": 0, "1": 1, "-1": -1, "i": 1j, "-i": -1j}
+    out, cur, name = {}, [], None
+    for line in open(os.path.join(GOLD, "gamma_chiral.txt")):
+        line = line.strip()
+        if not line or line.startswith("#"):
+            continue
+        if line.startswith("gamma"):
+            name = line.split()[1]
+            cur = []
+            out[name] = cur
+        else:
+            cur.append([tok[t] for t in line.split()])
+    return {k: np.array(v, dtype=np.complex128) for k, v in out.items()}
+
+
+def site_coords(dims):
+    lx, ly, lz, lt = dims
+    t, z, y, x = np.meshgrid(np.arange(lt), np.arange(lz), np.arange(ly), np.arange(lx), indexing="ij")
+    return x, y, z, t
+
+
+def random_site_su3(dims, seed, eps=1.0):
+    lx, ly, lz, lt = dims
+    g = wi.random_su3(seed, wi.STREAM_AUX, lx * ly * lz * lt, eps)
+    return g.reshape(lt, lz, ly, lx, 3, 3)
+
+
+def shift(a, mu, step=1):
+    """a(x) -> a(x + step*mu) for arrays [T][Lz][Ly][Lx][...]."""
+    return np.roll(a, -step, axis=3 - mu)
+
+
+def gauge_transform(U, g):
+    """U^g_mu(x) = g(x) U_mu(x) g(x+mu)^dag."""
+    Uc = cview(U)
+    out = np.empty_like(Uc)
+    for mu in range(4):
+        gp = shift(g, mu)
+        out[mu] = np.einsum("...ab,...bc,...dc->...ad", g, Uc[mu], np.conj(gp))
+    return rview(out)
+
+
+# ----------------------------------------------------------------------------- gamma algebra
+def test_gamma_table_matches_appendix_a_and_is_clifford():
+    gold = read_golden_gamma()
+    g = [orc.gamma(mu) for mu in range(5)]
+    for mu, name in enumerate("xyzt5"):
+        assert np.array_equal(g[mu], gold[name]), name
+    for mu in range(4):
+        assert np.array_equal(g[mu], g[mu].conj().T)
+        for nu in range(4):
+            acom = g[mu] @ g[nu] + g[nu] @ g[mu]
+            assert np.allclose(acom, 2.0 * np.eye(4) * (mu == nu), atol=0)
+    assert np.array_equal(g[0] @ g[1] @ g[2] @ g[3], np.diag([1, 1, -1, -1]).astype(complex))
+
+
+# ----------------------------------------------------------------------------- closed forms
+def _plane_wave(dims, k, u):
+    x, y, z, t = site_coords(dims)
+    p = [2 * np.pi * k[i] / dims[i] for i in range(4)]
+    phase = np.exp(1j * (p[0] * x + p[1] * y + p[2] * z + p[3] * t))
+    return p, phase[..., None, None] * u
+
+
+@pytest.mark.parametrize("dag", [0, 1])
+def test_free_field_plane_wave_closed_form(dag):
+    # north_star check (d): unit links, periodic => D psi = [1 - 2k sum cos p + 2ik sum gamma sin p] psi
+    dims = (4, 6, 2, 8)   # unequal extents: an axis mix-up cannot cancel
+    kappa = 0.11
+    rng = np.random.default_rng(5)
+    u = rng.normal(size=(4, 3)) + 1j * rng.normal(size=(4, 3))
+    p, psi = _plane_wave(dims, (1, 2, 1, 3), u)
+    out = cview(orc.apply(dims, kappa, wi.BC_PERIODIC, dag, wi.unit_gauge(dims), rview(psi)[None]))[0]
+    g = read_golden_gamma()
+    sgn = -1.0 if dag else 1.0
+    M = (1 - 2 * kappa * sum(np.cos(p))) * np.eye(4) + sgn * 2j * kappa * sum(
+        g[n] * np.sin(p[mu]) for mu, n in enumerate("xyzt"))
+    expect = np.einsum("rs,...sc->...rc", M, psi)
+    assert relerr(out, expect) < 1e-14
+
+
+def test_twisted_abelian_links_closed_form():
+    # constant U_mu = diag(exp(i theta_mu^a)), sum_a theta = 0  =>  p_mu -> p_mu + theta_mu^a for
+    # colour a.  Tells U from U^dag, which unit links cannot.
+    dims = (4, 2, 6, 4)
+    kappa = 0.12
+    theta = np.array([[0.3, -0.5, 0.2], [1.1, -0.4, -0.7], [-0.9, 0.6, 0.3], [0.25, 0.45, -0.7]])
+    U = np.zeros((4,) + dims[::-1] + (3, 3), dtype=np.complex128)
+    for mu in range(4):
+        for a in range(3):
+            U[mu, ..., a, a] = np.exp(1j * theta[mu, a])
+    g = read_golden_gamma()
+    rng = np.random.default_rng(7)
+    k = (1, 1, 2, 3)
+    expect = np.zeros(dims[::-1] + (4, 3), dtype=np.complex128)
+    psi = np.zeros_like(expect)
+    for a in range(3):
+        u = np.zeros((4, 3), dtype=np.complex128)
+        u[:, a] = rng.normal(size=4) + 1j * rng.normal(size=4)
+        p, w = _plane_wave(dims, k, u)
+        q = [p[mu] + theta[mu, a] for mu in range(4)]
+        M = (1 - 2 * kappa * sum(np.cos(q))) * np.eye(4) + 2j * kappa * sum(
+            g[n] * np.sin(q[mu]) for mu, n in enumerate("xyzt"))
+        psi += w
+        expect += np.einsum("rs,...sc->...rc", M, w)
+    out = cview(orc.apply(dims, kappa, wi.BC_PERIODIC, 0, rview(U), rview(psi)[None]))[0]
+    assert relerr(out, expect) < 1e-14
+    # and the wrong orientation is an O(1) error, so the pin has teeth
+    out_wrong = cview(orc.apply(dims, kappa, wi.BC_PERIODIC, 0, rview(np.conj(U)), rview(psi)[None]))[0]
+    assert relerr(out_wrong, expect) > 1e-2
+
+
+# ----------------------------------------------------------------------------- symmetries
+@pytest.mark.parametrize("bc", [wi.BC_PERIODIC, wi.BC_SF])
+def test_gamma5_hermiticity_and_dagger_flag(bc):
+    # north_star check (b): <y, D x> = <gamma5 D gamma5 y, x>; and the dag flag IS the adjoint.
+    dims = (4, 2, 4, 6)
+    kappa = 0.13
+    U = wi.gauge_field(dims, 0.4, 3, bc)
+    x = wi.spinor_field(dims, 2, 11, bc)
+    y = wi.spinor_field(dims, 2, 12, bc)
+    Dx = orc.apply(dims, kappa, bc, 0, U, x)
+    Ddy = orc.apply(dims, kappa, bc, 1, U, y)
+    g5 = np.array([1, 1, -1, -1.0])[:, None, None]
+    g5Dg5y = orc.apply(dims, kappa, bc, 0, U, y * g5) * g5
+    assert relerr(Ddy, g5Dg5y) < 1e-14
+    for r in range(2):
+        lhs = inner(y[r], Dx[r])
+        rhs = inner(g5Dg5y[r], x[r])
+        assert abs(lhs - rhs) / abs(lhs) < 1e-13
+
+
+@pytest.mark.parametrize("bc", [wi.BC_PERIODIC, wi.BC_SF])
+@pytest.mark.parametrize("dag", [0, 1])
+def test_gauge_covariance(bc, dag):
+    # north_star check (c): D[U^g](g psi) = g D[U] psi
+    dims = (4, 4, 2, 4)
+    kappa = 0.125
+    U = wi.gauge_field(dims, 0.4, 2, bc)
+    psi = wi.spinor_field(dims, 2, 21, bc)
+    g = random_site_su3(dims, 99)
+    gpsi = rview(np.einsum("...ab,n...sb->n...sa", g, cview(psi)))
+    lhs = orc.apply(dims, kappa, bc, dag, gauge_transform(U, g), gpsi)
+    rhs = rview(np.einsum("...ab,n...sb->n...sa", g, cview(orc.apply(dims, kappa, bc, dag, U, psi))))
+    assert relerr(lhs, rhs) < 1e-14
+
+
+def test_staggered_sign_symmetry_and_parity_structure():
+    # Gamma D Gamma = 2 - D with Gamma = (-1)^(x+y+z+t); H maps even sites to odd sites only.
+    dims = (4, 4, 4, 4)
+    kappa = 0.125
+    U = wi.gauge_field(dims, 0.3, 4, wi.BC_PERIODIC)
+    psi = wi.spinor_field(dims, 1, 8, wi.BC_PERIODIC)
+    x, y, z, t = site_coords(dims)
+    sign = (1.0 - 2.0 * ((x + y + z + t) % 2))[None, ..., None, None, None]
+    lhs = sign * orc.apply(dims, kappa, 0, 0, U, sign * psi)
+    rhs = 2.0 * psi - orc.apply(dims, kappa, 0, 0, U, psi)
+    assert relerr(lhs, rhs) < 1e-14
+    even = (sign > 0).astype(np.float64)
+    hop = orc.apply(dims, kappa, 0, 0, U, psi * even) - psi * even
+    assert np.all((hop * even) == 0.0)
+    assert np.linalg.norm(hop) > 1.0
+
+
+def test_identity_at_kappa_zero_and_linearity():
+    dims = (2, 4, 2, 4)
+    U = wi.gauge_field(dims, 0.4, 6, wi.BC_SF)
+    a = wi.spinor_field(dims, 1, 1, wi.BC_SF)
+    b = wi.spinor_field(dims, 1, 2, wi.BC_SF)
+    assert np.array_equal(orc.apply(dims, 0.0, wi.BC_SF, 0, U, a), a)
+    c = rview((0.3 - 1.2j) * cview(a) + (2.0 + 0.5j) * cview(b))
+    lhs = cview(orc.apply(dims, 0.14, wi.BC_SF, 0, U, c))
+    rhs = (0.3 - 1.2j) * cview(orc.apply(dims, 0.14, wi.BC_SF, 0, U, a)) + (2.0 + 0.5j) * cview(
+        orc.apply(dims, 0.14, wi.BC_SF, 0, U, b))
+    assert relerr(lhs, rhs) < 1e-14
+
+
+def test_sf_boundary_treatment():
+    # D_SF = P (1 - kappa H) P: output zero on t=0, input on t=0 ignored, links touching a boundary
+    # slice (all links at t=0, and U_t(t=T-1)) never enter.
+    dims = (4, 2, 2, 6)
+    kappa = 0.135
+    U = wi.gauge_field(dims, 0.4, 9, wi.BC_SF)
+    psi = wi.spinor_field(dims, 2, 5, wi.BC_SF)
+    ref = orc.apply(dims, kappa, wi.BC_SF, 0, U, psi)
+    assert np.all(ref[:, 0] == 0.0)
+    dirty = psi.copy()
+    dirty[:, 0] = wi.spinor_field(dims, 2, 77, wi.BC_PERIODIC)[:, 0]
+    assert np.array_equal(orc.apply(dims, kappa, wi.BC_SF, 0, U, dirty), ref)
+    U2 = U.copy()
+    junk = wi.gauge_field(dims, 1.0, 123, wi.BC_PERIODIC)
+    U2[:, 0] = junk[:, 0]
+    U2[3, dims[3] - 1] = junk[3, dims[3] - 1]
+    assert np.array_equal(orc.apply(dims, kappa, wi.BC_SF, 0, U2, psi), ref)
+    # the SF operator differs from the periodic one on the slices next to the boundary
+    per = orc.apply(dims, kappa, wi.BC_PERIODIC, 0, U, psi)
+    assert np.array_equal(per[:, 2:dims[3] - 1], ref[:, 2:dims[3] - 1])
+    # t=1 differs only through U_t(t=0)^dag psi(t=0), and psi(t=0)=0 here: equal.  t=T-1 sees
+    # psi(t=0)=0 through the wrap: equal as well -- the periodic stencil plus a zero slice IS D_SF.
+    assert np.array_equal(per[:, 1:], ref[:, 1:])
+
+
+# ----------------------------------------------------------------------------- solve
+SMALL = (2, 2, 2, 4)
+
+
+def test_dense_matrix_adjoint_and_lu_inverse():
+    # north_star check (a): dense brute-force inverse on 2^3 x 4.
+    kappa = 0.13
+    U = wi.gauge_field(SMALL, 0.4, 1, wi.BC_SF)
+    A = orc.dense_matrix(SMALL, kappa, wi.BC_SF, 0, U)
+    Ad = orc.dense_matrix(SMALL, kappa, wi.BC_SF, 1, U)
+    assert A.shape == (288, 288)
+    assert np.abs(Ad - A.conj().T).max() < 1e-15
+    phi = wi.spinor_field(SMALL, 3, 1, wi.BC_SF)
+    b = cview(phi)[:, 1:].reshape(3, -1)          # dynamical slices t = 1..T-1, site-major
+    x_lu = orc.lu_solve(A, b)
+    x_np = np.linalg.solve(A, b.T).T              # library routine as a second opinion on the LU
+    assert relerr(x_lu, x_np) < 1e-12
+    X, relres, iters, rc = orc.solve(SMALL, kappa, wi.BC_SF, 0, U, phi, tol=1e-14)
+    assert rc == 0 and relres.max() < 1e-13
+    assert np.all(X[:, 0] == 0.0)
+    assert relerr(cview(X)[:, 1:].reshape(3, -1), x_lu) < 1e-12
+    Y, relres, iters, rc = orc.solve(SMALL, kappa, wi.BC_SF, 1, U, X, tol=1e-14)
+    y_np = np.linalg.solve(A.conj().T, cview(X)[:, 1:].reshape(3, -1).T).T
+    assert rc == 0 and relerr(cview(Y)[:, 1:].reshape(3, -1), y_np) < 1e-12
+
+
+def test_dense_matrix_periodic_matches_apply():
+    dims = (2, 2, 2, 2)
+    U = wi.gauge_field(dims, 0.5, 3, wi.BC_PERIODIC)
+    A = orc.dense_matrix(dims, 0.12, wi.BC_PERIODIC, 0, U)
+    psi = wi.spinor_field(dims, 1, 4, wi.BC_PERIODIC)
+    out = cview(orc.apply(dims, 0.12, wi.BC_PERIODIC, 0, U, psi)).ravel()
+    assert relerr(A @ cview(psi).ravel(), out) < 1e-14
+
+
+def test_solve_true_residual_dagger_and_column_independence():
+    cfg, U, phi = wi.make_config(0)
+    dims, kappa, bc = cfg["dims"], cfg["kappa"], cfg["bc"]
+    X, relres, iters, rc = orc.solve(dims, kappa, bc, 0, U, phi, tol=1e-14)
+    assert rc == 0
+    # true residual recomputed here from D-apply, not taken from the solver
+    R = phi - orc.apply(dims, kappa, bc, 0, U, X)
+    for r in range(cfg["n_rhs"]):
+        assert np.linalg.norm(R[r]) / np.linalg.norm(phi[r]) < 1e-13
+    # Y = D^dag^-1 X equals gamma5 D^-1 gamma5 X
+    Y, _, _, rc = orc.solve(dims, kappa, bc, 1, U, X, tol=1e-14)
+    g5 = np.array([1, 1, -1, -1.0])[:, None, None]
+    Y2, _, _, rc2 = orc.solve(dims, kappa, bc, 0, U, X * g5, tol=1e-14)
+    assert rc == 0 and rc2 == 0
+    assert relerr(Y, Y2 * g5) < 1e-11
+    # Alg. 1 vs Alg. 2: a column solved alone equals the same column in the block
+    X1, _, _, _ = orc.solve(dims, kappa, bc, 0, U, phi[2:3], tol=1e-14)
+    # (to rounding: the OpenMP reductions inside the oracle's dot products are order-dependent)
+    assert relerr(X1[0], X[2]) < 1e-12
+
+
+# ----------------------------------------------------------------------------- force
+def random_antihermitian_traceless(seed):
+    h = wi.random_algebra(seed, wi.STREAM_AUX, 1)[0]
+    return 1j * h
+
+
+def action_dense(dims, kappa, bc, U, phi):
+    """S = sum_i |D^-1 phi_i|^2 (eq. 2.2) via the dense matrix and numpy's solver."""
+    A = orc.dense_matrix(dims, kappa, bc, 0, U)
+    lo = 1 if bc == wi.BC_SF else 0
+    b = cview(phi)[:, lo:].reshape(phi.shape[0], -1)
+    x = np.linalg.solve(A, b.T)
+    return float(np.sum(np.abs(x) ** 2))
+
+
+def perturbed(U, mu, site_tzyx, omega, eps):
+    Uc = cview(U).copy()
+    t, z, y, x = site_tzyx
+    Uc[mu, t, z, y, x] = wi.su3_exp(eps * omega) @ Uc[mu, t, z, y, x]
+    return rview(Uc)
+
+
+@pytest.mark.parametrize("bc", [wi.BC_SF, wi.BC_PERIODIC])
+def test_force_is_the_derivative_of_the_action_dense(bc):
+    # dS/deps |_0 = Re tr[Omega F_mu(x)] under U_mu(x) -> exp(eps Omega) U_mu(x).
+    dims, kappa, n = SMALL, 0.13, 3
+    U = wi.gauge_field(dims, 0.4, 1, bc)
+    phi = wi.spinor_field(dims, n, 1, bc)
+    X, _, _, rc1 = orc.solve(dims, kappa, bc, 0, U, phi, tol=1e-14)
+    Y, _, _, rc2 = orc.solve(dims, kappa, bc, 1, U, X, tol=1e-14)
+    assert rc1 == 0 and rc2 == 0
+    F = cview(orc.force(dims, kappa, bc, U, X, Y))
+    eps = 1e-4
+    # L = 2 in space: forward and backward neighbour coincide there -- the awkward case.
+    probes = [(0, (1, 0, 1, 0)), (1, (2, 1, 0, 1)), (2, (1, 1, 1, 1)), (3, (1, 0, 0, 1)), (3, (2, 1, 1, 0))]
+    for k, (mu, site) in enumerate(probes):
+        om = random_antihermitian_traceless(40 + k)
+        sp = action_dense(dims, kappa, bc, perturbed(U, mu, site, om, +eps), phi)
+        sm = action_dense(dims, kappa, bc, perturbed(U, mu, site, om, -eps), phi)
+        fd = (sp - sm) / (2 * eps)
+        an = np.real(np.trace(om @ F[(mu,) + site]))
+        assert abs(an) > 1e-3, "probe must be sensitive"
+        assert abs(fd - an) / abs(an) < 5e-7, (mu, site, fd, an)
+
+
+def test_force_is_the_derivative_of_the_action_config0():
+    # same identity on BASELINE.json configs[0] (4^3 x 4 SF, eps 0.2, kappa 0.125, 5 RHS), with the
+    # oracle's own iterative solves supplying S.
+    cfg, U, phi = wi.make_config(0)
+    dims, kappa, bc = cfg["dims"], cfg["kappa"], cfg["bc"]
+
+    def action(Uv):
+        X, _, _, rc = orc.solve(dims, kappa, bc, 0, Uv, phi, tol=1e-14)
+        assert rc == 0
+        return float(np.sum(X ** 2)), X
+
+    _, X = action(U)
+    Y, _, _, rc = orc.solve(dims, kappa, bc, 1, U, X, tol=1e-14)
+    F = cview(orc.force(dims, kappa, bc, U, X, Y))
+    eps = 1e-4
+    for k, (mu, site) in enumerate([(0, (2, 1, 3, 0)), (3, (1, 2, 0, 3)), (2, (3, 3, 1, 2))]):
+        om = random_antihermitian_traceless(60 + k)
+        sp, _ = action(perturbed(U, mu, site, om, +eps))
+        sm, _ = action(perturbed(U, mu, site, om, -eps))
+        fd = (sp - sm) / (2 * eps)
+        an = np.real(np.trace(om @ F[(mu,) + site]))
+        assert abs(fd - an) / abs(an) < 5e-7, (mu, site, fd, an)
+
+
+def test_force_structure_sf():
+    cfg, U, phi = wi.make_config(0)
+    dims, kappa, bc = cfg["dims"], cfg["kappa"], cfg["bc"]
+    X, _, _, _ = orc.solve(dims, kappa, bc, 0, U, phi, tol=1e-14)
+    Y, _, _, _ = orc.solve(dims, kappa, bc, 1, U, X, tol=1e-14)
+    F = cview(orc.force(dims, kappa, bc, U, X, Y))
+    Fd = np.conj(np.swapaxes(F, -1, -2))
+    assert np.abs(F + Fd).max() == 0.0                      # antihermitian
+    assert np.abs(np.trace(F, axis1=-2, axis2=-1)).max() < 1e-13   # traceless
+    # zero on every link touching a boundary slice: all links at t=0 and U_t(t=T-1)
+    assert np.all(F[:, 0] == 0.0)
+    assert np.all(F[3, dims[3] - 1] == 0.0)
+    assert np.abs(F[0, 1]).max() > 1e-3
+    # additivity over right-hand sides: Alg. 1 (sequential accumulation) == Alg. 2 (blocked)
+    Fseq = np.zeros(U.shape)
+    for i in range(cfg["n_rhs"]):
+        orc.force(dims, kappa, bc, U, X[i:i + 1], Y[i:i + 1], Fseq)
+    assert relerr(cview(Fseq), F) < 1e-14
+    # accumulation: F is added to, not overwritten
+    F2 = orc.force(dims, kappa, bc, U, X, Y, rview(F).copy())
+    assert relerr(cview(F2), 2 * F) < 1e-15
+
+
+def test_force_gauge_covariance():
+    # F[U^g; g x, g y] = g(x) F_mu(x) g(x)^dag
+    dims, kappa, bc = (4, 2, 2, 4), 0.13, wi.BC_PERIODIC
+    U = wi.gauge_field(dims, 0.4, 5, bc)
+    X = wi.spinor_field(dims, 2, 31, bc)
+    Y = wi.spinor_field(dims, 2, 32, bc)
+    g = random_site_su3(dims, 17)
+    rot = lambda psi: rview(np.einsum("...ab,n...sb->n...sa", g, cview(psi)))
+    F = cview(orc.force(dims, kappa, bc, U, X, Y))
+    Fg = cview(orc.force(dims, kappa, bc, gauge_transform(U, g), rot(X), rot(Y)))
+    expect = np.einsum("...ab,m...bc,...dc->m...ad", g, F, np.conj(g))
+    assert relerr(Fg, expect) < 1e-14
