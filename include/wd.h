@@ -1,0 +1,153 @@
+/* wd.h -- C ABI of the B200 (sm_100a) blocked Wilson-Dirac solve + fermion force library.
+ *
+ * What it computes (arxiv/paper_1009_5169, "Algorithm 2", eq. 2.3):
+ *     2: solve D X = Phi          X  = D^-1 Phi            (N_f/2 columns at once)
+ *     3: solve D^dag Y = X        Y  = D^dag^-1 X
+ *     5: F_mu = F_mu + f[x_i, y_i]   for every column i
+ * with D the Wilson-Dirac operator on a lattice with Schroedinger-functional (Dirichlet) time
+ * boundaries.  The paper fixes neither the normalisation of D, the gamma basis, the
+ * SF convention nor f[x,y]; the readings used are listed in DESIGN.md ("Readings"):
+ *     D = 1 - kappa H,
+ *     (H psi)(x) = sum_mu (1-gamma_mu) U_mu(x) psi(x+mu) + (1+gamma_mu) U_mu(x-mu)^dag psi(x-mu),
+ *     D^dag: gamma_mu -> -gamma_mu;   SF: psi(t=0) = psi(t=T) = 0, T slices stored (t = 0..T-1),
+ *     f[x,y]_mu(s) = 2 kappa TA[ U_mu(s) W ],  TA(M) = (M - M^dag)/2 - tr(M - M^dag)/6,
+ *     W = sum_spin x(s+mu) (x) ((1-gamma_mu) y(s))^dag + ((1+gamma_mu) y(s+mu)) (x) x(s)^dag.
+ *
+ * Conventions common to every call
+ *   - Every function returns an int: WD_OK (0) or a negative WD_E* code.  Nothing throws or aborts
+ *     across this boundary.  wd_last_error(ctx) gives a text for the last failure on that context.
+ *   - Pointers named *_dev are DEVICE pointers (cudaMalloc'ed by the caller, e.g. a torch tensor's
+ *     data_ptr()); pointers named *_host are HOST pointers.  The caller owns every buffer it
+ *     passes; the library owns only the context and never allocates device memory after
+ *     wd_set_workspace (all its scratch is carved from the caller's workspace).
+ *   - All work is enqueued on the CUDA stream given to wd_create.  wd_apply, wd_pack, wd_unpack,
+ *     wd_force and wd_set_gauge do not synchronise.  wd_solve_block synchronises the stream to
+ *     read convergence scalars.  The *_host entry points synchronise before returning.
+ *   - dims = (Lx, Ly, Lz, T), all even, >= 2 (>= 4 in T for WD_BC_SF).  mu = 0,1,2,3 = x,y,z,t.
+ *
+ * Layouts
+ *   CANONICAL (fp64, what a user holds):
+ *     gauge / force  double [mu=4][T][Lz][Ly][Lx][3][3][2]    row-major colour matrix, (re,im)
+ *     spinor block   double [n_rhs][T][Lz][Ly][Lx][4][3][2]   spin, colour, (re,im)
+ *   NATIVE (what the kernels read; produced by wd_pack, consumed by wd_unpack):
+ *     sites are split by parity (x+y+z+t) mod 2 (even = 0) and numbered 0..V/2-1 inside a parity
+ *     in the context's site order (wd_site_order); a full-lattice block of n_rhs spinors is
+ *       fp64:  double2 [parity=2][k=12][V/2][n_rhs]      k = spin*3+colour, one complex per double2
+ *       fp32:  float4  [parity=2][c=6 ][V/2][n_rhs]      complex 2c and 2c+1 per float4
+ *     i.e. structure-of-arrays, site-major / RHS-minor, 128-bit elements.  wd_native_bytes gives
+ *     the size.  In SF mode the t=0 slice is stored and is zero in every native field the library
+ *     produces; wd_pack writes zeros there whatever the canonical input holds.
+ */
+#ifndef WD_H
+#define WD_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct wd_ctx wd_ctx; /* opaque; created by wd_create, freed by wd_destroy */
+
+enum { WD_OK = 0, WD_EINVAL = -1, WD_ENOMEM = -2, WD_ECUDA = -3, WD_ENOCONV = -4, WD_ESTATE = -5 };
+enum { WD_BC_PERIODIC = 0, WD_BC_SF = 1 }; /* time direction; space is always periodic, theta=0 */
+enum { WD_OP_D = 0, WD_OP_DDAG = 1 };
+enum { WD_F64 = 0, WD_F32 = 1 };
+enum { WD_LINK18 = 0, WD_LINK12 = 1 }; /* 18 reals per link, or rows 1-2 only */
+enum { WD_ORDER_LINEAR = 0, WD_ORDER_TILED = 1 };
+
+#define WD_MAX_RHS 16
+
+/* Filled by wd_solve_block (all host memory, owned by the caller). */
+typedef struct wd_solve_info {
+    int    n_rhs;
+    int    outer_steps;               /* fp64 defect-correction steps taken (inner solver calls)     */
+    int    inner_iters_total;         /* fp32 BiCGStab iterations summed over the outer steps         */
+    int    converged;                 /* 1 if every column met tol                                    */
+    double relres[WD_MAX_RHS];        /* final TRUE fp64 residual |phi_i - A x_i| / |phi_i|            */
+    double bnorm[WD_MAX_RHS];         /* |phi_i|                                                      */
+    double seconds;                   /* host wall time of the call (includes its synchronisations)   */
+} wd_solve_info;
+
+/* Create a context for a lattice (problem statement: "SF setup ... Wilson quarks",
+ * kappa = hopping parameter).  time_bc = WD_BC_SF gives the Dirichlet time boundaries.  max_rhs
+ * (1..WD_MAX_RHS) bounds n_rhs of every later call and sizes the workspace.  cuda_stream is a
+ * cudaStream_t (NULL = legacy default stream).  Errors: WD_EINVAL (null, odd or too small dims,
+ * kappa not finite, max_rhs out of range), WD_ECUDA (no device), WD_ENOMEM (host). */
+int wd_create(wd_ctx** out, const int dims[4], double kappa, int time_bc, int max_rhs, void* cuda_stream);
+int wd_destroy(wd_ctx* ctx);
+
+/* Choose how sites are numbered inside a parity (affects only the native layout, hence speed):
+ * WD_ORDER_LINEAR: x/2 fastest, then y, z, t.  WD_ORDER_TILED: blocks of tile[] = (bx,by,bz,bt)
+ * full-lattice sites are contiguous (each must divide the matching dim; bx even).  Must be
+ * called before wd_set_workspace; default is WD_ORDER_LINEAR.  Errors: WD_EINVAL, WD_ESTATE. */
+int wd_site_order(wd_ctx* ctx, int order, const int tile[4]);
+
+/* Scratch memory: the caller allocates wd_workspace_bytes(ctx) bytes of device memory (256-byte
+ * aligned) and hands it over; it must stay valid until wd_destroy.  wd_set_workspace uploads the
+ * site tables.  Errors: WD_EINVAL (null, too small, misaligned), WD_ECUDA. */
+size_t wd_workspace_bytes(const wd_ctx* ctx);
+int    wd_set_workspace(wd_ctx* ctx, void* ws_dev, size_t bytes);
+
+/* Gauge ingest (hot-path step a0): canonical fp64 links -> the library's native fp64 and fp32
+ * copies, each in 18-real and 12-real form ("single-precision coefficient matrix D on the GPUs",
+ * PAPER.md:84; "3rd column ... dropped ... reconstructed on the fly").  The canonical
+ * buffer is not referenced after the enqueued kernels finish.  Errors: WD_ESTATE (no workspace). */
+int wd_set_gauge(wd_ctx* ctx, const double* U_canon_dev);
+
+/* Bytes of a native full-lattice block of n_rhs spinors in precision prec (WD_F64 / WD_F32). */
+size_t wd_native_bytes(const wd_ctx* ctx, int prec, int n_rhs);
+
+/* canonical fp64 block [n_rhs][T][Lz][Ly][Lx][4][3][2]  <->  native block of precision prec. */
+int wd_pack(wd_ctx* ctx, int prec, int n_rhs, const double* canon_dev, void* native_dev);
+int wd_unpack(wd_ctx* ctx, int prec, int n_rhs, const void* native_dev, double* canon_dev);
+
+/* out = D in (op = WD_OP_D) or D^dag in (WD_OP_DDAG) on a native full-lattice block, all n_rhs
+ * columns in one pass per output parity (two launches of the hopping kernel with the diagonal
+ * term fused).  prec picks fp64 or fp32 arithmetic and storage, recon the link form.  in and out
+ * must not overlap.  Errors: WD_ESTATE (no gauge), WD_EINVAL (n_rhs, enums, null). */
+int wd_apply(wd_ctx* ctx, int op, int prec, int recon, int n_rhs, const void* in_native_dev, void* out_native_dev);
+
+/* The bare hopping term on one output parity (hot-path step a2), exposed for measurement:
+ * out[out_parity] = H in[1-out_parity] ("dslash").  in/out are native HALF-lattice blocks, i.e.
+ * [k or c][V/2][n_rhs] (half of wd_native_bytes).  Same errors as wd_apply. */
+int wd_hop(wd_ctx* ctx, int op, int prec, int recon, int n_rhs, int out_parity, const void* in_half_dev, void* out_half_dev);
+
+/* Blocked solve (Algorithm 2 lines 2-3): A X = Phi with A = D (WD_OP_D) or D^dag
+ * (WD_OP_DDAG), Phi and X native fp64 full-lattice blocks (X may not alias Phi).  Route: site
+ * even/odd preconditioning, fp64 defect-correction outer loop around an fp32
+ * BiCGStab run in lock-step over the columns with per-column scalars.  Stops
+ * when every column has |phi_i - A x_i| <= tol |phi_i| in fp64 (true residual), or after
+ * max_outer outer steps of at most max_inner inner iterations each; inner_tol (0 = default 1e-5)
+ * is the relative reduction asked of each inner call; recon picks the inner (fp32) link form,
+ * the fp64 outer operator always uses 18 reals.  Returns WD_ENOCONV if tol was not met: X then
+ * holds the best iterate and info is still filled.  info may be NULL. */
+int wd_solve_block(wd_ctx* ctx, int op, int n_rhs, const double* Phi_native_dev, double* X_native_dev,
+                   double tol, int max_outer, int max_inner, double inner_tol, int recon,
+                   wd_solve_info* info);
+
+/* Force accumulation (Algorithm 2 lines 4-6): F += sum_i f[x_i, y_i] with X, Y
+ * native fp64 full-lattice blocks and F canonical fp64 [mu][T][Lz][Ly][Lx][3][3][2].  F is
+ * ACCUMULATED ("F_mu = F_mu + f[x_i,y_i]"); the caller zeroes it. */
+int wd_force(wd_ctx* ctx, int n_rhs, const double* X_native_dev, const double* Y_native_dev, double* F_canon_dev);
+
+/* One whole MD force evaluation from HOST buffers (Algorithm 2 as a single call): copies the
+ * canonical Phi to the device, packs, solves D X = Phi and D^dag Y = X, accumulates the force
+ * into a zeroed device buffer and copies it to F_canon_host (overwritten, not accumulated).
+ * Staging buffers come from the workspace.  info[0], info[1] (nullable) describe the two solves.
+ * Synchronises.  Phi_canon_host/F_canon_host should be pinned for full copy bandwidth. */
+int wd_md_force_host(wd_ctx* ctx, int n_rhs, const double* Phi_canon_host, double* F_canon_host,
+                     double tol, int max_outer, int max_inner, double inner_tol, int recon,
+                     wd_solve_info* info2);
+
+/* Number of kernel launches this context has enqueued since creation (for bench.py's count). */
+long long wd_launch_count(const wd_ctx* ctx);
+
+const char* wd_strerror(int code);
+const char* wd_last_error(const wd_ctx* ctx);
+const char* wd_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* WD_H */

@@ -1,0 +1,8 @@
+"""B200-native (sm_100a) blocked Wilson-Dirac solve + fermion force of arxiv/paper_1009_5169.
+
+The product is the C-ABI library `libwd.so` (include/wd.h, sources in csrc/); `wd` is its thin
+ctypes binding.  Build with `python -m paper_1009_5169_b200.build`.
+"""
+from . import wd  # noqa: F401
+from .wd import (BC_PERIODIC, BC_SF, F32, F64, LINK12, LINK18, OP_D, OP_DDAG, ORDER_LINEAR,  # noqa: F401
+                 ORDER_TILED, Context, WdError)

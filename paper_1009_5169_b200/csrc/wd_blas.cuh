@@ -1,0 +1,176 @@
+// wd_blas.cuh -- batched-per-RHS BLAS1 updates fused with their inner products (hot-path step a4)
+// and the device-side scalar recurrences of BiCGStab (restated in DESIGN.md).
+//
+// Thread mapping: a block has B = 32*n*m threads (m = ceil(8/n)), so B is a multiple of n and thread
+// t always works on column r = t % n of the flat RHS-minor vector index.  Per-column sums go
+// thread -> shared memory (transposed so one warp owns one column) -> warp shuffle -> one partial
+// per block and column in global memory -> the LAST block to finish (atomic ticket) adds the
+// partials in a fixed order and runs the scalar recurrence, so no scalar ever visits the host and
+// the result does not depend on block scheduling.  All sums are accumulated in fp64.
+#pragma once
+#include "wd_internal.h"
+
+namespace wdblas {
+
+// ---- layout of the per-column scalar table (doubles, column stride WD_MAX_RHS) -------------------
+enum {
+    S_RHO_RE = 0, S_RHO_IM, S_ALPHA_RE, S_ALPHA_IM, S_OMEGA_RE, S_OMEGA_IM, S_BETA_RE, S_BETA_IM,
+    S_RNORM2,     // recursive |r_i|^2 of the inner solver
+    S_THR2,       // inner stopping threshold on |r_i|^2
+    S_FLAG,       // 0 active, 1 converged (frozen), 2 breakdown (frozen)
+    S_OUT_R2,     // outer true residual |R_i|^2 (even/odd system)
+    S_PHI2,       // |phi_i|^2 over the full lattice
+    S_SCALE,      // |R_i| used to normalise the inner right-hand side
+    S_OUT_CONV,   // 1 if column met the outer tolerance
+    S_ROWS
+};
+// global (not per-column) slots after the table
+enum { G_DONE = S_ROWS * WD_MAX_RHS, G_ITERS, G_OUT_DONE, G_TOL2, G_INTOL2, G_COUNT };
+
+__device__ __forceinline__ double& SC(double* scal, int row, int r) { return scal[row * WD_MAX_RHS + r]; }
+
+enum Kind { K_SIGMA, K_OMEGA, K_RHO, K_PHI2, K_OUT_R2, K_INIT_RHO };
+
+struct RedBuf {
+    double* scal;
+    double* partials;
+    unsigned int* ticket;
+};
+
+template <typename T> struct V;
+template <> struct V<float> { typedef float4 type; enum { NC = 2 }; };
+template <> struct V<double> { typedef double2 type; enum { NC = 1 }; };
+
+struct cd { double re, im; };
+__device__ __forceinline__ cd cmul(cd a, cd b) { return {a.re * b.re - a.im * b.im, a.re * b.im + a.im * b.re}; }
+__device__ __forceinline__ cd cdiv(cd a, cd b) {
+    const double d = b.re * b.re + b.im * b.im;
+    return {(a.re * b.re + a.im * b.im) / d, (a.im * b.re - a.re * b.im) / d};
+}
+
+// ---- scalar recurrences, run by one thread per column in the last block ---------------------------
+template <int KIND>
+__device__ void finalize_column(double* scal, int r, const double* tot) {
+    const bool frozen = SC(scal, S_FLAG, r) != 0.0;
+    if (KIND == K_SIGMA) {  // tot = <rt, v>;  alpha = rho / sigma
+        cd alpha = {0.0, 0.0};
+        if (!frozen) {
+            const cd sigma = {tot[0], tot[1]};
+            if (sigma.re == 0.0 && sigma.im == 0.0) SC(scal, S_FLAG, r) = 2.0;
+            else alpha = cdiv({SC(scal, S_RHO_RE, r), SC(scal, S_RHO_IM, r)}, sigma);
+        }
+        SC(scal, S_ALPHA_RE, r) = alpha.re;
+        SC(scal, S_ALPHA_IM, r) = alpha.im;
+    } else if (KIND == K_OMEGA) {  // tot = <t, s>, <t, t>;  omega = <t,s>/<t,t>
+        cd omega = {0.0, 0.0};
+        if (!frozen && tot[2] > 0.0) omega = {tot[0] / tot[2], tot[1] / tot[2]};
+        SC(scal, S_OMEGA_RE, r) = omega.re;
+        SC(scal, S_OMEGA_IM, r) = omega.im;
+    } else if (KIND == K_RHO || KIND == K_INIT_RHO) {  // tot = <rt, r>, |r|^2
+        if (KIND == K_INIT_RHO) {
+            SC(scal, S_RHO_RE, r) = tot[0]; SC(scal, S_RHO_IM, r) = tot[1];
+            SC(scal, S_ALPHA_RE, r) = 1.0;  SC(scal, S_ALPHA_IM, r) = 0.0;
+            SC(scal, S_OMEGA_RE, r) = 1.0;  SC(scal, S_OMEGA_IM, r) = 0.0;
+            SC(scal, S_BETA_RE, r) = 0.0;   SC(scal, S_BETA_IM, r) = 0.0;
+            SC(scal, S_RNORM2, r) = tot[2];
+            // S_FLAG was set by the outer residual kernel (1 = column already converged)
+            if (!frozen && !(tot[2] > 0.0)) SC(scal, S_FLAG, r) = 1.0;
+            return;
+        }
+        if (frozen) {
+            SC(scal, S_BETA_RE, r) = 0.0; SC(scal, S_BETA_IM, r) = 0.0;
+            return;
+        }
+        SC(scal, S_RNORM2, r) = tot[2];
+        const cd rho1 = {tot[0], tot[1]};
+        const cd rho = {SC(scal, S_RHO_RE, r), SC(scal, S_RHO_IM, r)};
+        const cd alpha = {SC(scal, S_ALPHA_RE, r), SC(scal, S_ALPHA_IM, r)};
+        const cd omega = {SC(scal, S_OMEGA_RE, r), SC(scal, S_OMEGA_IM, r)};
+        cd beta = {0.0, 0.0};
+        if (tot[2] <= SC(scal, S_THR2, r)) {
+            SC(scal, S_FLAG, r) = 1.0;
+        } else if (!(tot[2] == tot[2]) || (omega.re == 0.0 && omega.im == 0.0) || (rho1.re == 0.0 && rho1.im == 0.0)) {
+            SC(scal, S_FLAG, r) = 2.0;  // breakdown or NaN: freeze; the outer loop restarts from the true residual
+        } else {
+            beta = cmul(cdiv(rho1, rho), cdiv(alpha, omega));
+        }
+        SC(scal, S_RHO_RE, r) = rho1.re; SC(scal, S_RHO_IM, r) = rho1.im;
+        SC(scal, S_BETA_RE, r) = beta.re; SC(scal, S_BETA_IM, r) = beta.im;
+    } else if (KIND == K_PHI2) {
+        SC(scal, S_PHI2, r) = tot[0];
+    } else if (KIND == K_OUT_R2) {  // tot = |R_i|^2 of the fp64 even/odd system
+        SC(scal, S_OUT_R2, r) = tot[0];
+        const double phi2 = SC(scal, S_PHI2, r);
+        const double tol2 = scal[G_TOL2];
+        const bool conv = tot[0] <= tol2 * phi2;
+        SC(scal, S_OUT_CONV, r) = conv ? 1.0 : 0.0;
+        SC(scal, S_SCALE, r) = sqrt(tot[0]);
+        SC(scal, S_FLAG, r) = conv ? 1.0 : 0.0;
+        // inner target: the asked reduction, but never far below what the outer tolerance needs
+        double thr2 = scal[G_INTOL2];
+        if (tot[0] > 0.0) thr2 = fmax(thr2, 0.01 * tol2 * phi2 / tot[0]);
+        SC(scal, S_THR2, r) = thr2;  // inner rhs is normalised to |b_i| = 1
+    }
+}
+
+template <int KIND>
+__device__ void finalize_global(double* scal, int n) {
+    if (KIND == K_RHO || KIND == K_INIT_RHO) {
+        bool all = true;
+        for (int r = 0; r < n; ++r) all = all && (SC(scal, S_FLAG, r) != 0.0);
+        scal[G_DONE] = all ? 1.0 : 0.0;
+        if (KIND == K_RHO) scal[G_ITERS] += 1.0;
+    } else if (KIND == K_OUT_R2) {
+        bool all = true;
+        for (int r = 0; r < n; ++r) all = all && (SC(scal, S_OUT_CONV, r) != 0.0);
+        scal[G_OUT_DONE] = all ? 1.0 : 0.0;
+    }
+}
+
+// Block + grid reduction of K per-thread fp64 sums for column r = threadIdx.x % n, then finalize.
+template <int K, int KIND>
+__device__ void reduce_finalize(double (&v)[K], int n, RedBuf rb) {
+    __shared__ double sh[4 * 512];
+    __shared__ bool is_last;
+    const int B = blockDim.x, t = threadIdx.x;
+    const int per = B / n;  // threads per column, a multiple of 32
+    const int r = t % n, q = t / n;
+#pragma unroll
+    for (int k = 0; k < K; ++k) sh[k * B + r * per + q] = v[k];
+    __syncthreads();
+    const int warp = t >> 5, lane = t & 31;
+    if (warp < n) {
+#pragma unroll
+        for (int k = 0; k < K; ++k) {
+            double s = 0.0;
+            for (int j = lane; j < per; j += 32) s += sh[k * B + warp * per + j];
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+            if (lane == 0) rb.partials[((long)blockIdx.x * n + warp) * K + k] = s;
+        }
+    }
+    __threadfence();
+    __syncthreads();
+    if (t == 0) is_last = (atomicAdd(rb.ticket, 1u) == gridDim.x - 1);
+    __syncthreads();
+    if (!is_last) return;
+    __threadfence();
+    // last block: column sums in fixed block order
+    const int nwarps = B >> 5;
+    for (int item = warp; item < n * K; item += nwarps) {
+        double s = 0.0;
+        for (int g = lane; g < (int)gridDim.x; g += 32) s += rb.partials[(long)g * n * K + item];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+        if (lane == 0) sh[item] = s;
+    }
+    __syncthreads();
+    if (t < n) finalize_column<KIND>(rb.scal, t, &sh[t * K]);
+    __syncthreads();
+    if (t == 0) {
+        finalize_global<KIND>(rb.scal, n);
+        *rb.ticket = 0u;
+    }
+}
+
+}  // namespace wdblas

@@ -1,0 +1,336 @@
+// wd_ctx.cu -- context life cycle, site tables, workspace map and the argument-checking front of
+// every C-ABI entry point declared in include/wd.h.
+#include <chrono>
+#include <cmath>
+#include <cstring>
+#include <new>
+
+#include "wd_internal.h"
+
+namespace {
+
+inline long canon_site(const wd_ctx* c, const int x[4]) {
+    return x[0] + (long)c->L[0] * (x[1] + (long)c->L[1] * (x[2] + (long)c->L[2] * x[3]));
+}
+
+// position of a site inside its parity for the chosen order
+long order_index(const wd_ctx* c, const int x[4]) {
+    if (c->order == WD_ORDER_LINEAR) return canon_site(c, x) >> 1;
+    const int* b = c->tile;
+    int nt[4], tc[4], ic[4];
+    for (int d = 0; d < 4; ++d) { nt[d] = c->L[d] / b[d]; tc[d] = x[d] / b[d]; ic[d] = x[d] % b[d]; }
+    long tile_idx = tc[0] + (long)nt[0] * (tc[1] + (long)nt[1] * (tc[2] + (long)nt[2] * tc[3]));
+    long in_tile = ic[0] + (long)b[0] * (ic[1] + (long)b[1] * (ic[2] + (long)b[2] * ic[3]));
+    long tile_half = (long)b[0] * b[1] * b[2] * b[3] / 2;
+    return tile_idx * tile_half + (in_tile >> 1);
+}
+
+void build_tables(wd_ctx* c) {
+    const long V = c->V, Vh = c->Vh;
+    c->h_site_of.assign(2 * Vh, -1);
+    c->h_nbr.assign(2 * Vh * WD_NDIR, 0);
+    std::vector<int32_t> idx_of(V);
+    int x[4];
+    for (x[3] = 0; x[3] < c->L[3]; ++x[3])
+        for (x[2] = 0; x[2] < c->L[2]; ++x[2])
+            for (x[1] = 0; x[1] < c->L[1]; ++x[1])
+                for (x[0] = 0; x[0] < c->L[0]; ++x[0]) {
+                    const int p = (x[0] + x[1] + x[2] + x[3]) & 1;
+                    const long h = order_index(c, x);
+                    const long s = canon_site(c, x);
+                    c->h_site_of[p * Vh + h] = (int32_t)s;
+                    idx_of[s] = (int32_t)h;
+                }
+    for (x[3] = 0; x[3] < c->L[3]; ++x[3])
+        for (x[2] = 0; x[2] < c->L[2]; ++x[2])
+            for (x[1] = 0; x[1] < c->L[1]; ++x[1])
+                for (x[0] = 0; x[0] < c->L[0]; ++x[0]) {
+                    const int p = (x[0] + x[1] + x[2] + x[3]) & 1;
+                    const long h = idx_of[canon_site(c, x)];
+                    int32_t* nb = &c->h_nbr[(p * Vh + h) * WD_NDIR];
+                    for (int mu = 0; mu < 4; ++mu)
+                        for (int s = 0; s < 2; ++s) {
+                            int y[4] = {x[0], x[1], x[2], x[3]};
+                            y[mu] = (y[mu] + (s == 0 ? 1 : c->L[mu] - 1)) % c->L[mu];
+                            nb[2 * mu + s] = idx_of[canon_site(c, y)];
+                        }
+                    // SF: the stored t=0 slice is not dynamical.  Its neighbours at t=1 / t=T-1 read it
+                    // as the zero field, which is exactly psi(t=0) = psi(t=T) = 0 (SF reading).
+                    if (c->bc == WD_BC_SF && x[3] == 0) nb[0] = (int32_t)((uint32_t)nb[0] | WD_SITE_FROZEN);
+                }
+}
+
+struct WsMap {
+    size_t site_of, nbr, u64[2], u32[2], scal, partials, ticket, solver, total;
+};
+
+const int kReals[2] = {18, 12};
+const size_t kScalDoubles = 64 * WD_MAX_RHS;
+const size_t kPartialDoubles = 4096 * 8;  // >= max blocks of any reduction * values per block
+
+WsMap ws_map(const wd_ctx* c) {
+    WsMap m;
+    size_t o = 0;
+    m.site_of = o; o += wd_align_up(sizeof(int32_t) * 2 * c->Vh);
+    m.nbr = o;     o += wd_align_up(sizeof(int32_t) * 2 * c->Vh * WD_NDIR);
+    for (int r = 0; r < 2; ++r) { m.u64[r] = o; o += wd_align_up(sizeof(double) * 4 * c->V * kReals[r]); }
+    for (int r = 0; r < 2; ++r) { m.u32[r] = o; o += wd_align_up(sizeof(float) * 4 * c->V * kReals[r]); }
+    m.scal = o;     o += wd_align_up(sizeof(double) * kScalDoubles);
+    m.partials = o; o += wd_align_up(sizeof(double) * kPartialDoubles * WD_MAX_RHS);
+    m.ticket = o;   o += wd_align_up(256);
+    m.solver = o;   o += wd_align_up(wd_solver_scratch_bytes(c));
+    m.total = o;
+    return m;
+}
+
+bool bad_n(const wd_ctx* c, int n) { return n < 1 || n > c->max_rhs; }
+
+}  // namespace
+
+extern "C" {
+
+const char* wd_version(void) { return "wd 0.1 (sm_100a)"; }
+
+const char* wd_strerror(int code) {
+    switch (code) {
+        case WD_OK: return "ok";
+        case WD_EINVAL: return "invalid argument";
+        case WD_ENOMEM: return "out of memory";
+        case WD_ECUDA: return "CUDA error";
+        case WD_ENOCONV: return "solver did not reach the tolerance";
+        case WD_ESTATE: return "call out of order (workspace or gauge field not set)";
+        default: return "unknown error code";
+    }
+}
+
+const char* wd_last_error(const wd_ctx* ctx) { return ctx ? ctx->err.c_str() : "null context"; }
+
+long long wd_launch_count(const wd_ctx* ctx) { return ctx ? ctx->launches : 0; }
+
+int wd_create(wd_ctx** out, const int dims[4], double kappa, int time_bc, int max_rhs, void* cuda_stream) {
+    if (!out || !dims) return WD_EINVAL;
+    *out = nullptr;
+    if (!std::isfinite(kappa)) return WD_EINVAL;
+    if (time_bc != WD_BC_PERIODIC && time_bc != WD_BC_SF) return WD_EINVAL;
+    if (max_rhs < 1 || max_rhs > WD_MAX_RHS) return WD_EINVAL;
+    long V = 1;
+    for (int d = 0; d < 4; ++d) {
+        if (dims[d] < 2 || (dims[d] & 1)) return WD_EINVAL;
+        V *= dims[d];
+        if (V > (1L << 30)) return WD_EINVAL;
+    }
+    if (time_bc == WD_BC_SF && dims[3] < 4) return WD_EINVAL;
+    int dev = 0;
+    cudaDeviceProp prop;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) {
+        cudaGetLastError();
+        return WD_ECUDA;
+    }
+    wd_ctx* c = new (std::nothrow) wd_ctx();
+    if (!c) return WD_ENOMEM;
+    for (int d = 0; d < 4; ++d) c->L[d] = dims[d];
+    c->V = V;
+    c->Vh = V / 2;
+    c->kappa = kappa;
+    c->bc = time_bc;
+    c->max_rhs = max_rhs;
+    c->stream = (cudaStream_t)cuda_stream;
+    c->n_sm = prop.multiProcessorCount;
+    c->order = WD_ORDER_LINEAR;
+    for (int d = 0; d < 4; ++d) c->tile[d] = dims[d];
+    c->ws = nullptr;
+    c->ws_bytes = 0;
+    c->have_ws = c->have_gauge = false;
+    c->launches = 0;
+    c->h_pinned = nullptr;
+    if (cudaMallocHost((void**)&c->h_pinned, sizeof(double) * kScalDoubles) != cudaSuccess) {
+        cudaGetLastError();
+        delete c;
+        return WD_ENOMEM;
+    }
+    try {
+        build_tables(c);
+    } catch (const std::bad_alloc&) {
+        cudaFreeHost(c->h_pinned);
+        delete c;
+        return WD_ENOMEM;
+    }
+    *out = c;
+    return WD_OK;
+}
+
+int wd_destroy(wd_ctx* ctx) {
+    if (!ctx) return WD_EINVAL;
+    if (ctx->h_pinned) cudaFreeHost(ctx->h_pinned);
+    delete ctx;
+    return WD_OK;
+}
+
+int wd_site_order(wd_ctx* ctx, int order, const int tile[4]) {
+    if (!ctx) return WD_EINVAL;
+    if (ctx->have_ws) return wd_fail(ctx, WD_ESTATE, "wd_site_order must precede wd_set_workspace");
+    if (order == WD_ORDER_LINEAR) {
+        ctx->order = order;
+    } else if (order == WD_ORDER_TILED) {
+        if (!tile) return wd_fail(ctx, WD_EINVAL, "tile is null");
+        for (int d = 0; d < 4; ++d)
+            if (tile[d] < 1 || ctx->L[d] % tile[d]) return wd_fail(ctx, WD_EINVAL, "tile must divide dims");
+        if (tile[0] & 1) return wd_fail(ctx, WD_EINVAL, "tile[0] must be even");
+        ctx->order = order;
+        for (int d = 0; d < 4; ++d) ctx->tile[d] = tile[d];
+    } else {
+        return wd_fail(ctx, WD_EINVAL, "unknown site order");
+    }
+    try {
+        build_tables(ctx);
+    } catch (const std::bad_alloc&) {
+        return wd_fail(ctx, WD_ENOMEM, "site tables");
+    }
+    return WD_OK;
+}
+
+size_t wd_workspace_bytes(const wd_ctx* ctx) { return ctx ? ws_map(ctx).total : 0; }
+
+int wd_set_workspace(wd_ctx* ctx, void* ws_dev, size_t bytes) {
+    if (!ctx) return WD_EINVAL;
+    if (!ws_dev) return wd_fail(ctx, WD_EINVAL, "workspace is null");
+    if (((uintptr_t)ws_dev) & 255) return wd_fail(ctx, WD_EINVAL, "workspace must be 256-byte aligned");
+    const WsMap m = ws_map(ctx);
+    if (bytes < m.total) return wd_fail(ctx, WD_EINVAL, "workspace too small");
+    char* w = (char*)ws_dev;
+    ctx->ws = w;
+    ctx->ws_bytes = bytes;
+    ctx->d_site_of = (int32_t*)(w + m.site_of);
+    ctx->d_nbr = (int32_t*)(w + m.nbr);
+    for (int r = 0; r < 2; ++r) { ctx->d_U64[r] = (double*)(w + m.u64[r]); ctx->d_U32[r] = (float*)(w + m.u32[r]); }
+    ctx->d_scal = (double*)(w + m.scal);
+    ctx->d_partials = (double*)(w + m.partials);
+    ctx->d_ticket = (unsigned int*)(w + m.ticket);
+    ctx->d_solver = w + m.solver;
+    ctx->solver_bytes = m.total - m.solver;
+    WD_CUDA_CHECK(ctx, cudaMemcpyAsync(ctx->d_site_of, ctx->h_site_of.data(), sizeof(int32_t) * 2 * ctx->Vh,
+                                       cudaMemcpyHostToDevice, ctx->stream));
+    WD_CUDA_CHECK(ctx, cudaMemcpyAsync(ctx->d_nbr, ctx->h_nbr.data(), sizeof(int32_t) * 2 * ctx->Vh * WD_NDIR,
+                                       cudaMemcpyHostToDevice, ctx->stream));
+    WD_CUDA_CHECK(ctx, cudaMemsetAsync(ctx->d_ticket, 0, 256, ctx->stream));
+    WD_CUDA_CHECK(ctx, cudaMemsetAsync(ctx->d_scal, 0, sizeof(double) * kScalDoubles, ctx->stream));
+    WD_CUDA_CHECK(ctx, cudaStreamSynchronize(ctx->stream));  // host tables may now change
+    ctx->have_ws = true;
+    ctx->have_gauge = false;
+    return WD_OK;
+}
+
+int wd_set_gauge(wd_ctx* ctx, const double* U) {
+    if (!ctx) return WD_EINVAL;
+    if (!U) return wd_fail(ctx, WD_EINVAL, "gauge pointer is null");
+    if (!ctx->have_ws) return wd_fail(ctx, WD_ESTATE, "wd_set_workspace first");
+    int rc = wd_layout_gauge(ctx, U);
+    if (rc == WD_OK) ctx->have_gauge = true;
+    return rc;
+}
+
+size_t wd_native_bytes(const wd_ctx* ctx, int prec, int n_rhs) {
+    if (!ctx || n_rhs < 0 || (prec != WD_F64 && prec != WD_F32)) return 0;
+    return 2 * wd_half_bytes(ctx, prec, n_rhs);
+}
+
+int wd_pack(wd_ctx* ctx, int prec, int n_rhs, const double* canon, void* native) {
+    if (!ctx) return WD_EINVAL;
+    if (!canon || !native || bad_n(ctx, n_rhs) || (prec != WD_F64 && prec != WD_F32))
+        return wd_fail(ctx, WD_EINVAL, "wd_pack: bad argument");
+    if (!ctx->have_ws) return wd_fail(ctx, WD_ESTATE, "wd_set_workspace first");
+    return wd_layout_pack(ctx, prec, n_rhs, canon, native);
+}
+
+int wd_unpack(wd_ctx* ctx, int prec, int n_rhs, const void* native, double* canon) {
+    if (!ctx) return WD_EINVAL;
+    if (!canon || !native || bad_n(ctx, n_rhs) || (prec != WD_F64 && prec != WD_F32))
+        return wd_fail(ctx, WD_EINVAL, "wd_unpack: bad argument");
+    if (!ctx->have_ws) return wd_fail(ctx, WD_ESTATE, "wd_set_workspace first");
+    return wd_layout_unpack(ctx, prec, n_rhs, native, canon);
+}
+
+static int check_op_args(wd_ctx* ctx, int op, int prec, int recon, int n_rhs, const void* a, const void* b) {
+    if (!ctx) return WD_EINVAL;
+    if (!a || !b || a == b) return wd_fail(ctx, WD_EINVAL, "null or aliased field pointer");
+    if (bad_n(ctx, n_rhs)) return wd_fail(ctx, WD_EINVAL, "n_rhs out of range");
+    if (op != WD_OP_D && op != WD_OP_DDAG) return wd_fail(ctx, WD_EINVAL, "bad op");
+    if (prec != WD_F64 && prec != WD_F32) return wd_fail(ctx, WD_EINVAL, "bad precision");
+    if (recon != WD_LINK18 && recon != WD_LINK12) return wd_fail(ctx, WD_EINVAL, "bad link form");
+    if (!ctx->have_gauge) return wd_fail(ctx, WD_ESTATE, "wd_set_gauge first");
+    return WD_OK;
+}
+
+int wd_apply(wd_ctx* ctx, int op, int prec, int recon, int n_rhs, const void* in, void* out) {
+    int rc = check_op_args(ctx, op, prec, recon, n_rhs, in, out);
+    if (rc) return rc;
+    const size_t hb = wd_half_bytes(ctx, prec, n_rhs);
+    const char* i = (const char*)in;
+    char* o = (char*)out;
+    // out_p = in_p - kappa H_{p,1-p} in_{1-p}   (D = 1 - kappa H)
+    for (int p = 0; p < 2; ++p) {
+        rc = wd_hop_launch(ctx, prec, recon, op == WD_OP_DDAG, n_rhs, p, i + (1 - p) * hb, o + p * hb, i + p * hb,
+                           1.0, -ctx->kappa);
+        if (rc) return rc;
+    }
+    return WD_OK;
+}
+
+int wd_hop(wd_ctx* ctx, int op, int prec, int recon, int n_rhs, int out_parity, const void* in, void* out) {
+    int rc = check_op_args(ctx, op, prec, recon, n_rhs, in, out);
+    if (rc) return rc;
+    if (out_parity != 0 && out_parity != 1) return wd_fail(ctx, WD_EINVAL, "bad parity");
+    return wd_hop_launch(ctx, prec, recon, op == WD_OP_DDAG, n_rhs, out_parity, in, out, nullptr, 0.0, 1.0);
+}
+
+int wd_solve_block(wd_ctx* ctx, int op, int n_rhs, const double* Phi, double* X, double tol, int max_outer,
+                   int max_inner, double inner_tol, int recon, wd_solve_info* info) {
+    int rc = check_op_args(ctx, op, WD_F64, recon, n_rhs, Phi, X);
+    if (rc) return rc;
+    if (!(tol > 0.0) || max_outer < 1 || max_inner < 1 || inner_tol < 0.0 || inner_tol >= 1.0)
+        return wd_fail(ctx, WD_EINVAL, "bad solver parameters");
+    return wd_solve_impl(ctx, op == WD_OP_DDAG, n_rhs, Phi, X, tol, max_outer, max_inner,
+                         inner_tol > 0.0 ? inner_tol : 1e-5, recon, info);
+}
+
+int wd_force(wd_ctx* ctx, int n_rhs, const double* X, const double* Y, double* F) {
+    if (!ctx) return WD_EINVAL;
+    if (!X || !Y || !F) return wd_fail(ctx, WD_EINVAL, "null pointer");
+    if (bad_n(ctx, n_rhs)) return wd_fail(ctx, WD_EINVAL, "n_rhs out of range");
+    if (!ctx->have_gauge) return wd_fail(ctx, WD_ESTATE, "wd_set_gauge first");
+    return wd_force_impl(ctx, n_rhs, X, Y, F);
+}
+
+int wd_md_force_host(wd_ctx* ctx, int n_rhs, const double* Phi_host, double* F_host, double tol, int max_outer,
+                     int max_inner, double inner_tol, int recon, wd_solve_info* info2) {
+    if (!ctx) return WD_EINVAL;
+    if (!Phi_host || !F_host) return wd_fail(ctx, WD_EINVAL, "null pointer");
+    if (bad_n(ctx, n_rhs)) return wd_fail(ctx, WD_EINVAL, "n_rhs out of range");
+    if (!ctx->have_gauge) return wd_fail(ctx, WD_ESTATE, "wd_set_gauge first");
+    // staging lives at the END of the solver scratch (sized for max_rhs in wd_solver_scratch_bytes)
+    const size_t full = wd_align_up(2 * wd_half_bytes(ctx, WD_F64, ctx->max_rhs));
+    const size_t fbytes = wd_align_up(sizeof(double) * 4 * ctx->V * 18);
+    char* end = ctx->d_solver + ctx->solver_bytes;
+    double* dF = (double*)(end - fbytes);
+    double* dY = (double*)(end - fbytes - full);
+    double* dX = (double*)(end - fbytes - 2 * full);
+    double* dPhi = (double*)(end - fbytes - 3 * full);
+    double* dCanon = (double*)(end - fbytes - 4 * full);
+    const size_t cbytes = sizeof(double) * 24 * ctx->V * n_rhs;
+    WD_CUDA_CHECK(ctx, cudaMemcpyAsync(dCanon, Phi_host, cbytes, cudaMemcpyHostToDevice, ctx->stream));
+    int rc = wd_layout_pack(ctx, WD_F64, n_rhs, dCanon, dPhi);
+    if (rc) return rc;
+    WD_CUDA_CHECK(ctx, cudaMemsetAsync(dF, 0, sizeof(double) * 4 * ctx->V * 18, ctx->stream));
+    const double itol = inner_tol > 0.0 ? inner_tol : 1e-5;
+    int rc1 = wd_solve_impl(ctx, 0, n_rhs, dPhi, dX, tol, max_outer, max_inner, itol, recon, info2 ? &info2[0] : nullptr);
+    if (rc1 != WD_OK && rc1 != WD_ENOCONV) return rc1;
+    int rc2 = wd_solve_impl(ctx, 1, n_rhs, dX, dY, tol, max_outer, max_inner, itol, recon, info2 ? &info2[1] : nullptr);
+    if (rc2 != WD_OK && rc2 != WD_ENOCONV) return rc2;
+    rc = wd_force_impl(ctx, n_rhs, dX, dY, dF);
+    if (rc) return rc;
+    WD_CUDA_CHECK(ctx, cudaMemcpyAsync(F_host, dF, sizeof(double) * 4 * ctx->V * 18, cudaMemcpyDeviceToHost, ctx->stream));
+    WD_CUDA_CHECK(ctx, cudaStreamSynchronize(ctx->stream));
+    return (rc1 == WD_OK && rc2 == WD_OK) ? WD_OK : WD_ENOCONV;
+}
+
+}  // extern "C"

@@ -1,0 +1,105 @@
+// wd_internal.h -- context, workspace map and launch helpers shared by the library's .cu files.
+// Not part of the public ABI (include/wd.h is).  Nothing here is shared with oracle/.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stdio.h>
+#include <string>
+#include <vector>
+
+#include "../../include/wd.h"
+
+#define WD_NDIR 8  // x+, x-, y+, y-, z+, z-, t+, t-
+
+// Bit 31 of nbr[.][0] marks a site that is not dynamical (SF: the stored t=0 slice).
+#define WD_SITE_FROZEN 0x80000000u
+
+struct wd_ctx {
+    int L[4];
+    long V, Vh;
+    double kappa;
+    int bc;
+    int max_rhs;
+    cudaStream_t stream;
+    int n_sm;
+
+    int order;
+    int tile[4];
+
+    // host copies of the site tables (uploaded by wd_set_workspace)
+    std::vector<int32_t> h_site_of;  // [2][Vh]   canonical site index of (parity, h)
+    std::vector<int32_t> h_nbr;      // [2][Vh][8] index (in parity 1-p) of the 8 neighbours of (p, h)
+
+    // workspace
+    char* ws;
+    size_t ws_bytes;
+    bool have_ws, have_gauge;
+
+    // device pointers carved from the workspace
+    int32_t* d_site_of;
+    int32_t* d_nbr;
+    double* d_U64[2];  // [recon] native fp64 links  [mu][parity][R][Vh]
+    float* d_U32[2];   // [recon] native fp32 links
+    // solver scratch
+    double* d_scal;        // per-RHS scalars (see wd_solve.cu)
+    double* d_partials;    // block partial sums
+    unsigned int* d_ticket;
+    double* h_pinned;      // pinned host mirror for convergence polling (cudaMallocHost, small)
+    char* d_solver;        // remaining scratch for solver vectors and host-path staging
+    size_t solver_bytes;
+
+    long long launches;
+    std::string err;
+};
+
+static inline size_t wd_align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
+
+// size in bytes of a native HALF-lattice block
+static inline size_t wd_half_bytes(const wd_ctx* c, int prec, int n) {
+    return (size_t)c->Vh * 24 * (prec == WD_F64 ? 8 : 4) * (size_t)n;
+}
+
+static inline int wd_fail(wd_ctx* c, int code, const char* msg) {
+    if (c) c->err = msg;
+    return code;
+}
+
+#define WD_CUDA_CHECK(ctx, expr)                                                     \
+    do {                                                                             \
+        cudaError_t e__ = (expr);                                                    \
+        if (e__ != cudaSuccess) {                                                    \
+            (ctx)->err = std::string(#expr) + ": " + cudaGetErrorString(e__);        \
+            return WD_ECUDA;                                                         \
+        }                                                                            \
+    } while (0)
+
+#define WD_LAUNCH_CHECK(ctx)                                                         \
+    do {                                                                             \
+        (ctx)->launches++;                                                           \
+        cudaError_t e__ = cudaGetLastError();                                        \
+        if (e__ != cudaSuccess) {                                                    \
+            (ctx)->err = std::string("kernel launch: ") + cudaGetErrorString(e__);   \
+            return WD_ECUDA;                                                         \
+        }                                                                            \
+    } while (0)
+
+// ---- internal entry points (device pointers, no argument checks) -------------------------------
+// wd_hop.cu
+// out[h][r] = (xpay ? a * in2 + b * (H in) : H in) on output parity `par`; in/out/in2 half-lattice blocks.
+// If dots != nullptr (fp32/fp64), see wd_hop.cu for the fused reductions.
+int wd_hop_launch(wd_ctx* c, int prec, int recon, int dag, int n, int par, const void* in, void* out,
+                  const void* in2, double a, double b);
+
+// wd_layout.cu
+int wd_layout_gauge(wd_ctx* c, const double* U);
+int wd_layout_pack(wd_ctx* c, int prec, int n, const double* canon, void* native);
+int wd_layout_unpack(wd_ctx* c, int prec, int n, const void* native, double* canon);
+
+// wd_solve.cu
+size_t wd_solver_scratch_bytes(const wd_ctx* c);
+int wd_solve_impl(wd_ctx* c, int dag, int n, const double* Phi, double* X, double tol, int max_outer,
+                  int max_inner, double inner_tol, int recon, wd_solve_info* info);
+
+// wd_force.cu
+int wd_force_impl(wd_ctx* c, int n, const double* X, const double* Y, double* F);

@@ -1,0 +1,361 @@
+// wd_solve.cu -- blocked mixed-precision solve (hot-path steps a1, a3-a7).
+//
+//   A X = Phi,  A = D or D^dag, all n_rhs columns in lock-step.
+//   even/odd:  Ahat = 1 - kappa^2 H_eo H_oe on even sites,
+//        Phihat_e = Phi_e + kappa H_eo Phi_o,   Ahat X_e = Phihat_e,   X_o = Phi_o + kappa H_oe X_e.
+//   outer loop, fp64 (defect correction, the "mixed-precision preconditioner technique" of
+//   PAPER.md:80-82 in its simplest form; reading c.6-2):
+//        R = Phihat_e - Ahat X_e;  stop when |R_i| <= tol |phi_i| for every i;
+//        E = BiCGStab_fp32(R_i / |R_i|);  X_e,i += |R_i| E_i.
+//   inner loop, fp32: textbook BiCGStab per column, per-column alpha, beta, omega kept
+//   on the device; a converged column is frozen (alpha = omega = beta = 0).
+#include <chrono>
+
+#include "wd_blas.cuh"
+
+using namespace wdblas;
+
+namespace {
+
+template <typename T>
+__device__ __forceinline__ void to_arr(const typename V<T>::type& v, T (&a)[2 * V<T>::NC]);
+template <> __device__ __forceinline__ void to_arr<float>(const float4& v, float (&a)[4]) { a[0] = v.x; a[1] = v.y; a[2] = v.z; a[3] = v.w; }
+template <> __device__ __forceinline__ void to_arr<double>(const double2& v, double (&a)[2]) { a[0] = v.x; a[1] = v.y; }
+__device__ __forceinline__ float4 from_arr(const float (&a)[4]) { return make_float4(a[0], a[1], a[2], a[3]); }
+__device__ __forceinline__ double2 from_arr(const double (&a)[2]) { return make_double2(a[0], a[1]); }
+
+#define WD_BLAS_PROLOGUE(T)                                                        \
+    typedef typename V<T>::type vec;                                               \
+    constexpr int NC = V<T>::NC;                                                   \
+    const int r = threadIdx.x % n;                                                 \
+    const long stride = (long)gridDim.x * blockDim.x;                              \
+    const long i0 = (long)blockIdx.x * blockDim.x + threadIdx.x;
+
+// P = R + beta (P - omega V)
+template <typename T>
+__global__ void p_update_kernel(long nvec, int n, const double* __restrict__ scal, const typename V<T>::type* __restrict__ R,
+                                typename V<T>::type* __restrict__ P, const typename V<T>::type* __restrict__ Vv) {
+    if (scal[G_DONE] != 0.0) return;
+    WD_BLAS_PROLOGUE(T)
+    const T br = (T)scal[S_BETA_RE * WD_MAX_RHS + r], bi = (T)scal[S_BETA_IM * WD_MAX_RHS + r];
+    const T wr = (T)scal[S_OMEGA_RE * WD_MAX_RHS + r], wi = (T)scal[S_OMEGA_IM * WD_MAX_RHS + r];
+    for (long i = i0; i < nvec; i += stride) {
+        T a[2 * NC], p[2 * NC], v[2 * NC];
+        to_arr<T>(R[i], a); to_arr<T>(P[i], p); to_arr<T>(Vv[i], v);
+#pragma unroll
+        for (int c = 0; c < NC; ++c) {
+            const T tr = p[2 * c] - (wr * v[2 * c] - wi * v[2 * c + 1]);
+            const T ti = p[2 * c + 1] - (wr * v[2 * c + 1] + wi * v[2 * c]);
+            p[2 * c] = a[2 * c] + (br * tr - bi * ti);
+            p[2 * c + 1] = a[2 * c + 1] + (br * ti + bi * tr);
+        }
+        P[i] = from_arr(p);
+    }
+}
+
+// sigma = <Rt, V>  ->  alpha = rho / sigma
+template <typename T>
+__global__ void dot_sigma_kernel(long nvec, int n, RedBuf rb, const typename V<T>::type* __restrict__ Rt,
+                                 const typename V<T>::type* __restrict__ Vv) {
+    if (rb.scal[G_DONE] != 0.0) return;
+    WD_BLAS_PROLOGUE(T)
+    (void)r;
+    double s[2] = {0.0, 0.0};
+    for (long i = i0; i < nvec; i += stride) {
+        T a[2 * NC], v[2 * NC];
+        to_arr<T>(Rt[i], a); to_arr<T>(Vv[i], v);
+#pragma unroll
+        for (int c = 0; c < NC; ++c) {  // conj(a) * v
+            s[0] += (double)a[2 * c] * v[2 * c] + (double)a[2 * c + 1] * v[2 * c + 1];
+            s[1] += (double)a[2 * c] * v[2 * c + 1] - (double)a[2 * c + 1] * v[2 * c];
+        }
+    }
+    reduce_finalize<2, K_SIGMA>(s, n, rb);
+}
+
+// S = R - alpha V   (in place on R)
+template <typename T>
+__global__ void s_update_kernel(long nvec, int n, const double* __restrict__ scal, typename V<T>::type* __restrict__ R,
+                                const typename V<T>::type* __restrict__ Vv) {
+    if (scal[G_DONE] != 0.0) return;
+    WD_BLAS_PROLOGUE(T)
+    const T ar = (T)scal[S_ALPHA_RE * WD_MAX_RHS + r], ai = (T)scal[S_ALPHA_IM * WD_MAX_RHS + r];
+    for (long i = i0; i < nvec; i += stride) {
+        T a[2 * NC], v[2 * NC];
+        to_arr<T>(R[i], a); to_arr<T>(Vv[i], v);
+#pragma unroll
+        for (int c = 0; c < NC; ++c) {
+            a[2 * c] -= ar * v[2 * c] - ai * v[2 * c + 1];
+            a[2 * c + 1] -= ar * v[2 * c + 1] + ai * v[2 * c];
+        }
+        R[i] = from_arr(a);
+    }
+}
+
+// <T, S>, <T, T>  ->  omega
+template <typename T>
+__global__ void dot_omega_kernel(long nvec, int n, RedBuf rb, const typename V<T>::type* __restrict__ Tt,
+                                 const typename V<T>::type* __restrict__ S) {
+    if (rb.scal[G_DONE] != 0.0) return;
+    WD_BLAS_PROLOGUE(T)
+    (void)r;
+    double s[3] = {0.0, 0.0, 0.0};
+    for (long i = i0; i < nvec; i += stride) {
+        T a[2 * NC], v[2 * NC];
+        to_arr<T>(Tt[i], a); to_arr<T>(S[i], v);
+#pragma unroll
+        for (int c = 0; c < NC; ++c) {
+            s[0] += (double)a[2 * c] * v[2 * c] + (double)a[2 * c + 1] * v[2 * c + 1];
+            s[1] += (double)a[2 * c] * v[2 * c + 1] - (double)a[2 * c + 1] * v[2 * c];
+            s[2] += (double)a[2 * c] * a[2 * c] + (double)a[2 * c + 1] * a[2 * c + 1];
+        }
+    }
+    reduce_finalize<3, K_OMEGA>(s, n, rb);
+}
+
+// X += alpha P + omega S;  R = S - omega T;  <Rt, R>, |R|^2  ->  rho, beta, convergence flags
+template <typename T>
+__global__ void xr_update_kernel(long nvec, int n, RedBuf rb, typename V<T>::type* __restrict__ X,
+                                 const typename V<T>::type* __restrict__ P, typename V<T>::type* __restrict__ R,
+                                 const typename V<T>::type* __restrict__ Tt, const typename V<T>::type* __restrict__ Rt) {
+    if (rb.scal[G_DONE] != 0.0) return;
+    WD_BLAS_PROLOGUE(T)
+    const double* scal = rb.scal;
+    const T ar = (T)scal[S_ALPHA_RE * WD_MAX_RHS + r], ai = (T)scal[S_ALPHA_IM * WD_MAX_RHS + r];
+    const T wr = (T)scal[S_OMEGA_RE * WD_MAX_RHS + r], wi = (T)scal[S_OMEGA_IM * WD_MAX_RHS + r];
+    double s[3] = {0.0, 0.0, 0.0};
+    for (long i = i0; i < nvec; i += stride) {
+        T x[2 * NC], p[2 * NC], sv[2 * NC], t[2 * NC], q[2 * NC];
+        to_arr<T>(X[i], x); to_arr<T>(P[i], p); to_arr<T>(R[i], sv); to_arr<T>(Tt[i], t); to_arr<T>(Rt[i], q);
+#pragma unroll
+        for (int c = 0; c < NC; ++c) {
+            x[2 * c] += (ar * p[2 * c] - ai * p[2 * c + 1]) + (wr * sv[2 * c] - wi * sv[2 * c + 1]);
+            x[2 * c + 1] += (ar * p[2 * c + 1] + ai * p[2 * c]) + (wr * sv[2 * c + 1] + wi * sv[2 * c]);
+            const T rr = sv[2 * c] - (wr * t[2 * c] - wi * t[2 * c + 1]);
+            const T ri = sv[2 * c + 1] - (wr * t[2 * c + 1] + wi * t[2 * c]);
+            sv[2 * c] = rr; sv[2 * c + 1] = ri;
+            s[0] += (double)q[2 * c] * rr + (double)q[2 * c + 1] * ri;
+            s[1] += (double)q[2 * c] * ri - (double)q[2 * c + 1] * rr;
+            s[2] += (double)rr * rr + (double)ri * ri;
+        }
+        X[i] = from_arr(x);
+        R[i] = from_arr(sv);
+    }
+    reduce_finalize<3, K_RHO>(s, n, rb);
+}
+
+// |phi_i|^2 over a full-lattice fp64 block
+__global__ void norm2_kernel(long nvec, int n, RedBuf rb, const double2* __restrict__ A) {
+    const long stride = (long)gridDim.x * blockDim.x;
+    double s[1] = {0.0};
+    for (long i = (long)blockIdx.x * blockDim.x + threadIdx.x; i < nvec; i += stride) {
+        const double2 a = A[i];
+        s[0] += a.x * a.x + a.y * a.y;
+    }
+    reduce_finalize<1, K_PHI2>(s, n, rb);
+}
+
+// R = B - W (W may be null: R = B), |R_i|^2 -> outer convergence flags, scale, inner threshold
+__global__ void outer_resid_kernel(long nvec, int n, RedBuf rb, const double2* __restrict__ Bv, const double2* W,
+                                   double2* R) {
+    const long stride = (long)gridDim.x * blockDim.x;
+    double s[1] = {0.0};
+    for (long i = (long)blockIdx.x * blockDim.x + threadIdx.x; i < nvec; i += stride) {
+        double2 b = Bv[i];
+        if (W) { const double2 w = W[i]; b.x -= w.x; b.y -= w.y; }
+        R[i] = b;
+        s[0] += b.x * b.x + b.y * b.y;
+    }
+    reduce_finalize<1, K_OUT_R2>(s, n, rb);
+}
+
+// inner start: b = R_i / |R_i| in fp32 -> r, rt;  x = p = v = 0;  rho = <b, b>.
+// fp64 vec index (k, h, r) k < 12  <->  fp32 vec index (k/2, h, r), components 2*(k%2)..
+__global__ void demote_kernel(long Vh, int n, RedBuf rb, const double2* __restrict__ R64, float4* __restrict__ r32,
+                              float4* __restrict__ rt32, float4* __restrict__ x32, float4* __restrict__ p32,
+                              float4* __restrict__ v32) {
+    const int r = threadIdx.x % n;
+    const long stride = (long)gridDim.x * blockDim.x;
+    const long nvec = 6 * Vh * n, half = Vh * n;
+    const double* scal = rb.scal;
+    const bool frozen = scal[S_FLAG * WD_MAX_RHS + r] != 0.0;
+    const double sc = scal[S_SCALE * WD_MAX_RHS + r];
+    const double inv = (frozen || !(sc > 0.0)) ? 0.0 : 1.0 / sc;
+    double s[3] = {0.0, 0.0, 0.0};
+    for (long i = (long)blockIdx.x * blockDim.x + threadIdx.x; i < nvec; i += stride) {
+        const long c = i / half, rem = i - c * half;
+        const double2 a = R64[(2 * c) * half + rem], b = R64[(2 * c + 1) * half + rem];
+        const float4 f = make_float4((float)(a.x * inv), (float)(a.y * inv), (float)(b.x * inv), (float)(b.y * inv));
+        r32[i] = f;
+        rt32[i] = f;
+        const float4 z = make_float4(0.f, 0.f, 0.f, 0.f);
+        x32[i] = z; p32[i] = z; v32[i] = z;
+        s[0] += (double)f.x * f.x + (double)f.y * f.y + (double)f.z * f.z + (double)f.w * f.w;
+    }
+    s[2] = s[0];
+    reduce_finalize<3, K_INIT_RHO>(s, n, rb);
+}
+
+// X_i += |R_i| E_i  (fp32 -> fp64)
+__global__ void promote_kernel(long Vh, int n, const double* __restrict__ scal, const float4* __restrict__ e32,
+                               double2* __restrict__ X64) {
+    const int r = threadIdx.x % n;
+    const long stride = (long)gridDim.x * blockDim.x;
+    const long nvec = 6 * Vh * n, half = Vh * n;
+    const double sc = scal[S_OUT_CONV * WD_MAX_RHS + r] != 0.0 ? 0.0 : scal[S_SCALE * WD_MAX_RHS + r];
+    for (long i = (long)blockIdx.x * blockDim.x + threadIdx.x; i < nvec; i += stride) {
+        const long c = i / half, rem = i - c * half;
+        const float4 f = e32[i];
+        double2 a = X64[(2 * c) * half + rem], b = X64[(2 * c + 1) * half + rem];
+        a.x += sc * f.x; a.y += sc * f.y; b.x += sc * f.z; b.y += sc * f.w;
+        X64[(2 * c) * half + rem] = a;
+        X64[(2 * c + 1) * half + rem] = b;
+    }
+}
+
+__global__ void set_globals_kernel(double* scal, double tol2, double intol2) {
+    scal[G_TOL2] = tol2;
+    scal[G_INTOL2] = intol2;
+    scal[G_DONE] = 0.0;
+    scal[G_ITERS] = 0.0;
+    scal[G_OUT_DONE] = 0.0;
+}
+
+struct Launch {
+    int B;
+    unsigned G;
+};
+Launch blas_cfg(const wd_ctx* c, long nvec, int n) {
+    Launch l;
+    const int m = (8 + n - 1) / n;
+    l.B = 32 * n * m;
+    long g = (nvec + l.B - 1) / l.B;
+    const long cap = (long)c->n_sm * 4;
+    l.G = (unsigned)(g < cap ? (g < 1 ? 1 : g) : cap);
+    return l;
+}
+
+}  // namespace
+
+size_t wd_solver_scratch_bytes(const wd_ctx* c) {
+    const int n = c->max_rhs;
+    size_t b = 0;
+    b += 3 * wd_align_up(wd_half_bytes(c, WD_F64, n));      // phihat, tmp_o, R/W
+    b += 7 * wd_align_up(wd_half_bytes(c, WD_F32, n));      // x, r, p, v, t, rt, tmp_o
+    b += 4 * wd_align_up(2 * wd_half_bytes(c, WD_F64, n));  // host path: canonical Phi, native Phi, X, Y
+    b += wd_align_up(sizeof(double) * 4 * c->V * 18);       // host path: F
+    return b;
+}
+
+int wd_solve_impl(wd_ctx* c, int dag, int n, const double* Phi, double* X, double tol, int max_outer,
+                  int max_inner, double inner_tol, int recon, wd_solve_info* info) {
+    const auto t_begin = std::chrono::steady_clock::now();
+    cudaStream_t st = c->stream;
+    const long Vh = c->Vh;
+    const size_t hb64 = wd_half_bytes(c, WD_F64, n), hb32 = wd_half_bytes(c, WD_F32, n);
+    const size_t sb64 = wd_align_up(wd_half_bytes(c, WD_F64, c->max_rhs)), sb32 = wd_align_up(wd_half_bytes(c, WD_F32, c->max_rhs));
+    char* w = c->d_solver;
+    double2* phihat = (double2*)w; w += sb64;
+    double2* tmp64 = (double2*)w;  w += sb64;
+    double2* R64 = (double2*)w;    w += sb64;
+    float4* x32 = (float4*)w;   w += sb32;
+    float4* r32 = (float4*)w;   w += sb32;
+    float4* p32 = (float4*)w;   w += sb32;
+    float4* v32 = (float4*)w;   w += sb32;
+    float4* t32 = (float4*)w;   w += sb32;
+    float4* rt32 = (float4*)w;  w += sb32;
+    float4* tmp32 = (float4*)w; w += sb32;
+
+    const char* PhiE = (const char*)Phi;
+    const char* PhiO = PhiE + hb64;
+    char* XE = (char*)X;
+    char* XO = XE + hb64;
+    const double kap = c->kappa;
+    RedBuf rb{c->d_scal, c->d_partials, c->d_ticket};
+    int rc;
+
+    set_globals_kernel<<<1, 1, 0, st>>>(c->d_scal, tol * tol, inner_tol * inner_tol);
+    WD_LAUNCH_CHECK(c);
+
+    const long nv64 = 12 * Vh * n, nv32 = 6 * Vh * n;
+    const Launch L64 = blas_cfg(c, nv64, n), L64f = blas_cfg(c, 2 * nv64, n), L32 = blas_cfg(c, nv32, n);
+
+    // |phi_i|^2 (full lattice) and the even/odd right-hand side
+    norm2_kernel<<<L64f.G, L64f.B, 0, st>>>(2 * nv64, n, rb, (const double2*)Phi);
+    WD_LAUNCH_CHECK(c);
+    rc = wd_hop_launch(c, WD_F64, WD_LINK18, dag, n, 0, PhiO, phihat, PhiE, 1.0, kap);
+    if (rc) return rc;
+    WD_CUDA_CHECK(c, cudaMemsetAsync(XE, 0, hb64, st));
+
+    int outer = 0, converged = 0;
+    double* hp = c->h_pinned;
+    for (;;) {
+        // true residual of the even/odd system in fp64
+        if (outer == 0) {
+            outer_resid_kernel<<<L64.G, L64.B, 0, st>>>(nv64, n, rb, phihat, nullptr, R64);
+        } else {
+            rc = wd_hop_launch(c, WD_F64, WD_LINK18, dag, n, 1, XE, tmp64, nullptr, 0.0, 1.0);
+            if (rc) return rc;
+            rc = wd_hop_launch(c, WD_F64, WD_LINK18, dag, n, 0, tmp64, R64, XE, 1.0, -kap * kap);
+            if (rc) return rc;
+            outer_resid_kernel<<<L64.G, L64.B, 0, st>>>(nv64, n, rb, phihat, R64, R64);
+        }
+        WD_LAUNCH_CHECK(c);
+        WD_CUDA_CHECK(c, cudaMemcpyAsync(hp, c->d_scal, sizeof(double) * G_COUNT, cudaMemcpyDeviceToHost, st));
+        WD_CUDA_CHECK(c, cudaStreamSynchronize(st));
+        if (hp[G_OUT_DONE] != 0.0) { converged = 1; break; }
+        if (outer >= max_outer) break;
+        ++outer;
+
+        // inner fp32 BiCGStab on the normalised residual
+        demote_kernel<<<L32.G, L32.B, 0, st>>>(Vh, n, rb, R64, r32, rt32, x32, p32, v32);
+        WD_LAUNCH_CHECK(c);
+        const double* done = c->d_scal + G_DONE;
+        (void)done;
+        for (int it = 1; it <= max_inner; ++it) {
+            p_update_kernel<float><<<L32.G, L32.B, 0, st>>>(nv32, n, c->d_scal, r32, p32, v32);
+            WD_LAUNCH_CHECK(c);
+            rc = wd_hop_launch(c, WD_F32, recon, dag, n, 1, p32, tmp32, nullptr, 0.0, 1.0);
+            if (rc) return rc;
+            rc = wd_hop_launch(c, WD_F32, recon, dag, n, 0, tmp32, v32, p32, 1.0, -kap * kap);
+            if (rc) return rc;
+            dot_sigma_kernel<float><<<L32.G, L32.B, 0, st>>>(nv32, n, rb, rt32, v32);
+            WD_LAUNCH_CHECK(c);
+            s_update_kernel<float><<<L32.G, L32.B, 0, st>>>(nv32, n, c->d_scal, r32, v32);
+            WD_LAUNCH_CHECK(c);
+            rc = wd_hop_launch(c, WD_F32, recon, dag, n, 1, r32, tmp32, nullptr, 0.0, 1.0);
+            if (rc) return rc;
+            rc = wd_hop_launch(c, WD_F32, recon, dag, n, 0, tmp32, t32, r32, 1.0, -kap * kap);
+            if (rc) return rc;
+            dot_omega_kernel<float><<<L32.G, L32.B, 0, st>>>(nv32, n, rb, t32, r32);
+            WD_LAUNCH_CHECK(c);
+            xr_update_kernel<float><<<L32.G, L32.B, 0, st>>>(nv32, n, rb, x32, p32, r32, t32, rt32);
+            WD_LAUNCH_CHECK(c);
+            // convergence poll (every iteration for now)
+            WD_CUDA_CHECK(c, cudaMemcpyAsync(hp + G_COUNT, c->d_scal + G_DONE, sizeof(double), cudaMemcpyDeviceToHost, st));
+            WD_CUDA_CHECK(c, cudaStreamSynchronize(st));
+            if (hp[G_COUNT] != 0.0) break;
+        }
+        promote_kernel<<<L32.G, L32.B, 0, st>>>(Vh, n, c->d_scal, x32, (double2*)XE);
+        WD_LAUNCH_CHECK(c);
+    }
+
+    // X_o = Phi_o + kappa H_oe X_e
+    rc = wd_hop_launch(c, WD_F64, WD_LINK18, dag, n, 1, XE, XO, PhiO, 1.0, kap);
+    if (rc) return rc;
+
+    if (info) {
+        info->n_rhs = n;
+        info->outer_steps = outer;
+        info->inner_iters_total = (int)hp[G_ITERS];
+        info->converged = converged;
+        for (int r = 0; r < n; ++r) {
+            const double phi2 = hp[S_PHI2 * WD_MAX_RHS + r], r2 = hp[S_OUT_R2 * WD_MAX_RHS + r];
+            info->bnorm[r] = sqrt(phi2);
+            info->relres[r] = phi2 > 0.0 ? sqrt(r2 / phi2) : 0.0;
+        }
+        for (int r = n; r < WD_MAX_RHS; ++r) info->bnorm[r] = info->relres[r] = 0.0;
+        info->seconds = std::chrono::duration<double>(std::chrono::steady_clock::now() - t_begin).count();
+    }
+    return converged ? WD_OK : WD_ENOCONV;
+}

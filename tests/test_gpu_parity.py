@@ -1,0 +1,231 @@
+"""Parity of the CUDA path (libwd.so through its C ABI) with the fp64 CPU oracle, element by
+element on the same seeded inputs.  Tolerances are BASELINE.json north_star's:
+D-apply 1e-13 (fp64) / 1e-5 (fp32) relative L2 per RHS; solutions 1e-9 at solver tolerance 1e-12;
+forces 1e-9 relative.  All tests here need a GPU.
+"""
+import numpy as np
+import pytest
+import torch
+
+import wd_inputs as wi
+from oracle import wd_oracle as orc
+
+pytestmark = pytest.mark.gpu
+
+
+def _wd():
+    import paper_1009_5169_b200 as pkg
+    return pkg
+
+
+def rel_per_rhs(a, b):
+    n = a.shape[0]
+    a = a.reshape(n, -1)
+    b = b.reshape(n, -1)
+    return np.linalg.norm(a - b, axis=1) / np.maximum(np.linalg.norm(b, axis=1), 1e-300)
+
+
+def dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def make_ctx(dims, kappa, bc, max_rhs, U, **kw):
+    pkg = _wd()
+    ctx = pkg.Context(dims, kappa, bc=bc, max_rhs=max_rhs, **kw)
+    ctx.set_gauge(dev(U))
+    return ctx
+
+
+APPLY_CASES = [
+    # dims, bc, n_rhs, eps
+    ((4, 4, 4, 4), wi.BC_SF, 5, 0.2),
+    ((4, 4, 4, 4), wi.BC_PERIODIC, 3, 0.4),
+    ((8, 4, 6, 10), wi.BC_SF, 5, 0.3),       # unequal dims, ragged tail of the last block
+    ((6, 6, 6, 8), wi.BC_PERIODIC, 1, 0.4),
+    ((2, 2, 2, 4), wi.BC_SF, 12, 0.4),       # smallest lattice, neighbours coincide
+    ((8, 8, 8, 8), wi.BC_SF, 16, 0.3),       # maximum n_rhs
+]
+
+
+@pytest.mark.parametrize("dims,bc,n_rhs,eps", APPLY_CASES)
+@pytest.mark.parametrize("op", [0, 1])
+def test_apply_fp64_matches_oracle(dims, bc, n_rhs, eps, op):
+    pkg = _wd()
+    kappa = 0.13
+    U = wi.gauge_field(dims, eps, 7, bc)
+    psi = wi.spinor_field(dims, n_rhs, 11, bc)
+    ref = orc.apply(dims, kappa, bc, op, U, psi)
+    ctx = make_ctx(dims, kappa, bc, n_rhs, U)
+    nat = ctx.pack(dev(psi), pkg.F64)
+    for recon in (pkg.LINK18, pkg.LINK12):
+        out = ctx.unpack(ctx.apply(op, nat, n_rhs, pkg.F64, recon), n_rhs, pkg.F64).cpu().numpy()
+        err = rel_per_rhs(out, ref)
+        assert err.max() < 1e-13, (recon, err)
+    ctx.close()
+
+
+@pytest.mark.parametrize("dims,bc,n_rhs,eps", APPLY_CASES)
+@pytest.mark.parametrize("op", [0, 1])
+def test_apply_fp32_matches_oracle_on_rounded_inputs(dims, bc, n_rhs, eps, op):
+    """fp32 arithmetic against the oracle applied to the SAME fp32-rounded inputs (DESIGN.md c.6-12)."""
+    pkg = _wd()
+    kappa = 0.13
+    U = wi.gauge_field(dims, eps, 7, bc)
+    psi = wi.spinor_field(dims, n_rhs, 11, bc)
+    U32 = U.astype(np.float32).astype(np.float64)
+    psi32 = psi.astype(np.float32).astype(np.float64)
+    ref = orc.apply(dims, kappa, bc, op, U32, psi32)
+    ctx = make_ctx(dims, kappa, bc, n_rhs, U)
+    nat = ctx.pack(dev(psi), pkg.F32)
+    out = ctx.unpack(ctx.apply(op, nat, n_rhs, pkg.F32, pkg.LINK18), n_rhs, pkg.F32).cpu().numpy()
+    assert rel_per_rhs(out, ref).max() < 1e-5
+    # 12-real form: row 3 is rebuilt from the rounded rows 1-2, which differs from the rounded row 3
+    # by fp32 rounding of a unit-modulus product, still inside the 1e-5 budget
+    out = ctx.unpack(ctx.apply(op, nat, n_rhs, pkg.F32, pkg.LINK12), n_rhs, pkg.F32).cpu().numpy()
+    assert rel_per_rhs(out, ref).max() < 1e-5
+    ctx.close()
+
+
+def test_pack_unpack_roundtrip_and_sf_zero_slice():
+    pkg = _wd()
+    dims = (4, 6, 2, 8)
+    U = wi.gauge_field(dims, 0.3, 1, wi.BC_SF)
+    psi = wi.spinor_field(dims, 3, 5, wi.BC_PERIODIC)  # non-zero on t=0 on purpose
+    ctx = make_ctx(dims, 0.1, wi.BC_SF, 3, U)
+    back = ctx.unpack(ctx.pack(dev(psi)), 3).cpu().numpy()
+    assert np.all(back[:, 0] == 0.0)
+    assert np.array_equal(back[:, 1:], psi[:, 1:])
+    back32 = ctx.unpack(ctx.pack(dev(psi), pkg.F32), 3, pkg.F32).cpu().numpy()
+    assert np.array_equal(back32[:, 1:], psi[:, 1:].astype(np.float32).astype(np.float64))
+    ctx.close()
+
+
+def test_hop_single_parity_matches_apply():
+    """wd_hop (bare dslash on one parity) is consistent with D = 1 - kappa H."""
+    pkg = _wd()
+    dims, bc, n = (4, 4, 4, 6), wi.BC_SF, 5
+    kappa = 0.125
+    U = wi.gauge_field(dims, 0.3, 3, bc)
+    psi = wi.spinor_field(dims, n, 4, bc)
+    ctx = make_ctx(dims, kappa, bc, n, U)
+    nat = ctx.pack(dev(psi))
+    half = nat.numel() // 2
+    Dpsi = ctx.apply(0, nat, n)
+    for par in (0, 1):
+        h = ctx.hop(0, nat[(1 - par) * half:(2 - par) * half], n, par)
+        expect = nat[par * half:(par + 1) * half] - kappa * h
+        got = Dpsi[par * half:(par + 1) * half]
+        assert torch.allclose(got, expect, rtol=0, atol=1e-13)
+    ctx.close()
+
+
+@pytest.mark.parametrize("order_tile", [None, (2, 2, 2, 2), (4, 2, 2, 4)])
+def test_tiled_site_order_gives_identical_results(order_tile):
+    pkg = _wd()
+    dims, bc, n = (4, 4, 4, 8), wi.BC_SF, 5
+    U = wi.gauge_field(dims, 0.3, 3, bc)
+    psi = wi.spinor_field(dims, n, 4, bc)
+    ref = orc.apply(dims, 0.13, bc, 0, U, psi)
+    kw = {} if order_tile is None else dict(order=pkg.ORDER_TILED, tile=order_tile)
+    ctx = make_ctx(dims, 0.13, bc, n, U, **kw)
+    out = ctx.unpack(ctx.apply(0, ctx.pack(dev(psi)), n), n).cpu().numpy()
+    assert rel_per_rhs(out, ref).max() < 1e-13
+    ctx.close()
+
+
+def _solve_force_case(cfg_idx, n_rhs=None, recon=0):
+    pkg = _wd()
+    cfg, U, Phi = wi.make_config(cfg_idx, n_rhs)
+    dims, kappa, bc, n = cfg["dims"], cfg["kappa"], cfg["bc"], cfg["n_rhs"]
+    Xr, rr, _, rc = orc.solve(dims, kappa, bc, 0, U, Phi, tol=1e-14)
+    assert rc == 0 and rr.max() < 1e-13
+    Yr, rr, _, rc = orc.solve(dims, kappa, bc, 1, U, Xr, tol=1e-14)
+    assert rc == 0 and rr.max() < 1e-13
+    Fr = orc.force(dims, kappa, bc, U, Xr, Yr)
+
+    ctx = make_ctx(dims, kappa, bc, n, U)
+    P = ctx.pack(dev(Phi))
+    X, ix = ctx.solve_block(pkg.OP_D, P, n, tol=1e-12, recon=recon)
+    Y, iy = ctx.solve_block(pkg.OP_DDAG, X, n, tol=1e-12, recon=recon)
+    F = ctx.force(X, Y, n).cpu().numpy()
+    Xc = ctx.unpack(X, n).cpu().numpy()
+    Yc = ctx.unpack(Y, n).cpu().numpy()
+    assert ix["converged"] and iy["converged"]
+    assert max(ix["relres"]) <= 1e-12 and max(iy["relres"]) <= 1e-12
+    # the reported residual is the true one: recompute it with the oracle's operator
+    res = rel_per_rhs(orc.apply(dims, kappa, bc, 0, U, Xc), Phi)
+    assert res.max() < 2e-12, res
+    assert rel_per_rhs(Xc, Xr).max() < 1e-9
+    assert rel_per_rhs(Yc, Yr).max() < 1e-9
+    assert np.linalg.norm(F - Fr) / np.linalg.norm(Fr) < 1e-9
+    ctx.close()
+    return ix, iy
+
+
+def test_solve_and_force_config0():
+    _solve_force_case(0)
+
+
+def test_solve_and_force_config0_recon12():
+    _solve_force_case(0, recon=1)
+
+
+def test_solve_and_force_config1():
+    _solve_force_case(1)
+
+
+@pytest.mark.slow
+def test_solve_and_force_config2():
+    _solve_force_case(2)
+
+
+def test_force_accumulates_and_matches_oracle_on_random_fields():
+    """wd_force alone on arbitrary X, Y (not solutions): F += semantics and parity."""
+    pkg = _wd()
+    dims, bc, n = (4, 6, 4, 6), wi.BC_SF, 5
+    kappa = 0.13
+    U = wi.gauge_field(dims, 0.4, 2, bc)
+    X = wi.spinor_field(dims, n, 21, bc)
+    Y = wi.spinor_field(dims, n, 22, bc)
+    Fr = orc.force(dims, kappa, bc, U, X, Y)
+    ctx = make_ctx(dims, kappa, bc, n, U)
+    Xn, Yn = ctx.pack(dev(X)), ctx.pack(dev(Y))
+    F = ctx.force(Xn, Yn, n)
+    assert np.linalg.norm(F.cpu().numpy() - Fr) / np.linalg.norm(Fr) < 1e-13
+    F = ctx.force(Xn, Yn, n, F=F)  # accumulate a second time
+    assert np.linalg.norm(F.cpu().numpy() - 2 * Fr) / np.linalg.norm(Fr) < 1e-13
+    ctx.close()
+
+
+def test_md_force_host_matches_device_path():
+    pkg = _wd()
+    cfg, U, Phi = wi.make_config(0)
+    dims, kappa, bc, n = cfg["dims"], cfg["kappa"], cfg["bc"], cfg["n_rhs"]
+    ctx = make_ctx(dims, kappa, bc, n, U)
+    P = ctx.pack(dev(Phi))
+    X, _ = ctx.solve_block(pkg.OP_D, P, n)
+    Y, _ = ctx.solve_block(pkg.OP_DDAG, X, n)
+    F = ctx.force(X, Y, n).cpu().numpy()
+    Fh, infos = ctx.md_force_host(torch.from_numpy(Phi).pin_memory())
+    assert np.array_equal(Fh.numpy(), F)
+    assert infos[0]["converged"] and infos[1]["converged"]
+    ctx.close()
+
+
+def test_error_codes():
+    pkg = _wd()
+    L = pkg.wd.lib()
+    import ctypes
+    h = ctypes.c_void_p()
+    bad = (ctypes.c_int * 4)(4, 4, 3, 4)
+    assert L.wd_create(ctypes.byref(h), bad, 0.1, 1, 5, None) == pkg.wd.EINVAL
+    ctx = pkg.Context((4, 4, 4, 4), 0.1, max_rhs=2)
+    t = torch.zeros(ctx.native_numel(pkg.F64, 2), dtype=torch.float64, device="cuda")
+    o = torch.zeros_like(t)
+    # gauge not set
+    assert L.wd_apply(ctx._h, 0, 0, 0, 2, ctypes.c_void_p(t.data_ptr()), ctypes.c_void_p(o.data_ptr())) == pkg.wd.ESTATE
+    ctx.set_gauge(dev(wi.unit_gauge((4, 4, 4, 4))))
+    assert L.wd_apply(ctx._h, 0, 0, 0, 3, ctypes.c_void_p(t.data_ptr()), ctypes.c_void_p(o.data_ptr())) == pkg.wd.EINVAL
+    assert L.wd_apply(ctx._h, 0, 0, 0, 2, ctypes.c_void_p(t.data_ptr()), ctypes.c_void_p(t.data_ptr())) == pkg.wd.EINVAL
+    assert L.wd_apply(ctx._h, 0, 0, 0, 2, ctypes.c_void_p(t.data_ptr()), ctypes.c_void_p(o.data_ptr())) == pkg.wd.OK
+    ctx.close()
