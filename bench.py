@@ -1,0 +1,377 @@
+#!/usr/bin/env python
+"""bench.py -- one JSON line for the hot path of arxiv/paper_1009_5169 on B200.
+
+A "step" is one MD force evaluation (Algorithm 2): the blocked mixed-precision solve
+D X = Phi, the blocked solve D^dag Y = X (both to a true fp64 relative residual of 1e-12) and the
+force accumulation F += sum_i f[x_i, y_i], over all n_rhs pseudo-fermion fields, all in the CUDA
+kernels of libwd.so through its C ABI.  Workload at N = 1: BASELINE.json configs[4] at n_rhs = 5
+(24^3 x 24 SF lattice, eps 0.4, kappa 0.135) -- the largest single-GPU config and the only one whose
+working set (about 0.65 GB of solver vectors + 96 MB of fp32 links) is far outside the 126 MB L2,
+so no L2 flush is needed between steps.  N > 1: independent replicas (the path has no exchange step,
+DESIGN.md "Multi-GPU"), weak scaling.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 4] [--n-rhs 5] [--impl reference]
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import tempfile
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "md_force_evals_per_s (2 blocked mixed-precision solves to 1e-12 + force; ms_per_step = solve time per MD force)"
+UNIT = "force_eval/s"
+TOL = 1e-12
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=4, help="index into BASELINE.json configs")
+    ap.add_argument("--n-rhs", type=int, default=5)
+    ap.add_argument("--recon", type=int, default=12, choices=(12, 18), help="inner fp32 link form")
+    ap.add_argument("--impl", default="ours", choices=("ours", "reference"))
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-hop-sweep", action="store_true")
+    return ap.parse_args()
+
+
+def workload_name(cfg, n):
+    lx, ly, lz, lt = cfg["dims"]
+    return f"{lx}x{ly}x{lz}x{lt} SF lattice, eps={cfg['eps']}, kappa={cfg['kappa']}, n_rhs={n}, seed={cfg['seed']}"
+
+
+# ------------------------------------------------------------------------------------------------
+# the oracle, timed on the host cores (cpu_baseline leg and --impl reference arm)
+# ------------------------------------------------------------------------------------------------
+# rough cost of one 1-RHS MD force evaluation of the oracle on 8 cores, seconds, by lattice size
+_ORACLE_SAMPLES = [(24, 90.0), (16, 14.0), (12, 3.5), (8, 0.6)]
+
+
+def oracle_sample_time(cfg_full, n_full, L):
+    """Time the oracle, as it stands, on a bounded sample of the workload: ONE right-hand side on an
+    L^3 x L SF lattice drawn from the same link/RHS distribution (eps, kappa, seed of the workload).
+    Returns (seconds, site*rhs of the sample, iterations)."""
+    import wd_inputs as wi
+    from oracle import wd_oracle as orc
+    dims = (L, L, L, L)
+    U = wi.gauge_field(dims, cfg_full["eps"], cfg_full["seed"], cfg_full["bc"])
+    Phi = wi.spinor_field(dims, 1, cfg_full["seed"], cfg_full["bc"])
+    k, bc = cfg_full["kappa"], cfg_full["bc"]
+    t0 = time.perf_counter()
+    X, r1, it1, _ = orc.solve(dims, k, bc, 0, U, Phi, tol=TOL)
+    Y, r2, it2, _ = orc.solve(dims, k, bc, 1, U, X, tol=TOL)
+    orc.force(dims, k, bc, U, X, Y)
+    dt = time.perf_counter() - t0
+    return dt, L ** 4, (int(it1[0]), int(it2[0]))
+
+
+def oracle_value(cfg_full, n_full, L):
+    """force_eval/s of the full workload extrapolated from the sample by site*rhs count."""
+    dt, units, iters = oracle_sample_time(cfg_full, n_full, L)
+    lx, ly, lz, lt = cfg_full["dims"]
+    full_units = lx * ly * lz * lt * n_full
+    est_full = dt * full_units / units
+    sample = (f"oracle (fp64, unpreconditioned BiCGStab, OpenMP over sites) on 1 RHS of a {L}^4 SF lattice of the "
+              f"same distribution: 2 solves to {TOL:g} + force took {dt:.2f} s ({iters[0]}+{iters[1]} iterations); "
+              f"scaled by site*rhs count x{full_units / units:.1f} to the full workload")
+    return 1.0 / est_full, sample, dt
+
+
+def run_reference(args):
+    """--impl reference: the oracle on the host cores (rank 0 only)."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import wd_inputs as wi
+    from oracle import wd_oracle as orc
+    cfg = dict(wi.CONFIGS[args.config])
+    n = args.n_rhs
+    budget = 200.0 / max(1, args.steps + args.warmup)
+    L = next((l for l, cost in _ORACLE_SAMPLES if cost <= budget and l <= cfg["dims"][0]), 8)
+    for _ in range(args.warmup):
+        oracle_value(cfg, n, L)
+    times, sample = [], ""
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        v, sample, dt = oracle_value(cfg, n, L)
+        times.append(1.0 / v)
+    total = time.perf_counter() - t0
+    value = args.steps / sum(times)
+    cores = orc.max_threads()
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 / value, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": workload_name(cfg, n), "l2": "n/a (CPU)"},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0, "wall_s": total,
+    }
+    print(json.dumps(line))
+
+
+# ------------------------------------------------------------------------------------------------
+# clocks during the timed region (B200_PROFILING.md "clocks line")
+# ------------------------------------------------------------------------------------------------
+class ClockSampler:
+    FIELDS = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
+              "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+              "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index):
+        self.gpu = gpu_index
+        self.proc = None
+        self.path = None
+
+    def start(self):
+        try:
+            f = tempfile.NamedTemporaryFile("w", suffix=".csv", delete=False)
+            self.path = f.name
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.gpu), f"--query-gpu={self.FIELDS}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"], stdout=f,
+                                         stderr=subprocess.DEVNULL)
+        except Exception:
+            self.proc = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.proc is None:
+            return out
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, smax, reasons = [], [], set()
+        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        try:
+            for ln in open(self.path):
+                p = [x.strip() for x in ln.split(",")]
+                if len(p) < 9:
+                    continue
+                try:
+                    sm.append(float(p[1]))
+                    smax.append(float(p[2]))
+                except ValueError:
+                    continue
+                for name, v in zip(names, p[5:9]):
+                    if v.lower().startswith("active"):
+                        reasons.add(name)
+            os.unlink(self.path)
+        except Exception:
+            pass
+        if sm:
+            out.update(sm_mhz=statistics.median(sm), sm_max_mhz=max(smax), samples=len(sm))
+        out["reasons"] = sorted(reasons)
+        return out
+
+
+# ------------------------------------------------------------------------------------------------
+# standalone hop (dslash) measurement: BASELINE.json metric "multi-RHS Wilson dslash GFLOP/s & HBM GB/s"
+# ------------------------------------------------------------------------------------------------
+def hop_bytes_per_launch(Vh, n, s, R, xpay_frac=0.0):
+    """Algorithmic bytes of one hop launch on one output parity: per output
+    site*RHS 24 reals in + 24 out (+24 for the fused xpay operand) and 8 links of R reals per site."""
+    return Vh * (n * (48 + 24 * xpay_frac) * s + 8 * R * s)
+
+
+def hop_sweep(pkg, ctx, torch, n, peak_gbs, reps=50):
+    """wd_hop back to back on native half-lattice blocks, fp32/fp64 x 18/12-real links; CUDA events
+    on the launching stream.  Fields rotate through enough copies to exceed 2x L2 (L2-cold)."""
+    res = {}
+    Vh = ctx.V // 2
+    for prec, pname, s in ((pkg.F32, "f32", 4), (pkg.F64, "f64", 8)):
+        half = ctx.native_numel(prec, n) // 2
+        dt = torch.float32 if prec == pkg.F32 else torch.float64
+        nbuf = max(2, int(2 * 130e6 / (half * s)) + 1)
+        bufs = [torch.randn(half, dtype=dt, device=ctx.device) for _ in range(nbuf)]
+        out = [torch.empty(half, dtype=dt, device=ctx.device) for _ in range(2)]
+        for recon, R in ((pkg.LINK18, 18), (pkg.LINK12, 12)):
+            for i in range(5):
+                ctx.hop(pkg.OP_D, bufs[i % nbuf], n, 0, prec, recon, out=out[i % 2])
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            torch.cuda.synchronize()
+            e0.record()
+            for i in range(reps):
+                ctx.hop(pkg.OP_D, bufs[i % nbuf], n, 0, prec, recon, out=out[i % 2])
+            e1.record()
+            torch.cuda.synchronize()
+            us = e0.elapsed_time(e1) * 1e3 / reps
+            b = hop_bytes_per_launch(Vh, n, s, R)
+            gbs = b / us * 1e-3
+            res[f"{pname}_r{R}"] = {"us": round(us, 2), "gbs": round(gbs, 1), "frac_hbm": round(gbs / peak_gbs, 4),
+                                    "gflops": round(1320.0 * Vh * n / us * 1e-3, 1),
+                                    "site_rhs_per_s": round(Vh * n / us * 1e6, 0)}
+        del bufs, out
+    return res
+
+
+# ------------------------------------------------------------------------------------------------
+# our arm
+# ------------------------------------------------------------------------------------------------
+def run_ours(args):
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+
+    import paper_1009_5169_b200 as pkg
+    import wd_inputs as wi
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback (use --impl reference for the oracle)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    peaks = {}
+    try:
+        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except Exception:
+        pass
+    peak_gbs = float(peaks.get("hbm_gbs", 6650.0))
+    peak_src = "measured (MEASURED_PEAKS.json hbm_gbs)" if "hbm_gbs" in peaks else "fallback 6650 GB/s"
+
+    cfg = dict(wi.CONFIGS[args.config])
+    cfg["seed"] = cfg["seed"] + rank  # independent replica per rank
+    n = args.n_rhs
+    dims, kappa, bc = cfg["dims"], cfg["kappa"], cfg["bc"]
+    recon = pkg.LINK12 if args.recon == 12 else pkg.LINK18
+    R = args.recon
+    U = wi.gauge_field(dims, cfg["eps"], cfg["seed"], bc)
+    Phi = wi.spinor_field(dims, n, cfg["seed"], bc)
+
+    ctx = pkg.Context(dims, kappa, bc=bc, max_rhs=n, device=f"cuda:{local}")
+    ctx.set_gauge(torch.from_numpy(U).cuda())
+    Phi_host = torch.from_numpy(Phi).pin_memory()
+    P = ctx.pack(Phi_host.cuda())
+    X = torch.empty_like(P)
+    Y = torch.empty_like(P)
+    F = torch.zeros((4,) + tuple(reversed(dims)) + (3, 3, 2), dtype=torch.float64, device=ctx.device)
+    F_host = torch.empty(F.shape, dtype=torch.float64).pin_memory()
+    V = ctx.V
+    Vh = V // 2
+
+    def step():
+        F.zero_()
+        _, ix = ctx.solve_block(pkg.OP_D, P, n, tol=TOL, recon=recon, out=X)
+        _, iy = ctx.solve_block(pkg.OP_DDAG, X, n, tol=TOL, recon=recon, out=Y)
+        ctx.force(X, Y, n, F=F)
+        return ix, iy
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def max_over_ranks(ms):
+        if world == 1:
+            return ms
+        t = torch.tensor([ms], dtype=torch.float64, device=ctx.device)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
+
+    for _ in range(max(args.warmup, 3)):
+        ix, iy = step()
+    # ---- timed region: device-resident inputs ---------------------------------------------------
+    sampler = ClockSampler(local)
+    barrier()
+    sampler.start()
+    l0 = ctx.launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(args.steps):
+        ix, iy = step()
+    e1.record()
+    barrier()
+    launches = ctx.launch_count() - l0
+    ms_total = max_over_ranks(e0.elapsed_time(e1))
+    ms_step = ms_total / args.steps
+    value = world * args.steps / (ms_total * 1e-3)
+
+    # ---- e2e: host buffers through the one-call C-ABI entry, copies inside the timed region ------
+    ctx.md_force_host(Phi_host, F_host, tol=TOL, recon=recon)
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        ctx.md_force_host(Phi_host, F_host, tol=TOL, recon=recon)
+    barrier()
+    e2e_ms = max_over_ranks((time.perf_counter() - t0) * 1e3)
+    e2e_value = world * args.steps / (e2e_ms * 1e-3)
+    clocks = sampler.stop()
+    f_check = float(F_host.abs().sum())
+    assert np.isfinite(f_check) and f_check > 0.0
+
+    # ---- per-class device time of one more step (event pairs inside the library) -----------------
+    ctx.profile(True)
+    ix, iy = step()
+    prof = ctx.profile_read()
+    ctx.profile(False)
+    hop_ms, hop_cnt = prof["hop32"]
+    tot_prof = sum(v[0] for v in prof.values())
+    # in the inner solver half of the hop launches carry the fused xpay operand
+    hop_bytes = hop_bytes_per_launch(Vh, n, 4, R, xpay_frac=0.5)
+    hop_us = hop_ms * 1e3 / max(1, hop_cnt)
+    achieved = hop_bytes / (hop_us * 1e-6) * 1e-9 if hop_cnt else 0.0
+    roofline = {"bound": "hbm", "kernel": f"hop_kernel<float,{R}> (fp32 multi-RHS Wilson hop inside the inner solver)",
+                "achieved": round(achieved, 1), "peak": peak_gbs, "unit": "GB/s", "frac": round(achieved / peak_gbs, 4),
+                "peak_source": peak_src, "traffic": None, "bytes_per_launch": hop_bytes,
+                "avg_launch_us": round(hop_us, 2), "launches_in_step": hop_cnt,
+                "share_of_step": round(hop_ms / tot_prof, 4) if tot_prof else None,
+                "gflops": round(1320.0 * Vh * n / hop_us * 1e-3, 1) if hop_cnt else None}
+    breakdown = {k: {"ms": round(v[0], 3), "launch_groups": v[1]} for k, v in prof.items()}
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
+        "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+        "data": "synthetic",
+        "config": {"workload": workload_name(cfg, n), "inner_links": f"{R}-real fp32", "outer": "fp64 defect correction",
+                   "tol": TOL, "l2": "no flush: solver working set >> 126 MB L2", "parallelism": f"replicas x{world}"},
+        "clocks": clocks,
+        "e2e": {"value": e2e_value, "unit": UNIT, "ms_per_step": e2e_ms / args.steps,
+                "h2d_bytes_per_step": Phi_host.numel() * 8, "d2h_bytes_per_step": F_host.numel() * 8},
+        "gpu_launches": int(launches),
+        "roofline": roofline,
+        "solver": {"outer_steps": [ix["outer_steps"], iy["outer_steps"]],
+                   "inner_iters": [ix["inner_iters_total"], iy["inner_iters_total"]],
+                   "max_relres": [max(ix["relres"]), max(iy["relres"])],
+                   "site_rhs_per_s": V * n * value},
+        "breakdown_ms": breakdown,
+    }
+    if rank == 0 and not args.no_hop_sweep:
+        line["hop"] = hop_sweep(pkg, ctx, torch, n, peak_gbs)
+    ctx.close()
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        from oracle import wd_oracle as orc
+        v, sample, _ = oracle_value(dict(wi.CONFIGS[args.config]), n, 16 if dims[0] >= 16 else dims[0])
+        line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": orc.max_threads(), "kind": "oracle", "sample": sample}
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+    if rank == 0:
+        print(json.dumps(line))
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

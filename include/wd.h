@@ -140,6 +140,16 @@ int wd_md_force_host(wd_ctx* ctx, int n_rhs, const double* Phi_canon_host, doubl
                      double tol, int max_outer, int max_inner, double inner_tol, int recon,
                      wd_solve_info* info2);
 
+/* Per-class device timing for measurement (bench.py's roofline line).  wd_profile(ctx, 1) makes every
+ * later hop / BLAS1 / force launch record a CUDA event pair on the context's stream (a few
+ * microseconds of host time each; leave it off when timing whole calls).  wd_profile_read
+ * synchronises the stream, adds up the event-pair durations recorded since the previous read into
+ * ms[class] (milliseconds) and count[class] (launch groups), class = WD_PROF_*, both arrays of
+ * WD_PROF_N, and resets the record.  Errors: WD_EINVAL (null), WD_ECUDA. */
+enum { WD_PROF_HOP32 = 0, WD_PROF_HOP64 = 1, WD_PROF_BLAS = 2, WD_PROF_FORCE = 3, WD_PROF_LAYOUT = 4, WD_PROF_N = 5 };
+int wd_profile(wd_ctx* ctx, int enable);
+int wd_profile_read(wd_ctx* ctx, double* ms_host, long long* count_host);
+
 /* Number of kernel launches this context has enqueued since creation (for bench.py's count). */
 long long wd_launch_count(const wd_ctx* ctx);
 

@@ -47,7 +47,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
         failed = failed or p.returncode != 0
     if failed:
         raise RuntimeError("nvcc failed")
-    subprocess.run([nvcc, "-shared", "-o", LIB] + objs + ["-lcudart"], check=True)
+    subprocess.run([nvcc, "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-o", LIB] + objs + ["-lcudart"], check=True)
     return LIB
 
 

@@ -142,6 +142,8 @@ int wd_create(wd_ctx** out, const int dims[4], double kappa, int time_bc, int ma
     c->ws_bytes = 0;
     c->have_ws = c->have_gauge = false;
     c->launches = 0;
+    c->prof_on = false;
+    c->prof_used = 0;
     c->h_pinned = nullptr;
     if (cudaMallocHost((void**)&c->h_pinned, sizeof(double) * kScalDoubles) != cudaSuccess) {
         cudaGetLastError();
@@ -162,7 +164,29 @@ int wd_create(wd_ctx** out, const int dims[4], double kappa, int time_bc, int ma
 int wd_destroy(wd_ctx* ctx) {
     if (!ctx) return WD_EINVAL;
     if (ctx->h_pinned) cudaFreeHost(ctx->h_pinned);
+    for (cudaEvent_t e : ctx->prof_ev) cudaEventDestroy(e);
     delete ctx;
+    return WD_OK;
+}
+
+int wd_profile(wd_ctx* ctx, int enable) {
+    if (!ctx) return WD_EINVAL;
+    ctx->prof_on = enable != 0;
+    return WD_OK;
+}
+
+int wd_profile_read(wd_ctx* ctx, double* ms, long long* count) {
+    if (!ctx) return WD_EINVAL;
+    if (!ms || !count) return wd_fail(ctx, WD_EINVAL, "null pointer");
+    for (int k = 0; k < WD_PROF_N; ++k) { ms[k] = 0.0; count[k] = 0; }
+    WD_CUDA_CHECK(ctx, cudaStreamSynchronize(ctx->stream));
+    for (size_t i = 0; i < ctx->prof_used; ++i) {
+        float t = 0.f;
+        WD_CUDA_CHECK(ctx, cudaEventElapsedTime(&t, ctx->prof_ev[2 * i], ctx->prof_ev[2 * i + 1]));
+        ms[ctx->prof_cls[i]] += t;
+        count[ctx->prof_cls[i]] += 1;
+    }
+    ctx->prof_used = 0;
     return WD_OK;
 }
 

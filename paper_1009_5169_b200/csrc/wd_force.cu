@@ -173,6 +173,7 @@ int wd_force_impl(wd_ctx* c, int n, const double* X, const double* Y, double* F)
         attr_set = true;
     }
     const unsigned G = (unsigned)((2 * c->Vh + A.spb - 1) / A.spb);
+    wd_prof_scope prof(c, WD_PROF_FORCE);
     force_kernel<<<G, B, smem, c->stream>>>(A);
     WD_LAUNCH_CHECK(c);
     return WD_OK;

@@ -112,6 +112,7 @@ void launch_t(wd_ctx* c, int dag, int n, int par, const void* in, void* out, con
 
 int wd_hop_launch(wd_ctx* c, int prec, int recon, int dag, int n, int par, const void* in, void* out,
                   const void* in2, double a, double b) {
+    wd_prof_scope prof(c, prec == WD_F64 ? WD_PROF_HOP64 : WD_PROF_HOP32);
     if (prec == WD_F64) {
         if (recon == WD_LINK18) launch_t<double, 18>(c, dag, n, par, in, out, in2, a, b, c->d_U64[0]);
         else                    launch_t<double, 12>(c, dag, n, par, in, out, in2, a, b, c->d_U64[1]);

@@ -51,6 +51,34 @@ struct wd_ctx {
 
     long long launches;
     std::string err;
+
+    // optional per-class device timing (wd_profile): CUDA event pairs around the classed launches
+    bool prof_on;
+    std::vector<cudaEvent_t> prof_ev;   // pairs (begin, end)
+    std::vector<int> prof_cls;          // class of pair i
+    size_t prof_used;                   // pairs used since the last wd_profile_read
+};
+
+// RAII bracket: records an event pair on the context's stream around the launches in its scope.
+struct wd_prof_scope {
+    wd_ctx* c;
+    long idx;
+    wd_prof_scope(wd_ctx* ctx, int cls) : c(ctx), idx(-1) {
+        if (!c->prof_on) return;
+        if (c->prof_used == c->prof_cls.size()) {
+            cudaEvent_t a, b;
+            if (cudaEventCreate(&a) != cudaSuccess || cudaEventCreate(&b) != cudaSuccess) return;
+            c->prof_ev.push_back(a);
+            c->prof_ev.push_back(b);
+            c->prof_cls.push_back(cls);
+        }
+        idx = (long)c->prof_used++;
+        c->prof_cls[idx] = cls;
+        cudaEventRecord(c->prof_ev[2 * idx], c->stream);
+    }
+    ~wd_prof_scope() {
+        if (idx >= 0) cudaEventRecord(c->prof_ev[2 * idx + 1], c->stream);
+    }
 };
 
 static inline size_t wd_align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }

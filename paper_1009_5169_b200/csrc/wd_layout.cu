@@ -120,6 +120,7 @@ __global__ void unpack_kernel(const T* __restrict__ native, const int32_t* __res
 int wd_layout_gauge(wd_ctx* c, const double* U) {
     const long total = 8 * c->Vh;
     const int B = 128;
+    wd_prof_scope prof(c, WD_PROF_LAYOUT);
     gauge_ingest_kernel<<<(unsigned)((total + B - 1) / B), B, 0, c->stream>>>(
         U, c->d_site_of, c->V, c->Vh, c->d_U64[0], c->d_U64[1], c->d_U32[0], c->d_U32[1]);
     WD_LAUNCH_CHECK(c);
@@ -130,6 +131,7 @@ int wd_layout_pack(wd_ctx* c, int prec, int n, const double* canon, void* native
     const long total = 2 * c->Vh * n;
     const int B = 128;
     const unsigned G = (unsigned)((total + B - 1) / B);
+    wd_prof_scope prof(c, WD_PROF_LAYOUT);
     if (prec == WD_F64)
         pack_kernel<double><<<G, B, 0, c->stream>>>(canon, c->d_site_of, c->d_nbr, c->V, c->Vh, n, (double*)native);
     else
@@ -142,6 +144,7 @@ int wd_layout_unpack(wd_ctx* c, int prec, int n, const void* native, double* can
     const long total = 2 * c->Vh * n;
     const int B = 128;
     const unsigned G = (unsigned)((total + B - 1) / B);
+    wd_prof_scope prof(c, WD_PROF_LAYOUT);
     if (prec == WD_F64)
         unpack_kernel<double><<<G, B, 0, c->stream>>>((const double*)native, c->d_site_of, c->V, c->Vh, n, canon);
     else

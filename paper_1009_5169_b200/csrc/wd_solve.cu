@@ -274,14 +274,14 @@ int wd_solve_impl(wd_ctx* c, int dag, int n, const double* Phi, double* X, doubl
     RedBuf rb{c->d_scal, c->d_partials, c->d_ticket};
     int rc;
 
-    set_globals_kernel<<<1, 1, 0, st>>>(c->d_scal, tol * tol, inner_tol * inner_tol);
+    { wd_prof_scope pr__(c, WD_PROF_BLAS); set_globals_kernel<<<1, 1, 0, st>>>(c->d_scal, tol * tol, inner_tol * inner_tol); }
     WD_LAUNCH_CHECK(c);
 
     const long nv64 = 12 * Vh * n, nv32 = 6 * Vh * n;
     const Launch L64 = blas_cfg(c, nv64, n), L64f = blas_cfg(c, 2 * nv64, n), L32 = blas_cfg(c, nv32, n);
 
     // |phi_i|^2 (full lattice) and the even/odd right-hand side
-    norm2_kernel<<<L64f.G, L64f.B, 0, st>>>(2 * nv64, n, rb, (const double2*)Phi);
+    { wd_prof_scope pr__(c, WD_PROF_BLAS); norm2_kernel<<<L64f.G, L64f.B, 0, st>>>(2 * nv64, n, rb, (const double2*)Phi); }
     WD_LAUNCH_CHECK(c);
     rc = wd_hop_launch(c, WD_F64, WD_LINK18, dag, n, 0, PhiO, phihat, PhiE, 1.0, kap);
     if (rc) return rc;
@@ -292,13 +292,13 @@ int wd_solve_impl(wd_ctx* c, int dag, int n, const double* Phi, double* X, doubl
     for (;;) {
         // true residual of the even/odd system in fp64
         if (outer == 0) {
-            outer_resid_kernel<<<L64.G, L64.B, 0, st>>>(nv64, n, rb, phihat, nullptr, R64);
+            { wd_prof_scope pr__(c, WD_PROF_BLAS); outer_resid_kernel<<<L64.G, L64.B, 0, st>>>(nv64, n, rb, phihat, nullptr, R64); }
         } else {
             rc = wd_hop_launch(c, WD_F64, WD_LINK18, dag, n, 1, XE, tmp64, nullptr, 0.0, 1.0);
             if (rc) return rc;
             rc = wd_hop_launch(c, WD_F64, WD_LINK18, dag, n, 0, tmp64, R64, XE, 1.0, -kap * kap);
             if (rc) return rc;
-            outer_resid_kernel<<<L64.G, L64.B, 0, st>>>(nv64, n, rb, phihat, R64, R64);
+            { wd_prof_scope pr__(c, WD_PROF_BLAS); outer_resid_kernel<<<L64.G, L64.B, 0, st>>>(nv64, n, rb, phihat, R64, R64); }
         }
         WD_LAUNCH_CHECK(c);
         WD_CUDA_CHECK(c, cudaMemcpyAsync(hp, c->d_scal, sizeof(double) * G_COUNT, cudaMemcpyDeviceToHost, st));
@@ -308,35 +308,35 @@ int wd_solve_impl(wd_ctx* c, int dag, int n, const double* Phi, double* X, doubl
         ++outer;
 
         // inner fp32 BiCGStab on the normalised residual
-        demote_kernel<<<L32.G, L32.B, 0, st>>>(Vh, n, rb, R64, r32, rt32, x32, p32, v32);
+        { wd_prof_scope pr__(c, WD_PROF_BLAS); demote_kernel<<<L32.G, L32.B, 0, st>>>(Vh, n, rb, R64, r32, rt32, x32, p32, v32); }
         WD_LAUNCH_CHECK(c);
         const double* done = c->d_scal + G_DONE;
         (void)done;
         for (int it = 1; it <= max_inner; ++it) {
-            p_update_kernel<float><<<L32.G, L32.B, 0, st>>>(nv32, n, c->d_scal, r32, p32, v32);
+            { wd_prof_scope pr__(c, WD_PROF_BLAS); p_update_kernel<float><<<L32.G, L32.B, 0, st>>>(nv32, n, c->d_scal, r32, p32, v32); }
             WD_LAUNCH_CHECK(c);
             rc = wd_hop_launch(c, WD_F32, recon, dag, n, 1, p32, tmp32, nullptr, 0.0, 1.0);
             if (rc) return rc;
             rc = wd_hop_launch(c, WD_F32, recon, dag, n, 0, tmp32, v32, p32, 1.0, -kap * kap);
             if (rc) return rc;
-            dot_sigma_kernel<float><<<L32.G, L32.B, 0, st>>>(nv32, n, rb, rt32, v32);
+            { wd_prof_scope pr__(c, WD_PROF_BLAS); dot_sigma_kernel<float><<<L32.G, L32.B, 0, st>>>(nv32, n, rb, rt32, v32); }
             WD_LAUNCH_CHECK(c);
-            s_update_kernel<float><<<L32.G, L32.B, 0, st>>>(nv32, n, c->d_scal, r32, v32);
+            { wd_prof_scope pr__(c, WD_PROF_BLAS); s_update_kernel<float><<<L32.G, L32.B, 0, st>>>(nv32, n, c->d_scal, r32, v32); }
             WD_LAUNCH_CHECK(c);
             rc = wd_hop_launch(c, WD_F32, recon, dag, n, 1, r32, tmp32, nullptr, 0.0, 1.0);
             if (rc) return rc;
             rc = wd_hop_launch(c, WD_F32, recon, dag, n, 0, tmp32, t32, r32, 1.0, -kap * kap);
             if (rc) return rc;
-            dot_omega_kernel<float><<<L32.G, L32.B, 0, st>>>(nv32, n, rb, t32, r32);
+            { wd_prof_scope pr__(c, WD_PROF_BLAS); dot_omega_kernel<float><<<L32.G, L32.B, 0, st>>>(nv32, n, rb, t32, r32); }
             WD_LAUNCH_CHECK(c);
-            xr_update_kernel<float><<<L32.G, L32.B, 0, st>>>(nv32, n, rb, x32, p32, r32, t32, rt32);
+            { wd_prof_scope pr__(c, WD_PROF_BLAS); xr_update_kernel<float><<<L32.G, L32.B, 0, st>>>(nv32, n, rb, x32, p32, r32, t32, rt32); }
             WD_LAUNCH_CHECK(c);
             // convergence poll (every iteration for now)
             WD_CUDA_CHECK(c, cudaMemcpyAsync(hp + G_COUNT, c->d_scal + G_DONE, sizeof(double), cudaMemcpyDeviceToHost, st));
             WD_CUDA_CHECK(c, cudaStreamSynchronize(st));
             if (hp[G_COUNT] != 0.0) break;
         }
-        promote_kernel<<<L32.G, L32.B, 0, st>>>(Vh, n, c->d_scal, x32, (double2*)XE);
+        { wd_prof_scope pr__(c, WD_PROF_BLAS); promote_kernel<<<L32.G, L32.B, 0, st>>>(Vh, n, c->d_scal, x32, (double2*)XE); }
         WD_LAUNCH_CHECK(c);
     }
 

@@ -27,11 +27,13 @@ F64, F32 = 0, 1
 LINK18, LINK12 = 0, 1
 ORDER_LINEAR, ORDER_TILED = 0, 1
 MAX_RHS = 16
+PROF_NAMES = ("hop32", "hop64", "blas", "force", "layout")
+PROF_N = len(PROF_NAMES)
 
 # every symbol include/wd.h declares (tests check that the library exports each one)
 SYMBOLS = ["wd_create", "wd_destroy", "wd_site_order", "wd_workspace_bytes", "wd_set_workspace",
            "wd_set_gauge", "wd_native_bytes", "wd_pack", "wd_unpack", "wd_apply", "wd_hop",
-           "wd_solve_block", "wd_force", "wd_md_force_host", "wd_launch_count", "wd_strerror",
+           "wd_solve_block", "wd_force", "wd_md_force_host", "wd_profile", "wd_profile_read", "wd_launch_count", "wd_strerror",
            "wd_last_error", "wd_version"]
 
 
@@ -84,6 +86,8 @@ def lib():
     L.wd_solve_block.argtypes = [vp, ci, ci, vp, vp, cd, ci, ci, cd, ci, ctypes.POINTER(SolveInfo)]
     L.wd_force.argtypes = [vp, ci, vp, vp, vp]
     L.wd_md_force_host.argtypes = [vp, ci, vp, vp, cd, ci, ci, cd, ci, ctypes.POINTER(SolveInfo)]
+    L.wd_profile.argtypes = [vp, ci]
+    L.wd_profile_read.argtypes = [vp, ctypes.POINTER(cd), ctypes.POINTER(ctypes.c_longlong)]
     L.wd_launch_count.argtypes = [vp]
     L.wd_launch_count.restype = ctypes.c_longlong
     L.wd_strerror.argtypes = [ci]
@@ -92,7 +96,8 @@ def lib():
     L.wd_last_error.restype = ctypes.c_char_p
     L.wd_version.restype = ctypes.c_char_p
     for name in ("wd_create", "wd_destroy", "wd_site_order", "wd_set_workspace", "wd_set_gauge", "wd_pack",
-                 "wd_unpack", "wd_apply", "wd_hop", "wd_solve_block", "wd_force", "wd_md_force_host"):
+                 "wd_unpack", "wd_apply", "wd_hop", "wd_solve_block", "wd_force", "wd_md_force_host", "wd_profile",
+                 "wd_profile_read"):
         getattr(L, name).restype = ci
     _lib = L
     return L
@@ -231,6 +236,16 @@ class Context:
                                      int(max_inner), float(inner_tol), int(recon), infos)
         self._check(rc)
         return F_host, [infos[0].as_dict(), infos[1].as_dict()]
+
+    def profile(self, enable=True):
+        self._check(self.L.wd_profile(self._h, 1 if enable else 0))
+
+    def profile_read(self):
+        """{class name: (milliseconds, launch groups)} since the previous read; synchronises."""
+        ms = (ctypes.c_double * PROF_N)()
+        cnt = (ctypes.c_longlong * PROF_N)()
+        self._check(self.L.wd_profile_read(self._h, ms, cnt))
+        return {name: (ms[i], int(cnt[i])) for i, name in enumerate(PROF_NAMES)}
 
     def launch_count(self):
         return int(self.L.wd_launch_count(self._h))
