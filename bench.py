@@ -180,10 +180,11 @@ class ClockSampler:
 # ------------------------------------------------------------------------------------------------
 # standalone hop (dslash) measurement: BASELINE.json metric "multi-RHS Wilson dslash GFLOP/s & HBM GB/s"
 # ------------------------------------------------------------------------------------------------
-def hop_bytes_per_launch(Vh, n, s, R, xpay_frac=0.0):
+def hop_bytes_per_launch(Vh, n, s, R, extra_operands=0.0):
     """Algorithmic bytes of one hop launch on one output parity: per output
-    site*RHS 24 reals in + 24 out (+24 for the fused xpay operand) and 8 links of R reals per site."""
-    return Vh * (n * (48 + 24 * xpay_frac) * s + 8 * R * s)
+    site*RHS 24 reals in + 24 out, +24 per extra operand the fused epilogue reads (xpay operand,
+    left operand of a fused inner product), and 8 links of R reals per site."""
+    return Vh * (n * (48 + 24 * extra_operands) * s + 8 * R * s)
 
 
 def hop_sweep(pkg, ctx, torch, n, peak_gbs, reps=50):
@@ -322,8 +323,9 @@ def run_ours(args):
     ctx.profile(False)
     hop_ms, hop_cnt = prof["hop32"]
     tot_prof = sum(v[0] for v in prof.values())
-    # in the inner solver half of the hop launches carry the fused xpay operand
-    hop_bytes = hop_bytes_per_launch(Vh, n, 4, R, xpay_frac=0.5)
+    # the four fp32 hop launches of one BiCGStab iteration: plain, xpay + <rt, v> (2 extra operands), plain,
+    # xpay + <t, s>, <t, t> (1 extra operand): 0.75 extra operands per launch on average
+    hop_bytes = hop_bytes_per_launch(Vh, n, 4, R, extra_operands=0.75)
     hop_us = hop_ms * 1e3 / max(1, hop_cnt)
     achieved = hop_bytes / (hop_us * 1e-6) * 1e-9 if hop_cnt else 0.0
     roofline = {"bound": "hbm", "kernel": f"hop_kernel<float,{R}> (fp32 multi-RHS Wilson hop inside the inner solver)",

@@ -83,6 +83,18 @@ int wd_destroy(wd_ctx* ctx);
  * called before wd_set_workspace; default is WD_ORDER_LINEAR.  Errors: WD_EINVAL, WD_ESTATE. */
 int wd_site_order(wd_ctx* ctx, int order, const int tile[4]);
 
+/* Launch tunables (speed only, never results).  Keys:
+ *   WD_OPT_HOP32_SITES / WD_OPT_HOP64_SITES  sites per CTA of the fp32 / fp64 hopping kernel (a CTA has
+ *       sites * n_rhs threads, halved until <= 1024).  Range 1..1024; defaults 32 / 16.
+ *   WD_OPT_HOP32_REGS / WD_OPT_HOP64_REGS    register budget per thread: picks among the compiled
+ *       variants (fp32: 64, 128; fp64: 128, 168), clamped so that one CTA fits an SM.
+ *   WD_OPT_POLL_EVERY   inner iterations enqueued between two convergence polls of the solver (>= 1).
+ * Errors: WD_EINVAL (null, unknown key, value out of range). */
+enum { WD_OPT_HOP32_SITES = 0, WD_OPT_HOP64_SITES = 1, WD_OPT_HOP32_REGS = 2, WD_OPT_HOP64_REGS = 3,
+       WD_OPT_POLL_EVERY = 4, WD_OPT_N = 8 };
+int wd_set_option(wd_ctx* ctx, int key, int value);
+int wd_get_option(const wd_ctx* ctx, int key, int* value_host);
+
 /* Scratch memory: the caller allocates wd_workspace_bytes(ctx) bytes of device memory (256-byte
  * aligned) and hands it over; it must stay valid until wd_destroy.  wd_set_workspace uploads the
  * site tables.  Errors: WD_EINVAL (null, too small, misaligned), WD_ECUDA. */

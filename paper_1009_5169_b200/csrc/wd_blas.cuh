@@ -128,12 +128,72 @@ __device__ void finalize_global(double* scal, int n) {
 }
 
 // Block + grid reduction of K per-thread fp64 sums for column r = threadIdx.x % n, then finalize.
+// Requires blockDim.x % n == 0, blockDim.x / 32 >= n, K * blockDim.x <= 2048.  Partials are stored
+// item-major ([column * K + k][block]) so that the last block reads them coalesced; it adds them in an
+// order fixed by (gridDim, blockDim) alone, so results do not depend on block scheduling.
 template <int K, int KIND>
 __device__ void reduce_finalize(double (&v)[K], int n, RedBuf rb) {
     __shared__ double sh[4 * 512];
     __shared__ bool is_last;
     const int B = blockDim.x, t = threadIdx.x;
-    const int per = B / n;  // threads per column, a multiple of 32
+    const int per = B / n;  // threads per column
+    const int r = t % n, q = t / n;
+#pragma unroll
+    for (int k = 0; k < K; ++k) sh[k * B + r * per + q] = v[k];
+    __syncthreads();
+    const int warp = t >> 5, lane = t & 31;
+    const int nwarps = B >> 5;
+    const unsigned grid = gridDim.x;
+    if (warp < n) {
+#pragma unroll
+        for (int k = 0; k < K; ++k) {
+            double s = 0.0;
+            for (int j = lane; j < per; j += 32) s += sh[k * B + warp * per + j];
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+            if (lane == 0) rb.partials[(size_t)(warp * K + k) * grid + blockIdx.x] = s;
+        }
+    }
+    __threadfence();
+    __syncthreads();
+    if (t == 0) is_last = (atomicAdd(rb.ticket, 1u) == grid - 1);
+    __syncthreads();
+    if (!is_last) return;
+    __threadfence();
+    // last block: every thread adds a strided slice of each item's partials, then warps, then thread `item`
+    const int items = n * K;  // <= 48
+    for (int item = 0; item < items; ++item) {
+        const double* p = rb.partials + (size_t)item * grid;
+        double s = 0.0;
+        for (unsigned g = t; g < grid; g += B) s += __ldcg(p + g);
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+        if (lane == 0) sh[item * 32 + warp] = s;
+    }
+    __syncthreads();
+    if (t < items) {
+        double s = 0.0;
+        for (int w = 0; w < nwarps; ++w) s += sh[t * 32 + w];
+        sh[1536 + t] = s;
+    }
+    __syncthreads();
+    if (t < n) finalize_column<KIND>(rb.scal, t, &sh[1536 + t * K]);
+    __syncthreads();
+    if (t == 0) {
+        finalize_global<KIND>(rb.scal, n);
+        *rb.ticket = 0u;
+    }
+}
+
+// Two-kernel form for reducing kernels with very many blocks (the hop with fused inner products):
+// block_partials() is the first half of reduce_finalize (no ticket); finalize_partials_kernel, launched
+// right after with one block per (column, value) item, adds that item's partials in a fixed order, and
+// the last of those blocks runs the scalar recurrences.  `totals` is n * K doubles of scratch.
+template <int K>
+__device__ void block_partials(double (&v)[K], int n, RedBuf rb) {
+    __shared__ double sh[3 * 512];  // K * blockDim.x <= 1536
+    const int B = blockDim.x, t = threadIdx.x;
+    const int per = B / n;
     const int r = t % n, q = t / n;
 #pragma unroll
     for (int k = 0; k < K; ++k) sh[k * B + r * per + q] = v[k];
@@ -146,26 +206,40 @@ __device__ void reduce_finalize(double (&v)[K], int n, RedBuf rb) {
             for (int j = lane; j < per; j += 32) s += sh[k * B + warp * per + j];
 #pragma unroll
             for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
-            if (lane == 0) rb.partials[((long)blockIdx.x * n + warp) * K + k] = s;
+            if (lane == 0) rb.partials[(size_t)(warp * K + k) * gridDim.x + blockIdx.x] = s;
         }
     }
-    __threadfence();
+}
+
+template <int K, int KIND>
+__global__ void __launch_bounds__(256) finalize_partials_kernel(int n, unsigned nblocks, RedBuf rb, double* totals) {
+    if (rb.scal[G_DONE] != 0.0) return;
+    __shared__ double shw[8];
+    __shared__ bool is_last;
+    const int t = threadIdx.x, warp = t >> 5, lane = t & 31;
+    const double* p = rb.partials + (size_t)blockIdx.x * nblocks;
+    double s = 0.0;
+    for (unsigned g = t; g < nblocks; g += 256) s += p[g];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+    if (lane == 0) shw[warp] = s;
     __syncthreads();
-    if (t == 0) is_last = (atomicAdd(rb.ticket, 1u) == gridDim.x - 1);
+    if (t == 0) {
+        double tot = 0.0;
+        for (int w = 0; w < 8; ++w) tot += shw[w];
+        totals[blockIdx.x] = tot;
+        __threadfence();
+        is_last = (atomicAdd(rb.ticket, 1u) == gridDim.x - 1);
+    }
     __syncthreads();
     if (!is_last) return;
     __threadfence();
-    // last block: column sums in fixed block order
-    const int nwarps = B >> 5;
-    for (int item = warp; item < n * K; item += nwarps) {
-        double s = 0.0;
-        for (int g = lane; g < (int)gridDim.x; g += 32) s += rb.partials[(long)g * n * K + item];
+    if (t < n) {
+        double tot[K];
 #pragma unroll
-        for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
-        if (lane == 0) sh[item] = s;
+        for (int k = 0; k < K; ++k) tot[k] = __ldcg(totals + t * K + k);
+        finalize_column<KIND>(rb.scal, t, tot);
     }
-    __syncthreads();
-    if (t < n) finalize_column<KIND>(rb.scal, t, &sh[t * K]);
     __syncthreads();
     if (t == 0) {
         finalize_global<KIND>(rb.scal, n);

@@ -66,7 +66,11 @@ struct WsMap {
 
 const int kReals[2] = {18, 12};
 const size_t kScalDoubles = 64 * WD_MAX_RHS;
-const size_t kPartialDoubles = 4096 * 8;  // >= max blocks of any reduction * values per block
+// per column: 3 values x the largest grid of any reducing kernel (BLAS1: 4 x SMs; hop with fused dots: V/2/32 + 1)
+size_t partial_doubles(const wd_ctx* c) {
+    const size_t blocks = (size_t)c->Vh / 32 + 1 > 4096 ? (size_t)c->Vh / 32 + 1 : 4096;
+    return 3 * blocks * WD_MAX_RHS;
+}
 
 WsMap ws_map(const wd_ctx* c) {
     WsMap m;
@@ -76,7 +80,7 @@ WsMap ws_map(const wd_ctx* c) {
     for (int r = 0; r < 2; ++r) { m.u64[r] = o; o += wd_align_up(sizeof(double) * 4 * c->V * kReals[r]); }
     for (int r = 0; r < 2; ++r) { m.u32[r] = o; o += wd_align_up(sizeof(float) * 4 * c->V * kReals[r]); }
     m.scal = o;     o += wd_align_up(sizeof(double) * kScalDoubles);
-    m.partials = o; o += wd_align_up(sizeof(double) * kPartialDoubles * WD_MAX_RHS);
+    m.partials = o; o += wd_align_up(sizeof(double) * partial_doubles(c));
     m.ticket = o;   o += wd_align_up(256);
     m.solver = o;   o += wd_align_up(wd_solver_scratch_bytes(c));
     m.total = o;
@@ -120,6 +124,7 @@ int wd_create(wd_ctx** out, const int dims[4], double kappa, int time_bc, int ma
         if (V > (1L << 30)) return WD_EINVAL;
     }
     if (time_bc == WD_BC_SF && dims[3] < 4) return WD_EINVAL;
+    if (6 * V * max_rhs >= (1L << 31)) return WD_EINVAL;  // kernels index 128-bit elements with 32 bits
     int dev = 0;
     cudaDeviceProp prop;
     if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) {
@@ -142,6 +147,12 @@ int wd_create(wd_ctx** out, const int dims[4], double kappa, int time_bc, int ma
     c->ws_bytes = 0;
     c->have_ws = c->have_gauge = false;
     c->launches = 0;
+    for (int k = 0; k < WD_OPT_N; ++k) c->opt[k] = 0;
+    c->opt[WD_OPT_HOP32_SITES] = 32;
+    c->opt[WD_OPT_HOP64_SITES] = 16;
+    c->opt[WD_OPT_HOP32_REGS] = 128;
+    c->opt[WD_OPT_HOP64_REGS] = 168;
+    c->opt[WD_OPT_POLL_EVERY] = 4;
     c->prof_on = false;
     c->prof_used = 0;
     c->h_pinned = nullptr;
@@ -166,6 +177,33 @@ int wd_destroy(wd_ctx* ctx) {
     if (ctx->h_pinned) cudaFreeHost(ctx->h_pinned);
     for (cudaEvent_t e : ctx->prof_ev) cudaEventDestroy(e);
     delete ctx;
+    return WD_OK;
+}
+
+int wd_set_option(wd_ctx* ctx, int key, int value) {
+    if (!ctx) return WD_EINVAL;
+    switch (key) {
+        case WD_OPT_HOP32_SITES:
+        case WD_OPT_HOP64_SITES:
+            if (value < 1 || value > 1024) return wd_fail(ctx, WD_EINVAL, "sites per CTA out of range");
+            break;
+        case WD_OPT_HOP32_REGS:
+        case WD_OPT_HOP64_REGS:
+            if (value < 32 || value > 255) return wd_fail(ctx, WD_EINVAL, "register budget out of range");
+            break;
+        case WD_OPT_POLL_EVERY:
+            if (value < 1 || value > 1024) return wd_fail(ctx, WD_EINVAL, "poll interval out of range");
+            break;
+        default:
+            return wd_fail(ctx, WD_EINVAL, "unknown option");
+    }
+    ctx->opt[key] = value;
+    return WD_OK;
+}
+
+int wd_get_option(const wd_ctx* ctx, int key, int* value) {
+    if (!ctx || !value || key < 0 || key >= WD_OPT_N) return WD_EINVAL;
+    *value = ctx->opt[key];
     return WD_OK;
 }
 
@@ -229,6 +267,7 @@ int wd_set_workspace(wd_ctx* ctx, void* ws_dev, size_t bytes) {
     for (int r = 0; r < 2; ++r) { ctx->d_U64[r] = (double*)(w + m.u64[r]); ctx->d_U32[r] = (float*)(w + m.u32[r]); }
     ctx->d_scal = (double*)(w + m.scal);
     ctx->d_partials = (double*)(w + m.partials);
+    ctx->d_totals = ctx->d_scal + 48 * WD_MAX_RHS;  // tail of the scalar block (kScalDoubles = 64 * WD_MAX_RHS)
     ctx->d_ticket = (unsigned int*)(w + m.ticket);
     ctx->d_solver = w + m.solver;
     ctx->solver_bytes = m.total - m.solver;

@@ -11,6 +11,7 @@
 // direction inside a row of the site order.  Spin projection to half spinors happens in registers
 // (table: DESIGN.md "Half-spinor projection"), so each direction costs 2 SU(3) x colour-vector
 // products: 1320 flop per output site and RHS.
+#include "wd_blas.cuh"
 #include "wd_su3.cuh"
 
 using namespace wdk;
@@ -21,105 +22,188 @@ template <typename T>
 struct HopArgs {
     const typename Vec<T>::type* in;   // half-lattice block of parity 1-par
     typename Vec<T>::type* out;        // half-lattice block of parity par
-    const typename Vec<T>::type* in2;  // parity par, used by the XPAY epilogue
+    const typename Vec<T>::type* in2;  // parity par, used by the xpay epilogue (EPI >= 1)
+    const typename Vec<T>::type* in3;  // parity par, left operand of the fused <in3, out> (EPI == 2)
+    wdblas::RedBuf rb;                 // per-column reduction scratch and scalar table (EPI >= 2)
+    const double* done;                // nullable: the solver's "all columns converged" flag -> no-op launch
     const T* U;                        // native links of this precision and form
     const int32_t* nbr;                // [Vh][8] of parity par
-    long Vh;
-    int n;
-    int par;
+    uint32_t Vh;
+    uint32_t n;
+    uint32_t par;
+    uint32_t total;                    // Vh * n  (wd_create bounds 12 * V/2 * max_rhs below 2^31: 32-bit indices)
     T a, b;
 };
 
 // one direction: FWD: U_mu(x) psi(x+mu) with (1 - sg gamma);  !FWD: U_mu(x-mu)^dag psi(x-mu) with (1 + sg gamma)
 template <typename T, int RECON, int MU, bool FWD, bool DAG>
-__device__ __forceinline__ void hop_dir(const HopArgs<T>& A, long h, int r, long nb, cx<T> (&acc)[12]) {
+__device__ __forceinline__ void hop_dir(const HopArgs<T>& A, uint32_t h, uint32_t r, uint32_t nb, cx<T> (&acc)[12]) {
     constexpr int SIGMA = (FWD ? 1 : -1) * (DAG ? -1 : 1);
-    const long stride = A.Vh * A.n;
     cx<T> psi[12], hs[6], chi[6], u[9];
-    load_spinor(A.in, stride, nb * A.n + r, psi);
-    if (FWD) load_link<RECON>(A.U + (long)(MU * 2 + A.par) * RECON * A.Vh, A.Vh, h, u);
-    else     load_link<RECON>(A.U + (long)(MU * 2 + 1 - A.par) * RECON * A.Vh, A.Vh, nb, u);
+    load_spinor(A.in, A.total, nb * A.n + r, psi);
+    if (FWD) load_link<RECON>(A.U + (size_t)(MU * 2 + A.par) * RECON * A.Vh, A.Vh, h, u);
+    else     load_link<RECON>(A.U + (size_t)(MU * 2 + 1 - A.par) * RECON * A.Vh, A.Vh, nb, u);
     if (RECON == 12) rebuild_row3(u);
     project<MU, SIGMA>(psi, hs);
     su3_mul<!FWD>(u, hs, chi);
     accumulate<MU, SIGMA>(acc, chi);
 }
 
-template <typename T, int RECON, bool DAG, bool XPAY>
-__global__ void __launch_bounds__(128) hop_kernel(const HopArgs<T> A) {
-    const long tid = (long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (tid >= A.Vh * A.n) return;
-    const long h = tid / A.n;
-    const int r = (int)(tid - h * A.n);
-    const long stride = A.Vh * A.n;
-    const int4 n0 = __ldg(reinterpret_cast<const int4*>(A.nbr + h * WD_NDIR));
-    const int4 n1 = __ldg(reinterpret_cast<const int4*>(A.nbr + h * WD_NDIR) + 1);
+// Epilogues fused into the hop (one kernel boundary per global reduction):
+//   EPI_NONE  out = H in
+//   EPI_XPAY  out = a in2 + b H in
+//   EPI_SIGMA EPI_XPAY, then sigma_i = <in3_i, out_i> per column  -> alpha_i = rho_i / sigma_i   (in3 = r~, out = v)
+//   EPI_OMEGA EPI_XPAY, then <out_i, in2_i>, <out_i, out_i>       -> omega_i                     (in2 = s,  out = t)
+// Each CTA leaves one partial per column and value; a tiny finalize_partials_kernel (one block per item)
+// adds them in a fixed order and runs the scalar recurrence, so no dot-product kernel re-reads the vectors.
+enum { EPI_NONE = 0, EPI_XPAY = 1, EPI_SIGMA = 2, EPI_OMEGA = 3 };
+
+// Launch shape: S sites x n columns per CTA (column fastest), S = WD_OPT_HOP*_SITES.
+template <typename T, int RECON, bool DAG, int EPI, int MAXREG>
+__global__ void __maxnreg__(MAXREG) hop_kernel(const HopArgs<T> A) {
+    if (A.done != nullptr && *A.done != 0.0) return;
+    const uint32_t tid = blockIdx.x * blockDim.x + threadIdx.x;
+    const bool in_range = tid < A.total;
+    if (EPI < EPI_SIGMA && !in_range) return;
+    const uint32_t h = in_range ? tid / A.n : 0u;
+    const uint32_t r = tid - (tid / A.n) * A.n;
+    const int4 n0 = __ldg(reinterpret_cast<const int4*>(A.nbr) + 2 * h);
+    const int4 n1 = __ldg(reinterpret_cast<const int4*>(A.nbr) + 2 * h + 1);
     cx<T> acc[12];
 #pragma unroll
     for (int k = 0; k < 12; ++k) { acc[k].re = 0; acc[k].im = 0; }
-    if ((uint32_t)n0.x & WD_SITE_FROZEN) {  // SF: t = 0 stays zero
-        store_spinor(A.out, stride, tid, acc);
+    const bool frozen = ((uint32_t)n0.x & WD_SITE_FROZEN) != 0;  // SF: t = 0 stays zero
+    if (EPI < EPI_SIGMA && frozen) {
+        store_spinor(A.out, A.total, tid, acc);
         return;
     }
-    hop_dir<T, RECON, 0, true, DAG>(A, h, r, n0.x, acc);
-    hop_dir<T, RECON, 0, false, DAG>(A, h, r, n0.y, acc);
-    hop_dir<T, RECON, 1, true, DAG>(A, h, r, n0.z, acc);
-    hop_dir<T, RECON, 1, false, DAG>(A, h, r, n0.w, acc);
-    hop_dir<T, RECON, 2, true, DAG>(A, h, r, n1.x, acc);
-    hop_dir<T, RECON, 2, false, DAG>(A, h, r, n1.y, acc);
-    hop_dir<T, RECON, 3, true, DAG>(A, h, r, n1.z, acc);
-    hop_dir<T, RECON, 3, false, DAG>(A, h, r, n1.w, acc);
-    if (XPAY) {
-        cx<T> q[12];
-        load_spinor(A.in2, stride, tid, q);
+    // per-thread partial sums over the 12 components of ONE site and column in working precision
+    // (fp32: 24-72 products); everything across threads is added in fp64 (wd_blas.cuh)
+    [[maybe_unused]] T sums[3] = {0, 0, 0};
+    if (in_range && !frozen) {
+        hop_dir<T, RECON, 0, true, DAG>(A, h, r, n0.x, acc);
+        hop_dir<T, RECON, 0, false, DAG>(A, h, r, n0.y, acc);
+        hop_dir<T, RECON, 1, true, DAG>(A, h, r, n0.z, acc);
+        hop_dir<T, RECON, 1, false, DAG>(A, h, r, n0.w, acc);
+        hop_dir<T, RECON, 2, true, DAG>(A, h, r, n1.x, acc);
+        hop_dir<T, RECON, 2, false, DAG>(A, h, r, n1.y, acc);
+        hop_dir<T, RECON, 3, true, DAG>(A, h, r, n1.z, acc);
+        hop_dir<T, RECON, 3, false, DAG>(A, h, r, n1.w, acc);
+        if (EPI >= EPI_XPAY) {
+            cx<T> q[12];
+            load_spinor(A.in2, A.total, tid, q);
 #pragma unroll
-        for (int k = 0; k < 12; ++k) {
-            acc[k].re = A.a * q[k].re + A.b * acc[k].re;
-            acc[k].im = A.a * q[k].im + A.b * acc[k].im;
+            for (int k = 0; k < 12; ++k) {
+                acc[k].re = fma(A.b, acc[k].re, A.a * q[k].re);
+                acc[k].im = fma(A.b, acc[k].im, A.a * q[k].im);
+            }
+            if (EPI == EPI_OMEGA) {  // <t, s>, <t, t> with t = acc, s = q
+#pragma unroll
+                for (int k = 0; k < 12; ++k) {
+                    sums[0] = fma(acc[k].re, q[k].re, sums[0]);  sums[0] = fma(acc[k].im, q[k].im, sums[0]);
+                    sums[1] = fma(acc[k].re, q[k].im, sums[1]);  sums[1] = fma(-acc[k].im, q[k].re, sums[1]);
+                    sums[2] = fma(acc[k].re, acc[k].re, sums[2]); sums[2] = fma(acc[k].im, acc[k].im, sums[2]);
+                }
+            }
+        }
+        if (EPI == EPI_SIGMA) {  // <r~, v> with v = acc
+            cx<T> q[12];
+            load_spinor(A.in3, A.total, tid, q);
+#pragma unroll
+            for (int k = 0; k < 12; ++k) {
+                sums[0] = fma(q[k].re, acc[k].re, sums[0]);  sums[0] = fma(q[k].im, acc[k].im, sums[0]);
+                sums[1] = fma(q[k].re, acc[k].im, sums[1]);  sums[1] = fma(-q[k].im, acc[k].re, sums[1]);
+            }
         }
     }
-    store_spinor(A.out, stride, tid, acc);
+    if (in_range) store_spinor(A.out, A.total, tid, acc);
+    if (EPI == EPI_SIGMA) {  // block partials; finalize_partials_kernel follows on the stream
+        double s2[2] = {(double)sums[0], (double)sums[1]};
+        wdblas::block_partials<2>(s2, (int)A.n, A.rb);
+    } else if (EPI == EPI_OMEGA) {
+        double s3[3] = {(double)sums[0], (double)sums[1], (double)sums[2]};
+        wdblas::block_partials<3>(s3, (int)A.n, A.rb);
+    }
+}
+
+template <typename T, int RECON, int MAXREG>
+void launch_r(wd_ctx* c, const HopArgs<T>& A, int dag, int epi, unsigned G, unsigned B) {
+#define WD_HOP_CASE(D, E) hop_kernel<T, RECON, D, E, MAXREG><<<G, B, 0, c->stream>>>(A)
+    if (dag) {
+        if (epi == EPI_NONE) WD_HOP_CASE(true, EPI_NONE);
+        else if (epi == EPI_XPAY) WD_HOP_CASE(true, EPI_XPAY);
+        else if constexpr (sizeof(T) == 4) { if (epi == EPI_SIGMA) WD_HOP_CASE(true, EPI_SIGMA); else WD_HOP_CASE(true, EPI_OMEGA); }
+    } else {
+        if (epi == EPI_NONE) WD_HOP_CASE(false, EPI_NONE);
+        else if (epi == EPI_XPAY) WD_HOP_CASE(false, EPI_XPAY);
+        else if constexpr (sizeof(T) == 4) { if (epi == EPI_SIGMA) WD_HOP_CASE(false, EPI_SIGMA); else WD_HOP_CASE(false, EPI_OMEGA); }
+    }
+#undef WD_HOP_CASE
 }
 
 template <typename T, int RECON>
-void launch_t(wd_ctx* c, int dag, int n, int par, const void* in, void* out, const void* in2, double a, double b,
-              const T* U) {
+void launch_t(wd_ctx* c, int dag, int n, int par, const wd_hop_ops& o, const T* U) {
     HopArgs<T> A;
-    A.in = (const typename Vec<T>::type*)in;
-    A.out = (typename Vec<T>::type*)out;
-    A.in2 = (const typename Vec<T>::type*)in2;
+    A.in = (const typename Vec<T>::type*)o.in;
+    A.out = (typename Vec<T>::type*)o.out;
+    A.in2 = (const typename Vec<T>::type*)o.in2;
+    A.in3 = (const typename Vec<T>::type*)o.in3;
+    A.rb = wdblas::RedBuf{c->d_scal, c->d_partials, c->d_ticket};
+    A.done = o.check_done ? c->d_scal + wdblas::G_DONE : nullptr;
     A.U = U;
     A.nbr = c->d_nbr + (long)par * c->Vh * WD_NDIR;
-    A.Vh = c->Vh;
-    A.n = n;
-    A.par = par;
-    A.a = (T)a;
-    A.b = (T)b;
-    const long total = c->Vh * n;
-    const int B = 128;
-    const unsigned G = (unsigned)((total + B - 1) / B);
-    const bool xpay = in2 != nullptr;
-    if (dag) {
-        if (xpay) hop_kernel<T, RECON, true, true><<<G, B, 0, c->stream>>>(A);
-        else      hop_kernel<T, RECON, true, false><<<G, B, 0, c->stream>>>(A);
+    A.Vh = (uint32_t)c->Vh;
+    A.n = (uint32_t)n;
+    A.par = (uint32_t)par;
+    A.total = (uint32_t)(c->Vh * n);
+    A.a = (T)o.a;
+    A.b = (T)o.b;
+    const bool f64 = sizeof(T) == 8;
+    // CTA = `sites` sites x n columns; the register budget decides how many CTAs share an SM
+    int sites = c->opt[f64 ? WD_OPT_HOP64_SITES : WD_OPT_HOP32_SITES];
+    while (sites * n > 1024) sites >>= 1;
+    if (o.epi >= EPI_SIGMA) sites = 32;  // the fused reduction wants one warp per column: B / 32 >= n
+    const unsigned B = (unsigned)(sites * n);
+    const unsigned G = (A.total + B - 1) / B;
+    // largest compiled register budget that the option allows and that lets one CTA of B threads fit
+    int regs = c->opt[f64 ? WD_OPT_HOP64_REGS : WD_OPT_HOP32_REGS];
+    if ((long)regs * B > 65536) regs = (int)(65536 / B);
+    if constexpr (sizeof(T) == 8) {
+        if (regs >= 168) launch_r<T, RECON, 168>(c, A, dag, o.epi, G, B);
+        else             launch_r<T, RECON, 128>(c, A, dag, o.epi, G, B);
     } else {
-        if (xpay) hop_kernel<T, RECON, false, true><<<G, B, 0, c->stream>>>(A);
-        else      hop_kernel<T, RECON, false, false><<<G, B, 0, c->stream>>>(A);
+        if (regs >= 128) launch_r<T, RECON, 128>(c, A, dag, o.epi, G, B);
+        else             launch_r<T, RECON, 64>(c, A, dag, o.epi, G, B);
     }
+    if (o.epi == EPI_SIGMA)
+        wdblas::finalize_partials_kernel<2, wdblas::K_SIGMA><<<2 * n, 256, 0, c->stream>>>(n, G, A.rb, c->d_totals);
+    else if (o.epi == EPI_OMEGA)
+        wdblas::finalize_partials_kernel<3, wdblas::K_OMEGA><<<3 * n, 256, 0, c->stream>>>(n, G, A.rb, c->d_totals);
+    if (o.epi >= EPI_SIGMA) c->launches++;
 }
 
 }  // namespace
 
-int wd_hop_launch(wd_ctx* c, int prec, int recon, int dag, int n, int par, const void* in, void* out,
-                  const void* in2, double a, double b) {
+int wd_hop_launch_ex(wd_ctx* c, int prec, int recon, int dag, int n, int par, const wd_hop_ops& o) {
     wd_prof_scope prof(c, prec == WD_F64 ? WD_PROF_HOP64 : WD_PROF_HOP32);
+    if (o.epi >= EPI_SIGMA && prec != WD_F32) return wd_fail(c, WD_EINVAL, "fused reductions are fp32 only");
     if (prec == WD_F64) {
-        if (recon == WD_LINK18) launch_t<double, 18>(c, dag, n, par, in, out, in2, a, b, c->d_U64[0]);
-        else                    launch_t<double, 12>(c, dag, n, par, in, out, in2, a, b, c->d_U64[1]);
+        if (recon == WD_LINK18) launch_t<double, 18>(c, dag, n, par, o, c->d_U64[0]);
+        else                    launch_t<double, 12>(c, dag, n, par, o, c->d_U64[1]);
     } else {
-        if (recon == WD_LINK18) launch_t<float, 18>(c, dag, n, par, in, out, in2, a, b, c->d_U32[0]);
-        else                    launch_t<float, 12>(c, dag, n, par, in, out, in2, a, b, c->d_U32[1]);
+        if (recon == WD_LINK18) launch_t<float, 18>(c, dag, n, par, o, c->d_U32[0]);
+        else                    launch_t<float, 12>(c, dag, n, par, o, c->d_U32[1]);
     }
     WD_LAUNCH_CHECK(c);
     return WD_OK;
+}
+
+int wd_hop_launch(wd_ctx* c, int prec, int recon, int dag, int n, int par, const void* in, void* out,
+                  const void* in2, double a, double b) {
+    wd_hop_ops o;
+    o.in = in; o.out = out; o.in2 = in2; o.in3 = nullptr;
+    o.a = a; o.b = b;
+    o.epi = in2 ? EPI_XPAY : EPI_NONE;
+    o.check_done = false;
+    return wd_hop_launch_ex(c, prec, recon, dag, n, par, o);
 }

@@ -44,10 +44,13 @@ struct wd_ctx {
     // solver scratch
     double* d_scal;        // per-RHS scalars (see wd_solve.cu)
     double* d_partials;    // block partial sums
+    double* d_totals;      // 3 * WD_MAX_RHS item totals of the two-kernel reductions
     unsigned int* d_ticket;
     double* h_pinned;      // pinned host mirror for convergence polling (cudaMallocHost, small)
     char* d_solver;        // remaining scratch for solver vectors and host-path staging
     size_t solver_bytes;
+
+    int opt[WD_OPT_N];  // tunables (wd_set_option)
 
     long long launches;
     std::string err;
@@ -116,6 +119,18 @@ static inline int wd_fail(wd_ctx* c, int code, const char* msg) {
 // wd_hop.cu
 // out[h][r] = (xpay ? a * in2 + b * (H in) : H in) on output parity `par`; in/out/in2 half-lattice blocks.
 // If dots != nullptr (fp32/fp64), see wd_hop.cu for the fused reductions.
+// general form: epi = 0 none, 1 xpay (in2), 2 xpay + sigma = <in3, out> -> alpha, 3 xpay + <out,in2>, <out,out> -> omega
+// (2, 3: fp32 only, scalars land in the solver's table);  check_done: no-op when the solver's done flag is set.
+struct wd_hop_ops {
+    const void* in;
+    void* out;
+    const void* in2;
+    const void* in3;
+    double a, b;
+    int epi;
+    bool check_done;
+};
+int wd_hop_launch_ex(wd_ctx* c, int prec, int recon, int dag, int n, int par, const wd_hop_ops& o);
 int wd_hop_launch(wd_ctx* c, int prec, int recon, int dag, int n, int par, const void* in, void* out,
                   const void* in2, double a, double b);
 

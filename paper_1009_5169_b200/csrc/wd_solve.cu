@@ -53,26 +53,6 @@ __global__ void p_update_kernel(long nvec, int n, const double* __restrict__ sca
     }
 }
 
-// sigma = <Rt, V>  ->  alpha = rho / sigma
-template <typename T>
-__global__ void dot_sigma_kernel(long nvec, int n, RedBuf rb, const typename V<T>::type* __restrict__ Rt,
-                                 const typename V<T>::type* __restrict__ Vv) {
-    if (rb.scal[G_DONE] != 0.0) return;
-    WD_BLAS_PROLOGUE(T)
-    (void)r;
-    double s[2] = {0.0, 0.0};
-    for (long i = i0; i < nvec; i += stride) {
-        T a[2 * NC], v[2 * NC];
-        to_arr<T>(Rt[i], a); to_arr<T>(Vv[i], v);
-#pragma unroll
-        for (int c = 0; c < NC; ++c) {  // conj(a) * v
-            s[0] += (double)a[2 * c] * v[2 * c] + (double)a[2 * c + 1] * v[2 * c + 1];
-            s[1] += (double)a[2 * c] * v[2 * c + 1] - (double)a[2 * c + 1] * v[2 * c];
-        }
-    }
-    reduce_finalize<2, K_SIGMA>(s, n, rb);
-}
-
 // S = R - alpha V   (in place on R)
 template <typename T>
 __global__ void s_update_kernel(long nvec, int n, const double* __restrict__ scal, typename V<T>::type* __restrict__ R,
@@ -90,27 +70,6 @@ __global__ void s_update_kernel(long nvec, int n, const double* __restrict__ sca
         }
         R[i] = from_arr(a);
     }
-}
-
-// <T, S>, <T, T>  ->  omega
-template <typename T>
-__global__ void dot_omega_kernel(long nvec, int n, RedBuf rb, const typename V<T>::type* __restrict__ Tt,
-                                 const typename V<T>::type* __restrict__ S) {
-    if (rb.scal[G_DONE] != 0.0) return;
-    WD_BLAS_PROLOGUE(T)
-    (void)r;
-    double s[3] = {0.0, 0.0, 0.0};
-    for (long i = i0; i < nvec; i += stride) {
-        T a[2 * NC], v[2 * NC];
-        to_arr<T>(Tt[i], a); to_arr<T>(S[i], v);
-#pragma unroll
-        for (int c = 0; c < NC; ++c) {
-            s[0] += (double)a[2 * c] * v[2 * c] + (double)a[2 * c + 1] * v[2 * c + 1];
-            s[1] += (double)a[2 * c] * v[2 * c + 1] - (double)a[2 * c + 1] * v[2 * c];
-            s[2] += (double)a[2 * c] * a[2 * c] + (double)a[2 * c + 1] * a[2 * c + 1];
-        }
-    }
-    reduce_finalize<3, K_OMEGA>(s, n, rb);
 }
 
 // X += alpha P + omega S;  R = S - omega T;  <Rt, R>, |R|^2  ->  rho, beta, convergence flags
@@ -310,31 +269,38 @@ int wd_solve_impl(wd_ctx* c, int dag, int n, const double* Phi, double* X, doubl
         // inner fp32 BiCGStab on the normalised residual
         { wd_prof_scope pr__(c, WD_PROF_BLAS); demote_kernel<<<L32.G, L32.B, 0, st>>>(Vh, n, rb, R64, r32, rt32, x32, p32, v32); }
         WD_LAUNCH_CHECK(c);
-        const double* done = c->d_scal + G_DONE;
-        (void)done;
+        // One iteration = 3 BLAS1 kernels + 4 hops; sigma and omega are reduced inside the even-parity hops.
+        // Kernels turn into no-ops once the device-side done flag is set, so iterations are enqueued
+        // poll_every at a time and the host only looks at the flag in between.
+        const int poll_every = c->opt[WD_OPT_POLL_EVERY];
+        wd_hop_ops o;
+        o.check_done = true;
         for (int it = 1; it <= max_inner; ++it) {
             { wd_prof_scope pr__(c, WD_PROF_BLAS); p_update_kernel<float><<<L32.G, L32.B, 0, st>>>(nv32, n, c->d_scal, r32, p32, v32); }
             WD_LAUNCH_CHECK(c);
-            rc = wd_hop_launch(c, WD_F32, recon, dag, n, 1, p32, tmp32, nullptr, 0.0, 1.0);
+            // v = Ahat p, sigma = <rt, v> -> alpha
+            o.in = p32; o.out = tmp32; o.in2 = nullptr; o.in3 = nullptr; o.a = 0.0; o.b = 1.0; o.epi = 0;
+            rc = wd_hop_launch_ex(c, WD_F32, recon, dag, n, 1, o);
             if (rc) return rc;
-            rc = wd_hop_launch(c, WD_F32, recon, dag, n, 0, tmp32, v32, p32, 1.0, -kap * kap);
+            o.in = tmp32; o.out = v32; o.in2 = p32; o.in3 = rt32; o.a = 1.0; o.b = -kap * kap; o.epi = 2;
+            rc = wd_hop_launch_ex(c, WD_F32, recon, dag, n, 0, o);
             if (rc) return rc;
-            { wd_prof_scope pr__(c, WD_PROF_BLAS); dot_sigma_kernel<float><<<L32.G, L32.B, 0, st>>>(nv32, n, rb, rt32, v32); }
-            WD_LAUNCH_CHECK(c);
             { wd_prof_scope pr__(c, WD_PROF_BLAS); s_update_kernel<float><<<L32.G, L32.B, 0, st>>>(nv32, n, c->d_scal, r32, v32); }
             WD_LAUNCH_CHECK(c);
-            rc = wd_hop_launch(c, WD_F32, recon, dag, n, 1, r32, tmp32, nullptr, 0.0, 1.0);
+            // t = Ahat s, <t, s>, <t, t> -> omega
+            o.in = r32; o.out = tmp32; o.in2 = nullptr; o.in3 = nullptr; o.a = 0.0; o.b = 1.0; o.epi = 0;
+            rc = wd_hop_launch_ex(c, WD_F32, recon, dag, n, 1, o);
             if (rc) return rc;
-            rc = wd_hop_launch(c, WD_F32, recon, dag, n, 0, tmp32, t32, r32, 1.0, -kap * kap);
+            o.in = tmp32; o.out = t32; o.in2 = r32; o.in3 = nullptr; o.a = 1.0; o.b = -kap * kap; o.epi = 3;
+            rc = wd_hop_launch_ex(c, WD_F32, recon, dag, n, 0, o);
             if (rc) return rc;
-            { wd_prof_scope pr__(c, WD_PROF_BLAS); dot_omega_kernel<float><<<L32.G, L32.B, 0, st>>>(nv32, n, rb, t32, r32); }
-            WD_LAUNCH_CHECK(c);
             { wd_prof_scope pr__(c, WD_PROF_BLAS); xr_update_kernel<float><<<L32.G, L32.B, 0, st>>>(nv32, n, rb, x32, p32, r32, t32, rt32); }
             WD_LAUNCH_CHECK(c);
-            // convergence poll (every iteration for now)
-            WD_CUDA_CHECK(c, cudaMemcpyAsync(hp + G_COUNT, c->d_scal + G_DONE, sizeof(double), cudaMemcpyDeviceToHost, st));
-            WD_CUDA_CHECK(c, cudaStreamSynchronize(st));
-            if (hp[G_COUNT] != 0.0) break;
+            if (it % poll_every == 0 || it == max_inner) {
+                WD_CUDA_CHECK(c, cudaMemcpyAsync(hp + G_COUNT, c->d_scal + G_DONE, sizeof(double), cudaMemcpyDeviceToHost, st));
+                WD_CUDA_CHECK(c, cudaStreamSynchronize(st));
+                if (hp[G_COUNT] != 0.0) break;
+            }
         }
         { wd_prof_scope pr__(c, WD_PROF_BLAS); promote_kernel<<<L32.G, L32.B, 0, st>>>(Vh, n, c->d_scal, x32, (double2*)XE); }
         WD_LAUNCH_CHECK(c);

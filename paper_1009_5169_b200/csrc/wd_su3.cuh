@@ -16,33 +16,37 @@ template <> struct Vec<float> { typedef float4 type; enum { NCH = 6 }; };
 template <> struct Vec<double> { typedef double2 type; enum { NCH = 12 }; };
 
 // ---- loads / stores of one spinor (12 complex) at vec index `e` of a half-lattice block ----------
-__device__ __forceinline__ void load_spinor(const float4* __restrict__ base, long stride, long e, cx<float> (&psi)[12]) {
+template <typename I>
+__device__ __forceinline__ void load_spinor(const float4* __restrict__ base, I stride, I e, cx<float> (&psi)[12]) {
 #pragma unroll
     for (int c = 0; c < 6; ++c) {
         const float4 v = __ldg(base + c * stride + e);
         psi[2 * c].re = v.x; psi[2 * c].im = v.y; psi[2 * c + 1].re = v.z; psi[2 * c + 1].im = v.w;
     }
 }
-__device__ __forceinline__ void load_spinor(const double2* __restrict__ base, long stride, long e, cx<double> (&psi)[12]) {
+template <typename I>
+__device__ __forceinline__ void load_spinor(const double2* __restrict__ base, I stride, I e, cx<double> (&psi)[12]) {
 #pragma unroll
     for (int c = 0; c < 12; ++c) {
         const double2 v = __ldg(base + c * stride + e);
         psi[c].re = v.x; psi[c].im = v.y;
     }
 }
-__device__ __forceinline__ void store_spinor(float4* __restrict__ base, long stride, long e, const cx<float> (&psi)[12]) {
+template <typename I>
+__device__ __forceinline__ void store_spinor(float4* __restrict__ base, I stride, I e, const cx<float> (&psi)[12]) {
 #pragma unroll
     for (int c = 0; c < 6; ++c)
         base[c * stride + e] = make_float4(psi[2 * c].re, psi[2 * c].im, psi[2 * c + 1].re, psi[2 * c + 1].im);
 }
-__device__ __forceinline__ void store_spinor(double2* __restrict__ base, long stride, long e, const cx<double> (&psi)[12]) {
+template <typename I>
+__device__ __forceinline__ void store_spinor(double2* __restrict__ base, I stride, I e, const cx<double> (&psi)[12]) {
 #pragma unroll
     for (int c = 0; c < 12; ++c) base[c * stride + e] = make_double2(psi[c].re, psi[c].im);
 }
 
 // ---- link load: 9 complex, row-major; RECON==12 rebuilds row 3 = conj(row1 x row2) ----------------
-template <int RECON>
-__device__ __forceinline__ void load_link(const float* __restrict__ blk, long Vh, long h, cx<float> (&u)[9]) {
+template <int RECON, typename I>
+__device__ __forceinline__ void load_link(const float* __restrict__ blk, I Vh, I h, cx<float> (&u)[9]) {
     const float4* q = reinterpret_cast<const float4*>(blk);
 #pragma unroll
     for (int c = 0; c < (RECON == 18 ? 4 : 3); ++c) {
@@ -50,12 +54,12 @@ __device__ __forceinline__ void load_link(const float* __restrict__ blk, long Vh
         u[2 * c].re = v.x; u[2 * c].im = v.y; u[2 * c + 1].re = v.z; u[2 * c + 1].im = v.w;
     }
     if (RECON == 18) {
-        const float2 w = __ldg(reinterpret_cast<const float2*>(blk + 16 * Vh) + h);
+        const float2 w = __ldg(reinterpret_cast<const float2*>(blk) + (8 * Vh + h));
         u[8].re = w.x; u[8].im = w.y;
     }
 }
-template <int RECON>
-__device__ __forceinline__ void load_link(const double* __restrict__ blk, long Vh, long h, cx<double> (&u)[9]) {
+template <int RECON, typename I>
+__device__ __forceinline__ void load_link(const double* __restrict__ blk, I Vh, I h, cx<double> (&u)[9]) {
     const double2* q = reinterpret_cast<const double2*>(blk);
 #pragma unroll
     for (int c = 0; c < (RECON == 18 ? 9 : 6); ++c) {
@@ -65,14 +69,20 @@ __device__ __forceinline__ void load_link(const double* __restrict__ blk, long V
 }
 template <typename T>
 __device__ __forceinline__ void rebuild_row3(cx<T> (&u)[9]) {
-    // u[6+k] = conj( u[(k+1)%3] * u[3+(k+2)%3] - u[(k+2)%3] * u[3+(k+1)%3] )
+    // u[6+k] = conj( u[(k+1)%3] * u[3+(k+2)%3] - u[(k+2)%3] * u[3+(k+1)%3] ), as explicit FMA chains
 #pragma unroll
     for (int k = 0; k < 3; ++k) {
         const int a = (k + 1) % 3, b = (k + 2) % 3;
-        const T re = u[a].re * u[3 + b].re - u[a].im * u[3 + b].im - (u[b].re * u[3 + a].re - u[b].im * u[3 + a].im);
-        const T im = u[a].re * u[3 + b].im + u[a].im * u[3 + b].re - (u[b].re * u[3 + a].im + u[b].im * u[3 + a].re);
+        T re = u[a].re * u[3 + b].re;
+        re = fma(-u[a].im, u[3 + b].im, re);
+        re = fma(-u[b].re, u[3 + a].re, re);
+        re = fma(u[b].im, u[3 + a].im, re);
+        T im = u[b].re * u[3 + a].im;          // this is -Im(...)
+        im = fma(u[b].im, u[3 + a].re, im);
+        im = fma(-u[a].re, u[3 + b].im, im);
+        im = fma(-u[a].im, u[3 + b].re, im);
         u[6 + k].re = re;
-        u[6 + k].im = -im;
+        u[6 + k].im = im;
     }
 }
 
@@ -124,24 +134,27 @@ __device__ __forceinline__ void accumulate(cx<T> (&acc)[12], const cx<T> (&chi)[
     }
 }
 
-// chi_j = U h_j (ADJ = false) or U^dag h_j (ADJ = true), j = 0, 1
+// chi_j = U h_j (ADJ = false) or U^dag h_j (ADJ = true), j = 0, 1.  Written as explicit FMA chains:
+// 12 FMUL + 60 FFMA per call (the compiler may not re-associate `re += a*b - c*d` into two FMAs).
 template <bool ADJ, typename T>
 __device__ __forceinline__ void su3_mul(const cx<T> (&u)[9], const cx<T> (&hs)[6], cx<T> (&chi)[6]) {
 #pragma unroll
     for (int j = 0; j < 2; ++j)
 #pragma unroll
         for (int a = 0; a < 3; ++a) {
-            T re = 0, im = 0;
+            T re, im;
 #pragma unroll
             for (int c = 0; c < 3; ++c) {
                 const cx<T> m = ADJ ? u[c * 3 + a] : u[a * 3 + c];
                 const cx<T> v = hs[3 * j + c];
+                if (c == 0) { re = m.re * v.re; im = m.re * v.im; }
+                else        { re = fma(m.re, v.re, re); im = fma(m.re, v.im, im); }
                 if (ADJ) {  // conj(m) * v
-                    re += m.re * v.re + m.im * v.im;
-                    im += m.re * v.im - m.im * v.re;
+                    re = fma(m.im, v.im, re);
+                    im = fma(-m.im, v.re, im);
                 } else {
-                    re += m.re * v.re - m.im * v.im;
-                    im += m.re * v.im + m.im * v.re;
+                    re = fma(-m.im, v.im, re);
+                    im = fma(m.im, v.re, im);
                 }
             }
             chi[3 * j + a].re = re;

@@ -27,12 +27,13 @@ F64, F32 = 0, 1
 LINK18, LINK12 = 0, 1
 ORDER_LINEAR, ORDER_TILED = 0, 1
 MAX_RHS = 16
+OPT_HOP32_SITES, OPT_HOP64_SITES, OPT_HOP32_REGS, OPT_HOP64_REGS, OPT_POLL_EVERY = 0, 1, 2, 3, 4
 PROF_NAMES = ("hop32", "hop64", "blas", "force", "layout")
 PROF_N = len(PROF_NAMES)
 
 # every symbol include/wd.h declares (tests check that the library exports each one)
 SYMBOLS = ["wd_create", "wd_destroy", "wd_site_order", "wd_workspace_bytes", "wd_set_workspace",
-           "wd_set_gauge", "wd_native_bytes", "wd_pack", "wd_unpack", "wd_apply", "wd_hop",
+           "wd_set_option", "wd_get_option", "wd_set_gauge", "wd_native_bytes", "wd_pack", "wd_unpack", "wd_apply", "wd_hop",
            "wd_solve_block", "wd_force", "wd_md_force_host", "wd_profile", "wd_profile_read", "wd_launch_count", "wd_strerror",
            "wd_last_error", "wd_version"]
 
@@ -73,6 +74,8 @@ def lib():
     L.wd_create.argtypes = [ctypes.POINTER(vp), ip, cd, ci, ci, vp]
     L.wd_destroy.argtypes = [vp]
     L.wd_site_order.argtypes = [vp, ci, ip]
+    L.wd_set_option.argtypes = [vp, ci, ci]
+    L.wd_get_option.argtypes = [vp, ci, ip]
     L.wd_workspace_bytes.argtypes = [vp]
     L.wd_workspace_bytes.restype = sz
     L.wd_set_workspace.argtypes = [vp, vp, sz]
@@ -95,7 +98,7 @@ def lib():
     L.wd_last_error.argtypes = [vp]
     L.wd_last_error.restype = ctypes.c_char_p
     L.wd_version.restype = ctypes.c_char_p
-    for name in ("wd_create", "wd_destroy", "wd_site_order", "wd_set_workspace", "wd_set_gauge", "wd_pack",
+    for name in ("wd_create", "wd_destroy", "wd_site_order", "wd_set_option", "wd_get_option", "wd_set_workspace", "wd_set_gauge", "wd_pack",
                  "wd_unpack", "wd_apply", "wd_hop", "wd_solve_block", "wd_force", "wd_md_force_host", "wd_profile",
                  "wd_profile_read"):
         getattr(L, name).restype = ci
@@ -246,6 +249,14 @@ class Context:
         cnt = (ctypes.c_longlong * PROF_N)()
         self._check(self.L.wd_profile_read(self._h, ms, cnt))
         return {name: (ms[i], int(cnt[i])) for i, name in enumerate(PROF_NAMES)}
+
+    def set_option(self, key, value):
+        self._check(self.L.wd_set_option(self._h, int(key), int(value)))
+
+    def get_option(self, key):
+        v = ctypes.c_int()
+        self._check(self.L.wd_get_option(self._h, int(key), ctypes.byref(v)))
+        return v.value
 
     def launch_count(self):
         return int(self.L.wd_launch_count(self._h))
