@@ -88,10 +88,15 @@ int wd_site_order(wd_ctx* ctx, int order, const int tile[4]);
  *       sites * n_rhs threads, halved until <= 1024).  Range 1..1024; defaults 32 / 16.
  *   WD_OPT_HOP32_REGS / WD_OPT_HOP64_REGS    register budget per thread: picks among the compiled
  *       variants (fp32: 64, 128; fp64: 128, 168), clamped so that one CTA fits an SM.
+ *   WD_OPT_HOP_IMPL     0 (default): the register kernel (one thread per site and column, operands loaded
+ *       straight into registers).  1: the kernel that stages whole lattice rows through shared memory with
+ *       bulk copies (cp.async.bulk + mbarrier, persistent CTAs, producer/consumer warps) wherever it applies
+ *       (linear site order; else the register kernel runs).  Same results bit for bit; 0 is faster up to
+ *       n_rhs ~ 8, 1 from n_rhs ~ 12 (measured at 24^4).
  *   WD_OPT_POLL_EVERY   inner iterations enqueued between two convergence polls of the solver (>= 1).
  * Errors: WD_EINVAL (null, unknown key, value out of range). */
 enum { WD_OPT_HOP32_SITES = 0, WD_OPT_HOP64_SITES = 1, WD_OPT_HOP32_REGS = 2, WD_OPT_HOP64_REGS = 3,
-       WD_OPT_POLL_EVERY = 4, WD_OPT_N = 8 };
+       WD_OPT_POLL_EVERY = 4, WD_OPT_HOP_IMPL = 5, WD_OPT_N = 8 };
 int wd_set_option(wd_ctx* ctx, int key, int value);
 int wd_get_option(const wd_ctx* ctx, int key, int* value_host);
 

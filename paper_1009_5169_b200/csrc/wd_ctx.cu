@@ -191,6 +191,9 @@ int wd_set_option(wd_ctx* ctx, int key, int value) {
         case WD_OPT_HOP64_REGS:
             if (value < 32 || value > 255) return wd_fail(ctx, WD_EINVAL, "register budget out of range");
             break;
+        case WD_OPT_HOP_IMPL:
+            if (value != 0 && value != 1) return wd_fail(ctx, WD_EINVAL, "hop implementation is 0 or 1");
+            break;
         case WD_OPT_POLL_EVERY:
             if (value < 1 || value > 1024) return wd_fail(ctx, WD_EINVAL, "poll interval out of range");
             break;

@@ -187,6 +187,13 @@ void launch_t(wd_ctx* c, int dag, int n, int par, const wd_hop_ops& o, const T* 
 int wd_hop_launch_ex(wd_ctx* c, int prec, int recon, int dag, int n, int par, const wd_hop_ops& o) {
     wd_prof_scope prof(c, prec == WD_F64 ? WD_PROF_HOP64 : WD_PROF_HOP32);
     if (o.epi >= EPI_SIGMA && prec != WD_F32) return wd_fail(c, WD_EINVAL, "fused reductions are fp32 only");
+    if (c->opt[WD_OPT_HOP_IMPL] == 1) {  // shared-memory-staged kernel where it applies, else fall through
+        const int rc = wd_hop_tma_launch(c, prec, recon, dag, n, par, o);
+        if (rc <= 0) {
+            if (rc == WD_OK) WD_LAUNCH_CHECK(c);
+            return rc;
+        }
+    }
     if (prec == WD_F64) {
         if (recon == WD_LINK18) launch_t<double, 18>(c, dag, n, par, o, c->d_U64[0]);
         else                    launch_t<double, 12>(c, dag, n, par, o, c->d_U64[1]);

@@ -131,6 +131,8 @@ struct wd_hop_ops {
     bool check_done;
 };
 int wd_hop_launch_ex(wd_ctx* c, int prec, int recon, int dag, int n, int par, const wd_hop_ops& o);
+// wd_hop_tma.cu: the shared-memory-staged (bulk copy + mbarrier) form; > 0 = not applicable, use the plain kernel
+int wd_hop_tma_launch(wd_ctx* c, int prec, int recon, int dag, int n, int par, const wd_hop_ops& o);
 int wd_hop_launch(wd_ctx* c, int prec, int recon, int dag, int n, int par, const void* in, void* out,
                   const void* in2, double a, double b);
 

@@ -229,3 +229,94 @@ def test_error_codes():
     assert L.wd_apply(ctx._h, 0, 0, 0, 2, ctypes.c_void_p(t.data_ptr()), ctypes.c_void_p(t.data_ptr())) == pkg.wd.EINVAL
     assert L.wd_apply(ctx._h, 0, 0, 0, 2, ctypes.c_void_p(t.data_ptr()), ctypes.c_void_p(o.data_ptr())) == pkg.wd.OK
     ctx.close()
+
+
+# ---- the two hopping-kernel implementations and the launch tunables (WD_OPT_*) -------------------------
+STAGED_CASES = [
+    # dims, bc, n_rhs  (linear site order; Lx/2 even and odd, row groups with and without y wrap-around)
+    ((4, 4, 4, 4), wi.BC_SF, 5),
+    ((8, 4, 6, 4), wi.BC_PERIODIC, 3),
+    ((12, 8, 4, 6), wi.BC_SF, 5),
+    ((6, 4, 4, 4), wi.BC_PERIODIC, 2),      # Lx/2 odd: 18-real fp32 links fall back to the register kernel
+    ((2, 2, 2, 4), wi.BC_SF, 12),
+    ((8, 8, 8, 8), wi.BC_SF, 16),
+]
+
+
+@pytest.mark.parametrize("dims,bc,n_rhs", STAGED_CASES)
+def test_staged_hop_kernel_matches_oracle_and_register_kernel(dims, bc, n_rhs):
+    """WD_OPT_HOP_IMPL = 1 (bulk-copy staged kernel): parity with the oracle at the D-apply tolerances and
+    bit-for-bit agreement with the register kernel (same per-site arithmetic in the same order)."""
+    pkg = _wd()
+    kappa = 0.13
+    U = wi.gauge_field(dims, 0.4, 7, bc)
+    psi = wi.spinor_field(dims, n_rhs, 11, bc)
+    ctx = make_ctx(dims, kappa, bc, n_rhs, U)
+    for op in (0, 1):
+        ref64 = orc.apply(dims, kappa, bc, op, U, psi)
+        ref32 = orc.apply(dims, kappa, bc, op, U.astype(np.float32).astype(np.float64),
+                          psi.astype(np.float32).astype(np.float64))
+        for prec, ref, tol in ((pkg.F64, ref64, 1e-13), (pkg.F32, ref32, 1e-5)):
+            nat = ctx.pack(dev(psi), prec)
+            for recon in (pkg.LINK18, pkg.LINK12):
+                ctx.set_option(pkg.OPT_HOP_IMPL, 0)
+                a = ctx.apply(op, nat, n_rhs, prec, recon)
+                ctx.set_option(pkg.OPT_HOP_IMPL, 1)
+                b = ctx.apply(op, nat, n_rhs, prec, recon)
+                assert torch.equal(a, b), (op, prec, recon)
+                out = ctx.unpack(b, n_rhs, prec).cpu().numpy()
+                assert rel_per_rhs(out, ref).max() < tol, (op, prec, recon)
+    ctx.close()
+
+
+@pytest.mark.parametrize("impl", [0, 1])
+@pytest.mark.parametrize("recon", [0, 1])
+def test_solve_and_force_with_either_hop_kernel(impl, recon):
+    """The fused <rt,v> / <t,s>,<t,t> epilogues of both hop kernels drive the inner BiCGStab: X, Y, F parity."""
+    pkg = _wd()
+    cfg, U, Phi = wi.make_config(1, 3)
+    dims, kappa, bc, n = cfg["dims"], cfg["kappa"], cfg["bc"], cfg["n_rhs"]
+    Xr, rr, _, rc = orc.solve(dims, kappa, bc, 0, U, Phi, tol=1e-14)
+    Yr, rr, _, rc = orc.solve(dims, kappa, bc, 1, U, Xr, tol=1e-14)
+    Fr = orc.force(dims, kappa, bc, U, Xr, Yr)
+    ctx = make_ctx(dims, kappa, bc, n, U)
+    ctx.set_option(pkg.OPT_HOP_IMPL, impl)
+    P = ctx.pack(dev(Phi))
+    X, ix = ctx.solve_block(pkg.OP_D, P, n, tol=1e-12, recon=recon)
+    Y, iy = ctx.solve_block(pkg.OP_DDAG, X, n, tol=1e-12, recon=recon)
+    F = ctx.force(X, Y, n).cpu().numpy()
+    assert ix["converged"] and iy["converged"]
+    assert rel_per_rhs(ctx.unpack(X, n).cpu().numpy(), Xr).max() < 1e-9
+    assert rel_per_rhs(ctx.unpack(Y, n).cpu().numpy(), Yr).max() < 1e-9
+    assert np.linalg.norm(F - Fr) / np.linalg.norm(Fr) < 1e-9
+    ctx.close()
+
+
+def test_launch_options_change_speed_only():
+    """CTA shape, register budget and poll interval never change results; bad keys and values are rejected."""
+    pkg = _wd()
+    dims, bc, n = (8, 4, 6, 10), wi.BC_SF, 5
+    U = wi.gauge_field(dims, 0.3, 7, bc)
+    psi = wi.spinor_field(dims, n, 11, bc)
+    ctx = make_ctx(dims, 0.13, bc, n, U)
+    assert ctx.get_option(pkg.OPT_HOP_IMPL) == 0
+    for prec, ks, kr, sites, regs in ((pkg.F32, pkg.OPT_HOP32_SITES, pkg.OPT_HOP32_REGS, (7, 16, 32, 64, 1024), (64, 128)),
+                                      (pkg.F64, pkg.OPT_HOP64_SITES, pkg.OPT_HOP64_REGS, (5, 16, 32, 64), (128, 168, 255))):
+        nat = ctx.pack(dev(psi), prec)
+        ref = ctx.apply(0, nat, n, prec, pkg.LINK12)
+        for s in sites:
+            for r in regs:
+                ctx.set_option(ks, s)
+                ctx.set_option(kr, r)
+                assert torch.equal(ctx.apply(0, nat, n, prec, pkg.LINK12), ref), (prec, s, r)
+    for key, val in ((99, 1), (pkg.OPT_HOP32_SITES, 0), (pkg.OPT_HOP32_REGS, 1000), (pkg.OPT_POLL_EVERY, 0),
+                     (pkg.OPT_HOP_IMPL, 2)):
+        with pytest.raises(pkg.WdError):
+            ctx.set_option(key, val)
+    P = ctx.pack(dev(psi))
+    ctx.set_option(pkg.OPT_POLL_EVERY, 1)
+    X1, i1 = ctx.solve_block(pkg.OP_D, P, n)
+    ctx.set_option(pkg.OPT_POLL_EVERY, 7)
+    X7, i7 = ctx.solve_block(pkg.OP_D, P, n)
+    assert torch.equal(X1, X7) and i1["inner_iters_total"] == i7["inner_iters_total"]
+    ctx.close()
