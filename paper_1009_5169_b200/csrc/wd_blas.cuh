@@ -191,22 +191,22 @@ __device__ void reduce_finalize(double (&v)[K], int n, RedBuf rb) {
 // the last of those blocks runs the scalar recurrences.  `totals` is n * K doubles of scratch.
 template <int K>
 __device__ void block_partials(double (&v)[K], int n, RedBuf rb) {
-    __shared__ double sh[3 * 512];  // K * blockDim.x <= 1536
+    __shared__ double sh[3 * 512];  // K * blockDim.x <= 1536; blockDim.x a multiple of 32 and of n
     const int B = blockDim.x, t = threadIdx.x;
     const int per = B / n;
     const int r = t % n, q = t / n;
 #pragma unroll
     for (int k = 0; k < K; ++k) sh[k * B + r * per + q] = v[k];
     __syncthreads();
-    const int warp = t >> 5, lane = t & 31;
-    if (warp < n) {
+    const int warp = t >> 5, lane = t & 31, nwarps = B >> 5;
+    for (int col = warp; col < n; col += nwarps) {
 #pragma unroll
         for (int k = 0; k < K; ++k) {
             double s = 0.0;
-            for (int j = lane; j < per; j += 32) s += sh[k * B + warp * per + j];
+            for (int j = lane; j < per; j += 32) s += sh[k * B + col * per + j];
 #pragma unroll
             for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
-            if (lane == 0) rb.partials[(size_t)(warp * K + k) * gridDim.x + blockIdx.x] = s;
+            if (lane == 0) rb.partials[(size_t)(col * K + k) * gridDim.x + blockIdx.x] = s;
         }
     }
 }

@@ -148,11 +148,9 @@ int wd_create(wd_ctx** out, const int dims[4], double kappa, int time_bc, int ma
     c->have_ws = c->have_gauge = false;
     c->launches = 0;
     for (int k = 0; k < WD_OPT_N; ++k) c->opt[k] = 0;
-    c->opt[WD_OPT_HOP32_SITES] = 32;
-    c->opt[WD_OPT_HOP64_SITES] = 16;
-    c->opt[WD_OPT_HOP32_REGS] = 128;
-    c->opt[WD_OPT_HOP64_REGS] = 168;
+    // hop CTA shape and register budget: 0 = chosen per launch from n_rhs (wd_hop.cu)
     c->opt[WD_OPT_POLL_EVERY] = 4;
+    c->opt[WD_OPT_ALTERNATE_SWEEP] = 1;
     c->prof_on = false;
     c->prof_used = 0;
     c->h_pinned = nullptr;
@@ -185,14 +183,15 @@ int wd_set_option(wd_ctx* ctx, int key, int value) {
     switch (key) {
         case WD_OPT_HOP32_SITES:
         case WD_OPT_HOP64_SITES:
-            if (value < 1 || value > 1024) return wd_fail(ctx, WD_EINVAL, "sites per CTA out of range");
+            if (value < 0 || value > 1024) return wd_fail(ctx, WD_EINVAL, "sites per CTA out of range");
             break;
         case WD_OPT_HOP32_REGS:
         case WD_OPT_HOP64_REGS:
-            if (value < 32 || value > 255) return wd_fail(ctx, WD_EINVAL, "register budget out of range");
+            if (value != 0 && (value < 32 || value > 255)) return wd_fail(ctx, WD_EINVAL, "register budget out of range");
             break;
         case WD_OPT_HOP_IMPL:
-            if (value != 0 && value != 1) return wd_fail(ctx, WD_EINVAL, "hop implementation is 0 or 1");
+        case WD_OPT_ALTERNATE_SWEEP:
+            if (value != 0 && value != 1) return wd_fail(ctx, WD_EINVAL, "this option is 0 or 1");
             break;
         case WD_OPT_POLL_EVERY:
             if (value < 1 || value > 1024) return wd_fail(ctx, WD_EINVAL, "poll interval out of range");

@@ -31,6 +31,7 @@ struct HopArgs {
     uint32_t Vh;
     uint32_t n;
     uint32_t par;
+    uint32_t rev;                      // 1: CTA b works on block gridDim-1-b
     uint32_t total;                    // Vh * n  (wd_create bounds 12 * V/2 * max_rhs below 2^31: 32-bit indices)
     T a, b;
 };
@@ -62,7 +63,7 @@ enum { EPI_NONE = 0, EPI_XPAY = 1, EPI_SIGMA = 2, EPI_OMEGA = 3 };
 template <typename T, int RECON, bool DAG, int EPI, int MAXREG>
 __global__ void __maxnreg__(MAXREG) hop_kernel(const HopArgs<T> A) {
     if (A.done != nullptr && *A.done != 0.0) return;
-    const uint32_t tid = blockIdx.x * blockDim.x + threadIdx.x;
+    const uint32_t tid = (A.rev ? gridDim.x - 1 - blockIdx.x : blockIdx.x) * blockDim.x + threadIdx.x;
     const bool in_range = tid < A.total;
     if (EPI < EPI_SIGMA && !in_range) return;
     const uint32_t h = in_range ? tid / A.n : 0u;
@@ -155,18 +156,29 @@ void launch_t(wd_ctx* c, int dag, int n, int par, const wd_hop_ops& o, const T* 
     A.Vh = (uint32_t)c->Vh;
     A.n = (uint32_t)n;
     A.par = (uint32_t)par;
+    A.rev = o.rev ? 1u : 0u;
     A.total = (uint32_t)(c->Vh * n);
     A.a = (T)o.a;
     A.b = (T)o.b;
     const bool f64 = sizeof(T) == 8;
-    // CTA = `sites` sites x n columns; the register budget decides how many CTAs share an SM
+    // CTA = `sites` sites x n columns.  Measured at 24^4 (fp32, R=12): about 64-160 threads per CTA is best for
+    // every n_rhs (n=5: 32 sites, n=8: 8-16, n=12, 16: 8), and 64 registers (more CTAs per SM) from n = 3 up.
     int sites = c->opt[f64 ? WD_OPT_HOP64_SITES : WD_OPT_HOP32_SITES];
-    while (sites * n > 1024) sites >>= 1;
-    if (o.epi >= EPI_SIGMA) sites = 32;  // the fused reduction wants one warp per column: B / 32 >= n
+    const bool fused = o.epi >= EPI_SIGMA;
+    if (sites == 0) {
+        sites = 32;
+        if (!f64)
+            for (int s = 8; s < 32; s <<= 1)
+                if ((s * n) % 32 == 0 && s * n >= 64) { sites = s; break; }
+        if (f64) sites = 16;
+    }
+    while (sites * n > (fused ? 512 : 1024)) sites >>= 1;
+    if (fused && (sites * n) % 32 != 0) sites = 32;  // the block reduction shuffles whole warps (n <= 16: 512 threads)
     const unsigned B = (unsigned)(sites * n);
     const unsigned G = (A.total + B - 1) / B;
     // largest compiled register budget that the option allows and that lets one CTA of B threads fit
     int regs = c->opt[f64 ? WD_OPT_HOP64_REGS : WD_OPT_HOP32_REGS];
+    if (regs == 0) regs = f64 ? 168 : ((n <= 2 || RECON == 18) ? 128 : 64);  // 18-real links: 64 registers spill
     if ((long)regs * B > 65536) regs = (int)(65536 / B);
     if constexpr (sizeof(T) == 8) {
         if (regs >= 168) launch_r<T, RECON, 168>(c, A, dag, o.epi, G, B);
@@ -212,5 +224,6 @@ int wd_hop_launch(wd_ctx* c, int prec, int recon, int dag, int n, int par, const
     o.a = a; o.b = b;
     o.epi = in2 ? EPI_XPAY : EPI_NONE;
     o.check_done = false;
+    o.rev = 0;
     return wd_hop_launch_ex(c, prec, recon, dag, n, par, o);
 }

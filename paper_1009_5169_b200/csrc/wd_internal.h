@@ -129,6 +129,7 @@ struct wd_hop_ops {
     double a, b;
     int epi;
     bool check_done;
+    int rev;  // 1: sweep the sites from the top (L2 reuse between consecutive kernels)
 };
 int wd_hop_launch_ex(wd_ctx* c, int prec, int recon, int dag, int n, int par, const wd_hop_ops& o);
 // wd_hop_tma.cu: the shared-memory-staged (bulk copy + mbarrier) form; > 0 = not applicable, use the plain kernel

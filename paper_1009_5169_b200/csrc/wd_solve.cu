@@ -29,17 +29,19 @@ __device__ __forceinline__ double2 from_arr(const double (&a)[2]) { return make_
     constexpr int NC = V<T>::NC;                                                   \
     const int r = threadIdx.x % n;                                                 \
     const long stride = (long)gridDim.x * blockDim.x;                              \
-    const long i0 = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    const long i0 = (long)blockIdx.x * blockDim.x + threadIdx.x;                   \
+    const long cnt = i0 < nvec ? (nvec - 1 - i0) / stride + 1 : 0;
 
 // P = R + beta (P - omega V)
 template <typename T>
-__global__ void p_update_kernel(long nvec, int n, const double* __restrict__ scal, const typename V<T>::type* __restrict__ R,
+__global__ void p_update_kernel(long nvec, int n, int rev, const double* __restrict__ scal, const typename V<T>::type* __restrict__ R,
                                 typename V<T>::type* __restrict__ P, const typename V<T>::type* __restrict__ Vv) {
     if (scal[G_DONE] != 0.0) return;
     WD_BLAS_PROLOGUE(T)
     const T br = (T)scal[S_BETA_RE * WD_MAX_RHS + r], bi = (T)scal[S_BETA_IM * WD_MAX_RHS + r];
     const T wr = (T)scal[S_OMEGA_RE * WD_MAX_RHS + r], wi = (T)scal[S_OMEGA_IM * WD_MAX_RHS + r];
-    for (long i = i0; i < nvec; i += stride) {
+    for (long k = 0; k < cnt; ++k) {
+        const long i = i0 + (rev ? cnt - 1 - k : k) * stride;  // rev: sweep from the top, see wd_solve_impl
         T a[2 * NC], p[2 * NC], v[2 * NC];
         to_arr<T>(R[i], a); to_arr<T>(P[i], p); to_arr<T>(Vv[i], v);
 #pragma unroll
@@ -55,12 +57,13 @@ __global__ void p_update_kernel(long nvec, int n, const double* __restrict__ sca
 
 // S = R - alpha V   (in place on R)
 template <typename T>
-__global__ void s_update_kernel(long nvec, int n, const double* __restrict__ scal, typename V<T>::type* __restrict__ R,
+__global__ void s_update_kernel(long nvec, int n, int rev, const double* __restrict__ scal, typename V<T>::type* __restrict__ R,
                                 const typename V<T>::type* __restrict__ Vv) {
     if (scal[G_DONE] != 0.0) return;
     WD_BLAS_PROLOGUE(T)
     const T ar = (T)scal[S_ALPHA_RE * WD_MAX_RHS + r], ai = (T)scal[S_ALPHA_IM * WD_MAX_RHS + r];
-    for (long i = i0; i < nvec; i += stride) {
+    for (long k = 0; k < cnt; ++k) {
+        const long i = i0 + (rev ? cnt - 1 - k : k) * stride;  // rev: sweep from the top, see wd_solve_impl
         T a[2 * NC], v[2 * NC];
         to_arr<T>(R[i], a); to_arr<T>(Vv[i], v);
 #pragma unroll
@@ -74,7 +77,7 @@ __global__ void s_update_kernel(long nvec, int n, const double* __restrict__ sca
 
 // X += alpha P + omega S;  R = S - omega T;  <Rt, R>, |R|^2  ->  rho, beta, convergence flags
 template <typename T>
-__global__ void xr_update_kernel(long nvec, int n, RedBuf rb, typename V<T>::type* __restrict__ X,
+__global__ void xr_update_kernel(long nvec, int n, int rev, RedBuf rb, typename V<T>::type* __restrict__ X,
                                  const typename V<T>::type* __restrict__ P, typename V<T>::type* __restrict__ R,
                                  const typename V<T>::type* __restrict__ Tt, const typename V<T>::type* __restrict__ Rt) {
     if (rb.scal[G_DONE] != 0.0) return;
@@ -83,7 +86,8 @@ __global__ void xr_update_kernel(long nvec, int n, RedBuf rb, typename V<T>::typ
     const T ar = (T)scal[S_ALPHA_RE * WD_MAX_RHS + r], ai = (T)scal[S_ALPHA_IM * WD_MAX_RHS + r];
     const T wr = (T)scal[S_OMEGA_RE * WD_MAX_RHS + r], wi = (T)scal[S_OMEGA_IM * WD_MAX_RHS + r];
     double s[3] = {0.0, 0.0, 0.0};
-    for (long i = i0; i < nvec; i += stride) {
+    for (long k = 0; k < cnt; ++k) {
+        const long i = i0 + (rev ? cnt - 1 - k : k) * stride;  // rev: sweep from the top, see wd_solve_impl
         T x[2 * NC], p[2 * NC], sv[2 * NC], t[2 * NC], q[2 * NC];
         to_arr<T>(X[i], x); to_arr<T>(P[i], p); to_arr<T>(R[i], sv); to_arr<T>(Tt[i], t); to_arr<T>(Rt[i], q);
 #pragma unroll
@@ -273,28 +277,36 @@ int wd_solve_impl(wd_ctx* c, int dag, int n, const double* Phi, double* X, doubl
         // Kernels turn into no-ops once the device-side done flag is set, so iterations are enqueued
         // poll_every at a time and the host only looks at the flag in between.
         const int poll_every = c->opt[WD_OPT_POLL_EVERY];
+        // Consecutive kernels sweep the vectors in opposite directions: what one kernel wrote last (and the
+        // 126 MB L2 still holds) is what the next one reads first.
+        int sweep_dir = 0;
+        auto sweep = [&]() { sweep_dir ^= c->opt[WD_OPT_ALTERNATE_SWEEP] ? 1 : 0; return sweep_dir; };
         wd_hop_ops o;
         o.check_done = true;
         for (int it = 1; it <= max_inner; ++it) {
-            { wd_prof_scope pr__(c, WD_PROF_BLAS); p_update_kernel<float><<<L32.G, L32.B, 0, st>>>(nv32, n, c->d_scal, r32, p32, v32); }
+            { wd_prof_scope pr__(c, WD_PROF_BLAS); p_update_kernel<float><<<L32.G, L32.B, 0, st>>>(nv32, n, sweep(), c->d_scal, r32, p32, v32); }
             WD_LAUNCH_CHECK(c);
             // v = Ahat p, sigma = <rt, v> -> alpha
             o.in = p32; o.out = tmp32; o.in2 = nullptr; o.in3 = nullptr; o.a = 0.0; o.b = 1.0; o.epi = 0;
+            o.rev = sweep();
             rc = wd_hop_launch_ex(c, WD_F32, recon, dag, n, 1, o);
             if (rc) return rc;
             o.in = tmp32; o.out = v32; o.in2 = p32; o.in3 = rt32; o.a = 1.0; o.b = -kap * kap; o.epi = 2;
+            o.rev = sweep();
             rc = wd_hop_launch_ex(c, WD_F32, recon, dag, n, 0, o);
             if (rc) return rc;
-            { wd_prof_scope pr__(c, WD_PROF_BLAS); s_update_kernel<float><<<L32.G, L32.B, 0, st>>>(nv32, n, c->d_scal, r32, v32); }
+            { wd_prof_scope pr__(c, WD_PROF_BLAS); s_update_kernel<float><<<L32.G, L32.B, 0, st>>>(nv32, n, sweep(), c->d_scal, r32, v32); }
             WD_LAUNCH_CHECK(c);
             // t = Ahat s, <t, s>, <t, t> -> omega
             o.in = r32; o.out = tmp32; o.in2 = nullptr; o.in3 = nullptr; o.a = 0.0; o.b = 1.0; o.epi = 0;
+            o.rev = sweep();
             rc = wd_hop_launch_ex(c, WD_F32, recon, dag, n, 1, o);
             if (rc) return rc;
             o.in = tmp32; o.out = t32; o.in2 = r32; o.in3 = nullptr; o.a = 1.0; o.b = -kap * kap; o.epi = 3;
+            o.rev = sweep();
             rc = wd_hop_launch_ex(c, WD_F32, recon, dag, n, 0, o);
             if (rc) return rc;
-            { wd_prof_scope pr__(c, WD_PROF_BLAS); xr_update_kernel<float><<<L32.G, L32.B, 0, st>>>(nv32, n, rb, x32, p32, r32, t32, rt32); }
+            { wd_prof_scope pr__(c, WD_PROF_BLAS); xr_update_kernel<float><<<L32.G, L32.B, 0, st>>>(nv32, n, sweep(), rb, x32, p32, r32, t32, rt32); }
             WD_LAUNCH_CHECK(c);
             if (it % poll_every == 0 || it == max_inner) {
                 WD_CUDA_CHECK(c, cudaMemcpyAsync(hp + G_COUNT, c->d_scal + G_DONE, sizeof(double), cudaMemcpyDeviceToHost, st));

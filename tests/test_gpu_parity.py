@@ -300,7 +300,7 @@ def test_launch_options_change_speed_only():
     psi = wi.spinor_field(dims, n, 11, bc)
     ctx = make_ctx(dims, 0.13, bc, n, U)
     assert ctx.get_option(pkg.OPT_HOP_IMPL) == 0
-    for prec, ks, kr, sites, regs in ((pkg.F32, pkg.OPT_HOP32_SITES, pkg.OPT_HOP32_REGS, (7, 16, 32, 64, 1024), (64, 128)),
+    for prec, ks, kr, sites, regs in ((pkg.F32, pkg.OPT_HOP32_SITES, pkg.OPT_HOP32_REGS, (0, 7, 16, 32, 64, 1024), (0, 64, 128)),
                                       (pkg.F64, pkg.OPT_HOP64_SITES, pkg.OPT_HOP64_REGS, (5, 16, 32, 64), (128, 168, 255))):
         nat = ctx.pack(dev(psi), prec)
         ref = ctx.apply(0, nat, n, prec, pkg.LINK12)
@@ -309,7 +309,7 @@ def test_launch_options_change_speed_only():
                 ctx.set_option(ks, s)
                 ctx.set_option(kr, r)
                 assert torch.equal(ctx.apply(0, nat, n, prec, pkg.LINK12), ref), (prec, s, r)
-    for key, val in ((99, 1), (pkg.OPT_HOP32_SITES, 0), (pkg.OPT_HOP32_REGS, 1000), (pkg.OPT_POLL_EVERY, 0),
+    for key, val in ((99, 1), (pkg.OPT_HOP32_SITES, -1), (pkg.OPT_HOP32_REGS, 1000), (pkg.OPT_POLL_EVERY, 0),
                      (pkg.OPT_HOP_IMPL, 2)):
         with pytest.raises(pkg.WdError):
             ctx.set_option(key, val)
