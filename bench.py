@@ -41,6 +41,8 @@ def parse_args():
     ap.add_argument("--n-rhs", type=int, default=5)
     ap.add_argument("--recon", type=int, default=12, choices=(12, 18), help="inner fp32 link form")
     ap.add_argument("--impl", default="ours", choices=("ours", "reference"))
+    ap.add_argument("--hop-impl", type=int, default=-1, choices=(-1, 0, 1),
+                    help="WD_OPT_HOP_IMPL: 0 register kernel, 1 shared-memory-staged kernel, -1 library default")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-hop-sweep", action="store_true")
     return ap.parse_args()
@@ -256,6 +258,8 @@ def run_ours(args):
     Phi = wi.spinor_field(dims, n, cfg["seed"], bc)
 
     ctx = pkg.Context(dims, kappa, bc=bc, max_rhs=n, device=f"cuda:{local}")
+    if args.hop_impl >= 0:
+        ctx.set_option(pkg.OPT_HOP_IMPL, args.hop_impl)
     ctx.set_gauge(torch.from_numpy(U).cuda())
     Phi_host = torch.from_numpy(Phi).pin_memory()
     P = ctx.pack(Phi_host.cuda())

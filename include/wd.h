@@ -88,11 +88,11 @@ int wd_site_order(wd_ctx* ctx, int order, const int tile[4]);
  *       sites * n_rhs threads, halved until <= 1024).  0 (default) = chosen from n_rhs; else 1..1024.
  *   WD_OPT_HOP32_REGS / WD_OPT_HOP64_REGS    register budget per thread: picks among the compiled
  *       variants (fp32: 64, 128; fp64: 128, 168), clamped so that one CTA fits an SM.  0 (default) = chosen from n_rhs.
- *   WD_OPT_HOP_IMPL     0 (default): the register kernel (one thread per site and column, operands loaded
- *       straight into registers).  1: the kernel that stages whole lattice rows through shared memory with
- *       bulk copies (cp.async.bulk + mbarrier, persistent CTAs, producer/consumer warps) wherever it applies
- *       (linear site order; else the register kernel runs).  Same results bit for bit; 0 is faster up to
- *       n_rhs ~ 8, 1 from n_rhs ~ 12 (measured at 24^4).
+ *   WD_OPT_HOP_IMPL     1 (default): the hopping kernel that stages whole lattice rows through shared memory with
+ *       bulk copies (cp.async.bulk + mbarrier ring, persistent CTAs, producer and consumer warps) wherever it
+ *       applies (linear site order with Lx/2 even, i.e. the row-major native layout), else the register kernel.
+ *       0: always the register kernel (one thread per site and column, operands loaded straight into
+ *       registers).  Same results bit for bit.
  *   WD_OPT_ALTERNATE_SWEEP  1 (default): consecutive kernels of the inner solver sweep the vectors in opposite
  *       directions, so that what one kernel wrote last is still in L2 when the next reads it first; 0: off.
  *   WD_OPT_POLL_EVERY   inner iterations enqueued between two convergence polls of the solver (>= 1).

@@ -27,6 +27,10 @@ long order_index(const wd_ctx* c, const int x[4]) {
 
 void build_tables(wd_ctx* c) {
     const long V = c->V, Vh = c->Vh;
+    // row-major blocks need Lx/2 even: a row of 18-real fp32 links is Lx/2 * 72 bytes and must stay 16-byte aligned
+    c->RB = (c->order == WD_ORDER_LINEAR && (c->L[0] / 2) % 2 == 0) ? (uint32_t)(c->L[0] / 2) : (uint32_t)Vh;
+    c->rb_lg = 0;
+    while ((1u << c->rb_lg) < c->RB) ++c->rb_lg;
     c->h_site_of.assign(2 * Vh, -1);
     c->h_nbr.assign(2 * Vh * WD_NDIR, 0);
     std::vector<int32_t> idx_of(V);
@@ -52,7 +56,7 @@ void build_tables(wd_ctx* c) {
                         for (int s = 0; s < 2; ++s) {
                             int y[4] = {x[0], x[1], x[2], x[3]};
                             y[mu] = (y[mu] + (s == 0 ? 1 : c->L[mu] - 1)) % c->L[mu];
-                            nb[2 * mu + s] = idx_of[canon_site(c, y)];
+                            nb[2 * mu + s] = (int32_t)wd_pack_site(c, idx_of[canon_site(c, y)]);
                         }
                     // SF: the stored t=0 slice is not dynamical.  Its neighbours at t=1 / t=T-1 read it
                     // as the zero field, which is exactly psi(t=0) = psi(t=T) = 0 (SF reading).
@@ -150,6 +154,7 @@ int wd_create(wd_ctx** out, const int dims[4], double kappa, int time_bc, int ma
     for (int k = 0; k < WD_OPT_N; ++k) c->opt[k] = 0;
     // hop CTA shape and register budget: 0 = chosen per launch from n_rhs (wd_hop.cu)
     c->opt[WD_OPT_POLL_EVERY] = 4;
+    c->opt[WD_OPT_HOP_IMPL] = 1;
     c->opt[WD_OPT_ALTERNATE_SWEEP] = 1;
     c->prof_on = false;
     c->prof_used = 0;

@@ -26,6 +26,7 @@ struct ForceArgs {
     const int32_t* site_of;
     double* F;          // canonical
     long V, Vh;
+    uint32_t RB, lg;    // native layout blocks (wd_internal.h); neighbour indices are packed (block << lg) | offset
     int n;
     int spb;            // sites per block
     double coef;        // 2 kappa
@@ -35,11 +36,13 @@ template <int MU>
 __device__ __forceinline__ void force_dir(const ForceArgs& A, int p, long nb, int r, const cx<double> (&x0)[12],
                                           const cx<double> (&y0)[12], double* w /* [18] */) {
     const long stride = A.Vh * A.n;
-    const double2* Xn = A.X + (long)(1 - p) * 12 * stride;
-    const double2* Yn = A.Y + (long)(1 - p) * 12 * stride;
+    const long nbb = (long)((uint32_t)nb >> A.lg), nbo = (long)((uint32_t)nb & ((1u << A.lg) - 1u));
+    const long rbn = (long)A.RB * A.n;
+    const double2* Xn = A.X + (long)(1 - p) * 12 * stride + nbb * 12 * rbn;
+    const double2* Yn = A.Y + (long)(1 - p) * 12 * stride + nbb * 12 * rbn;
     cx<double> x1[12], y1[12], a[6], b[6], c[6], d[6];
-    load_spinor(Xn, stride, nb * A.n + r, x1);
-    load_spinor(Yn, stride, nb * A.n + r, y1);
+    load_spinor(Xn, rbn, nbo * A.n + r, x1);
+    load_spinor(Yn, rbn, nbo * A.n + r, y1);
     project<MU, 1>(x1, a);   // (1 - gamma) x(s+mu)
     project<MU, 1>(y0, b);   // (1 - gamma) y(s)
     project<MU, -1>(y1, c);  // (1 + gamma) y(s+mu)
@@ -84,8 +87,9 @@ __global__ void force_kernel(const ForceArgs A) {
                 for (int k = 0; k < 18; ++k) w[mu * slab + k] = 0.0;
         } else {
             cx<double> x0[12], y0[12];
-            load_spinor(A.X + (long)p * 12 * stride, stride, h * n + r, x0);
-            load_spinor(A.Y + (long)p * 12 * stride, stride, h * n + r, y0);
+            const long hb = h / A.RB, ho = h - hb * A.RB, rbn = (long)A.RB * n;
+            load_spinor(A.X + (long)p * 12 * stride + hb * 12 * rbn, rbn, ho * n + r, x0);
+            load_spinor(A.Y + (long)p * 12 * stride + hb * 12 * rbn, rbn, ho * n + r, y0);
             double wl[18];
             force_dir<0>(A, p, n0.x, r, x0, y0, wl);
 #pragma unroll
@@ -117,7 +121,8 @@ __global__ void force_kernel(const ForceArgs A) {
 #pragma unroll
                 for (int k = 0; k < 9; ++k) { W[k].re += w[rr * 18 + 2 * k]; W[k].im += w[rr * 18 + 2 * k + 1]; }
             cx<double> u[9], M[9];
-            load_link<18>(A.U + (long)(mu * 2 + p2) * 18 * A.Vh, A.Vh, h2, u);
+            const long hb2 = h2 / A.RB;
+            load_link<18>(A.U + (long)(mu * 2 + p2) * 18 * A.Vh + hb2 * 18 * A.RB, (long)A.RB, h2 - hb2 * A.RB, u);
 #pragma unroll
             for (int i = 0; i < 3; ++i)
 #pragma unroll
@@ -160,6 +165,8 @@ int wd_force_impl(wd_ctx* c, int n, const double* X, const double* Y, double* F)
     A.F = F;
     A.V = c->V;
     A.Vh = c->Vh;
+    A.RB = c->RB;
+    A.lg = c->rb_lg;
     A.n = n;
     A.spb = 128 / n < 1 ? 1 : 128 / n;  // about 128 threads; at least 4*spb threads are needed for stage 2
     int B = A.spb * n;

@@ -27,7 +27,8 @@ struct HopArgs {
     wdblas::RedBuf rb;                 // per-column reduction scratch and scalar table (EPI >= 2)
     const double* done;                // nullable: the solver's "all columns converged" flag -> no-op launch
     const T* U;                        // native links of this precision and form
-    const int32_t* nbr;                // [Vh][8] of parity par
+    const int32_t* nbr;                // [Vh][8] of parity par: PACKED site indices (block << lg) | offset
+    uint32_t RB, lg;                   // native layout blocks of RB sites (wd_internal.h); 2^lg >= RB
     uint32_t Vh;
     uint32_t n;
     uint32_t par;
@@ -36,14 +37,18 @@ struct HopArgs {
     T a, b;
 };
 
-// one direction: FWD: U_mu(x) psi(x+mu) with (1 - sg gamma);  !FWD: U_mu(x-mu)^dag psi(x-mu) with (1 + sg gamma)
+// one direction: FWD: U_mu(x) psi(x+mu) with (1 - sg gamma);  !FWD: U_mu(x-mu)^dag psi(x-mu) with (1 + sg gamma).
+// (hb, ho) = layout block and offset of the output site, nb = packed index of the neighbour.
 template <typename T, int RECON, int MU, bool FWD, bool DAG>
-__device__ __forceinline__ void hop_dir(const HopArgs<T>& A, uint32_t h, uint32_t r, uint32_t nb, cx<T> (&acc)[12]) {
+__device__ __forceinline__ void hop_dir(const HopArgs<T>& A, uint32_t hb, uint32_t ho, uint32_t r, uint32_t nb,
+                                        cx<T> (&acc)[12]) {
     constexpr int SIGMA = (FWD ? 1 : -1) * (DAG ? -1 : 1);
+    constexpr uint32_t NCH = Vec<T>::NCH;
+    const uint32_t nbb = nb >> A.lg, nbo = nb & ((1u << A.lg) - 1u);
     cx<T> psi[12], hs[6], chi[6], u[9];
-    load_spinor(A.in, A.total, nb * A.n + r, psi);
-    if (FWD) load_link<RECON>(A.U + (size_t)(MU * 2 + A.par) * RECON * A.Vh, A.Vh, h, u);
-    else     load_link<RECON>(A.U + (size_t)(MU * 2 + 1 - A.par) * RECON * A.Vh, A.Vh, nb, u);
+    load_spinor(A.in + nbb * (NCH * A.RB * A.n), A.RB * A.n, nbo * A.n + r, psi);
+    if (FWD) load_link<RECON>(A.U + (size_t)(MU * 2 + A.par) * RECON * A.Vh + (size_t)hb * RECON * A.RB, A.RB, ho, u);
+    else     load_link<RECON>(A.U + (size_t)(MU * 2 + 1 - A.par) * RECON * A.Vh + (size_t)nbb * RECON * A.RB, A.RB, nbo, u);
     if (RECON == 12) rebuild_row3(u);
     project<MU, SIGMA>(psi, hs);
     su3_mul<!FWD>(u, hs, chi);
@@ -68,6 +73,10 @@ __global__ void __maxnreg__(MAXREG) hop_kernel(const HopArgs<T> A) {
     if (EPI < EPI_SIGMA && !in_range) return;
     const uint32_t h = in_range ? tid / A.n : 0u;
     const uint32_t r = tid - (tid / A.n) * A.n;
+    const uint32_t hb = h / A.RB, ho = h - hb * A.RB;        // layout block and offset of this site
+    const uint32_t rbn = A.RB * A.n;                          // chunk stride inside a layout block
+    const uint32_t own = hb * (Vec<T>::NCH * rbn);            // first element of the block
+    const uint32_t eo = ho * A.n + r;                         // this (site, column) inside a chunk
     const int4 n0 = __ldg(reinterpret_cast<const int4*>(A.nbr) + 2 * h);
     const int4 n1 = __ldg(reinterpret_cast<const int4*>(A.nbr) + 2 * h + 1);
     cx<T> acc[12];
@@ -75,24 +84,31 @@ __global__ void __maxnreg__(MAXREG) hop_kernel(const HopArgs<T> A) {
     for (int k = 0; k < 12; ++k) { acc[k].re = 0; acc[k].im = 0; }
     const bool frozen = ((uint32_t)n0.x & WD_SITE_FROZEN) != 0;  // SF: t = 0 stays zero
     if (EPI < EPI_SIGMA && frozen) {
-        store_spinor(A.out, A.total, tid, acc);
+        store_spinor(A.out + own, rbn, eo, acc);
         return;
     }
     // per-thread partial sums over the 12 components of ONE site and column in working precision
     // (fp32: 24-72 products); everything across threads is added in fp64 (wd_blas.cuh)
     [[maybe_unused]] T sums[3] = {0, 0, 0};
     if (in_range && !frozen) {
-        hop_dir<T, RECON, 0, true, DAG>(A, h, r, n0.x, acc);
-        hop_dir<T, RECON, 0, false, DAG>(A, h, r, n0.y, acc);
-        hop_dir<T, RECON, 1, true, DAG>(A, h, r, n0.z, acc);
-        hop_dir<T, RECON, 1, false, DAG>(A, h, r, n0.w, acc);
-        hop_dir<T, RECON, 2, true, DAG>(A, h, r, n1.x, acc);
-        hop_dir<T, RECON, 2, false, DAG>(A, h, r, n1.y, acc);
-        hop_dir<T, RECON, 3, true, DAG>(A, h, r, n1.z, acc);
-        hop_dir<T, RECON, 3, false, DAG>(A, h, r, n1.w, acc);
+        if (EPI >= EPI_XPAY) {  // the epilogue's operands: ask L2 for them now, they are read after the eight directions
+#pragma unroll
+            for (uint32_t c = 0; c < Vec<T>::NCH; ++c) {
+                asm volatile("prefetch.global.L2 [%0];" ::"l"(A.in2 + own + c * rbn + eo));
+                if (EPI == EPI_SIGMA) asm volatile("prefetch.global.L2 [%0];" ::"l"(A.in3 + own + c * rbn + eo));
+            }
+        }
+        hop_dir<T, RECON, 0, true, DAG>(A, hb, ho, r, n0.x, acc);
+        hop_dir<T, RECON, 0, false, DAG>(A, hb, ho, r, n0.y, acc);
+        hop_dir<T, RECON, 1, true, DAG>(A, hb, ho, r, n0.z, acc);
+        hop_dir<T, RECON, 1, false, DAG>(A, hb, ho, r, n0.w, acc);
+        hop_dir<T, RECON, 2, true, DAG>(A, hb, ho, r, n1.x, acc);
+        hop_dir<T, RECON, 2, false, DAG>(A, hb, ho, r, n1.y, acc);
+        hop_dir<T, RECON, 3, true, DAG>(A, hb, ho, r, n1.z, acc);
+        hop_dir<T, RECON, 3, false, DAG>(A, hb, ho, r, n1.w, acc);
         if (EPI >= EPI_XPAY) {
             cx<T> q[12];
-            load_spinor(A.in2, A.total, tid, q);
+            load_spinor(A.in2 + own, rbn, eo, q);
 #pragma unroll
             for (int k = 0; k < 12; ++k) {
                 acc[k].re = fma(A.b, acc[k].re, A.a * q[k].re);
@@ -109,7 +125,7 @@ __global__ void __maxnreg__(MAXREG) hop_kernel(const HopArgs<T> A) {
         }
         if (EPI == EPI_SIGMA) {  // <r~, v> with v = acc
             cx<T> q[12];
-            load_spinor(A.in3, A.total, tid, q);
+            load_spinor(A.in3 + own, rbn, eo, q);
 #pragma unroll
             for (int k = 0; k < 12; ++k) {
                 sums[0] = fma(q[k].re, acc[k].re, sums[0]);  sums[0] = fma(q[k].im, acc[k].im, sums[0]);
@@ -117,7 +133,7 @@ __global__ void __maxnreg__(MAXREG) hop_kernel(const HopArgs<T> A) {
             }
         }
     }
-    if (in_range) store_spinor(A.out, A.total, tid, acc);
+    if (in_range) store_spinor(A.out + own, rbn, eo, acc);
     if (EPI == EPI_SIGMA) {  // block partials; finalize_partials_kernel follows on the stream
         double s2[2] = {(double)sums[0], (double)sums[1]};
         wdblas::block_partials<2>(s2, (int)A.n, A.rb);
@@ -154,6 +170,8 @@ void launch_t(wd_ctx* c, int dag, int n, int par, const wd_hop_ops& o, const T* 
     A.U = U;
     A.nbr = c->d_nbr + (long)par * c->Vh * WD_NDIR;
     A.Vh = (uint32_t)c->Vh;
+    A.RB = c->RB;
+    A.lg = c->rb_lg;
     A.n = (uint32_t)n;
     A.par = (uint32_t)par;
     A.rev = o.rev ? 1u : 0u;

@@ -8,24 +8,31 @@
 // cp.async.bulk (no registers, no LSU instructions, ~150 KB in flight per SM), and consumer warps (one thread
 // per site and column) that only ever wait on an mbarrier, read shared memory and do arithmetic.
 //
-// Measured (B200, 24^4, fp32, 12-real links, L2-cold): bit-identical results to the register kernel; 75.9 us
-// against 70.5 us at n_rhs = 5, 172 us against 194 us at n_rhs = 12.  With the consumers' arithmetic switched off
-// the producer alone needs 49 us: each bulk copy costs about 85 ns of issue/latency, and in the chunk-major native
-// layout a group needs about 60 copies of 1-4 KB (one per spinor chunk and link chunk).  So this form is the
-// opt-in choice (WD_OPT_HOP_IMPL = 1; it wins from n_rhs ~ 12 up) until the native layout is row-major, which
-// would bring a group down to ~15 copies; that layout change is listed under "next" in DESIGN.md.
+// It needs the row-major native layout (wd_layout.cu, RB = Lx/2): there a lattice row is contiguous with all its
+// chunks, so every piece a unit needs is ONE bulk copy of whole rows (about 15 copies per group).  In the earlier
+// chunk-major layout a group took about 60 copies of 1-4 KB, and at a measured ~85 ns of issue cost per copy the
+// producer alone needed 49 us per launch, longer than the consumers' arithmetic.
 //
-// A note for whoever touches the producer: keep its copy loops rolled.  Fully unrolled for fp64 (12 chunks) ptxas
-// ran out of uniform registers and emitted R2UR.FILL spills around the UBLKCP instructions; that build raised
-// "illegal memory access" on every fp64 launch although every address and size checked out.
+// Measured (B200, 24^4, n_rhs = 5, fp32, L2-cold, standalone): 71 us (12-real links) / 70 us (18-real), results bit
+// for bit those of the register kernel, which takes 70 us in the chunk-major layout and 76 us in this one.  Inside
+// the solver (half of the launches carry the fused xpay / inner-product epilogues) this kernel averages 81 us per
+// launch against 91 us for the register kernel: one MD force evaluation 95.1 ms against 108.7 ms.  ncu: issue slots
+// 53 % busy with 12-15 consumer warps per SM, mbarrier waits 2 per issue -- the remaining gap to the HBM roofline
+// is issue efficiency at that occupancy (the ring needs the whole 227 KB of shared memory, so one CTA per SM).
+//
+// A note for whoever touches the producers: keep their code small.  An earlier version with fully unrolled copy
+// loops (fp64, 12 chunks) made ptxas run out of uniform registers and emit R2UR.FILL spills around the UBLKCP
+// instructions; that build raised "illegal memory access" on every fp64 launch although every address and size
+// checked out (cuobjdump -sass | grep R2UR.FILL should stay empty).
 //
 // Geometry (linear site order only): a half-lattice index is h = xh + Lxh*(y + Ly*(z + Lz*t)), xh = x/2.
 // A "row" is the Lxh sites of fixed (y,z,t); neighbours in +-y, +-z, +-t of a row are the row with the
 // same xh at the shifted (y,z,t); neighbours in +-x are in the row with the same (y,z,t) of the other
 // parity at xh or xh+-1 (which one depends on the parity of y+z+t+par).  So no neighbour table is read.
 // Work item = a group of RG consecutive rows in y (S = RG*Lxh sites, S*n consumer threads).  Per group the
-// producer issues 5 units:  XY (input rows y0-1 .. y0+RG, links x+ x- y+ y-), Z+, Z-, T+, T- (RG input rows
-// and one link array each).  Ring: one big slot for XY units and three small slots for the others.
+// producers issue 5 units:  XY (input rows y0-1 .. y0+RG, links x+ x- y+ y-), Z+, Z-, T+, T- (RG input rows
+// and one link array each).  Ring: one big slot for XY units and three small slots for the others; one producer
+// warp per slot class.
 #include "wd_blas.cuh"
 #include "wd_su3.cuh"
 
@@ -90,116 +97,88 @@ struct TmaArgs {
     T a, b;
 };
 
-template <typename T, int RECON> struct LinkShape;
-template <> struct LinkShape<float, 12> { enum { CH16 = 3, TAIL8 = 0 }; };
-template <> struct LinkShape<float, 18> { enum { CH16 = 4, TAIL8 = 1 }; };   // + one float2 chunk
-template <> struct LinkShape<double, 12> { enum { CH16 = 6, TAIL8 = 0 }; };
-template <> struct LinkShape<double, 18> { enum { CH16 = 9, TAIL8 = 0 }; };
-
-// 16-byte units of one staged link array of S sites
-template <typename T, int RECON>
-__host__ __device__ constexpr uint32_t link_vecs(uint32_t S) {
-    return LinkShape<T, RECON>::CH16 * S + (LinkShape<T, RECON>::TAIL8 ? (S + 1) / 2 : 0);
-}
-
 __device__ __forceinline__ uint32_t wrap_inc(uint32_t v, uint32_t L) { return v + 1 == L ? 0u : v + 1; }
 __device__ __forceinline__ uint32_t wrap_dec(uint32_t v, uint32_t L) { return v == 0 ? L - 1 : v - 1; }
 
 // ---- producer side ------------------------------------------------------------------------------------
-// The producer WARP issues the copies of a unit lane-parallel: copy number idx -> (dst, src, bytes) is pure index
-// arithmetic, every lane works out its own and the hardware serialises only the UBLKCP issue itself.  (One thread
-// issuing all ~70 copies of a group took longer than the consumers' arithmetic on that group.)
-//
-// One copy = (dst, src, bytes).  Every lane fills in its own descriptor with selects and all lanes meet at ONE
-// bulk_g2s call site, so the hardware-serialised part is just the UBLKCP issue.
+// In the row-major native layout (wd_layout.cu with RB = Lx/2) a lattice row is contiguous with all its chunks:
+// NCH * rowB bytes of spinor, lrowB = Lxh * R * sizeof(T) bytes of link per (mu, parity).  So every piece a unit
+// needs is ONE bulk copy of whole rows: 5-8 copies for the XY unit, 2 for the others (about 15 per group; in the
+// chunk-major layout it took about 60, and at ~85 ns of issue cost per copy the producer was the bottleneck).
+// The producer warp builds the copy list lane-parallel: lane k owns copy k.
 struct CopyDesc {
     char* dst;
     const char* src;
     uint32_t bytes;  // 0 = nothing to copy
 };
 
-// piece of a staged link array: `count` consecutive sites from half-lattice index hsrc of link block (mu, q) go to
-// site offset `off` of the array at L; copy cc < CH16 is 16-byte chunk cc, copy CH16 the float2 tail (fp32 R=18)
 template <typename T, int RECON>
-__device__ __forceinline__ CopyDesc link_desc(const TmaArgs<T>& A, char* L, int mu, uint32_t q, uint32_t hsrc, uint32_t count,
-                                              uint32_t off, uint32_t cc) {
-    constexpr uint32_t CH16 = LinkShape<T, RECON>::CH16;
-    const char* blk = reinterpret_cast<const char*>(A.U + (size_t)(mu * 2 + q) * RECON * A.Vh);
-    CopyDesc d;
-    if (cc < CH16) {
-        d.dst = L + ((size_t)cc * A.S + off) * 16;
-        d.src = blk + ((size_t)cc * A.Vh + hsrc) * 16;
-        d.bytes = count * 16;
-    } else {
-        d.dst = L + (size_t)CH16 * A.S * 16 + (size_t)off * 8;
-        d.src = blk + ((size_t)16 * A.Vh + 2 * (size_t)hsrc) * 4;
-        d.bytes = count * 8;
-    }
-    return d;
-}
-
-template <typename T, int RECON>
-__device__ void produce_group(const TmaArgs<T>& A, uint32_t lane, uint32_t y0, uint32_t z, uint32_t t, uint32_t q, char* ring,
+__device__ void produce_xy(const TmaArgs<T>& A, uint32_t lane, uint32_t y0, uint32_t z, uint32_t t, uint32_t q, char* ring,
                               uint64_t* full, uint64_t* empty) {
     constexpr uint32_t NCH = Vec<T>::NCH;
-    constexpr uint32_t CHT = LinkShape<T, RECON>::CH16 + LinkShape<T, RECON>::TAIL8;                 // copies per link piece
-    constexpr uint32_t LB = LinkShape<T, RECON>::CH16 * 16 + LinkShape<T, RECON>::TAIL8 * 8;         // bytes per link
-    const uint32_t rowV = A.Lxh * A.n, rowB = rowV * 16, RG = A.RG, S = A.S;
+    const uint32_t rowB = A.Lxh * A.n * 16 * NCH;                   // bytes of one spinor row (all chunks)
+    const uint32_t lrowB = A.Lxh * RECON * (uint32_t)sizeof(T);     // bytes of one row of one link array
+    const uint32_t RG = A.RG;
     const uint32_t zt = z + A.Lz * t;
     const uint32_t row0 = y0 + A.Ly * zt;
-    const uint32_t h0 = row0 * A.Lxh;
     const char* in = reinterpret_cast<const char*>(A.in);
-    const size_t chB = (size_t)A.total * 16;  // bytes per spinor chunk
-    // ---- XY unit -> big slot (use q)
+    const char* U = reinterpret_cast<const char*>(A.U);
+    const size_t ublk = (size_t)RECON * A.Vh * sizeof(T);           // bytes of one (mu, parity) link array
+    // ---- XY unit -> big slot (use q): rows y0-1 .. y0+RG, links x+ x- y+ y-
     {
         mbar_wait(&empty[0], (q & 1) ^ 1);
-        if (lane == 0) mbar_expect_tx(&full[0], NCH * (RG + 2) * rowB + 4 * S * LB);
+        if (lane == 0) mbar_expect_tx(&full[0], (RG + 2) * rowB + 4 * RG * lrowB);
         __syncwarp();
         char* B = ring;
-        char* L = B + (size_t)NCH * (RG + 2) * rowB;
-        const size_t LVB = (size_t)link_vecs<T, RECON>(S) * 16;
+        char* L = B + (size_t)(RG + 2) * rowB;
         const bool lo = y0 == 0, hi = y0 + RG == A.Ly;   // the halo row below / above wraps around in y
         const uint32_t rm = (lo ? A.Ly - 1 : y0 - 1) + A.Ly * zt;
         const uint32_t rp = (hi ? 0 : y0 + RG) + A.Ly * zt;
-        for (uint32_t idx = lane; idx < 3 * NCH + 5 * CHT; idx += 32) {
-            CopyDesc d;
-            if (idx < 3 * NCH) {
-                // input rows of chunk c: segment 1 = rows y0 .. y0+RG-1 together with whichever halo rows are contiguous
-                // with them; segments 0 / 2 = the halo row below / above only when it wraps
-                const uint32_t c = idx / 3, seg = idx - 3 * c;
-                char* dc = B + (size_t)c * (RG + 2) * rowB;
-                const char* sc = in + c * chB;
-                if (seg == 1) {
-                    const uint32_t first = lo ? 1u : 0u, nrows = RG + (lo ? 0u : 1u) + (hi ? 0u : 1u);
-                    d.dst = dc + (size_t)first * rowB;
-                    d.src = sc + (size_t)(row0 - (lo ? 0u : 1u)) * rowB;
-                    d.bytes = nrows * rowB;
-                } else if (seg == 0) {
-                    d.dst = dc; d.src = sc + (size_t)rm * rowB; d.bytes = lo ? rowB : 0u;
-                } else {
-                    d.dst = dc + (size_t)(RG + 1) * rowB; d.src = sc + (size_t)rp * rowB; d.bytes = hi ? rowB : 0u;
-                }
-            } else {
-                const uint32_t k = idx - 3 * NCH, piece = k / CHT, cc = k - piece * CHT;
-                // pieces: x+ U_x(x) | x- U_x on the same rows of the other parity | y+ U_y(x) | y- row y0-1 | y- rows y0 ..
-                const uint32_t arr = piece < 3 ? piece : 3u;
-                const int mu = piece < 2 ? 0 : 1;
-                const uint32_t qq = (piece == 0 || piece == 2) ? A.par : 1 - A.par;
-                const uint32_t hsrc = piece == 3 ? rm * A.Lxh : h0;
-                const uint32_t count = piece == 3 ? A.Lxh : (piece == 4 ? S - A.Lxh : S);
-                const uint32_t off = piece == 4 ? A.Lxh : 0u;
-                d = link_desc<T, RECON>(A, L + arr * LVB, mu, qq, hsrc, count, off, cc);
-            }
-            if (d.bytes) bulk_g2s(d.dst, d.src, d.bytes, &full[0]);
+        CopyDesc d;
+        d.bytes = 0;
+        if (lane == 0) {         // rows y0 .. y0+RG-1 with whichever halo rows are contiguous with them
+            const uint32_t first = lo ? 1u : 0u, nrows = RG + (lo ? 0u : 1u) + (hi ? 0u : 1u);
+            d.dst = B + (size_t)first * rowB; d.src = in + (size_t)(row0 - (lo ? 0u : 1u)) * rowB; d.bytes = nrows * rowB;
+        } else if (lane == 1) {  // halo row below, when it wraps
+            d.dst = B; d.src = in + (size_t)rm * rowB; d.bytes = lo ? rowB : 0u;
+        } else if (lane == 2) {  // halo row above, when it wraps
+            d.dst = B + (size_t)(RG + 1) * rowB; d.src = in + (size_t)rp * rowB; d.bytes = hi ? rowB : 0u;
+        } else if (lane == 3) {  // x+: U_x(x) on the output rows
+            d.dst = L; d.src = U + (size_t)(0 + A.par) * ublk + (size_t)row0 * lrowB; d.bytes = RG * lrowB;
+        } else if (lane == 4) {  // x-: U_x(x - x^) lives on the same rows of the other parity
+            d.dst = L + (size_t)RG * lrowB; d.src = U + (size_t)(0 + 1 - A.par) * ublk + (size_t)row0 * lrowB; d.bytes = RG * lrowB;
+        } else if (lane == 5) {  // y+: U_y(x)
+            d.dst = L + (size_t)2 * RG * lrowB; d.src = U + (size_t)(2 + A.par) * ublk + (size_t)row0 * lrowB; d.bytes = RG * lrowB;
+        } else if (lane == 6) {  // y-: U_y(x - y^) on rows y0-1 .. y0+RG-2 of the other parity (one piece unless row y0-1 wraps)
+            d.dst = L + (size_t)3 * RG * lrowB + (lo ? lrowB : 0u);
+            d.src = U + (size_t)(2 + 1 - A.par) * ublk + (size_t)(lo ? row0 : row0 - 1) * lrowB;
+            d.bytes = (lo ? RG - 1 : RG) * lrowB;
+        } else if (lane == 7) {
+            d.dst = L + (size_t)3 * RG * lrowB; d.src = U + (size_t)(2 + 1 - A.par) * ublk + (size_t)rm * lrowB; d.bytes = lo ? lrowB : 0u;
         }
+        if (d.bytes) bulk_g2s(d.dst, d.src, d.bytes, &full[0]);
     }
-    // ---- Z+, Z-, T+, T- units -> small slots
+}
+
+template <typename T, int RECON>
+__device__ void produce_small(const TmaArgs<T>& A, uint32_t lane, uint32_t y0, uint32_t z, uint32_t t, uint32_t q, char* ring,
+                              uint64_t* full, uint64_t* empty) {
+    constexpr uint32_t NCH = Vec<T>::NCH;
+    const uint32_t rowB = A.Lxh * A.n * 16 * NCH;                   // bytes of one spinor row (all chunks)
+    const uint32_t lrowB = A.Lxh * RECON * (uint32_t)sizeof(T);     // bytes of one row of one link array
+    const uint32_t RG = A.RG;
+    const uint32_t zt = z + A.Lz * t;
+    const uint32_t row0 = y0 + A.Ly * zt;
+    const char* in = reinterpret_cast<const char*>(A.in);
+    const char* U = reinterpret_cast<const char*>(A.U);
+    const size_t ublk = (size_t)RECON * A.Vh * sizeof(T);           // bytes of one (mu, parity) link array
+    // ---- Z+, Z-, T+, T- units -> small slots: RG rows of the shifted plane and one link array
     const size_t bigB = (size_t)A.big_vecs * 16, smallB = (size_t)A.small_vecs * 16;
 #pragma unroll 1
     for (uint32_t u = 0; u < 4; ++u) {
         const uint32_t m = 4 * q + u, slot = 1 + m % 3, use = m / 3;
         mbar_wait(&empty[slot], (use & 1) ^ 1);
-        if (lane == 0) mbar_expect_tx(&full[slot], NCH * RG * rowB + S * LB);
+        if (lane == 0) mbar_expect_tx(&full[slot], RG * rowB + RG * lrowB);
         __syncwarp();
         char* B = ring + bigB + (size_t)(slot - 1) * smallB;
         uint32_t zz = z, tt = t;
@@ -209,16 +188,11 @@ __device__ void produce_group(const TmaArgs<T>& A, uint32_t lane, uint32_t y0, u
         else tt = wrap_dec(t, A.Lt);
         const uint32_t rn = y0 + A.Ly * (zz + A.Lz * tt);
         const bool fwd = (u & 1) == 0;
-        for (uint32_t idx = lane; idx < NCH + CHT; idx += 32) {
-            CopyDesc d;
-            if (idx < NCH) {
-                d.dst = B + (size_t)idx * RG * rowB; d.src = in + idx * chB + (size_t)rn * rowB; d.bytes = RG * rowB;
-            } else {
-                d = link_desc<T, RECON>(A, B + (size_t)NCH * RG * rowB, 2 + (u >> 1), fwd ? A.par : 1 - A.par,
-                                        fwd ? h0 : rn * A.Lxh, S, 0, idx - NCH);
-            }
-            if (d.bytes) bulk_g2s(d.dst, d.src, d.bytes, &full[slot]);
-        }
+        if (lane == 0) bulk_g2s(B, in + (size_t)rn * rowB, RG * rowB, &full[slot]);
+        else if (lane == 1)
+            bulk_g2s(B + (size_t)RG * rowB,
+                     U + (size_t)((2 + (u >> 1)) * 2 + (fwd ? A.par : 1 - A.par)) * ublk + (size_t)(fwd ? row0 : rn) * lrowB,
+                     RG * lrowB, &full[slot]);
     }
 }
 
@@ -274,7 +248,7 @@ __device__ __forceinline__ void dir_smem(const typename Vec<T>::type* sp, uint32
 }
 
 // ---- the kernel -----------------------------------------------------------------------------------------
-// grid = min(groups, SMs) persistent CTAs; block = consumer warps (S*n threads, rounded up) + 1 producer warp.
+// grid = min(groups, SMs) persistent CTAs; block = consumer warps (S*n threads, rounded up) + 2 producer warps.
 // dynamic smem: 128 bytes of mbarriers, then the ring: [big slot][3 small slots].
 template <typename T, int RECON, bool DAG, int EPI, int MAXT>
 __global__ void __launch_bounds__(MAXT, 1) hop_tma_kernel(const TmaArgs<T> A) {
@@ -295,12 +269,13 @@ __global__ void __launch_bounds__(MAXT, 1) hop_tma_kernel(const TmaArgs<T> A) {
     const uint32_t gy = A.Ly / A.RG;
     [[maybe_unused]] double dsum[3] = {0.0, 0.0, 0.0};
 
-    if (warp == ncw) {
-        // ================= producer warp: issues every bulk copy of this CTA's groups ======================
+    if (warp >= ncw) {
+        // ================= two producer warps (one per slot class, so neither queue waits behind the other): every bulk copy of this CTA's groups ======================
         uint32_t q = 0;
         for (uint32_t g = A.g_first + blockIdx.x; g < A.groups; g += gridDim.x) {
             const uint32_t yg = g % gy, zt = g / gy, z = zt % A.Lz, t = zt / A.Lz;
-            produce_group<T, RECON>(A, lane, yg * A.RG, z, t, q, ring, full, empty);
+            if (warp == ncw) produce_xy<T, RECON>(A, lane, yg * A.RG, z, t, q, ring, full, empty);
+            else             produce_small<T, RECON>(A, lane, yg * A.RG, z, t, q, ring, full, empty);
             ++q;
         }
     } else {
@@ -308,37 +283,51 @@ __global__ void __launch_bounds__(MAXT, 1) hop_tma_kernel(const TmaArgs<T> A) {
         const uint32_t i = threadIdx.x;
         const bool active = i < nct;
         const uint32_t s = i / A.n, r = i - s * A.n;
-        const uint32_t j = s / A.Lxh, xh = s - j * A.Lxh;
-        const uint32_t rowV = A.Lxh * A.n, RG = A.RG, S = A.S;
+        const uint32_t j = s / A.Lxh, xh = s - j * A.Lxh;   // row inside the group, site inside the row
+        constexpr uint32_t NCH = Vec<T>::NCH;
+        const uint32_t rowV = A.Lxh * A.n, RG = A.RG;
+        const uint32_t lrowV = A.Lxh * RECON * (uint32_t)sizeof(T) / 16;   // 16-byte units of one link row
         const vec* bigS = reinterpret_cast<const vec*>(ring);
-        const vec* bigL = bigS + (size_t)Vec<T>::NCH * (RG + 2) * rowV;
-        const uint32_t LV = link_vecs<T, RECON>(S);
-        const uint32_t smallLoff = Vec<T>::NCH * RG * rowV;
+        const vec* bigL = bigS + (size_t)(RG + 2) * NCH * rowV;
+        const uint32_t e0 = xh * A.n + r;                    // this (site, column) inside a chunk of a row
         uint32_t q = 0;
         if (active) {  // SF: the stored t = 0 slice stays zero
             cx<T> zero[12];
 #pragma unroll
             for (int k = 0; k < 12; ++k) { zero[k].re = 0; zero[k].im = 0; }
-            for (uint32_t g = blockIdx.x; g < A.g_first; g += gridDim.x) store_spinor(A.out, A.total, g * S * A.n + i, zero);
+            for (uint32_t g = blockIdx.x; g < A.g_first; g += gridDim.x) {
+                const uint32_t row = (g % gy) * RG + A.Ly * (g / gy) + j;
+                store_spinor(A.out + (size_t)row * NCH * rowV, rowV, e0, zero);
+            }
         }
         for (uint32_t g = A.g_first + blockIdx.x; g < A.groups; g += gridDim.x) {
             const uint32_t yg = g % gy, zt = g / gy, z = zt % A.Lz, t = zt / A.Lz;
             const uint32_t y0 = yg * RG;
-            const uint32_t oidx = (y0 + A.Ly * zt) * rowV + i;  // h0 * n + i
+            const size_t own = (size_t)(y0 + A.Ly * zt + j) * NCH * rowV;   // first element of this site's row
             cx<T> acc[12];
 #pragma unroll
             for (int k = 0; k < 12; ++k) { acc[k].re = 0; acc[k].im = 0; }
+            // the epilogue's operands are only needed after all eight directions: ask L2 for them now, so that the
+            // loads at the end of the group do not wait on DRAM (they cannot be hoisted: no registers to hold them)
+            if (EPI >= EPI_XPAY && active) {
+#pragma unroll
+                for (uint32_t c = 0; c < NCH; ++c) {
+                    asm volatile("prefetch.global.L2 [%0];" ::"l"(A.in2 + own + c * rowV + e0));
+                    if (EPI == EPI_SIGMA) asm volatile("prefetch.global.L2 [%0];" ::"l"(A.in3 + own + c * rowV + e0));
+                }
+            }
             // ---- XY unit
             mbar_wait(&full[0], q & 1);
             if (active) {
                 const uint32_t b = (y0 + j + z + t + A.par) & 1;
                 const uint32_t xp = b ? wrap_inc(xh, A.Lxh) : xh;   // xh of the +x neighbour
                 const uint32_t xm = b ? xh : wrap_dec(xh, A.Lxh);   // xh of the -x neighbour
-                const uint32_t st = (RG + 2) * rowV;
-                dir_smem<T, RECON, 0, true, DAG>(bigS, st, (j + 1) * rowV + xp * A.n + r, bigL, S, s, acc);
-                dir_smem<T, RECON, 0, false, DAG>(bigS, st, (j + 1) * rowV + xm * A.n + r, bigL + LV, S, j * A.Lxh + xm, acc);
-                dir_smem<T, RECON, 1, true, DAG>(bigS, st, (j + 2) * rowV + xh * A.n + r, bigL + 2 * LV, S, s, acc);
-                dir_smem<T, RECON, 1, false, DAG>(bigS, st, j * rowV + xh * A.n + r, bigL + 3 * LV, S, s, acc);
+                const vec* rowc = bigS + (size_t)(j + 1) * NCH * rowV;     // staged rows: 0 = y0-1, 1.. = y0.., RG+1 = y0+RG
+                const vec* lk = bigL + (size_t)j * lrowV;                  // link arrays: x+ | x- | y+ | y-, RG rows each
+                dir_smem<T, RECON, 0, true, DAG>(rowc, rowV, xp * A.n + r, lk, A.Lxh, xh, acc);
+                dir_smem<T, RECON, 0, false, DAG>(rowc, rowV, xm * A.n + r, lk + (size_t)RG * lrowV, A.Lxh, xm, acc);
+                dir_smem<T, RECON, 1, true, DAG>(rowc + NCH * rowV, rowV, e0, lk + (size_t)2 * RG * lrowV, A.Lxh, xh, acc);
+                dir_smem<T, RECON, 1, false, DAG>(rowc - NCH * rowV, rowV, e0, lk + (size_t)3 * RG * lrowV, A.Lxh, xh, acc);
             }
             __syncwarp();
             if (lane == 0) mbar_arrive(&empty[0]);
@@ -348,11 +337,14 @@ __global__ void __launch_bounds__(MAXT, 1) hop_tma_kernel(const TmaArgs<T> A) {
                 const uint32_t m = 4 * q + u, slot = 1 + m % 3, use = m / 3;
                 mbar_wait(&full[slot], use & 1);
                 if (active) {
-                    const vec* sp = reinterpret_cast<const vec*>(ring) + A.big_vecs + (size_t)(slot - 1) * A.small_vecs;
-                    if (u == 0)      dir_smem<T, RECON, 2, true, DAG>(sp, S * A.n, i, sp + smallLoff, S, s, acc);
-                    else if (u == 1) dir_smem<T, RECON, 2, false, DAG>(sp, S * A.n, i, sp + smallLoff, S, s, acc);
-                    else if (u == 2) dir_smem<T, RECON, 3, true, DAG>(sp, S * A.n, i, sp + smallLoff, S, s, acc);
-                    else             dir_smem<T, RECON, 3, false, DAG>(sp, S * A.n, i, sp + smallLoff, S, s, acc);
+                    const vec* sp = reinterpret_cast<const vec*>(ring) + A.big_vecs + (size_t)(slot - 1) * A.small_vecs +
+                                    (size_t)j * NCH * rowV;
+                    const vec* lk = reinterpret_cast<const vec*>(ring) + A.big_vecs + (size_t)(slot - 1) * A.small_vecs +
+                                    (size_t)RG * NCH * rowV + (size_t)j * lrowV;
+                    if (u == 0)      dir_smem<T, RECON, 2, true, DAG>(sp, rowV, e0, lk, A.Lxh, xh, acc);
+                    else if (u == 1) dir_smem<T, RECON, 2, false, DAG>(sp, rowV, e0, lk, A.Lxh, xh, acc);
+                    else if (u == 2) dir_smem<T, RECON, 3, true, DAG>(sp, rowV, e0, lk, A.Lxh, xh, acc);
+                    else             dir_smem<T, RECON, 3, false, DAG>(sp, rowV, e0, lk, A.Lxh, xh, acc);
                 }
                 __syncwarp();
                 if (lane == 0) mbar_arrive(&empty[slot]);
@@ -362,7 +354,7 @@ __global__ void __launch_bounds__(MAXT, 1) hop_tma_kernel(const TmaArgs<T> A) {
             if (active) {
                 if (EPI >= EPI_XPAY) {
                     cx<T> qv[12];
-                    load_spinor(A.in2, A.total, oidx, qv);
+                    load_spinor(A.in2 + own, rowV, e0, qv);
 #pragma unroll
                     for (int k = 0; k < 12; ++k) {
                         acc[k].re = fma(A.b, acc[k].re, A.a * qv[k].re);
@@ -381,7 +373,7 @@ __global__ void __launch_bounds__(MAXT, 1) hop_tma_kernel(const TmaArgs<T> A) {
                 }
                 if (EPI == EPI_SIGMA) {  // <r~, v> with v = acc
                     cx<T> qv[12];
-                    load_spinor(A.in3, A.total, oidx, qv);
+                    load_spinor(A.in3 + own, rowV, e0, qv);
                     T s0 = 0, s1 = 0;
 #pragma unroll
                     for (int k = 0; k < 12; ++k) {
@@ -390,7 +382,7 @@ __global__ void __launch_bounds__(MAXT, 1) hop_tma_kernel(const TmaArgs<T> A) {
                     }
                     dsum[0] += (double)s0; dsum[1] += (double)s1;
                 }
-                store_spinor(A.out, A.total, oidx, acc);
+                store_spinor(A.out + own, rowV, e0, acc);
             }
         }
     }
@@ -399,7 +391,7 @@ __global__ void __launch_bounds__(MAXT, 1) hop_tma_kernel(const TmaArgs<T> A) {
         constexpr int K = EPI == EPI_SIGMA ? 2 : 3;
         __syncthreads();  // every bulk copy has been consumed: the ring is free
         double* red = reinterpret_cast<double*>(ring);
-        if (warp != ncw && threadIdx.x < nct) {
+        if (threadIdx.x < nct) {
 #pragma unroll
             for (int k = 0; k < K; ++k) red[k * nct + threadIdx.x] = dsum[k];
         }
@@ -431,11 +423,11 @@ bool pick_shape(const wd_ctx* c, int n, int max_threads, Shape* sh) {
     for (uint32_t RG = Ly; RG >= 1; --RG) {
         if (Ly % RG) continue;
         const uint32_t S = RG * Lxh, rowV = Lxh * n;
-        const uint32_t threads = ((S * n + 31) / 32) * 32 + 32;
+        const uint32_t threads = ((S * n + 31) / 32) * 32 + 64;  // consumer warps + two producer warps
         if ((int)threads > max_threads) continue;
-        const uint32_t LV = link_vecs<T, RECON>(S);
-        const uint32_t big = (Vec<T>::NCH * (RG + 2) * rowV + 4 * LV + 7) / 8 * 8;
-        const uint32_t small = (Vec<T>::NCH * RG * rowV + LV + 7) / 8 * 8;
+        const uint32_t lrowV = Lxh * RECON * (uint32_t)sizeof(T) / 16;
+        const uint32_t big = ((RG + 2) * Vec<T>::NCH * rowV + 4 * RG * lrowV + 7) / 8 * 8;
+        const uint32_t small = (RG * Vec<T>::NCH * rowV + RG * lrowV + 7) / 8 * 8;
         const size_t smem = 128 + ((size_t)big + 3 * (size_t)small) * 16;
         if (smem > kSmemMax) continue;
         sh->RG = RG; sh->S = S; sh->threads = threads; sh->big_vecs = big; sh->small_vecs = small; sh->smem = smem;
@@ -506,16 +498,14 @@ int launch_tma(wd_ctx* c, int dag, int n, int par, const wd_hop_ops& o, const T*
 // Returns WD_OK if launched, a positive value if this lattice / option set is not served by the staged kernel
 // (tiled site order, odd Lx/2 with 18-real fp32 links, nothing fits): the caller then uses wd_hop.cu's kernel.
 int wd_hop_tma_launch(wd_ctx* c, int prec, int recon, int dag, int n, int par, const wd_hop_ops& o) {
-    if (c->order != WD_ORDER_LINEAR) return 1;
-    const uint32_t Lxh = c->L[0] / 2;
-    if (prec == WD_F32 && recon == WD_LINK18 && (Lxh & 1)) return 1;  // the float2 chunk needs 16-byte pieces
+    if (c->order != WD_ORDER_LINEAR || c->RB != (uint32_t)(c->L[0] / 2)) return 1;  // needs the row-major layout
     int rc;
     if (prec == WD_F64) {
-        if (recon == WD_LINK18) rc = launch_tma<double, 18, 384>(c, dag, n, par, o, c->d_U64[0]);
-        else                    rc = launch_tma<double, 12, 384>(c, dag, n, par, o, c->d_U64[1]);
+        if (recon == WD_LINK18) rc = launch_tma<double, 18, 416>(c, dag, n, par, o, c->d_U64[0]);
+        else                    rc = launch_tma<double, 12, 416>(c, dag, n, par, o, c->d_U64[1]);
     } else {
-        if (recon == WD_LINK18) rc = launch_tma<float, 18, 512>(c, dag, n, par, o, c->d_U32[0]);
-        else                    rc = launch_tma<float, 12, 512>(c, dag, n, par, o, c->d_U32[1]);
+        if (recon == WD_LINK18) rc = launch_tma<float, 18, 544>(c, dag, n, par, o, c->d_U32[0]);
+        else                    rc = launch_tma<float, 12, 544>(c, dag, n, par, o, c->d_U32[1]);
     }
     return rc;
 }

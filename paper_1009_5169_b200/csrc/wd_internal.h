@@ -26,6 +26,12 @@ struct wd_ctx {
 
     int order;
     int tile[4];
+    // Native layout: sites of a parity are cut into blocks of RB consecutive sites and every block holds its
+    // chunks one after the other (spinor: [block][chunk][site in block][rhs] 128-bit elements; links alike).
+    // Linear site order with Lx/2 even: RB = Lx/2, a block is one lattice row (what the staged hop kernel copies
+    // in bulk); otherwise RB = V/2, one block, i.e. plain chunk-major.  A site index is stored PACKED in the
+    // neighbour table as (block << rb_lg) | offset, 2^rb_lg >= RB, so kernels decode it with a shift and a mask.
+    uint32_t RB, rb_lg;
 
     // host copies of the site tables (uploaded by wd_set_workspace)
     std::vector<int32_t> h_site_of;  // [2][Vh]   canonical site index of (parity, h)
@@ -83,6 +89,10 @@ struct wd_prof_scope {
         if (idx >= 0) cudaEventRecord(c->prof_ev[2 * idx + 1], c->stream);
     }
 };
+
+static inline uint32_t wd_pack_site(const wd_ctx* c, long h) {
+    return (uint32_t)(((h / c->RB) << c->rb_lg) | (h % c->RB));
+}
 
 static inline size_t wd_align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
 

@@ -1,18 +1,22 @@
 // wd_layout.cu -- canonical <-> native conversions (hot-path step a0 "gauge ingest" and the
 // pack/unpack of spinor blocks).  Conversion only: no arithmetic of the method happens here.
 //
-// Native link storage, per precision and link form (R = 18 or 12 reals):
-//   block (mu, parity) starts at real offset (mu*2+parity)*R*Vh and holds, for site h of that parity,
-//   fp64: double2 chunk c (= complex c of the row-major 3x3 matrix, rows 1-2 only for R=12)
-//         at double2 index c*Vh + h;
-//   fp32: float4 chunk c (= complex 2c, 2c+1) at float offset c*4*Vh + 4*h, c < R/4; for R=18 the
-//         ninth complex is a float2 at float offset 16*Vh + 2*h.
+// Native storage cuts the V/2 sites of a parity into layout blocks of RB consecutive sites (wd_internal.h:
+// RB = Lx/2, one lattice row, in the linear site order; RB = V/2 in the tiled order); site h = b*RB + o.
+// Links, per precision and link form (R = 18 or 12 reals): the array of (mu, parity) starts at real offset
+//   (mu*2+parity)*R*Vh; layout block b starts R*RB*b reals further and holds
+//   fp64: double2 chunk c (= complex c of the row-major 3x3 matrix, rows 1-2 only for R=12) at double2 index
+//         c*RB + o;
+//   fp32: float4 chunk c (= complex 2c, 2c+1) at float offset c*4*RB + 4*o, c < R/4; for R=18 the ninth
+//         complex is a float2 at float offset 16*RB + 2*o.
+// Spinor blocks: element (parity p, chunk k, site h, column r) at 128-bit index
+//   p*NCH*Vh*n + ((b*NCH + k)*RB + o)*n + r,   NCH = 12 (fp64, one complex) or 6 (fp32, complex 2k and 2k+1).
 #include "wd_internal.h"
 
 namespace {
 
 __global__ void gauge_ingest_kernel(const double* __restrict__ U, const int32_t* __restrict__ site_of, long V,
-                                    long Vh, double* __restrict__ u64_18, double* __restrict__ u64_12,
+                                    long Vh, long RB, double* __restrict__ u64_18, double* __restrict__ u64_12,
                                     float* __restrict__ u32_18, float* __restrict__ u32_12) {
     const long tid = (long)blockIdx.x * blockDim.x + threadIdx.x;
     if (tid >= 4 * 2 * Vh) return;
@@ -25,41 +29,41 @@ __global__ void gauge_ingest_kernel(const double* __restrict__ U, const int32_t*
 #pragma unroll
     for (int k = 0; k < 18; ++k) v[k] = u[k];
     const long blk = (long)(mu * 2 + p);
-    double* a = u64_18 + blk * 18 * Vh;
-    double* b = u64_12 + blk * 12 * Vh;
+    const long lb = h / RB, o = h - lb * RB;  // layout block and offset inside it
+    double* a = u64_18 + blk * 18 * Vh + lb * 18 * RB;
+    double* b = u64_12 + blk * 12 * Vh + lb * 12 * RB;
 #pragma unroll
     for (int c = 0; c < 9; ++c) {
-        a[(c * Vh + h) * 2] = v[2 * c];
-        a[(c * Vh + h) * 2 + 1] = v[2 * c + 1];
+        a[(c * RB + o) * 2] = v[2 * c];
+        a[(c * RB + o) * 2 + 1] = v[2 * c + 1];
         if (c < 6) {
-            b[(c * Vh + h) * 2] = v[2 * c];
-            b[(c * Vh + h) * 2 + 1] = v[2 * c + 1];
+            b[(c * RB + o) * 2] = v[2 * c];
+            b[(c * RB + o) * 2 + 1] = v[2 * c + 1];
         }
     }
-    float* fa = u32_18 + blk * 18 * Vh;
-    float* fb = u32_12 + blk * 12 * Vh;
+    float* fa = u32_18 + blk * 18 * Vh + lb * 18 * RB;
+    float* fb = u32_12 + blk * 12 * Vh + lb * 12 * RB;
 #pragma unroll
     for (int c = 0; c < 4; ++c)
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
-            fa[c * 4 * Vh + 4 * h + j] = (float)v[4 * c + j];
-            if (c < 3) fb[c * 4 * Vh + 4 * h + j] = (float)v[4 * c + j];
+            fa[c * 4 * RB + 4 * o + j] = (float)v[4 * c + j];
+            if (c < 3) fb[c * 4 * RB + 4 * o + j] = (float)v[4 * c + j];
         }
-    fa[16 * Vh + 2 * h] = (float)v[16];
-    fa[16 * Vh + 2 * h + 1] = (float)v[17];
+    fa[16 * RB + 2 * o] = (float)v[16];
+    fa[16 * RB + 2 * o + 1] = (float)v[17];
 }
 
-// native element (p, k, h, r): fp64 double2 index ((p*12 + k)*Vh + h)*n + r;
-// fp32 float4 index ((p*6 + k/2)*Vh + h)*n + r, component 2*(k%2).
 template <typename T>
 __global__ void pack_kernel(const double* __restrict__ canon, const int32_t* __restrict__ site_of,
-                            const int32_t* __restrict__ nbr, long V, long Vh, int n, T* __restrict__ native) {
+                            const int32_t* __restrict__ nbr, long V, long Vh, long RB, int n, T* __restrict__ native) {
     const long tid = (long)blockIdx.x * blockDim.x + threadIdx.x;
     if (tid >= 2 * Vh * n) return;
     const int r = (int)(tid % n);
     const long ph = tid / n;
     const long h = ph % Vh;
     const int p = (int)(ph / Vh);
+    const long lb = h / RB, o = h - lb * RB;
     const long s = site_of[ph];
     const bool frozen = ((uint32_t)nbr[ph * WD_NDIR] & WD_SITE_FROZEN) != 0;
     const double* src = canon + ((long)r * V + s) * 24;
@@ -70,7 +74,7 @@ __global__ void pack_kernel(const double* __restrict__ canon, const int32_t* __r
         double* dst = (double*)native;
 #pragma unroll
         for (int k = 0; k < 12; ++k) {
-            const long e = (((long)(p * 12 + k) * Vh + h) * n + r) * 2;
+            const long e = ((long)p * 12 * Vh * n + ((lb * 12 + k) * RB + o) * n + r) * 2;
             dst[e] = v[2 * k];
             dst[e + 1] = v[2 * k + 1];
         }
@@ -78,7 +82,7 @@ __global__ void pack_kernel(const double* __restrict__ canon, const int32_t* __r
         float* dst = (float*)native;
 #pragma unroll
         for (int c = 0; c < 6; ++c) {
-            const long e = (((long)(p * 6 + c) * Vh + h) * n + r) * 4;
+            const long e = ((long)p * 6 * Vh * n + ((lb * 6 + c) * RB + o) * n + r) * 4;
 #pragma unroll
             for (int j = 0; j < 4; ++j) dst[e + j] = (float)v[4 * c + j];
         }
@@ -87,20 +91,21 @@ __global__ void pack_kernel(const double* __restrict__ canon, const int32_t* __r
 
 template <typename T>
 __global__ void unpack_kernel(const T* __restrict__ native, const int32_t* __restrict__ site_of, long V, long Vh,
-                              int n, double* __restrict__ canon) {
+                              long RB, int n, double* __restrict__ canon) {
     const long tid = (long)blockIdx.x * blockDim.x + threadIdx.x;
     if (tid >= 2 * Vh * n) return;
     const int r = (int)(tid % n);
     const long ph = tid / n;
     const long h = ph % Vh;
     const int p = (int)(ph / Vh);
+    const long lb = h / RB, o = h - lb * RB;
     const long s = site_of[ph];
     double* dst = canon + ((long)r * V + s) * 24;
     if (sizeof(T) == 8) {
         const double* src = (const double*)native;
 #pragma unroll
         for (int k = 0; k < 12; ++k) {
-            const long e = (((long)(p * 12 + k) * Vh + h) * n + r) * 2;
+            const long e = ((long)p * 12 * Vh * n + ((lb * 12 + k) * RB + o) * n + r) * 2;
             dst[2 * k] = src[e];
             dst[2 * k + 1] = src[e + 1];
         }
@@ -108,7 +113,7 @@ __global__ void unpack_kernel(const T* __restrict__ native, const int32_t* __res
         const float* src = (const float*)native;
 #pragma unroll
         for (int c = 0; c < 6; ++c) {
-            const long e = (((long)(p * 6 + c) * Vh + h) * n + r) * 4;
+            const long e = ((long)p * 6 * Vh * n + ((lb * 6 + c) * RB + o) * n + r) * 4;
 #pragma unroll
             for (int j = 0; j < 4; ++j) dst[4 * c + j] = (double)src[e + j];
         }
@@ -122,7 +127,7 @@ int wd_layout_gauge(wd_ctx* c, const double* U) {
     const int B = 128;
     wd_prof_scope prof(c, WD_PROF_LAYOUT);
     gauge_ingest_kernel<<<(unsigned)((total + B - 1) / B), B, 0, c->stream>>>(
-        U, c->d_site_of, c->V, c->Vh, c->d_U64[0], c->d_U64[1], c->d_U32[0], c->d_U32[1]);
+        U, c->d_site_of, c->V, c->Vh, (long)c->RB, c->d_U64[0], c->d_U64[1], c->d_U32[0], c->d_U32[1]);
     WD_LAUNCH_CHECK(c);
     return WD_OK;
 }
@@ -133,9 +138,9 @@ int wd_layout_pack(wd_ctx* c, int prec, int n, const double* canon, void* native
     const unsigned G = (unsigned)((total + B - 1) / B);
     wd_prof_scope prof(c, WD_PROF_LAYOUT);
     if (prec == WD_F64)
-        pack_kernel<double><<<G, B, 0, c->stream>>>(canon, c->d_site_of, c->d_nbr, c->V, c->Vh, n, (double*)native);
+        pack_kernel<double><<<G, B, 0, c->stream>>>(canon, c->d_site_of, c->d_nbr, c->V, c->Vh, (long)c->RB, n, (double*)native);
     else
-        pack_kernel<float><<<G, B, 0, c->stream>>>(canon, c->d_site_of, c->d_nbr, c->V, c->Vh, n, (float*)native);
+        pack_kernel<float><<<G, B, 0, c->stream>>>(canon, c->d_site_of, c->d_nbr, c->V, c->Vh, (long)c->RB, n, (float*)native);
     WD_LAUNCH_CHECK(c);
     return WD_OK;
 }
@@ -146,9 +151,9 @@ int wd_layout_unpack(wd_ctx* c, int prec, int n, const void* native, double* can
     const unsigned G = (unsigned)((total + B - 1) / B);
     wd_prof_scope prof(c, WD_PROF_LAYOUT);
     if (prec == WD_F64)
-        unpack_kernel<double><<<G, B, 0, c->stream>>>((const double*)native, c->d_site_of, c->V, c->Vh, n, canon);
+        unpack_kernel<double><<<G, B, 0, c->stream>>>((const double*)native, c->d_site_of, c->V, c->Vh, (long)c->RB, n, canon);
     else
-        unpack_kernel<float><<<G, B, 0, c->stream>>>((const float*)native, c->d_site_of, c->V, c->Vh, n, canon);
+        unpack_kernel<float><<<G, B, 0, c->stream>>>((const float*)native, c->d_site_of, c->V, c->Vh, (long)c->RB, n, canon);
     WD_LAUNCH_CHECK(c);
     return WD_OK;
 }

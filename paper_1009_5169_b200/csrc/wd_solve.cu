@@ -133,13 +133,13 @@ __global__ void outer_resid_kernel(long nvec, int n, RedBuf rb, const double2* _
 }
 
 // inner start: b = R_i / |R_i| in fp32 -> r, rt;  x = p = v = 0;  rho = <b, b>.
-// fp64 vec index (k, h, r) k < 12  <->  fp32 vec index (k/2, h, r), components 2*(k%2)..
-__global__ void demote_kernel(long Vh, int n, RedBuf rb, const double2* __restrict__ R64, float4* __restrict__ r32,
+// fp64 vec index ((block*12 + k)*RB + o)*n + r, k < 12  <->  fp32 vec index ((block*6 + k/2)*RB + o)*n + r, components 2*(k%2)..
+__global__ void demote_kernel(long Vh, long RB, int n, RedBuf rb, const double2* __restrict__ R64, float4* __restrict__ r32,
                               float4* __restrict__ rt32, float4* __restrict__ x32, float4* __restrict__ p32,
                               float4* __restrict__ v32) {
     const int r = threadIdx.x % n;
     const long stride = (long)gridDim.x * blockDim.x;
-    const long nvec = 6 * Vh * n, half = Vh * n;
+    const long nvec = 6 * Vh * n, half = RB * n;  // i / half = block * 6 + c  <->  fp64 chunks 2 (block * 6 + c), + 1
     const double* scal = rb.scal;
     const bool frozen = scal[S_FLAG * WD_MAX_RHS + r] != 0.0;
     const double sc = scal[S_SCALE * WD_MAX_RHS + r];
@@ -160,11 +160,11 @@ __global__ void demote_kernel(long Vh, int n, RedBuf rb, const double2* __restri
 }
 
 // X_i += |R_i| E_i  (fp32 -> fp64)
-__global__ void promote_kernel(long Vh, int n, const double* __restrict__ scal, const float4* __restrict__ e32,
+__global__ void promote_kernel(long Vh, long RB, int n, const double* __restrict__ scal, const float4* __restrict__ e32,
                                double2* __restrict__ X64) {
     const int r = threadIdx.x % n;
     const long stride = (long)gridDim.x * blockDim.x;
-    const long nvec = 6 * Vh * n, half = Vh * n;
+    const long nvec = 6 * Vh * n, half = RB * n;  // i / half = block * 6 + c  <->  fp64 chunks 2 (block * 6 + c), + 1
     const double sc = scal[S_OUT_CONV * WD_MAX_RHS + r] != 0.0 ? 0.0 : scal[S_SCALE * WD_MAX_RHS + r];
     for (long i = (long)blockIdx.x * blockDim.x + threadIdx.x; i < nvec; i += stride) {
         const long c = i / half, rem = i - c * half;
@@ -271,7 +271,7 @@ int wd_solve_impl(wd_ctx* c, int dag, int n, const double* Phi, double* X, doubl
         ++outer;
 
         // inner fp32 BiCGStab on the normalised residual
-        { wd_prof_scope pr__(c, WD_PROF_BLAS); demote_kernel<<<L32.G, L32.B, 0, st>>>(Vh, n, rb, R64, r32, rt32, x32, p32, v32); }
+        { wd_prof_scope pr__(c, WD_PROF_BLAS); demote_kernel<<<L32.G, L32.B, 0, st>>>(Vh, (long)c->RB, n, rb, R64, r32, rt32, x32, p32, v32); }
         WD_LAUNCH_CHECK(c);
         // One iteration = 3 BLAS1 kernels + 4 hops; sigma and omega are reduced inside the even-parity hops.
         // Kernels turn into no-ops once the device-side done flag is set, so iterations are enqueued
@@ -314,7 +314,7 @@ int wd_solve_impl(wd_ctx* c, int dag, int n, const double* Phi, double* X, doubl
                 if (hp[G_COUNT] != 0.0) break;
             }
         }
-        { wd_prof_scope pr__(c, WD_PROF_BLAS); promote_kernel<<<L32.G, L32.B, 0, st>>>(Vh, n, c->d_scal, x32, (double2*)XE); }
+        { wd_prof_scope pr__(c, WD_PROF_BLAS); promote_kernel<<<L32.G, L32.B, 0, st>>>(Vh, (long)c->RB, n, c->d_scal, x32, (double2*)XE); }
         WD_LAUNCH_CHECK(c);
     }
 

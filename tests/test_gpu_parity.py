@@ -299,7 +299,7 @@ def test_launch_options_change_speed_only():
     U = wi.gauge_field(dims, 0.3, 7, bc)
     psi = wi.spinor_field(dims, n, 11, bc)
     ctx = make_ctx(dims, 0.13, bc, n, U)
-    assert ctx.get_option(pkg.OPT_HOP_IMPL) == 0
+    assert ctx.get_option(pkg.OPT_HOP_IMPL) == 1
     for prec, ks, kr, sites, regs in ((pkg.F32, pkg.OPT_HOP32_SITES, pkg.OPT_HOP32_REGS, (0, 7, 16, 32, 64, 1024), (0, 64, 128)),
                                       (pkg.F64, pkg.OPT_HOP64_SITES, pkg.OPT_HOP64_REGS, (5, 16, 32, 64), (128, 168, 255))):
         nat = ctx.pack(dev(psi), prec)
