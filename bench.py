@@ -43,6 +43,8 @@ def parse_args():
     ap.add_argument("--impl", default="ours", choices=("ours", "reference"))
     ap.add_argument("--hop-impl", type=int, default=-1, choices=(-1, 0, 1),
                     help="WD_OPT_HOP_IMPL: 0 register kernel, 1 shared-memory-staged kernel, -1 library default")
+    ap.add_argument("--rhs-sweep", action="store_true", help="configs[4]: blocked solve at n_rhs = 1, 2, 5, 8, 12")
+    ap.add_argument("--apply-sweep", action="store_true", help="configs[3]: D, D^dag apply on 16^4, fp32/fp64 x 18/12 reals")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-hop-sweep", action="store_true")
     return ap.parse_args()
@@ -92,8 +94,8 @@ def oracle_value(cfg_full, n_full, L):
 
 def run_reference(args):
     """--impl reference: the oracle on the host cores (rank 0 only)."""
-    rank = int(os.environ.get("RANK", "0"))
-    if rank != 0:
+    from paper_1009_5169_b200 import replicas as rp
+    if not rp.reference_arm_runs_here(rp.env_world()[1]):
         return
     import wd_inputs as wi
     from oracle import wd_oracle as orc
@@ -189,18 +191,22 @@ def hop_bytes_per_launch(Vh, n, s, R, extra_operands=0.0):
     return Vh * (n * (48 + 24 * extra_operands) * s + 8 * R * s)
 
 
-def hop_sweep(pkg, ctx, torch, n, peak_gbs, reps=50):
+def hop_sweep(pkg, ctx, torch, n, peak_gbs, reps=50, only=None):
     """wd_hop back to back on native half-lattice blocks, fp32/fp64 x 18/12-real links; CUDA events
     on the launching stream.  Fields rotate through enough copies to exceed 2x L2 (L2-cold)."""
     res = {}
     Vh = ctx.V // 2
     for prec, pname, s in ((pkg.F32, "f32", 4), (pkg.F64, "f64", 8)):
+        if only and only[0] != pname:
+            continue
         half = ctx.native_numel(prec, n) // 2
         dt = torch.float32 if prec == pkg.F32 else torch.float64
         nbuf = max(2, int(2 * 130e6 / (half * s)) + 1)
         bufs = [torch.randn(half, dtype=dt, device=ctx.device) for _ in range(nbuf)]
         out = [torch.empty(half, dtype=dt, device=ctx.device) for _ in range(2)]
         for recon, R in ((pkg.LINK18, 18), (pkg.LINK12, 12)):
+            if only and only[1] != R:
+                continue
             for i in range(5):
                 ctx.hop(pkg.OP_D, bufs[i % nbuf], n, 0, prec, recon, out=out[i % 2])
             e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -220,6 +226,79 @@ def hop_sweep(pkg, ctx, torch, n, peak_gbs, reps=50):
     return res
 
 
+def rhs_sweep(pkg, wi, torch, peak_gbs, R, recon):
+    """BASELINE.json configs[4]: the blocked mixed-precision solve D X = Phi on 24^4 at n_rhs = 1, 2, 5, 8, 12:
+    time per solve, per RHS and per inner iteration, and the standalone fp32 hop (L2-cold) at that n_rhs."""
+    cfg = dict(wi.CONFIGS[4])
+    dims, kappa, bc = cfg["dims"], cfg["kappa"], cfg["bc"]
+    U = torch.from_numpy(wi.gauge_field(dims, cfg["eps"], cfg["seed"], bc)).cuda()
+    out = {}
+    for n in (1, 2, 5, 8, 12):
+        ctx = pkg.Context(dims, kappa, bc=bc, max_rhs=n)
+        ctx.set_gauge(U)
+        P = ctx.pack(torch.from_numpy(wi.spinor_field(dims, n, cfg["seed"], bc)).cuda())
+        X = torch.empty_like(P)
+        for _ in range(2):
+            ctx.solve_block(pkg.OP_D, P, n, tol=TOL, recon=recon, out=X)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        e0.record()
+        reps = 3
+        for _ in range(reps):
+            _, info = ctx.solve_block(pkg.OP_D, P, n, tol=TOL, recon=recon, out=X)
+        e1.record()
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1) / reps
+        del P, X
+        hop = hop_sweep(pkg, ctx, torch, n, peak_gbs, reps=30, only=("f32", R))
+        out[str(n)] = {"solve_ms": round(ms, 3), "ms_per_rhs": round(ms / n, 3), "inner_iters": info["inner_iters_total"],
+                       "us_per_inner_iter": round(ms * 1e3 / max(1, info["inner_iters_total"]), 1),
+                       "max_relres": max(info["relres"]), "hop_f32": hop[f"f32_r{R}"]}
+        ctx.close()
+        del ctx
+    return out
+
+
+def apply_sweep(pkg, wi, torch, peak_gbs, reps=50):
+    """BASELINE.json configs[3]: standalone D and D^dag apply (two hop launches, diagonal term fused) on the 16^4
+    SF lattice, n_rhs = 5, fp32/fp64 x 18/12-real links.  L2-warm = same buffers every call (the 50-100 MB working
+    set sits in the 126 MB L2); L2-cold = inputs rotated through more than 2x L2 of buffers.  GB/s counts the
+    two-launch form: per site*RHS 72 reals (in twice, out once) plus 8 R reals of links per site."""
+    cfg = dict(wi.CONFIGS[3])
+    dims, kappa, bc, n = cfg["dims"], cfg["kappa"], cfg["bc"], 5
+    U = torch.from_numpy(wi.gauge_field(dims, cfg["eps"], cfg["seed"], bc)).cuda()
+    ctx = pkg.Context(dims, kappa, bc=bc, max_rhs=n)
+    ctx.set_gauge(U)
+    V = ctx.V
+    res = {}
+    for prec, pname, s in ((pkg.F32, "f32", 4), (pkg.F64, "f64", 8)):
+        numel = ctx.native_numel(prec, n)
+        dt = torch.float32 if prec == pkg.F32 else torch.float64
+        nbuf = max(2, int(2 * 130e6 / (numel * s)) + 1)
+        bufs = [torch.randn(numel, dtype=dt, device=ctx.device) for _ in range(nbuf)]
+        out = torch.empty(numel, dtype=dt, device=ctx.device)
+        for recon, R in ((pkg.LINK18, 18), (pkg.LINK12, 12)):
+            for op, oname in ((pkg.OP_D, "D"), (pkg.OP_DDAG, "Ddag")):
+                for mode in ("warm", "cold"):
+                    for i in range(5):
+                        ctx.apply(op, bufs[i % nbuf if mode == "cold" else 0], n, prec, recon, out=out)
+                    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                    torch.cuda.synchronize()
+                    e0.record()
+                    for i in range(reps):
+                        ctx.apply(op, bufs[i % nbuf if mode == "cold" else 0], n, prec, recon, out=out)
+                    e1.record()
+                    torch.cuda.synchronize()
+                    us = e0.elapsed_time(e1) * 1e3 / reps
+                    b = V * (n * 72 * s + 8 * R * s)
+                    res[f"{oname}_{pname}_r{R}_{mode}"] = {
+                        "us": round(us, 2), "gbs": round(b / us * 1e-3, 1), "frac_hbm": round(b / us * 1e-3 / peak_gbs, 4),
+                        "gflops": round(1368.0 * V * n / us * 1e-3, 1), "site_rhs_per_s": round(V * n / us * 1e6, 0)}
+        del bufs, out
+    ctx.close()
+    return res
+
+
 # ------------------------------------------------------------------------------------------------
 # our arm
 # ------------------------------------------------------------------------------------------------
@@ -231,9 +310,8 @@ def run_ours(args):
     import paper_1009_5169_b200 as pkg
     import wd_inputs as wi
 
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    rank = int(os.environ.get("RANK", "0"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
+    from paper_1009_5169_b200 import replicas as rp
+    world, rank, local = rp.env_world()
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback (use --impl reference for the oracle)")
     torch.cuda.set_device(local)
@@ -249,7 +327,7 @@ def run_ours(args):
     peak_src = "measured (MEASURED_PEAKS.json hbm_gbs)" if "hbm_gbs" in peaks else "fallback 6650 GB/s"
 
     cfg = dict(wi.CONFIGS[args.config])
-    cfg["seed"] = cfg["seed"] + rank  # independent replica per rank
+    cfg["seed"] = rp.replica_seed(cfg["seed"], rank)  # independent replica per rank
     n = args.n_rhs
     dims, kappa, bc = cfg["dims"], cfg["kappa"], cfg["bc"]
     recon = pkg.LINK12 if args.recon == 12 else pkg.LINK18
@@ -278,16 +356,11 @@ def run_ours(args):
         return ix, iy
 
     def barrier():
-        if world > 1:
-            dist.barrier()
+        rp.barrier(dist, world)
         torch.cuda.synchronize()
 
     def max_over_ranks(ms):
-        if world == 1:
-            return ms
-        t = torch.tensor([ms], dtype=torch.float64, device=ctx.device)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        return float(t.item())
+        return rp.max_over_ranks(dist, torch, world, ms, ctx.device)
 
     for _ in range(max(args.warmup, 3)):
         ix, iy = step()
@@ -305,7 +378,7 @@ def run_ours(args):
     launches = ctx.launch_count() - l0
     ms_total = max_over_ranks(e0.elapsed_time(e1))
     ms_step = ms_total / args.steps
-    value = world * args.steps / (ms_total * 1e-3)
+    value = rp.job_throughput(world, args.steps, ms_total)
 
     # ---- e2e: host buffers through the one-call C-ABI entry, copies inside the timed region ------
     ctx.md_force_host(Phi_host, F_host, tol=TOL, recon=recon)
@@ -315,7 +388,7 @@ def run_ours(args):
         ctx.md_force_host(Phi_host, F_host, tol=TOL, recon=recon)
     barrier()
     e2e_ms = max_over_ranks((time.perf_counter() - t0) * 1e3)
-    e2e_value = world * args.steps / (e2e_ms * 1e-3)
+    e2e_value = rp.job_throughput(world, args.steps, e2e_ms)
     clocks = sampler.stop()
     f_check = float(F_host.abs().sum())
     assert np.isfinite(f_check) and f_check > 0.0
@@ -325,16 +398,29 @@ def run_ours(args):
     ix, iy = step()
     prof = ctx.profile_read()
     ctx.profile(False)
-    hop_ms, hop_cnt = prof["hop32"]
+    hop_ms, hop_groups = prof["hop32"]
+    # real fp32 hop launches of that step: 4 per BiCGStab iteration.  (The class also counts the no-op launches
+    # enqueued between the last iteration and the next convergence poll; they must not dilute the average.)
+    hop_cnt = 4 * (ix["inner_iters_total"] + iy["inner_iters_total"])
     tot_prof = sum(v[0] for v in prof.values())
     # the four fp32 hop launches of one BiCGStab iteration: plain, xpay + <rt, v> (2 extra operands), plain,
     # xpay + <t, s>, <t, t> (1 extra operand): 0.75 extra operands per launch on average
     hop_bytes = hop_bytes_per_launch(Vh, n, 4, R, extra_operands=0.75)
     hop_us = hop_ms * 1e3 / max(1, hop_cnt)
     achieved = hop_bytes / (hop_us * 1e-6) * 1e-9 if hop_cnt else 0.0
-    roofline = {"bound": "hbm", "kernel": f"hop_kernel<float,{R}> (fp32 multi-RHS Wilson hop inside the inner solver)",
+    staged = ctx.get_option(pkg.OPT_HOP_IMPL) == 1 and (dims[0] // 2) % 2 == 0
+    kname = f"hop_tma_kernel<float,{R}>" if staged else f"hop_kernel<float,{R}>"
+    traffic = None
+    try:  # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu --set full capture
+        tr = json.load(open(os.path.join(ROOT, "profiles", "r01b_hop_traffic.json.txt")))
+        if tr.get("kernel") == kname and tr.get("workload") == workload_name(dict(wi.CONFIGS[args.config]), n):
+            traffic = tr["dram_bytes_per_launch"]
+    except Exception:
+        pass
+    roofline = {"bound": "hbm", "kernel": f"{kname} (fp32 multi-RHS Wilson hop inside the inner solver; launch time includes "
+                                          "the 15-block finalize kernel that follows the two fused-reduction launches)",
                 "achieved": round(achieved, 1), "peak": peak_gbs, "unit": "GB/s", "frac": round(achieved / peak_gbs, 4),
-                "peak_source": peak_src, "traffic": None, "bytes_per_launch": hop_bytes,
+                "peak_source": peak_src, "traffic": traffic, "bytes_per_launch": hop_bytes,
                 "avg_launch_us": round(hop_us, 2), "launches_in_step": hop_cnt,
                 "share_of_step": round(hop_ms / tot_prof, 4) if tot_prof else None,
                 "gflops": round(1320.0 * Vh * n / hop_us * 1e-3, 1) if hop_cnt else None}
@@ -360,6 +446,11 @@ def run_ours(args):
     if rank == 0 and not args.no_hop_sweep:
         line["hop"] = hop_sweep(pkg, ctx, torch, n, peak_gbs)
     ctx.close()
+    del ctx, P, X, Y, F
+    if rank == 0 and args.rhs_sweep:
+        line["rhs_sweep"] = rhs_sweep(pkg, wi, torch, peak_gbs, R, recon)
+    if rank == 0 and args.apply_sweep:
+        line["apply_16"] = apply_sweep(pkg, wi, torch, peak_gbs)
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         from oracle import wd_oracle as orc
         v, sample, _ = oracle_value(dict(wi.CONFIGS[args.config]), n, 16 if dims[0] >= 16 else dims[0])
