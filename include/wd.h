@@ -90,15 +90,19 @@ int wd_site_order(wd_ctx* ctx, int order, const int tile[4]);
  *       variants (fp32: 64, 128; fp64: 128, 168), clamped so that one CTA fits an SM.  0 (default) = chosen from n_rhs.
  *   WD_OPT_HOP_IMPL     1 (default): the hopping kernel that stages whole lattice rows through shared memory with
  *       bulk copies (cp.async.bulk + mbarrier ring, persistent CTAs, producer and consumer warps) wherever it
- *       applies (linear site order with Lx/2 even, i.e. the row-major native layout), else the register kernel.
+ *       applies (linear site order with Lx/2 even, i.e. the row-major native layout, and n_rhs >= 3), else the
+ *       register kernel.
  *       0: always the register kernel (one thread per site and column, operands loaded straight into
  *       registers).  Same results bit for bit.
+ *   WD_OPT_HOP_ROWS     staged kernel: upper bound on the lattice rows (consecutive in y) one CTA works on at a
+ *       time; 0 (default) = as many as the thread and shared-memory budgets allow.  Fewer rows = smaller
+ *       units, more ring slots (deeper prefetch), fewer consumer warps.
  *   WD_OPT_ALTERNATE_SWEEP  1 (default): consecutive kernels of the inner solver sweep the vectors in opposite
  *       directions, so that what one kernel wrote last is still in L2 when the next reads it first; 0: off.
  *   WD_OPT_POLL_EVERY   inner iterations enqueued between two convergence polls of the solver (>= 1).
  * Errors: WD_EINVAL (null, unknown key, value out of range). */
 enum { WD_OPT_HOP32_SITES = 0, WD_OPT_HOP64_SITES = 1, WD_OPT_HOP32_REGS = 2, WD_OPT_HOP64_REGS = 3,
-       WD_OPT_POLL_EVERY = 4, WD_OPT_HOP_IMPL = 5, WD_OPT_ALTERNATE_SWEEP = 6, WD_OPT_N = 8 };
+       WD_OPT_POLL_EVERY = 4, WD_OPT_HOP_IMPL = 5, WD_OPT_ALTERNATE_SWEEP = 6, WD_OPT_HOP_ROWS = 7, WD_OPT_N = 8 };
 int wd_set_option(wd_ctx* ctx, int key, int value);
 int wd_get_option(const wd_ctx* ctx, int key, int* value_host);
 

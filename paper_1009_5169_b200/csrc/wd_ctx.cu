@@ -198,6 +198,9 @@ int wd_set_option(wd_ctx* ctx, int key, int value) {
         case WD_OPT_ALTERNATE_SWEEP:
             if (value != 0 && value != 1) return wd_fail(ctx, WD_EINVAL, "this option is 0 or 1");
             break;
+        case WD_OPT_HOP_ROWS:
+            if (value < 0 || value > 1024) return wd_fail(ctx, WD_EINVAL, "rows per group out of range");
+            break;
         case WD_OPT_POLL_EVERY:
             if (value < 1 || value > 1024) return wd_fail(ctx, WD_EINVAL, "poll interval out of range");
             break;

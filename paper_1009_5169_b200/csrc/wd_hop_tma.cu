@@ -94,6 +94,7 @@ struct TmaArgs {
     uint32_t groups;                   // (Ly / RG) * Lz * Lt
     uint32_t g_first;                  // groups [0, g_first) are the frozen t = 0 slice (Schroedinger functional), else 0
     uint32_t big_vecs, small_vecs;     // slot sizes in 16-byte units
+    uint32_t NS;                       // number of small slots in the ring (3..7)
     T a, b;
 };
 
@@ -176,7 +177,7 @@ __device__ void produce_small(const TmaArgs<T>& A, uint32_t lane, uint32_t y0, u
     const size_t bigB = (size_t)A.big_vecs * 16, smallB = (size_t)A.small_vecs * 16;
 #pragma unroll 1
     for (uint32_t u = 0; u < 4; ++u) {
-        const uint32_t m = 4 * q + u, slot = 1 + m % 3, use = m / 3;
+        const uint32_t m = 4 * q + u, slot = 1 + m % A.NS, use = m / A.NS;
         mbar_wait(&empty[slot], (use & 1) ^ 1);
         if (lane == 0) mbar_expect_tx(&full[slot], RG * rowB + RG * lrowB);
         __syncwarp();
@@ -249,20 +250,20 @@ __device__ __forceinline__ void dir_smem(const typename Vec<T>::type* sp, uint32
 
 // ---- the kernel -----------------------------------------------------------------------------------------
 // grid = min(groups, SMs) persistent CTAs; block = consumer warps (S*n threads, rounded up) + 2 producer warps.
-// dynamic smem: 128 bytes of mbarriers, then the ring: [big slot][3 small slots].
+// dynamic smem: 128 bytes of mbarriers, then the ring: [big slot][NS small slots], NS = as many as fit (>= 3).
 template <typename T, int RECON, bool DAG, int EPI, int MAXT>
 __global__ void __launch_bounds__(MAXT, 1) hop_tma_kernel(const TmaArgs<T> A) {
     typedef typename Vec<T>::type vec;
     if (A.done != nullptr && *A.done != 0.0) return;
     extern __shared__ __align__(128) unsigned char smem[];
     uint64_t* full = reinterpret_cast<uint64_t*>(smem);
-    uint64_t* empty = full + 4;
+    uint64_t* empty = full + 8;   // up to 1 + 7 slots
     char* ring = reinterpret_cast<char*>(smem) + 128;
     const uint32_t nct = A.S * A.n;            // consumer threads
     const uint32_t ncw = (nct + 31) >> 5;      // consumer warps
     const uint32_t warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     if (threadIdx.x == 0) {
-        for (int s = 0; s < 4; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], ncw); }
+        for (uint32_t s = 0; s < 1 + A.NS; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], ncw); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
@@ -334,7 +335,7 @@ __global__ void __launch_bounds__(MAXT, 1) hop_tma_kernel(const TmaArgs<T> A) {
             // ---- Z+, Z-, T+, T- units
 #pragma unroll
             for (int u = 0; u < 4; ++u) {
-                const uint32_t m = 4 * q + u, slot = 1 + m % 3, use = m / 3;
+                const uint32_t m = 4 * q + u, slot = 1 + m % A.NS, use = m / A.NS;
                 mbar_wait(&full[slot], use & 1);
                 if (active) {
                     const vec* sp = reinterpret_cast<const vec*>(ring) + A.big_vecs + (size_t)(slot - 1) * A.small_vecs +
@@ -412,7 +413,7 @@ __global__ void __launch_bounds__(MAXT, 1) hop_tma_kernel(const TmaArgs<T> A) {
 constexpr size_t kSmemMax = 227 * 1024;
 
 struct Shape {
-    uint32_t RG, S, threads, big_vecs, small_vecs;
+    uint32_t RG, S, threads, big_vecs, small_vecs, NS;
     size_t smem;
 };
 
@@ -420,16 +421,20 @@ struct Shape {
 template <typename T, int RECON>
 bool pick_shape(const wd_ctx* c, int n, int max_threads, Shape* sh) {
     const uint32_t Lxh = c->L[0] / 2, Ly = c->L[1];
+    const uint32_t cap = c->opt[WD_OPT_HOP_ROWS] > 0 ? (uint32_t)c->opt[WD_OPT_HOP_ROWS] : Ly;
     for (uint32_t RG = Ly; RG >= 1; --RG) {
-        if (Ly % RG) continue;
+        if (Ly % RG || RG > cap) continue;
         const uint32_t S = RG * Lxh, rowV = Lxh * n;
         const uint32_t threads = ((S * n + 31) / 32) * 32 + 64;  // consumer warps + two producer warps
         if ((int)threads > max_threads) continue;
         const uint32_t lrowV = Lxh * RECON * (uint32_t)sizeof(T) / 16;
         const uint32_t big = ((RG + 2) * Vec<T>::NCH * rowV + 4 * RG * lrowV + 7) / 8 * 8;
         const uint32_t small = (RG * Vec<T>::NCH * rowV + RG * lrowV + 7) / 8 * 8;
-        const size_t smem = 128 + ((size_t)big + 3 * (size_t)small) * 16;
-        if (smem > kSmemMax) continue;
+        if (128 + ((size_t)big + 3 * (size_t)small) * 16 > kSmemMax) continue;
+        uint32_t NS = 3;  // as many small slots as fit (deeper prefetch), at least 3
+        while (NS < 7 && 128 + ((size_t)big + (NS + 1) * (size_t)small) * 16 <= kSmemMax) ++NS;
+        const size_t smem = 128 + ((size_t)big + NS * (size_t)small) * 16;
+        sh->NS = NS;
         sh->RG = RG; sh->S = S; sh->threads = threads; sh->big_vecs = big; sh->small_vecs = small; sh->smem = smem;
         return true;
     }
@@ -466,7 +471,7 @@ int launch_tma(wd_ctx* c, int dag, int n, int par, const wd_hop_ops& o, const T*
     const uint32_t gy = A.Ly / sh.RG;
     A.groups = gy * A.Lz * A.Lt;
     A.g_first = c->bc == WD_BC_SF ? gy * A.Lz : 0;
-    A.big_vecs = sh.big_vecs; A.small_vecs = sh.small_vecs;
+    A.big_vecs = sh.big_vecs; A.small_vecs = sh.small_vecs; A.NS = sh.NS;
     A.a = (T)o.a; A.b = (T)o.b;
     const uint32_t real = A.groups - A.g_first;
     const unsigned G = real < (uint32_t)c->n_sm ? real : (unsigned)c->n_sm;

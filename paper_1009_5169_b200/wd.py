@@ -27,7 +27,7 @@ F64, F32 = 0, 1
 LINK18, LINK12 = 0, 1
 ORDER_LINEAR, ORDER_TILED = 0, 1
 MAX_RHS = 16
-OPT_HOP32_SITES, OPT_HOP64_SITES, OPT_HOP32_REGS, OPT_HOP64_REGS, OPT_POLL_EVERY, OPT_HOP_IMPL, OPT_ALTERNATE_SWEEP = 0, 1, 2, 3, 4, 5, 6
+OPT_HOP32_SITES, OPT_HOP64_SITES, OPT_HOP32_REGS, OPT_HOP64_REGS, OPT_POLL_EVERY, OPT_HOP_IMPL, OPT_ALTERNATE_SWEEP, OPT_HOP_ROWS = 0, 1, 2, 3, 4, 5, 6, 7
 PROF_NAMES = ("hop32", "hop64", "blas", "force", "layout")
 PROF_N = len(PROF_NAMES)
 
