@@ -320,3 +320,41 @@ def test_launch_options_change_speed_only():
     X7, i7 = ctx.solve_block(pkg.OP_D, P, n)
     assert torch.equal(X1, X7) and i1["inner_iters_total"] == i7["inner_iters_total"]
     ctx.close()
+
+
+def test_full_size_bench_configuration_properties():
+    """BASELINE.json configs[4] at n_rhs = 5, exactly as bench.py runs it (24^4 SF, 12-real inner links, default
+    launch options = staged hop kernel).  The oracle cannot solve this size in test time, so: D-apply parity on
+    the whole lattice (the oracle's apply is cheap), and for the solves the properties that pin X and Y at any size --
+    the TRUE residuals |Phi - D X| / |Phi| and |X - D^dag Y| / |X| recomputed with the oracle's operator -- plus the
+    force's exact symmetries (anti-hermitian, traceless, zero on links touching the SF boundary)."""
+    pkg = _wd()
+    cfg, U, Phi = wi.make_config(4, 5)
+    dims, kappa, bc, n = cfg["dims"], cfg["kappa"], cfg["bc"], 5
+    ctx = make_ctx(dims, kappa, bc, n, U)
+    assert ctx.get_option(pkg.OPT_HOP_IMPL) == 1
+    P = ctx.pack(dev(Phi))
+    ref = orc.apply(dims, kappa, bc, 0, U, Phi)
+    out = ctx.unpack(ctx.apply(pkg.OP_D, P, n), n).cpu().numpy()
+    assert rel_per_rhs(out, ref).max() < 1e-13
+    P32 = ctx.pack(dev(Phi), pkg.F32)
+    ref32 = orc.apply(dims, kappa, bc, 0, U.astype(np.float32).astype(np.float64), Phi.astype(np.float32).astype(np.float64))
+    out32 = ctx.unpack(ctx.apply(pkg.OP_D, P32, n, pkg.F32, pkg.LINK12), n, pkg.F32).cpu().numpy()
+    assert rel_per_rhs(out32, ref32).max() < 1e-5
+    del ref, out, ref32, out32
+    X, ix = ctx.solve_block(pkg.OP_D, P, n, tol=1e-12, recon=pkg.LINK12)
+    Y, iy = ctx.solve_block(pkg.OP_DDAG, X, n, tol=1e-12, recon=pkg.LINK12)
+    assert ix["converged"] and iy["converged"]
+    Xc = ctx.unpack(X, n).cpu().numpy()
+    Yc = ctx.unpack(Y, n).cpu().numpy()
+    assert rel_per_rhs(orc.apply(dims, kappa, bc, 0, U, Xc), Phi).max() < 2e-12
+    assert rel_per_rhs(orc.apply(dims, kappa, bc, 1, U, Yc), Xc).max() < 2e-12
+    assert np.all(Xc[:, 0] == 0.0) and np.all(Yc[:, 0] == 0.0)          # SF: the stored t = 0 slice stays zero
+    F = ctx.force(X, Y, n).cpu().numpy()                                  # [mu][T][Lz][Ly][Lx][3][3][2]
+    Fm = F[..., 0] + 1j * F[..., 1]
+    scale = np.abs(Fm).max()
+    assert scale > 0
+    assert np.abs(Fm + np.conj(np.swapaxes(Fm, -1, -2))).max() < 1e-13 * scale   # anti-hermitian
+    assert np.abs(np.trace(Fm, axis1=-2, axis2=-1)).max() < 1e-12 * scale        # traceless
+    assert np.all(F[:, 0] == 0.0) and np.all(F[3, -1] == 0.0)                     # links touching t = 0 / t = T
+    ctx.close()
