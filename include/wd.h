@@ -31,10 +31,14 @@
  *     spinor block   double [n_rhs][T][Lz][Ly][Lx][4][3][2]   spin, colour, (re,im)
  *   NATIVE (what the kernels read; produced by wd_pack, consumed by wd_unpack):
  *     sites are split by parity (x+y+z+t) mod 2 (even = 0) and numbered 0..V/2-1 inside a parity
- *     in the context's site order (wd_site_order); a full-lattice block of n_rhs spinors is
- *       fp64:  double2 [parity=2][k=12][V/2][n_rhs]      k = spin*3+colour, one complex per double2
- *       fp32:  float4  [parity=2][c=6 ][V/2][n_rhs]      complex 2c and 2c+1 per float4
- *     i.e. structure-of-arrays, site-major / RHS-minor, 128-bit elements.  wd_native_bytes gives
+ *     in the context's site order (wd_site_order); the V/2 sites of a parity are cut into layout blocks of
+ *     RB consecutive sites (site h = b*RB + o) and a full-lattice block of n_rhs spinors is
+ *       fp64:  double2 [parity=2][b][k=12][o=RB][n_rhs]    k = spin*3+colour, one complex per double2
+ *       fp32:  float4  [parity=2][b][c=6 ][o=RB][n_rhs]    complex 2c and 2c+1 per float4
+ *     i.e. structure-of-arrays, site-major / RHS-minor, 128-bit elements.  RB = Lx/2 (a block is one
+ *     lattice row with all its chunks: what the staged hopping kernel copies in bulk) for the linear site
+ *     order when Lx/2 is even and max_rhs >= 3, else RB = V/2 (plain chunk-major).  The layout is an
+ *     internal matter of the library: wd_pack / wd_unpack are the way in and out.  wd_native_bytes gives
  *     the size.  In SF mode the t=0 slice is stored and is zero in every native field the library
  *     produces; wd_pack writes zeros there whatever the canonical input holds.
  */

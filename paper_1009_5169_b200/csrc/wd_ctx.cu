@@ -28,7 +28,8 @@ long order_index(const wd_ctx* c, const int x[4]) {
 void build_tables(wd_ctx* c) {
     const long V = c->V, Vh = c->Vh;
     // row-major blocks need Lx/2 even: a row of 18-real fp32 links is Lx/2 * 72 bytes and must stay 16-byte aligned
-    c->RB = (c->order == WD_ORDER_LINEAR && (c->L[0] / 2) % 2 == 0) ? (uint32_t)(c->L[0] / 2) : (uint32_t)Vh;
+    // and only pay when the staged kernel can run at all (n_rhs >= 3): the register kernel is ~8 % faster chunk-major
+    c->RB = (c->order == WD_ORDER_LINEAR && (c->L[0] / 2) % 2 == 0 && c->max_rhs >= 3) ? (uint32_t)(c->L[0] / 2) : (uint32_t)Vh;
     c->rb_lg = 0;
     while ((1u << c->rb_lg) < c->RB) ++c->rb_lg;
     c->h_site_of.assign(2 * Vh, -1);

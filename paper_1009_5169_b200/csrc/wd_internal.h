@@ -28,7 +28,7 @@ struct wd_ctx {
     int tile[4];
     // Native layout: sites of a parity are cut into blocks of RB consecutive sites and every block holds its
     // chunks one after the other (spinor: [block][chunk][site in block][rhs] 128-bit elements; links alike).
-    // Linear site order with Lx/2 even: RB = Lx/2, a block is one lattice row (what the staged hop kernel copies
+    // Linear site order with Lx/2 even and max_rhs >= 3: RB = Lx/2, a block is one lattice row (what the staged hop kernel copies
     // in bulk); otherwise RB = V/2, one block, i.e. plain chunk-major.  A site index is stored PACKED in the
     // neighbour table as (block << rb_lg) | offset, 2^rb_lg >= RB, so kernels decode it with a shift and a mask.
     uint32_t RB, rb_lg;
