@@ -6,7 +6,7 @@
  *     5: F_mu = F_mu + f[x_i, y_i]   for every column i
  * with D the Wilson-Dirac operator on a lattice with Schroedinger-functional (Dirichlet) time
  * boundaries.  The paper fixes neither the normalisation of D, the gamma basis, the
- * SF convention nor f[x,y]; the readings used are listed in DESIGN.md ("Readings"):
+ * SF convention nor f[x,y]; the readings used are listed in DESIGN.md section 2:
  *     D = 1 - kappa H,
  *     (H psi)(x) = sum_mu (1-gamma_mu) U_mu(x) psi(x+mu) + (1+gamma_mu) U_mu(x-mu)^dag psi(x-mu),
  *     D^dag: gamma_mu -> -gamma_mu;   SF: psi(t=0) = psi(t=T) = 0, T slices stored (t = 0..T-1),

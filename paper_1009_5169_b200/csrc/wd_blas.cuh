@@ -1,5 +1,5 @@
 // wd_blas.cuh -- batched-per-RHS BLAS1 updates fused with their inner products (hot-path step a4)
-// and the device-side scalar recurrences of BiCGStab (restated in DESIGN.md).
+// and the device-side scalar recurrences of BiCGStab (textbook BiCGStab per column; the schedule is DESIGN.md section 6).
 //
 // Thread mapping: a block has B = 32*n*m threads (m = ceil(8/n)), so B is a multiple of n and thread
 // t always works on column r = t % n of the flat RHS-minor vector index.  Per-column sums go

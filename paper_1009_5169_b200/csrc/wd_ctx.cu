@@ -60,7 +60,7 @@ void build_tables(wd_ctx* c) {
                             nb[2 * mu + s] = (int32_t)wd_pack_site(c, idx_of[canon_site(c, y)]);
                         }
                     // SF: the stored t=0 slice is not dynamical.  Its neighbours at t=1 / t=T-1 read it
-                    // as the zero field, which is exactly psi(t=0) = psi(t=T) = 0 (SF reading).
+                    // as the zero field, which is exactly psi(t=0) = psi(t=T) = 0 (reading R6).
                     if (c->bc == WD_BC_SF && x[3] == 0) nb[0] = (int32_t)((uint32_t)nb[0] | WD_SITE_FROZEN);
                 }
 }
@@ -341,7 +341,7 @@ int wd_apply(wd_ctx* ctx, int op, int prec, int recon, int n_rhs, const void* in
     const size_t hb = wd_half_bytes(ctx, prec, n_rhs);
     const char* i = (const char*)in;
     char* o = (char*)out;
-    // out_p = in_p - kappa H_{p,1-p} in_{1-p}   (D = 1 - kappa H)
+    // out_p = in_p - kappa H_{p,1-p} in_{1-p}   (D = 1 - kappa H; reading R4)
     for (int p = 0; p < 2; ++p) {
         rc = wd_hop_launch(ctx, prec, recon, op == WD_OP_DDAG, n_rhs, p, i + (1 - p) * hb, o + p * hb, i + p * hb,
                            1.0, -ctx->kappa);

@@ -1,12 +1,12 @@
 // wd_force.cu -- fermion force accumulation (hot-path step a8; Algorithm 2 lines 4-6, PAPER.md:56-58,
-// eq. 2.3; the functional f[x,y] is DESIGN.md reading c.5):
+// eq. 2.3; the functional f[x,y] is DESIGN.md reading R9):
 //
 //   W_mu(s)  = sum_i sum_spin  x_i(s+mu) (x) ((1-gamma_mu) y_i(s))^dag + ((1+gamma_mu) y_i(s+mu)) (x) x_i(s)^dag
 //   F_mu(s) += 2 kappa TA[ U_mu(s) W_mu(s) ],   TA(M) = (M - M^dag)/2 - tr(M - M^dag)/6.
 //
 // Because P = 1 -+ gamma_mu satisfies P = P^dag = P^2/2, sum_spin a (x) (P b)^dag equals
 // sum_{j=0,1} h(a)_j (x) h(b)_j^dag with h the half-spinor projection of the hop kernel, so each term
-// costs 2 colour outer products instead of 4 (DESIGN.md "Force kernel").
+// costs 2 colour outer products instead of 4 (DESIGN.md section 6a).
 //
 // One thread owns one (site, rhs) pair, rhs fastest (the same coalesced 128-bit loads as the hop);
 // it forms its column's contribution to W for the four forward links of its site.  The sum over

@@ -3,13 +3,17 @@
 //
 //   (H psi)(x) = sum_mu (1 -+ gamma_mu) U_mu(x) psi(x+mu) + (1 +- gamma_mu) U_mu(x-mu)^dag psi(x-mu)
 //   (upper sign D, lower sign D^dag) on ONE output parity, for all n_rhs columns in one launch,
-//   optionally with the fused epilogue out = a*in2 + b*(H psi).
+//   optionally with a fused epilogue (out = a*in2 + b*(H psi), per-column inner products; see EPI_* below).
+//
+// This is the REGISTER kernel: operands go straight from global memory into registers.  It serves every site
+// order and layout; where the layout is row-major and n_rhs >= 3 the staged kernel of wd_hop_tma.cu runs instead
+// (WD_OPT_HOP_IMPL) and this one is the fallback and the reference for bit-equality.
 //
 // One thread owns one (site, rhs) pair, rhs fastest: thread tid = h*n + r.  The n threads of a site
 // read the same link addresses (one L1 transaction, one HBM read per link per launch), the spinor
 // loads of a warp are 128-bit and contiguous in memory for the centre site and for every neighbour
 // direction inside a row of the site order.  Spin projection to half spinors happens in registers
-// (table: DESIGN.md "Half-spinor projection"), so each direction costs 2 SU(3) x colour-vector
+// (table: DESIGN.md section 6a "Half-spinor projection"), so each direction costs 2 SU(3) x colour-vector
 // products: 1320 flop per output site and RHS.
 #include "wd_blas.cuh"
 #include "wd_su3.cuh"

@@ -4,7 +4,7 @@
 //   even/odd:  Ahat = 1 - kappa^2 H_eo H_oe on even sites,
 //        Phihat_e = Phi_e + kappa H_eo Phi_o,   Ahat X_e = Phihat_e,   X_o = Phi_o + kappa H_oe X_e.
 //   outer loop, fp64 (defect correction, the "mixed-precision preconditioner technique" of
-//   PAPER.md:80-82 in its simplest form; reading c.6-2):
+//   PAPER.md:80-82 in its simplest form; reading R11):
 //        R = Phihat_e - Ahat X_e;  stop when |R_i| <= tol |phi_i| for every i;
 //        E = BiCGStab_fp32(R_i / |R_i|);  X_e,i += |R_i| E_i.
 //   inner loop, fp32: textbook BiCGStab per column, per-column alpha, beta, omega kept
@@ -20,9 +20,7 @@ namespace {
 template <typename T>
 __device__ __forceinline__ void to_arr(const typename V<T>::type& v, T (&a)[2 * V<T>::NC]);
 template <> __device__ __forceinline__ void to_arr<float>(const float4& v, float (&a)[4]) { a[0] = v.x; a[1] = v.y; a[2] = v.z; a[3] = v.w; }
-template <> __device__ __forceinline__ void to_arr<double>(const double2& v, double (&a)[2]) { a[0] = v.x; a[1] = v.y; }
 __device__ __forceinline__ float4 from_arr(const float (&a)[4]) { return make_float4(a[0], a[1], a[2], a[3]); }
-__device__ __forceinline__ double2 from_arr(const double (&a)[2]) { return make_double2(a[0], a[1]); }
 
 #define WD_BLAS_PROLOGUE(T)                                                        \
     typedef typename V<T>::type vec;                                               \

@@ -1,6 +1,6 @@
 // wd_su3.cuh -- register-level building blocks shared by the hop and force kernels: complex type,
 // 128-bit spinor/link loads from the native layouts, 12-real link rebuild, half-spinor projection
-// (chiral gamma basis), SU(3) x colour-vector product.
+// (DESIGN.md section 6a "Half-spinor projection"; chiral gamma basis), SU(3) x colour-vector product.
 #pragma once
 #include "wd_internal.h"
 
