@@ -67,7 +67,7 @@ def test_apply_fp64_matches_oracle(dims, bc, n_rhs, eps, op):
 @pytest.mark.parametrize("dims,bc,n_rhs,eps", APPLY_CASES)
 @pytest.mark.parametrize("op", [0, 1])
 def test_apply_fp32_matches_oracle_on_rounded_inputs(dims, bc, n_rhs, eps, op):
-    """fp32 arithmetic against the oracle applied to the SAME fp32-rounded inputs (DESIGN.md c.6-12)."""
+    """fp32 arithmetic against the oracle applied to the SAME fp32-rounded inputs."""
     pkg = _wd()
     kappa = 0.13
     U = wi.gauge_field(dims, eps, 7, bc)
