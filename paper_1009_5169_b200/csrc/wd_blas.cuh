@@ -108,7 +108,7 @@ __device__ void finalize_column(double* scal, int r, const double* tot) {
         SC(scal, S_FLAG, r) = conv ? 1.0 : 0.0;
         // inner target: the asked reduction, but never far below what the outer tolerance needs
         double thr2 = scal[G_INTOL2];
-        if (tot[0] > 0.0) thr2 = fmax(thr2, 0.01 * tol2 * phi2 / tot[0]);
+        if (tot[0] > 0.0) thr2 = fmax(thr2, 0.25 * tol2 * phi2 / tot[0]);
         SC(scal, S_THR2, r) = thr2;  // inner rhs is normalised to |b_i| = 1
     }
 }
