@@ -17,7 +17,7 @@
 // for bit those of the register kernel, which takes 70 us in the chunk-major layout and 76 us in this one.  Inside
 // the solver (half of the launches carry the fused xpay / inner-product epilogues) this kernel averages 81 us per
 // launch against 91 us for the register kernel: one MD force evaluation 95.1 ms against 108.7 ms.  ncu: issue slots
-// 53 % busy with 12-15 consumer warps per SM, mbarrier waits 2 per issue -- the remaining gap to the HBM roofline
+// 53 % busy with 15 consumer warps per SM, mbarrier waits 2.5-4 per issue -- the remaining gap to the HBM roofline
 // is issue efficiency at that occupancy (the ring needs the whole 227 KB of shared memory, so one CTA per SM).
 //
 // A note for whoever touches the producers: keep their code small.  An earlier version with fully unrolled copy
@@ -31,8 +31,7 @@
 // parity at xh or xh+-1 (which one depends on the parity of y+z+t+par).  So no neighbour table is read.
 // Work item = a group of RG consecutive rows in y (S = RG*Lxh sites, S*n consumer threads).  Per group the
 // producers issue 5 units:  XY (input rows y0-1 .. y0+RG, links x+ x- y+ y-), Z+, Z-, T+, T- (RG input rows
-// and one link array each).  Ring: one big slot for XY units and three small slots for the others; one producer
-// warp per slot class.
+// and one link array each).  Ring: one big slot for XY units and three small slots for the others.
 #include "wd_blas.cuh"
 #include "wd_su3.cuh"
 
@@ -249,7 +248,8 @@ __device__ __forceinline__ void dir_smem(const typename Vec<T>::type* sp, uint32
 }
 
 // ---- the kernel -----------------------------------------------------------------------------------------
-// grid = min(groups, SMs) persistent CTAs; block = consumer warps (S*n threads, rounded up) + 2 producer warps.
+// grid = min(groups, SMs) persistent CTAs; block = consumer warps (S*n threads, rounded up) + 1 producer warp
+// (16 warps in all at n = 5, so the consumers get 128 registers; a second producer warp bought nothing).
 // dynamic smem: 128 bytes of mbarriers, then the ring: [big slot][NS small slots], NS = as many as fit (>= 3).
 template <typename T, int RECON, bool DAG, int EPI, int MAXT>
 __global__ void __launch_bounds__(MAXT, 1) hop_tma_kernel(const TmaArgs<T> A) {
@@ -271,12 +271,12 @@ __global__ void __launch_bounds__(MAXT, 1) hop_tma_kernel(const TmaArgs<T> A) {
     [[maybe_unused]] double dsum[3] = {0.0, 0.0, 0.0};
 
     if (warp >= ncw) {
-        // ================= two producer warps (one per slot class, so neither queue waits behind the other): every bulk copy of this CTA's groups ======================
+        // ================= producer warp: every bulk copy of this CTA's groups ======================
         uint32_t q = 0;
         for (uint32_t g = A.g_first + blockIdx.x; g < A.groups; g += gridDim.x) {
             const uint32_t yg = g % gy, zt = g / gy, z = zt % A.Lz, t = zt / A.Lz;
-            if (warp == ncw) produce_xy<T, RECON>(A, lane, yg * A.RG, z, t, q, ring, full, empty);
-            else             produce_small<T, RECON>(A, lane, yg * A.RG, z, t, q, ring, full, empty);
+            produce_xy<T, RECON>(A, lane, yg * A.RG, z, t, q, ring, full, empty);
+            produce_small<T, RECON>(A, lane, yg * A.RG, z, t, q, ring, full, empty);
             ++q;
         }
     } else {
@@ -333,9 +333,11 @@ __global__ void __launch_bounds__(MAXT, 1) hop_tma_kernel(const TmaArgs<T> A) {
             __syncwarp();
             if (lane == 0) mbar_arrive(&empty[0]);
             // ---- Z+, Z-, T+, T- units
+            [[maybe_unused]] cx<T> qv[12];   // the xpay operand: requested before the wait for the last unit
 #pragma unroll
             for (int u = 0; u < 4; ++u) {
                 const uint32_t m = 4 * q + u, slot = 1 + m % A.NS, use = m / A.NS;
+                if (EPI >= EPI_XPAY && u == 3 && active) load_spinor(A.in2 + own, rowV, e0, qv);
                 mbar_wait(&full[slot], use & 1);
                 if (active) {
                     const vec* sp = reinterpret_cast<const vec*>(ring) + A.big_vecs + (size_t)(slot - 1) * A.small_vecs +
@@ -354,8 +356,6 @@ __global__ void __launch_bounds__(MAXT, 1) hop_tma_kernel(const TmaArgs<T> A) {
             // ---- epilogue and store
             if (active) {
                 if (EPI >= EPI_XPAY) {
-                    cx<T> qv[12];
-                    load_spinor(A.in2 + own, rowV, e0, qv);
 #pragma unroll
                     for (int k = 0; k < 12; ++k) {
                         acc[k].re = fma(A.b, acc[k].re, A.a * qv[k].re);
@@ -373,7 +373,6 @@ __global__ void __launch_bounds__(MAXT, 1) hop_tma_kernel(const TmaArgs<T> A) {
                     }
                 }
                 if (EPI == EPI_SIGMA) {  // <r~, v> with v = acc
-                    cx<T> qv[12];
                     load_spinor(A.in3 + own, rowV, e0, qv);
                     T s0 = 0, s1 = 0;
 #pragma unroll
@@ -425,7 +424,7 @@ bool pick_shape(const wd_ctx* c, int n, int max_threads, Shape* sh) {
     for (uint32_t RG = Ly; RG >= 1; --RG) {
         if (Ly % RG || RG > cap) continue;
         const uint32_t S = RG * Lxh, rowV = Lxh * n;
-        const uint32_t threads = ((S * n + 31) / 32) * 32 + 64;  // consumer warps + two producer warps
+        const uint32_t threads = ((S * n + 31) / 32) * 32 + 32;  // consumer warps + one producer warp
         if ((int)threads > max_threads) continue;
         const uint32_t lrowV = Lxh * RECON * (uint32_t)sizeof(T) / 16;
         const uint32_t big = ((RG + 2) * Vec<T>::NCH * rowV + 4 * RG * lrowV + 7) / 8 * 8;
@@ -506,11 +505,11 @@ int wd_hop_tma_launch(wd_ctx* c, int prec, int recon, int dag, int n, int par, c
     if (c->order != WD_ORDER_LINEAR || c->RB != (uint32_t)(c->L[0] / 2)) return 1;  // needs the row-major layout
     int rc;
     if (prec == WD_F64) {
-        if (recon == WD_LINK18) rc = launch_tma<double, 18, 416>(c, dag, n, par, o, c->d_U64[0]);
-        else                    rc = launch_tma<double, 12, 416>(c, dag, n, par, o, c->d_U64[1]);
+        if (recon == WD_LINK18) rc = launch_tma<double, 18, 384>(c, dag, n, par, o, c->d_U64[0]);
+        else                    rc = launch_tma<double, 12, 384>(c, dag, n, par, o, c->d_U64[1]);
     } else {
-        if (recon == WD_LINK18) rc = launch_tma<float, 18, 544>(c, dag, n, par, o, c->d_U32[0]);
-        else                    rc = launch_tma<float, 12, 544>(c, dag, n, par, o, c->d_U32[1]);
+        if (recon == WD_LINK18) rc = launch_tma<float, 18, 512>(c, dag, n, par, o, c->d_U32[0]);
+        else                    rc = launch_tma<float, 12, 512>(c, dag, n, par, o, c->d_U32[1]);
     }
     return rc;
 }
