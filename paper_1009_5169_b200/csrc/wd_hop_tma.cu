@@ -94,6 +94,7 @@ struct TmaArgs {
     uint32_t g_first;                  // groups [0, g_first) are the frozen t = 0 slice (Schroedinger functional), else 0
     uint32_t big_vecs, small_vecs;     // slot sizes in 16-byte units
     uint32_t NS;                       // number of small slots in the ring (3..7)
+    uint32_t NP;                       // producer warps: 2 when they fit beside the consumers, else 1
     T a, b;
 };
 
@@ -248,8 +249,8 @@ __device__ __forceinline__ void dir_smem(const typename Vec<T>::type* sp, uint32
 }
 
 // ---- the kernel -----------------------------------------------------------------------------------------
-// grid = min(groups, SMs) persistent CTAs; block = consumer warps (S*n threads, rounded up) + 1 producer warp
-// (16 warps in all at n = 5, so the consumers get 128 registers; a second producer warp bought nothing).
+// grid = min(groups, SMs) persistent CTAs; block = consumer warps (S*n threads, rounded up) + 1 or 2 producer warps
+// (at n = 5: 15 + 1 = 16 warps, so the consumers get 128 registers; a second producer warp bought nothing there).
 // dynamic smem: 128 bytes of mbarriers, then the ring: [big slot][NS small slots], NS = as many as fit (>= 3).
 template <typename T, int RECON, bool DAG, int EPI, int MAXT>
 __global__ void __launch_bounds__(MAXT, 1) hop_tma_kernel(const TmaArgs<T> A) {
@@ -275,8 +276,9 @@ __global__ void __launch_bounds__(MAXT, 1) hop_tma_kernel(const TmaArgs<T> A) {
         uint32_t q = 0;
         for (uint32_t g = A.g_first + blockIdx.x; g < A.groups; g += gridDim.x) {
             const uint32_t yg = g % gy, zt = g / gy, z = zt % A.Lz, t = zt / A.Lz;
-            produce_xy<T, RECON>(A, lane, yg * A.RG, z, t, q, ring, full, empty);
-            produce_small<T, RECON>(A, lane, yg * A.RG, z, t, q, ring, full, empty);
+            // one producer warp issues both slot classes; with two, warp ncw takes the XY units and warp ncw+1 the others
+            if (A.NP == 1 || warp == ncw) produce_xy<T, RECON>(A, lane, yg * A.RG, z, t, q, ring, full, empty);
+            if (A.NP == 1 || warp != ncw) produce_small<T, RECON>(A, lane, yg * A.RG, z, t, q, ring, full, empty);
             ++q;
         }
     } else {
@@ -412,7 +414,7 @@ __global__ void __launch_bounds__(MAXT, 1) hop_tma_kernel(const TmaArgs<T> A) {
 constexpr size_t kSmemMax = 227 * 1024;
 
 struct Shape {
-    uint32_t RG, S, threads, big_vecs, small_vecs, NS;
+    uint32_t RG, S, threads, big_vecs, small_vecs, NS, NP;
     size_t smem;
 };
 
@@ -424,8 +426,12 @@ bool pick_shape(const wd_ctx* c, int n, int max_threads, Shape* sh) {
     for (uint32_t RG = Ly; RG >= 1; --RG) {
         if (Ly % RG || RG > cap) continue;
         const uint32_t S = RG * Lxh, rowV = Lxh * n;
-        const uint32_t threads = ((S * n + 31) / 32) * 32 + 32;  // consumer warps + one producer warp
-        if ((int)threads > max_threads) continue;
+        // consumer warps + a producer warp; a second one (it helps when groups are small and frequent: 146 against
+        // 166 us at n = 12) only if the block stays within the thread budget, i.e. keeps its registers
+        const uint32_t cthreads = ((S * n + 31) / 32) * 32;
+        if ((int)cthreads + 32 > max_threads) continue;
+        const uint32_t NP = (int)cthreads + 64 <= max_threads ? 2u : 1u;
+        const uint32_t threads = cthreads + 32 * NP;
         const uint32_t lrowV = Lxh * RECON * (uint32_t)sizeof(T) / 16;
         const uint32_t big = ((RG + 2) * Vec<T>::NCH * rowV + 4 * RG * lrowV + 7) / 8 * 8;
         const uint32_t small = (RG * Vec<T>::NCH * rowV + RG * lrowV + 7) / 8 * 8;
@@ -434,6 +440,7 @@ bool pick_shape(const wd_ctx* c, int n, int max_threads, Shape* sh) {
         while (NS < 7 && 128 + ((size_t)big + (NS + 1) * (size_t)small) * 16 <= kSmemMax) ++NS;
         const size_t smem = 128 + ((size_t)big + NS * (size_t)small) * 16;
         sh->NS = NS;
+        sh->NP = NP;
         sh->RG = RG; sh->S = S; sh->threads = threads; sh->big_vecs = big; sh->small_vecs = small; sh->smem = smem;
         return true;
     }
@@ -470,7 +477,7 @@ int launch_tma(wd_ctx* c, int dag, int n, int par, const wd_hop_ops& o, const T*
     const uint32_t gy = A.Ly / sh.RG;
     A.groups = gy * A.Lz * A.Lt;
     A.g_first = c->bc == WD_BC_SF ? gy * A.Lz : 0;
-    A.big_vecs = sh.big_vecs; A.small_vecs = sh.small_vecs; A.NS = sh.NS;
+    A.big_vecs = sh.big_vecs; A.small_vecs = sh.small_vecs; A.NS = sh.NS; A.NP = sh.NP;
     A.a = (T)o.a; A.b = (T)o.b;
     const uint32_t real = A.groups - A.g_first;
     const unsigned G = real < (uint32_t)c->n_sm ? real : (unsigned)c->n_sm;
