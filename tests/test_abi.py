@@ -54,3 +54,30 @@ def test_create_rejects_bad_arguments_without_a_gpu_call():
     assert L.wd_create(ctypes.byref(h), (ctypes.c_int * 4)(4, 4, 4, 2), 0.1, 1, 5, None) == wd.EINVAL
     assert L.wd_destroy(None) == wd.EINVAL
     assert L.wd_workspace_bytes(None) == 0
+
+
+def test_option_and_enum_constants_match_header():
+    """The binding's integer constants are the header's (the binding only marshals arguments)."""
+    from paper_1009_5169_b200 import wd
+    hdr = open(os.path.join(ROOT, "include", "wd.h")).read()
+    hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
+    consts = {k: int(v) for k, v in re.findall(r"\b(WD_[A-Z0-9_]+)\s*=\s*(-?\d+)", hdr)}
+    pairs = {"WD_OK": wd.OK, "WD_EINVAL": wd.EINVAL, "WD_ENOCONV": wd.ENOCONV, "WD_BC_PERIODIC": wd.BC_PERIODIC,
+             "WD_BC_SF": wd.BC_SF, "WD_OP_D": wd.OP_D, "WD_OP_DDAG": wd.OP_DDAG, "WD_F64": wd.F64, "WD_F32": wd.F32,
+             "WD_LINK18": wd.LINK18, "WD_LINK12": wd.LINK12, "WD_ORDER_LINEAR": wd.ORDER_LINEAR,
+             "WD_ORDER_TILED": wd.ORDER_TILED, "WD_OPT_HOP32_SITES": wd.OPT_HOP32_SITES,
+             "WD_OPT_HOP64_SITES": wd.OPT_HOP64_SITES, "WD_OPT_HOP32_REGS": wd.OPT_HOP32_REGS,
+             "WD_OPT_HOP64_REGS": wd.OPT_HOP64_REGS, "WD_OPT_POLL_EVERY": wd.OPT_POLL_EVERY,
+             "WD_OPT_HOP_IMPL": wd.OPT_HOP_IMPL, "WD_OPT_ALTERNATE_SWEEP": wd.OPT_ALTERNATE_SWEEP,
+             "WD_OPT_HOP_ROWS": wd.OPT_HOP_ROWS}
+    for name, val in pairs.items():
+        assert consts[name] == val, name
+    assert len(wd.PROF_NAMES) == consts["WD_PROF_N"]
+
+
+def test_set_option_rejects_null_context():
+    from paper_1009_5169_b200 import wd
+    L = wd.lib()
+    assert L.wd_set_option(None, 0, 1) == wd.EINVAL
+    v = ctypes.c_int()
+    assert L.wd_get_option(None, 0, ctypes.byref(v)) == wd.EINVAL
