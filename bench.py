@@ -417,8 +417,8 @@ def run_ours(args):
             traffic = tr["dram_bytes_per_launch"]
     except Exception:
         pass
-    roofline = {"bound": "hbm", "kernel": f"{kname} (fp32 multi-RHS Wilson hop inside the inner solver; launch time includes "
-                                          "the 15-block finalize kernel that follows the two fused-reduction launches)",
+    roofline = {"bound": "hbm", "kernel": f"{kname} (fp32 multi-RHS Wilson hop inside the inner solver, 2 of 4 launches per iteration with "
+                                          "fused xpay + inner-product epilogues)",
                 "achieved": round(achieved, 1), "peak": peak_gbs, "unit": "GB/s", "frac": round(achieved / peak_gbs, 4),
                 "peak_source": peak_src, "traffic": traffic, "bytes_per_launch": hop_bytes,
                 "avg_launch_us": round(hop_us, 2), "launches_in_step": hop_cnt,

@@ -389,7 +389,7 @@ __global__ void __launch_bounds__(MAXT, 1) hop_tma_kernel(const TmaArgs<T> A) {
         }
     }
     if (EPI >= EPI_SIGMA) {
-        // per-column sums of this CTA -> one partial per (column, value); finalize_partials_kernel follows
+        // per-column sums of this CTA -> one partial per (column, value)
         constexpr int K = EPI == EPI_SIGMA ? 2 : 3;
         __syncthreads();  // every bulk copy has been consumed: the ring is free
         double* red = reinterpret_cast<double*>(ring);
@@ -407,6 +407,28 @@ __global__ void __launch_bounds__(MAXT, 1) hop_tma_kernel(const TmaArgs<T> A) {
             for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
             if (lane == 0) A.rb.partials[(size_t)item * gridDim.x + blockIdx.x] = v;
         }
+        // With at most one CTA per SM there are few partials: the last CTA to get here adds them (fixed order) and
+        // runs the scalar recurrence itself, so no finalize kernel follows this launch.
+        double* tot = red + K * nct;   // n * K totals behind the per-thread sums, then the "last CTA" flag
+        volatile uint32_t* is_last = reinterpret_cast<volatile uint32_t*>(tot + A.n * K);  // (no static shared memory: the
+        __threadfence();                                                                    //  ring may take all 227 KB)
+        __syncthreads();
+        if (threadIdx.x == 0) *is_last = (atomicAdd(A.rb.ticket, 1u) == gridDim.x - 1) ? 1u : 0u;
+        __syncthreads();
+        if (*is_last == 0u) return;
+        __threadfence();
+        for (uint32_t item = warp; item < A.n * K; item += nwarps) {
+            const double* p = A.rb.partials + (size_t)item * gridDim.x;
+            double v = 0.0;
+            for (uint32_t g = lane; g < gridDim.x; g += 32) v += __ldcg(p + g);
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+            if (lane == 0) tot[item] = v;
+        }
+        __syncthreads();
+        if (threadIdx.x < A.n)
+            wdblas::finalize_column<EPI == EPI_SIGMA ? wdblas::K_SIGMA : wdblas::K_OMEGA>(A.rb.scal, (int)threadIdx.x, tot + threadIdx.x * K);
+        if (threadIdx.x == 0) *A.rb.ticket = 0u;
     }
 }
 
@@ -496,11 +518,6 @@ int launch_tma(wd_ctx* c, int dag, int n, int par, const wd_hop_ops& o, const T*
     }
 #undef WD_TMA_CASE
     if (rc) return rc;
-    if (o.epi == EPI_SIGMA)
-        wdblas::finalize_partials_kernel<2, wdblas::K_SIGMA><<<2 * n, 256, 0, c->stream>>>(n, G, A.rb, c->d_totals);
-    else if (o.epi == EPI_OMEGA)
-        wdblas::finalize_partials_kernel<3, wdblas::K_OMEGA><<<3 * n, 256, 0, c->stream>>>(n, G, A.rb, c->d_totals);
-    if (o.epi >= EPI_SIGMA) c->launches++;
     return WD_OK;
 }
 
