@@ -15,10 +15,11 @@
 //
 // Measured (B200, 24^4, n_rhs = 5, fp32, L2-cold, standalone): 71 us (12-real links) / 70 us (18-real), results bit
 // for bit those of the register kernel, which takes 70 us in the chunk-major layout and 76 us in this one.  Inside
-// the solver (half of the launches carry the fused xpay / inner-product epilogues) this kernel averages 81 us per
-// launch against 91 us for the register kernel: one MD force evaluation 95.1 ms against 108.7 ms.  ncu: issue slots
-// 53 % busy with 15 consumer warps per SM, mbarrier waits 2.5-4 per issue -- the remaining gap to the HBM roofline
-// is issue efficiency at that occupancy (the ring needs the whole 227 KB of shared memory, so one CTA per SM).
+// the solver (half of the launches carry the fused xpay / inner-product epilogues) this kernel averages 84 us per
+// launch against 91 us for the register kernel.  Where the time goes: producers alone 43 us,
+// consumers alone 51 us (32 us of pure issue time), together 70: the ring is one group deep (it takes the whole
+// 227 KB of shared memory, one CTA per SM), so the fourth small unit of a group and the next XY unit arrive late
+// (mbarrier waits: 18 % of the stall samples).
 //
 // A note for whoever touches the producers: keep their code small.  An earlier version with fully unrolled copy
 // loops (fp64, 12 chunks) made ptxas run out of uniform registers and emit R2UR.FILL spills around the UBLKCP
