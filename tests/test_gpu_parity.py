@@ -240,6 +240,8 @@ STAGED_CASES = [
     ((6, 4, 4, 4), wi.BC_PERIODIC, 2),      # Lx/2 odd: 18-real fp32 links fall back to the register kernel
     ((2, 2, 2, 4), wi.BC_SF, 12),
     ((8, 8, 8, 8), wi.BC_SF, 16),
+    ((8, 6, 4, 4), wi.BC_SF, 7),            # Ly = 6: row groups of 6, 3, 2 or 1 rows
+    ((4, 10, 2, 6), wi.BC_PERIODIC, 4),     # Ly = 10, Lz = 2 (z+ and z- neighbours coincide)
 ]
 
 
