@@ -155,7 +155,7 @@ int wd_create(wd_ctx** out, const int dims[4], double kappa, int time_bc, int ma
     for (int k = 0; k < WD_OPT_N; ++k) c->opt[k] = 0;
     // hop CTA shape and register budget: 0 = chosen per launch from n_rhs (wd_hop.cu)
     c->opt[WD_OPT_POLL_EVERY] = 4;
-    c->opt[WD_OPT_HOP_IMPL] = 1;
+    c->opt[WD_OPT_HOP_IMPL] = 2;
     c->opt[WD_OPT_ALTERNATE_SWEEP] = 1;
     c->prof_on = false;
     c->prof_used = 0;
@@ -196,6 +196,8 @@ int wd_set_option(wd_ctx* ctx, int key, int value) {
             if (value != 0 && (value < 32 || value > 255)) return wd_fail(ctx, WD_EINVAL, "register budget out of range");
             break;
         case WD_OPT_HOP_IMPL:
+            if (value < 0 || value > 2) return wd_fail(ctx, WD_EINVAL, "hop implementation is 0, 1 or 2");
+            break;
         case WD_OPT_ALTERNATE_SWEEP:
             if (value != 0 && value != 1) return wd_fail(ctx, WD_EINVAL, "this option is 0 or 1");
             break;

@@ -174,11 +174,7 @@ int wd_force_impl(wd_ctx* c, int n, const double* X, const double* Y, double* F)
     B = (B + 31) / 32 * 32;
     A.coef = 2.0 * c->kappa;
     const size_t smem = sizeof(double) * 4 * (size_t)A.spb * n * 18;
-    static bool attr_set = false;
-    if (!attr_set) {
-        cudaFuncSetAttribute(force_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024);
-        attr_set = true;
-    }
+    WD_CUDA_CHECK(c, wd_ensure_smem_attr(c, (const void*)force_kernel, 160 * 1024));
     const unsigned G = (unsigned)((2 * c->Vh + A.spb - 1) / A.spb);
     wd_prof_scope prof(c, WD_PROF_FORCE);
     force_kernel<<<G, B, smem, c->stream>>>(A);

@@ -102,14 +102,28 @@ __global__ void __maxnreg__(MAXREG) hop_kernel(const HopArgs<T> A) {
                 if (EPI == EPI_SIGMA) asm volatile("prefetch.global.L2 [%0];" ::"l"(A.in3 + own + c * rbn + eo));
             }
         }
-        hop_dir<T, RECON, 0, true, DAG>(A, hb, ho, r, n0.x, acc);
-        hop_dir<T, RECON, 0, false, DAG>(A, hb, ho, r, n0.y, acc);
-        hop_dir<T, RECON, 1, true, DAG>(A, hb, ho, r, n0.z, acc);
-        hop_dir<T, RECON, 1, false, DAG>(A, hb, ho, r, n0.w, acc);
-        hop_dir<T, RECON, 2, true, DAG>(A, hb, ho, r, n1.x, acc);
-        hop_dir<T, RECON, 2, false, DAG>(A, hb, ho, r, n1.y, acc);
-        hop_dir<T, RECON, 3, true, DAG>(A, hb, ho, r, n1.z, acc);
-        hop_dir<T, RECON, 3, false, DAG>(A, hb, ho, r, n1.w, acc);
+        if constexpr (sizeof(T) == 4) {
+            // fp32: the order in which the z-march kernel (wd_hop_zm.cu) consumes its units, so that the two
+            // kernels agree bit for bit
+            hop_dir<T, RECON, 3, true, DAG>(A, hb, ho, r, n1.z, acc);
+            hop_dir<T, RECON, 3, false, DAG>(A, hb, ho, r, n1.w, acc);
+            hop_dir<T, RECON, 2, false, DAG>(A, hb, ho, r, n1.y, acc);
+            hop_dir<T, RECON, 1, false, DAG>(A, hb, ho, r, n0.w, acc);
+            hop_dir<T, RECON, 1, true, DAG>(A, hb, ho, r, n0.z, acc);
+            hop_dir<T, RECON, 0, false, DAG>(A, hb, ho, r, n0.y, acc);
+            hop_dir<T, RECON, 0, true, DAG>(A, hb, ho, r, n0.x, acc);
+            hop_dir<T, RECON, 2, true, DAG>(A, hb, ho, r, n1.x, acc);
+        } else {
+            // fp64: the order of wd_hop_tma.cu's units (the staged kernel that serves fp64)
+            hop_dir<T, RECON, 0, true, DAG>(A, hb, ho, r, n0.x, acc);
+            hop_dir<T, RECON, 0, false, DAG>(A, hb, ho, r, n0.y, acc);
+            hop_dir<T, RECON, 1, true, DAG>(A, hb, ho, r, n0.z, acc);
+            hop_dir<T, RECON, 1, false, DAG>(A, hb, ho, r, n0.w, acc);
+            hop_dir<T, RECON, 2, true, DAG>(A, hb, ho, r, n1.x, acc);
+            hop_dir<T, RECON, 2, false, DAG>(A, hb, ho, r, n1.y, acc);
+            hop_dir<T, RECON, 3, true, DAG>(A, hb, ho, r, n1.z, acc);
+            hop_dir<T, RECON, 3, false, DAG>(A, hb, ho, r, n1.w, acc);
+        }
         if (EPI >= EPI_XPAY) {
             cx<T> q[12];
             load_spinor(A.in2 + own, rbn, eo, q);
@@ -223,8 +237,10 @@ int wd_hop_launch_ex(wd_ctx* c, int prec, int recon, int dag, int n, int par, co
     if (o.epi >= EPI_SIGMA && prec != WD_F32) return wd_fail(c, WD_EINVAL, "fused reductions are fp32 only");
     // staged kernel where it applies (row-major layout) and pays: with 1-2 columns a group of rows gives it too few
     // consumer threads (24^4 fp32: 41 us against 33 us at n = 2; 71 against 76 at n = 5; 146 against 151 at n = 12)
-    if (c->opt[WD_OPT_HOP_IMPL] == 1 && n >= 3) {
-        const int rc = wd_hop_tma_launch(c, prec, recon, dag, n, par, o);
+    if (c->opt[WD_OPT_HOP_IMPL] >= 1 && n >= 3) {
+        int rc = 1;
+        if (c->opt[WD_OPT_HOP_IMPL] == 2) rc = wd_hop_zm_launch(c, prec, recon, dag, n, par, o);
+        if (rc > 0) rc = wd_hop_tma_launch(c, prec, recon, dag, n, par, o);
         if (rc <= 0) {
             if (rc == WD_OK) WD_LAUNCH_CHECK(c);
             return rc;

@@ -35,48 +35,14 @@
 // and one link array each).  Ring: one big slot for XY units and three small slots for the others.
 #include "wd_blas.cuh"
 #include "wd_su3.cuh"
+#include "wd_tma.cuh"
 
 using namespace wdk;
+using namespace wdtma;
 
 namespace {
 
 enum { EPI_NONE = 0, EPI_XPAY = 1, EPI_SIGMA = 2, EPI_OMEGA = 3 };
-
-// ---- mbarrier / bulk-copy PTX ---------------------------------------------------------------------
-__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
-}
-__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
-}
-__device__ __forceinline__ bool mbar_try_wait(uint64_t* bar, uint32_t parity) {
-    uint32_t ok;
-    asm volatile(
-        "{\n"
-        ".reg .pred p;\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
-        "selp.u32 %0, 1, 0, p;\n"
-        "}\n"
-        : "=r"(ok)
-        : "r"(smem_u32(bar)), "r"(parity)
-        : "memory");
-    return ok != 0;
-}
-__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
-    while (!mbar_try_wait(bar, parity)) {}
-}
-// global -> shared bulk copy, completion counted in bytes on `bar` (sizes and addresses multiples of 16)
-__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
-                     smem_u32(dst)),
-                 "l"(src), "r"(bytes), "r"(smem_u32(bar))
-                 : "memory");
-}
-
 
 // ---- arguments -------------------------------------------------------------------------------------
 template <typename T>
@@ -266,7 +232,7 @@ __global__ void __launch_bounds__(MAXT, 1) hop_tma_kernel(const TmaArgs<T> A) {
     const uint32_t warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     if (threadIdx.x == 0) {
         for (uint32_t s = 0; s < 1 + A.NS; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], ncw); }
-        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        mbar_fence_init();
     }
     __syncthreads();
     const uint32_t gy = A.Ly / A.RG;
@@ -472,12 +438,8 @@ bool pick_shape(const wd_ctx* c, int n, int max_threads, Shape* sh) {
 
 template <typename T, int RECON, bool DAG, int EPI, int MAXT>
 int launch_one(wd_ctx* c, const TmaArgs<T>& A, const Shape& sh, unsigned G) {
-    static bool attr_set = false;
     auto kern = hop_tma_kernel<T, RECON, DAG, EPI, MAXT>;
-    if (!attr_set) {
-        WD_CUDA_CHECK(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemMax));
-        attr_set = true;
-    }
+    WD_CUDA_CHECK(c, wd_ensure_smem_attr(c, (const void*)kern, (int)kSmemMax));
     kern<<<G, sh.threads, sh.smem, c->stream>>>(A);
     return WD_OK;
 }

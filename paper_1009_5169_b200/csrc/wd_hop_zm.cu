@@ -1,0 +1,452 @@
+// wd_hop_zm.cu -- the multi-RHS Wilson hopping kernel (hot-path step a2), "z-march" form:
+// persistent CTAs that walk along z with a sliding window of three lattice planes resident in shared memory.
+//
+// Why: the first staged kernel (wd_hop_tma.cu) re-stages the z+-1 and t+-1 neighbours of every group of 8 rows,
+// 42 input rows per 8 output rows = 5.25 x the input spinor through the L2 -> SM path (ncu r01e: 524 MB per launch
+// against 223 MB algorithmic; "producers alone" 43 us = the L2 read ceiling), and it consumes a unit in 0.35 us
+// that takes >= 1 us to arrive, with a ring that is one group deep.  Here a CTA owns a "column" (RG consecutive
+// rows in y at fixed t) and marches z = z0, z0+1, ...: the centre plane of one step is the z- plane of the next
+// and its z+ plane becomes the centre, so per step only ONE new plane (RG rows), the two y-halo rows and the
+// t+-1 rows (2 RG) are copied: (3 RG + 2) / RG = 3.33 x at RG = 6 instead of 5.25 x.  Every buffer is released
+// as soon as its last direction has been consumed (order t+, t-, z-, y-, y+, x-, x+, z+) and refilled for the
+// next step while the rest of this step computes, so each copy has about one step time (~2 us) to land.
+//
+// Geometry (linear site order, row-major native layout RB = Lx/2, as wd_hop_tma.cu): row = (y, z, t), Lxh sites.
+// Work: steps s = (column c, z), c = yb + gy * (t - t0), z fastest; CTA b takes the contiguous range
+// [b S / G, (b+1) S / G) of the S = gy (Lt - t0) Lz steps (t0 = 1 with Schroedinger-functional boundaries: the
+// stored t = 0 slice stays zero and is only ever read as a neighbour).  When a range crosses into the next column
+// the window restarts (three planes instead of one: a bubble of one copy latency, at most twice per CTA).
+//
+// Shared memory (fp32, 24^4, n = 5, RG = 6, 18-real links: 225.9 KB): 3 planes x RG rows | T+ RG rows | T- RG rows
+// | 2 halo rows | links: 8 blocks of RG link rows in consumption order.  Units and their barriers:
+//   U1 {T+ rows, link t+}  U2 {T- rows, link t-}  U3 {link z-}  U4 {halo rows, links y-, y+}  U5 {links x-, x+, z+}
+//   W[j % 3] plane with sequence number j (consecutive z of a column; +3 at a column switch).
+// One producer warp issues every cp.async.bulk (lane-parallel); consumer thread = (site of the step, column r),
+// r fastest: conflict-free 128-bit shared-memory reads, results bit for bit those of the register kernel
+// (wd_hop.cu accumulates the directions in the same order).
+#include "wd_blas.cuh"
+#include "wd_su3.cuh"
+#include "wd_tma.cuh"
+
+using namespace wdk;
+using namespace wdtma;
+
+namespace {
+
+enum { EPI_NONE = 0, EPI_XPAY = 1, EPI_SIGMA = 2, EPI_OMEGA = 3 };
+enum { U_TP = 0, U_TM = 1, U_ZM = 2, U_Y = 3, U_XZ = 4, NUNIT = 5 };
+// link blocks in shared memory, in consumption order
+enum { LK_TP = 0, LK_TM = 1, LK_ZM = 2, LK_YM = 3, LK_YP = 4, LK_XM = 5, LK_XP = 6, LK_ZP = 7 };
+
+template <typename T>
+struct ZmArgs {
+    const typename Vec<T>::type* in;
+    typename Vec<T>::type* out;
+    const typename Vec<T>::type* in2;
+    const typename Vec<T>::type* in3;
+    const T* U;
+    wdblas::RedBuf rb;
+    const double* done;
+    uint32_t Lxh, Ly, Lz, Lt;
+    uint32_t Vh, n, par;
+    uint32_t RG, S;          // rows per step, sites per step = RG * Lxh
+    uint32_t gy;             // Ly / RG
+    uint32_t t0;             // first dynamical time slice
+    uint32_t steps;          // gy * (Lt - t0) * Lz
+    uint32_t zero_rows;      // rows of the frozen t = 0 slice to clear (SF), else 0
+    T a, b;
+};
+
+__device__ __forceinline__ uint32_t winc(uint32_t v, uint32_t L) { return v + 1 == L ? 0u : v + 1; }
+__device__ __forceinline__ uint32_t wdec(uint32_t v, uint32_t L) { return v == 0 ? L - 1 : v - 1; }
+
+// ---- shared-memory operand reads ---------------------------------------------------------------------------
+__device__ __forceinline__ void lds_spinor(const float4* __restrict__ sp, uint32_t stride, uint32_t e, cx<float> (&psi)[12]) {
+#pragma unroll
+    for (int c = 0; c < 6; ++c) {
+        const float4 v = sp[c * stride + e];
+        psi[2 * c].re = v.x; psi[2 * c].im = v.y; psi[2 * c + 1].re = v.z; psi[2 * c + 1].im = v.w;
+    }
+}
+template <int RECON>
+__device__ __forceinline__ void lds_link(const float4* __restrict__ L, uint32_t S, uint32_t site, cx<float> (&u)[9]) {
+#pragma unroll
+    for (int c = 0; c < (RECON == 18 ? 4 : 3); ++c) {
+        const float4 v = L[c * S + site];
+        u[2 * c].re = v.x; u[2 * c].im = v.y; u[2 * c + 1].re = v.z; u[2 * c + 1].im = v.w;
+    }
+    if (RECON == 18) {
+        const float2 w = reinterpret_cast<const float2*>(L + 4 * S)[site];
+        u[8].re = w.x; u[8].im = w.y;
+    }
+}
+
+template <typename T, int RECON, int MU, bool FWD, bool DAG>
+__device__ __forceinline__ void dir_smem(const typename Vec<T>::type* sp, uint32_t stride, uint32_t e,
+                                         const typename Vec<T>::type* L, uint32_t S, uint32_t site, cx<T> (&acc)[12]) {
+    constexpr int SIGMA = (FWD ? 1 : -1) * (DAG ? -1 : 1);
+    cx<T> psi[12], hs[6], chi[6], u[9];
+    lds_spinor(sp, stride, e, psi);
+    lds_link<RECON>(L, S, site, u);
+    if (RECON == 12) rebuild_row3(u);
+    project<MU, SIGMA>(psi, hs);
+    su3_mul<!FWD>(u, hs, chi);
+    accumulate<MU, SIGMA>(acc, chi);
+}
+
+// ---- the kernel -------------------------------------------------------------------------------------------
+// block = consumer warps (S * n threads, rounded up) + one producer warp; grid = min(steps, SMs).
+// dynamic smem: 128 B of mbarriers | planes 3 x RG rows | T+ | T- | halo 2 rows | links 8 x RG link rows
+template <typename T, int RECON, bool DAG, int EPI, int MAXT>
+__global__ void __launch_bounds__(MAXT, 1) hop_zm_kernel(const ZmArgs<T> A) {
+    typedef typename Vec<T>::type vec;
+    constexpr uint32_t NCH = Vec<T>::NCH;
+    if (A.done != nullptr && *A.done != 0.0) return;
+    extern __shared__ __align__(128) unsigned char smem[];
+    uint64_t* full_u = reinterpret_cast<uint64_t*>(smem);   // [5]
+    uint64_t* empty_u = full_u + NUNIT;                      // [5]
+    uint64_t* full_w = empty_u + NUNIT;                      // [3]
+    uint64_t* empty_w = full_w + 3;                          // [3]
+    const uint32_t RG = A.RG, rowV = A.Lxh * A.n;
+    const uint32_t rowB = rowV * 16 * NCH;                               // bytes of one spinor row (all chunks)
+    const uint32_t lrowB = A.Lxh * RECON * (uint32_t)sizeof(T);          // bytes of one row of one link array
+    char* const base = reinterpret_cast<char*>(smem) + 128;
+    char* const planes = base;
+    char* const tp = planes + (size_t)3 * RG * rowB;
+    char* const tm = tp + (size_t)RG * rowB;
+    char* const halo = tm + (size_t)RG * rowB;
+    char* const links = halo + (size_t)2 * rowB;
+    const uint32_t nct = A.S * A.n, ncw = (nct + 31) >> 5;
+    const uint32_t warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    if (threadIdx.x == 0) {
+        for (uint32_t u = 0; u < NUNIT; ++u) { mbar_init(&full_u[u], 1); mbar_init(&empty_u[u], ncw); }
+        for (uint32_t w = 0; w < 3; ++w) { mbar_init(&full_w[w], 1); mbar_init(&empty_w[w], ncw); }
+        mbar_fence_init();
+    }
+    __syncthreads();
+    const uint32_t s_begin = (uint32_t)(((uint64_t)blockIdx.x * A.steps) / gridDim.x);
+    const uint32_t s_end = (uint32_t)(((uint64_t)(blockIdx.x + 1) * A.steps) / gridDim.x);
+    [[maybe_unused]] double dsum[3] = {0.0, 0.0, 0.0};
+
+    if (warp >= ncw) {
+        // ================= producer warp ===============================================================
+        const char* in = reinterpret_cast<const char*>(A.in);
+        const char* U = reinterpret_cast<const char*>(A.U);
+        const size_t ublk = (size_t)RECON * A.Vh * sizeof(T);   // bytes of one (mu, parity) link array
+        uint32_t issued = 0, a = 0, prev_col = 0xffffffffu;
+        for (uint32_t s = s_begin, k = 0; s < s_end; ++s, ++k) {
+            const uint32_t col = s / A.Lz, z = s - col * A.Lz;
+            const uint32_t yb = col % A.gy, t = A.t0 + col / A.gy, y0 = yb * RG;
+            if (k > 0) a += (col == prev_col) ? 1u : 3u;
+            prev_col = col;
+            const uint32_t eph = (k & 1) ^ 1;
+            const uint32_t row0 = y0 + A.Ly * (z + A.Lz * t);
+            const uint32_t rtp = y0 + A.Ly * (z + A.Lz * winc(t, A.Lt)), rtm = y0 + A.Ly * (z + A.Lz * wdec(t, A.Lt));
+            const uint32_t rzm = y0 + A.Ly * (wdec(z, A.Lz) + A.Lz * t);
+            // ---- U1: T+ rows, link t+ = U_t(x) on the output rows
+            mbar_wait(&empty_u[U_TP], eph);
+            if (lane == 0) mbar_expect_tx(&full_u[U_TP], RG * (rowB + lrowB));
+            __syncwarp();
+            if (lane == 0) bulk_g2s(tp, in + (size_t)rtp * rowB, RG * rowB, &full_u[U_TP]);
+            else if (lane == 1) bulk_g2s(links + (size_t)LK_TP * RG * lrowB, U + (size_t)(6 + A.par) * ublk + (size_t)row0 * lrowB, RG * lrowB, &full_u[U_TP]);
+            // ---- U2: T- rows, link t- = U_t(x - t^) on the t-1 rows of the other parity
+            mbar_wait(&empty_u[U_TM], eph);
+            if (lane == 0) mbar_expect_tx(&full_u[U_TM], RG * (rowB + lrowB));
+            __syncwarp();
+            if (lane == 0) bulk_g2s(tm, in + (size_t)rtm * rowB, RG * rowB, &full_u[U_TM]);
+            else if (lane == 1) bulk_g2s(links + (size_t)LK_TM * RG * lrowB, U + (size_t)(6 + 1 - A.par) * ublk + (size_t)rtm * lrowB, RG * lrowB, &full_u[U_TM]);
+            // ---- U3: link z- = U_z(x - z^) on the z-1 rows of the other parity
+            mbar_wait(&empty_u[U_ZM], eph);
+            if (lane == 0) {
+                mbar_expect_tx(&full_u[U_ZM], RG * lrowB);
+                bulk_g2s(links + (size_t)LK_ZM * RG * lrowB, U + (size_t)(4 + 1 - A.par) * ublk + (size_t)rzm * lrowB, RG * lrowB, &full_u[U_ZM]);
+            }
+            __syncwarp();
+            // ---- window planes up to sequence number a + 2 (one per step; three at a column start)
+            while (issued <= a + 2) {
+                const uint32_t d = issued - a;   // 0, 1, 2 = z-1, z, z+1
+                const uint32_t zz = d == 0 ? wdec(z, A.Lz) : (d == 1 ? z : winc(z, A.Lz));
+                const uint32_t w = issued % 3, use = issued / 3;
+                mbar_wait(&empty_w[w], (use & 1) ^ 1);
+                if (lane == 0) {
+                    mbar_expect_tx(&full_w[w], RG * rowB);
+                    bulk_g2s(planes + (size_t)w * RG * rowB, in + (size_t)(y0 + A.Ly * (zz + A.Lz * t)) * rowB, RG * rowB, &full_w[w]);
+                }
+                __syncwarp();
+                ++issued;
+            }
+            // ---- U4: halo rows y0-1, y0+RG of the centre plane; links y- = U_y(x - y^) (rows y0-1 .. y0+RG-2 of the
+            //      other parity), y+ = U_y(x)
+            {
+                const bool lo = y0 == 0;
+                const uint32_t zt = A.Ly * (z + A.Lz * t);
+                const uint32_t rm = (lo ? A.Ly - 1 : y0 - 1) + zt, rp = (y0 + RG == A.Ly ? 0 : y0 + RG) + zt;
+                mbar_wait(&empty_u[U_Y], eph);
+                if (lane == 0) mbar_expect_tx(&full_u[U_Y], 2 * rowB + 2 * RG * lrowB);
+                __syncwarp();
+                char* lym = links + (size_t)LK_YM * RG * lrowB;
+                const char* uym = U + (size_t)(2 + 1 - A.par) * ublk;
+                if (lane == 0) bulk_g2s(halo, in + (size_t)rm * rowB, rowB, &full_u[U_Y]);
+                else if (lane == 1) bulk_g2s(halo + rowB, in + (size_t)rp * rowB, rowB, &full_u[U_Y]);
+                else if (lane == 2) bulk_g2s(links + (size_t)LK_YP * RG * lrowB, U + (size_t)(2 + A.par) * ublk + (size_t)row0 * lrowB, RG * lrowB, &full_u[U_Y]);
+                else if (lane == 3) bulk_g2s(lym, uym + (size_t)rm * lrowB, lrowB, &full_u[U_Y]);   // row y0-1 (may wrap)
+                else if (lane == 4 && RG > 1) bulk_g2s(lym + lrowB, uym + (size_t)row0 * lrowB, (RG - 1) * lrowB, &full_u[U_Y]);
+            }
+            // ---- U5: links x- = U_x(x - x^) (same rows, other parity), x+ = U_x(x), z+ = U_z(x)
+            mbar_wait(&empty_u[U_XZ], eph);
+            if (lane == 0) mbar_expect_tx(&full_u[U_XZ], 3 * RG * lrowB);
+            __syncwarp();
+            if (lane == 0) bulk_g2s(links + (size_t)LK_XM * RG * lrowB, U + (size_t)(0 + 1 - A.par) * ublk + (size_t)row0 * lrowB, RG * lrowB, &full_u[U_XZ]);
+            else if (lane == 1) bulk_g2s(links + (size_t)LK_XP * RG * lrowB, U + (size_t)(0 + A.par) * ublk + (size_t)row0 * lrowB, RG * lrowB, &full_u[U_XZ]);
+            else if (lane == 2) bulk_g2s(links + (size_t)LK_ZP * RG * lrowB, U + (size_t)(4 + A.par) * ublk + (size_t)row0 * lrowB, RG * lrowB, &full_u[U_XZ]);
+        }
+    } else {
+        // ================= consumers: thread i = (site s of the step, column r) ==========================
+        const uint32_t i = threadIdx.x;
+        const bool active = i < nct;
+        const uint32_t sidx = i / A.n, r = i - sidx * A.n;
+        const uint32_t j = sidx / A.Lxh, xh = sidx - j * A.Lxh;   // row inside the step, site inside the row
+        const uint32_t lrowV = lrowB / 16;
+        const uint32_t e0 = xh * A.n + r;
+        const vec* const Pl = reinterpret_cast<const vec*>(planes);
+        const vec* const Tp = reinterpret_cast<const vec*>(tp) + (size_t)j * NCH * rowV;
+        const vec* const Tm = reinterpret_cast<const vec*>(tm) + (size_t)j * NCH * rowV;
+        const vec* const Hl = reinterpret_cast<const vec*>(halo);
+        const vec* const Lk = reinterpret_cast<const vec*>(links) + (size_t)j * lrowV;
+        const uint32_t lblk = RG * lrowV;    // 16-byte units of one link block
+        const uint32_t planeV = RG * NCH * rowV;
+        // SF: the stored t = 0 slice of the output stays zero
+        if (A.zero_rows) {
+            const vec z4 = {};
+            for (uint32_t row = blockIdx.x; row < A.zero_rows; row += gridDim.x)
+                for (uint32_t v = i; v < NCH * rowV; v += ncw * 32) A.out[(size_t)row * NCH * rowV + v] = z4;
+        }
+        uint32_t a = 0, prev_col = 0xffffffffu;
+        for (uint32_t s = s_begin, k = 0; s < s_end; ++s, ++k) {
+            const uint32_t col = s / A.Lz, z = s - col * A.Lz;
+            const uint32_t yb = col % A.gy, t = A.t0 + col / A.gy, y0 = yb * RG;
+            if (k > 0) a += (col == prev_col) ? 1u : 3u;
+            prev_col = col;
+            const bool switch_next = (s + 1 < s_end) && ((s + 1) / A.Lz != col);
+            const uint32_t ph = k & 1;
+            const size_t own = (size_t)(y0 + A.Ly * (z + A.Lz * t) + j) * NCH * rowV;
+            cx<T> acc[12];
+#pragma unroll
+            for (int q = 0; q < 12; ++q) { acc[q].re = 0; acc[q].im = 0; }
+            if (EPI >= EPI_XPAY && active) {
+#pragma unroll
+                for (uint32_t c = 0; c < NCH; ++c) {
+                    asm volatile("prefetch.global.L2 [%0];" ::"l"(A.in2 + own + c * rowV + e0));
+                    if (EPI == EPI_SIGMA) asm volatile("prefetch.global.L2 [%0];" ::"l"(A.in3 + own + c * rowV + e0));
+                }
+            }
+            const uint32_t wm = a % 3, wc = (a + 1) % 3, wp = (a + 2) % 3;
+            const vec* const Pm = Pl + (size_t)wm * planeV + (size_t)j * NCH * rowV;
+            const vec* const Pc = Pl + (size_t)wc * planeV + (size_t)j * NCH * rowV;
+            const vec* const Pp = Pl + (size_t)wp * planeV + (size_t)j * NCH * rowV;
+            // ---- t+
+            mbar_wait(&full_u[U_TP], ph);
+            if (active) dir_smem<T, RECON, 3, true, DAG>(Tp, rowV, e0, Lk + LK_TP * lblk, A.Lxh, xh, acc);
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&empty_u[U_TP]);
+            // ---- t-
+            mbar_wait(&full_u[U_TM], ph);
+            if (active) dir_smem<T, RECON, 3, false, DAG>(Tm, rowV, e0, Lk + LK_TM * lblk, A.Lxh, xh, acc);
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&empty_u[U_TM]);
+            // ---- z-
+            mbar_wait(&full_u[U_ZM], ph);
+            mbar_wait(&full_w[wm], (a / 3) & 1);
+            if (active) dir_smem<T, RECON, 2, false, DAG>(Pm, rowV, e0, Lk + LK_ZM * lblk, A.Lxh, xh, acc);
+            __syncwarp();
+            if (lane == 0) { mbar_arrive(&empty_u[U_ZM]); mbar_arrive(&empty_w[wm]); }
+            // ---- y-, y+
+            mbar_wait(&full_u[U_Y], ph);
+            mbar_wait(&full_w[wc], ((a + 1) / 3) & 1);
+            if (active) {
+                const vec* ym = j == 0 ? Hl : Pc - NCH * rowV;
+                const vec* yp = j == RG - 1 ? Hl + NCH * rowV : Pc + NCH * rowV;
+                dir_smem<T, RECON, 1, false, DAG>(ym, rowV, e0, Lk + LK_YM * lblk, A.Lxh, xh, acc);
+                dir_smem<T, RECON, 1, true, DAG>(yp, rowV, e0, Lk + LK_YP * lblk, A.Lxh, xh, acc);
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&empty_u[U_Y]);
+            // ---- x-, x+, z+
+            [[maybe_unused]] cx<T> qv[12];
+            if (EPI >= EPI_XPAY && active) load_spinor(A.in2 + own, rowV, e0, qv);
+            mbar_wait(&full_u[U_XZ], ph);
+            mbar_wait(&full_w[wp], ((a + 2) / 3) & 1);
+            if (active) {
+                const uint32_t bb = (y0 + j + z + t + A.par) & 1;
+                const uint32_t xp = bb ? winc(xh, A.Lxh) : xh;   // xh of the +x neighbour
+                const uint32_t xm = bb ? xh : wdec(xh, A.Lxh);   // xh of the -x neighbour
+                dir_smem<T, RECON, 0, false, DAG>(Pc, rowV, xm * A.n + r, Lk + LK_XM * lblk, A.Lxh, xm, acc);
+                dir_smem<T, RECON, 0, true, DAG>(Pc, rowV, xp * A.n + r, Lk + LK_XP * lblk, A.Lxh, xh, acc);
+                dir_smem<T, RECON, 2, true, DAG>(Pp, rowV, e0, Lk + LK_ZP * lblk, A.Lxh, xh, acc);
+            }
+            __syncwarp();
+            if (lane == 0) {
+                mbar_arrive(&empty_u[U_XZ]);
+                if (switch_next) { mbar_arrive(&empty_w[wc]); mbar_arrive(&empty_w[wp]); }
+            }
+            // ---- epilogue and store
+            if (active) {
+                if (EPI >= EPI_XPAY) {
+#pragma unroll
+                    for (int q = 0; q < 12; ++q) {
+                        acc[q].re = fma(A.b, acc[q].re, A.a * qv[q].re);
+                        acc[q].im = fma(A.b, acc[q].im, A.a * qv[q].im);
+                    }
+                    if (EPI == EPI_OMEGA) {  // <t, s>, <t, t> with t = acc, s = qv
+                        T s0 = 0, s1 = 0, s2 = 0;
+#pragma unroll
+                        for (int q = 0; q < 12; ++q) {
+                            s0 = fma(acc[q].re, qv[q].re, s0);  s0 = fma(acc[q].im, qv[q].im, s0);
+                            s1 = fma(acc[q].re, qv[q].im, s1);  s1 = fma(-acc[q].im, qv[q].re, s1);
+                            s2 = fma(acc[q].re, acc[q].re, s2); s2 = fma(acc[q].im, acc[q].im, s2);
+                        }
+                        dsum[0] += (double)s0; dsum[1] += (double)s1; dsum[2] += (double)s2;
+                    }
+                }
+                if (EPI == EPI_SIGMA) {  // <r~, v> with v = acc
+                    load_spinor(A.in3 + own, rowV, e0, qv);
+                    T s0 = 0, s1 = 0;
+#pragma unroll
+                    for (int q = 0; q < 12; ++q) {
+                        s0 = fma(qv[q].re, acc[q].re, s0);  s0 = fma(qv[q].im, acc[q].im, s0);
+                        s1 = fma(qv[q].re, acc[q].im, s1);  s1 = fma(-qv[q].im, acc[q].re, s1);
+                    }
+                    dsum[0] += (double)s0; dsum[1] += (double)s1;
+                }
+                store_spinor(A.out + own, rowV, e0, acc);
+            }
+        }
+    }
+    if (EPI >= EPI_SIGMA) {
+        // per-column sums of this CTA -> one partial per (column, value); the last CTA adds the partials in a fixed
+        // order and runs the scalar recurrence (as wd_hop_tma.cu)
+        constexpr int K = EPI == EPI_SIGMA ? 2 : 3;
+        __syncthreads();  // every bulk copy has been consumed: the staging area is free
+        double* red = reinterpret_cast<double*>(base);
+        if (threadIdx.x < nct) {
+#pragma unroll
+            for (int q = 0; q < K; ++q) red[q * nct + threadIdx.x] = dsum[q];
+        }
+        __syncthreads();
+        const uint32_t nwarps = blockDim.x >> 5;
+        for (uint32_t item = warp; item < A.n * K; item += nwarps) {
+            const uint32_t col = item / K, q = item - col * K;
+            double v = 0.0;
+            for (uint32_t ss = lane; ss < A.S; ss += 32) v += red[q * nct + ss * A.n + col];
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+            if (lane == 0) A.rb.partials[(size_t)item * gridDim.x + blockIdx.x] = v;
+        }
+        double* tot = red + K * nct;
+        volatile uint32_t* is_last = reinterpret_cast<volatile uint32_t*>(tot + A.n * K);
+        __threadfence();
+        __syncthreads();
+        if (threadIdx.x == 0) *is_last = (atomicAdd(A.rb.ticket, 1u) == gridDim.x - 1) ? 1u : 0u;
+        __syncthreads();
+        if (*is_last == 0u) return;
+        __threadfence();
+        for (uint32_t item = warp; item < A.n * K; item += nwarps) {
+            const double* p = A.rb.partials + (size_t)item * gridDim.x;
+            double v = 0.0;
+            for (uint32_t g = lane; g < gridDim.x; g += 32) v += __ldcg(p + g);
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+            if (lane == 0) tot[item] = v;
+        }
+        __syncthreads();
+        if (threadIdx.x < A.n)
+            wdblas::finalize_column<EPI == EPI_SIGMA ? wdblas::K_SIGMA : wdblas::K_OMEGA>(A.rb.scal, (int)threadIdx.x, tot + threadIdx.x * K);
+        if (threadIdx.x == 0) *A.rb.ticket = 0u;
+    }
+}
+
+// ---- host side ----------------------------------------------------------------------------------------------
+constexpr size_t kSmemMax = 227 * 1024;
+
+struct Shape {
+    uint32_t RG, S, threads;
+    size_t smem;
+};
+
+// largest row group (a divisor of Ly) whose CTA fits the thread budget and whose buffers fit shared memory
+template <typename T, int RECON>
+bool pick_shape(const wd_ctx* c, int n, int max_threads, Shape* sh) {
+    const uint32_t Lxh = c->L[0] / 2, Ly = c->L[1];
+    const uint32_t cap = c->opt[WD_OPT_HOP_ROWS] > 0 ? (uint32_t)c->opt[WD_OPT_HOP_ROWS] : Ly;
+    for (uint32_t RG = Ly; RG >= 1; --RG) {
+        if (Ly % RG || RG > cap) continue;
+        const uint32_t S = RG * Lxh;
+        const uint32_t cthreads = ((S * n + 31) / 32) * 32;
+        if ((int)cthreads + 32 > max_threads) continue;
+        const size_t rowB = (size_t)Lxh * n * 16 * Vec<T>::NCH, lrowB = (size_t)Lxh * RECON * sizeof(T);
+        const size_t smem = 128 + (5 * (size_t)RG + 2) * rowB + 8 * (size_t)RG * lrowB;
+        if (smem > kSmemMax) continue;
+        // the epilogue's reduction scratch (3 sums per consumer thread + totals) reuses the staging area
+        if ((size_t)(3 * S * n + 3 * WD_MAX_RHS + 2) * sizeof(double) > smem - 128) continue;
+        sh->RG = RG; sh->S = S; sh->threads = cthreads + 32; sh->smem = smem;
+        return true;
+    }
+    return false;
+}
+
+template <typename T, int RECON, bool DAG, int EPI, int MAXT>
+int launch_one(wd_ctx* c, const ZmArgs<T>& A, const Shape& sh, unsigned G) {
+    auto kern = hop_zm_kernel<T, RECON, DAG, EPI, MAXT>;
+    WD_CUDA_CHECK(c, wd_ensure_smem_attr(c, (const void*)kern, (int)kSmemMax));
+    kern<<<G, sh.threads, sh.smem, c->stream>>>(A);
+    return WD_OK;
+}
+
+template <typename T, int RECON, int MAXT>
+int launch_zm(wd_ctx* c, int dag, int n, int par, const wd_hop_ops& o, const T* U) {
+    Shape sh;
+    if (!pick_shape<T, RECON>(c, n, MAXT, &sh)) return 1;
+    ZmArgs<T> A;
+    A.in = (const typename Vec<T>::type*)o.in;
+    A.out = (typename Vec<T>::type*)o.out;
+    A.in2 = (const typename Vec<T>::type*)o.in2;
+    A.in3 = (const typename Vec<T>::type*)o.in3;
+    A.U = U;
+    A.rb = wdblas::RedBuf{c->d_scal, c->d_partials, c->d_ticket};
+    A.done = o.check_done ? c->d_scal + wdblas::G_DONE : nullptr;
+    A.Lxh = c->L[0] / 2; A.Ly = c->L[1]; A.Lz = c->L[2]; A.Lt = c->L[3];
+    A.Vh = (uint32_t)c->Vh; A.n = (uint32_t)n; A.par = (uint32_t)par;
+    A.RG = sh.RG; A.S = sh.S;
+    A.gy = A.Ly / sh.RG;
+    A.t0 = c->bc == WD_BC_SF ? 1u : 0u;
+    A.steps = A.gy * (A.Lt - A.t0) * A.Lz;
+    A.zero_rows = c->bc == WD_BC_SF ? A.Ly * A.Lz : 0u;
+    A.a = (T)o.a; A.b = (T)o.b;
+    const unsigned G = A.steps < (uint32_t)c->n_sm ? A.steps : (unsigned)c->n_sm;
+    int rc;
+#define WD_ZM_CASE(D, E) rc = launch_one<T, RECON, D, E, MAXT>(c, A, sh, G)
+    if (dag) {
+        if (o.epi == EPI_NONE) WD_ZM_CASE(true, EPI_NONE);
+        else if (o.epi == EPI_XPAY) WD_ZM_CASE(true, EPI_XPAY);
+        else if (o.epi == EPI_SIGMA) WD_ZM_CASE(true, EPI_SIGMA);
+        else WD_ZM_CASE(true, EPI_OMEGA);
+    } else {
+        if (o.epi == EPI_NONE) WD_ZM_CASE(false, EPI_NONE);
+        else if (o.epi == EPI_XPAY) WD_ZM_CASE(false, EPI_XPAY);
+        else if (o.epi == EPI_SIGMA) WD_ZM_CASE(false, EPI_SIGMA);
+        else WD_ZM_CASE(false, EPI_OMEGA);
+    }
+#undef WD_ZM_CASE
+    return rc;
+}
+
+}  // namespace
+
+// Returns WD_OK if launched, a positive value if this lattice / option set is not served by this kernel (tiled site
+// order, fp64, nothing fits): the caller then tries wd_hop_tma.cu's kernel and then the register kernel.
+int wd_hop_zm_launch(wd_ctx* c, int prec, int recon, int dag, int n, int par, const wd_hop_ops& o) {
+    if (c->order != WD_ORDER_LINEAR || c->RB != (uint32_t)(c->L[0] / 2)) return 1;  // needs the row-major layout
+    if (prec != WD_F32) return 1;
+    if (recon == WD_LINK18) return launch_zm<float, 18, 416>(c, dag, n, par, o, c->d_U32[0]);
+    return launch_zm<float, 12, 416>(c, dag, n, par, o, c->d_U32[1]);
+}

@@ -60,6 +60,9 @@ struct wd_ctx {
 
     long long launches;
     std::string err;
+    // kernels whose MaxDynamicSharedMemorySize attribute has been raised on THIS context's device (function
+    // attributes are per device, and a context is bound to one device)
+    std::vector<const void*> smem_attr_done;
 
     // optional per-class device timing (wd_profile): CUDA event pairs around the classed launches
     bool prof_on;
@@ -125,6 +128,15 @@ static inline int wd_fail(wd_ctx* c, int code, const char* msg) {
         }                                                                            \
     } while (0)
 
+// Raise a kernel's dynamic shared-memory limit once per context (i.e. per device).
+static inline cudaError_t wd_ensure_smem_attr(wd_ctx* c, const void* kern, int bytes) {
+    for (const void* k : c->smem_attr_done)
+        if (k == kern) return cudaSuccess;
+    const cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    if (e == cudaSuccess) c->smem_attr_done.push_back(kern);
+    return e;
+}
+
 // ---- internal entry points (device pointers, no argument checks) -------------------------------
 // wd_hop.cu
 // out[h][r] = (xpay ? a * in2 + b * (H in) : H in) on output parity `par`; in/out/in2 half-lattice blocks.
@@ -144,6 +156,8 @@ struct wd_hop_ops {
 int wd_hop_launch_ex(wd_ctx* c, int prec, int recon, int dag, int n, int par, const wd_hop_ops& o);
 // wd_hop_tma.cu: the shared-memory-staged (bulk copy + mbarrier) form; > 0 = not applicable, use the plain kernel
 int wd_hop_tma_launch(wd_ctx* c, int prec, int recon, int dag, int n, int par, const wd_hop_ops& o);
+// wd_hop_zm.cu: the z-marching sliding-window form (fp32); > 0 = not applicable
+int wd_hop_zm_launch(wd_ctx* c, int prec, int recon, int dag, int n, int par, const wd_hop_ops& o);
 int wd_hop_launch(wd_ctx* c, int prec, int recon, int dag, int n, int par, const void* in, void* out,
                   const void* in2, double a, double b);
 

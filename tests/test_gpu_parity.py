@@ -247,7 +247,7 @@ STAGED_CASES = [
 
 @pytest.mark.parametrize("dims,bc,n_rhs", STAGED_CASES)
 def test_staged_hop_kernel_matches_oracle_and_register_kernel(dims, bc, n_rhs):
-    """WD_OPT_HOP_IMPL = 1 (bulk-copy staged kernel): parity with the oracle at the D-apply tolerances and
+    """WD_OPT_HOP_IMPL = 1, 2 (the bulk-copy staged kernels): parity with the oracle at the D-apply tolerances and
     bit-for-bit agreement with the register kernel (same per-site arithmetic in the same order)."""
     pkg = _wd()
     kappa = 0.13
@@ -263,15 +263,20 @@ def test_staged_hop_kernel_matches_oracle_and_register_kernel(dims, bc, n_rhs):
             for recon in (pkg.LINK18, pkg.LINK12):
                 ctx.set_option(pkg.OPT_HOP_IMPL, 0)
                 a = ctx.apply(op, nat, n_rhs, prec, recon)
-                ctx.set_option(pkg.OPT_HOP_IMPL, 1)
-                b = ctx.apply(op, nat, n_rhs, prec, recon)
-                assert torch.equal(a, b), (op, prec, recon)
-                out = ctx.unpack(b, n_rhs, prec).cpu().numpy()
-                assert rel_per_rhs(out, ref).max() < tol, (op, prec, recon)
+                for impl in (1, 2):
+                    ctx.set_option(pkg.OPT_HOP_IMPL, impl)
+                    b = ctx.apply(op, nat, n_rhs, prec, recon)
+                    # The register kernel adds the eight directions in the order of the kernel that serves that
+                    # precision by default (fp32: z-march, impl 2; fp64: row-group ring, impl 1, which impl 2 falls
+                    # back to): those pairs agree bit for bit.  fp32 with impl 1 differs by summation order only.
+                    if not (prec == pkg.F32 and impl == 1):
+                        assert torch.equal(a, b), (op, prec, recon, impl)
+                    out = ctx.unpack(b, n_rhs, prec).cpu().numpy()
+                    assert rel_per_rhs(out, ref).max() < tol, (op, prec, recon, impl)
     ctx.close()
 
 
-@pytest.mark.parametrize("impl", [0, 1])
+@pytest.mark.parametrize("impl", [0, 1, 2])
 @pytest.mark.parametrize("recon", [0, 1])
 def test_solve_and_force_with_either_hop_kernel(impl, recon):
     """The fused <rt,v> / <t,s>,<t,t> epilogues of both hop kernels drive the inner BiCGStab: X, Y, F parity."""
@@ -279,7 +284,9 @@ def test_solve_and_force_with_either_hop_kernel(impl, recon):
     cfg, U, Phi = wi.make_config(1, 3)
     dims, kappa, bc, n = cfg["dims"], cfg["kappa"], cfg["bc"], cfg["n_rhs"]
     Xr, rr, _, rc = orc.solve(dims, kappa, bc, 0, U, Phi, tol=1e-14)
+    assert rc == 0 and rr.max() < 1e-13
     Yr, rr, _, rc = orc.solve(dims, kappa, bc, 1, U, Xr, tol=1e-14)
+    assert rc == 0 and rr.max() < 1e-13
     Fr = orc.force(dims, kappa, bc, U, Xr, Yr)
     ctx = make_ctx(dims, kappa, bc, n, U)
     ctx.set_option(pkg.OPT_HOP_IMPL, impl)
@@ -301,7 +308,7 @@ def test_launch_options_change_speed_only():
     U = wi.gauge_field(dims, 0.3, 7, bc)
     psi = wi.spinor_field(dims, n, 11, bc)
     ctx = make_ctx(dims, 0.13, bc, n, U)
-    assert ctx.get_option(pkg.OPT_HOP_IMPL) == 1
+    assert ctx.get_option(pkg.OPT_HOP_IMPL) == 2
     for prec, ks, kr, sites, regs in ((pkg.F32, pkg.OPT_HOP32_SITES, pkg.OPT_HOP32_REGS, (0, 7, 16, 32, 64, 1024), (0, 64, 128)),
                                       (pkg.F64, pkg.OPT_HOP64_SITES, pkg.OPT_HOP64_REGS, (5, 16, 32, 64), (128, 168, 255))):
         nat = ctx.pack(dev(psi), prec)
@@ -312,7 +319,7 @@ def test_launch_options_change_speed_only():
                 ctx.set_option(kr, r)
                 assert torch.equal(ctx.apply(0, nat, n, prec, pkg.LINK12), ref), (prec, s, r)
     for key, val in ((99, 1), (pkg.OPT_HOP32_SITES, -1), (pkg.OPT_HOP32_REGS, 1000), (pkg.OPT_POLL_EVERY, 0),
-                     (pkg.OPT_HOP_IMPL, 2)):
+                     (pkg.OPT_HOP_IMPL, 3)):
         with pytest.raises(pkg.WdError):
             ctx.set_option(key, val)
     P = ctx.pack(dev(psi))
@@ -334,7 +341,7 @@ def test_full_size_bench_configuration_properties():
     cfg, U, Phi = wi.make_config(4, 5)
     dims, kappa, bc, n = cfg["dims"], cfg["kappa"], cfg["bc"], 5
     ctx = make_ctx(dims, kappa, bc, n, U)
-    assert ctx.get_option(pkg.OPT_HOP_IMPL) == 1
+    assert ctx.get_option(pkg.OPT_HOP_IMPL) == 2
     P = ctx.pack(dev(Phi))
     ref = orc.apply(dims, kappa, bc, 0, U, Phi)
     out = ctx.unpack(ctx.apply(pkg.OP_D, P, n), n).cpu().numpy()
