@@ -12,16 +12,16 @@
 // next step while the rest of this step computes, so each copy has about one step time (~2 us) to land.
 //
 // Geometry (linear site order, row-major native layout RB = Lx/2, as wd_hop_tma.cu): row = (y, z, t), Lxh sites.
-// Work: steps s = (column c, z), c = yb + gy * (t - t0), z fastest; CTA b takes the contiguous range
-// [b S / G, (b+1) S / G) of the S = gy (Lt - t0) Lz steps (t0 = 1 with Schroedinger-functional boundaries: the
-// stored t = 0 slice stays zero and is only ever read as a neighbour).  When a range crosses into the next column
-// the window restarts (three planes instead of one: a bubble of one copy latency, at most twice per CTA).
+// Work: steps s = (column c, z), c = yb + gy * (t - t0), z fastest, S = gy (Lt - t0) Lz of them (t0 = 1 with
+// Schroedinger-functional boundaries: the stored t = 0 slice stays zero and is only ever read as a neighbour),
+// cut into chunks of `chunk` consecutive steps; CTA b takes chunks b, b + G, ...  When a chunk crosses into the
+// next column the window restarts (three planes instead of one: a bubble of one copy latency).
 //
 // Shared memory (fp32, 24^4, n = 5, RG = 6, 18-real links: 225.9 KB): 3 planes x RG rows | T+ RG rows | T- RG rows
 // | 2 halo rows | links: 8 blocks of RG link rows in consumption order.  Units and their barriers:
 //   U1 {T+ rows, link t+}  U2 {T- rows, link t-}  U3 {link z-}  U4 {halo rows, links y-, y+}  U5 {links x-, x+, z+}
 //   W[j % 3] plane with sequence number j (consecutive z of a column; +3 at a column switch).
-// One producer warp issues every cp.async.bulk (lane-parallel); consumer thread = (site of the step, column r),
+// Four producer warps issue the cp.async.bulk copies; consumer thread = (site of the step, column r),
 // r fastest: conflict-free 128-bit shared-memory reads, results bit for bit those of the register kernel
 // (wd_hop.cu accumulates the directions in the same order).
 #include "wd_blas.cuh"
@@ -32,6 +32,15 @@ using namespace wdk;
 using namespace wdtma;
 
 namespace {
+#ifndef WD_ZM_ABLATE
+#define WD_ZM_ABLATE 0   // measurement builds only (_work/): 1 = consumers skip the arithmetic, 2 = no copies, no waits
+#endif
+#if WD_ZM_ABLATE == 2
+#define mbar_wait(b, p) ((void)0)
+#define mbar_wait_relaxed(b, p) ((void)0)
+#define bulk_g2s(d, s, n, b) ((void)0)
+#define mbar_expect_tx(b, n) ((void)0)
+#endif
 
 enum { EPI_NONE = 0, EPI_XPAY = 1, EPI_SIGMA = 2, EPI_OMEGA = 3 };
 enum { U_TP = 0, U_TM = 1, U_ZM = 2, U_Y = 3, U_XZ = 4, NUNIT = 5 };
@@ -53,12 +62,23 @@ struct ZmArgs {
     uint32_t gy;             // Ly / RG
     uint32_t t0;             // first dynamical time slice
     uint32_t steps;          // gy * (Lt - t0) * Lz
+    uint32_t chunk;          // steps per chunk; CTA b takes chunks b, b + G, ...
     uint32_t zero_rows;      // rows of the frozen t = 0 slice to clear (SF), else 0
     T a, b;
 };
 
 __device__ __forceinline__ uint32_t winc(uint32_t v, uint32_t L) { return v + 1 == L ? 0u : v + 1; }
 __device__ __forceinline__ uint32_t wdec(uint32_t v, uint32_t L) { return v == 0 ? L - 1 : v - 1; }
+
+// Step sequence of a CTA: chunks b, b + G, ... of `chunk` consecutive steps each.  NO_STEP ends it.
+constexpr uint32_t NO_STEP = 0xffffffffu;
+__device__ __forceinline__ uint32_t next_step(uint32_t s, uint32_t chunk, uint32_t steps) {
+    if ((s + 1) % chunk != 0 && s + 1 < steps) return s + 1;
+    const uint32_t f = (s / chunk + gridDim.x) * chunk;
+    return f < steps ? f : NO_STEP;
+}
+// does step s2 continue the z-march of step s1 (same column, next z)?  Then the window slides by one plane.
+__device__ __forceinline__ bool continues(uint32_t s1, uint32_t s2, uint32_t Lz) { return s2 == s1 + 1 && s2 / Lz == s1 / Lz; }
 
 // ---- shared-memory operand reads ---------------------------------------------------------------------------
 __device__ __forceinline__ void lds_spinor(const float4* __restrict__ sp, uint32_t stride, uint32_t e, cx<float> (&psi)[12]) {
@@ -81,9 +101,16 @@ __device__ __forceinline__ void lds_link(const float4* __restrict__ L, uint32_t 
     }
 }
 
-template <typename T, int RECON, int MU, bool FWD, bool DAG>
+template <typename T, int RECON, int MU, bool FWD, bool DAG, bool FIRST = false>
 __device__ __forceinline__ void dir_smem(const typename Vec<T>::type* sp, uint32_t stride, uint32_t e,
                                          const typename Vec<T>::type* L, uint32_t S, uint32_t site, cx<T> (&acc)[12]) {
+    if (WD_ZM_ABLATE == 1) {
+        if (FIRST) {
+#pragma unroll
+            for (int q = 0; q < 12; ++q) { acc[q].re = 0; acc[q].im = 0; }
+        }
+        return;
+    }
     constexpr int SIGMA = (FWD ? 1 : -1) * (DAG ? -1 : 1);
     cx<T> psi[12], hs[6], chi[6], u[9];
     lds_spinor(sp, stride, e, psi);
@@ -91,32 +118,36 @@ __device__ __forceinline__ void dir_smem(const typename Vec<T>::type* sp, uint32
     if (RECON == 12) rebuild_row3(u);
     project<MU, SIGMA>(psi, hs);
     su3_mul<!FWD>(u, hs, chi);
-    accumulate<MU, SIGMA>(acc, chi);
+    accumulate<MU, SIGMA, FIRST>(acc, chi);
 }
 
 // ---- the kernel -------------------------------------------------------------------------------------------
-// block = consumer warps (S * n threads, rounded up) + one producer warp; grid = min(steps, SMs).
+// block = consumer warps (S * n threads, rounded up) + four producer warps; grid = min(steps, SMs).
 // dynamic smem: 128 B of mbarriers | planes 3 x RG rows | T+ | T- | halo 2 rows | links 8 x RG link rows
-template <typename T, int RECON, bool DAG, int EPI, int MAXT>
+// LXH, NR, RGT: Lx/2, n_rhs and rows per step as compile-time constants (0 = taken from the arguments).  With all
+// three fixed every shared-memory operand address is one per-thread base register plus an immediate; with run-time
+// strides the kernel spent 220 integer instructions per step and ~40 registers on addresses (ncu r02b).
+template <typename T, int RECON, bool DAG, int EPI, int MAXT, int LXH, int NR, int RGT>
 __global__ void __launch_bounds__(MAXT, 1) hop_zm_kernel(const ZmArgs<T> A) {
     typedef typename Vec<T>::type vec;
     constexpr uint32_t NCH = Vec<T>::NCH;
     if (A.done != nullptr && *A.done != 0.0) return;
+    const uint32_t Lxh = LXH ? (uint32_t)LXH : A.Lxh, nr = NR ? (uint32_t)NR : A.n;
     extern __shared__ __align__(128) unsigned char smem[];
     uint64_t* full_u = reinterpret_cast<uint64_t*>(smem);   // [5]
     uint64_t* empty_u = full_u + NUNIT;                      // [5]
     uint64_t* full_w = empty_u + NUNIT;                      // [3]
     uint64_t* empty_w = full_w + 3;                          // [3]
-    const uint32_t RG = A.RG, rowV = A.Lxh * A.n;
+    const uint32_t RG = RGT ? (uint32_t)RGT : A.RG, rowV = Lxh * nr;
     const uint32_t rowB = rowV * 16 * NCH;                               // bytes of one spinor row (all chunks)
-    const uint32_t lrowB = A.Lxh * RECON * (uint32_t)sizeof(T);          // bytes of one row of one link array
+    const uint32_t lrowB = Lxh * RECON * (uint32_t)sizeof(T);            // bytes of one row of one link array
     char* const base = reinterpret_cast<char*>(smem) + 128;
     char* const planes = base;
     char* const tp = planes + (size_t)3 * RG * rowB;
     char* const tm = tp + (size_t)RG * rowB;
     char* const halo = tm + (size_t)RG * rowB;
     char* const links = halo + (size_t)2 * rowB;
-    const uint32_t nct = A.S * A.n, ncw = (nct + 31) >> 5;
+    const uint32_t nct = RG * Lxh * nr, ncw = (nct + 31) >> 5;
     const uint32_t warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     if (threadIdx.x == 0) {
         for (uint32_t u = 0; u < NUNIT; ++u) { mbar_init(&full_u[u], 1); mbar_init(&empty_u[u], ncw); }
@@ -124,64 +155,71 @@ __global__ void __launch_bounds__(MAXT, 1) hop_zm_kernel(const ZmArgs<T> A) {
         mbar_fence_init();
     }
     __syncthreads();
-    const uint32_t s_begin = (uint32_t)(((uint64_t)blockIdx.x * A.steps) / gridDim.x);
-    const uint32_t s_end = (uint32_t)(((uint64_t)(blockIdx.x + 1) * A.steps) / gridDim.x);
+    const uint32_t s_first = blockIdx.x * A.chunk;   // < steps: the grid has at most ceil(steps / chunk) CTAs
     [[maybe_unused]] double dsum[3] = {0.0, 0.0, 0.0};
 
     if (warp >= ncw) {
-        // ================= producer warp ===============================================================
+        // ================= producer warps ================================================================
+        // One thread can start a bulk copy only every ~280 ns (measured: _work/ubench/tma_stream2.cu; the copy engine
+        // itself takes 8 issuers in parallel at 85-92 GB/s per SM), and a step needs 13-14 copies, so the units are
+        // dealt to FOUR producer warps, each walking the steps on its own and waiting only for its own buffers:
+        //   P0: U1 {T+ rows, link t+}, U3 {link z-}      P1: U2 {T- rows, link t-}, window planes
+        //   P2: U4 {halo rows, links y-, y+}             P3: U5 {links x-, x+, z+}
+        const uint32_t role = warp - ncw;
         const char* in = reinterpret_cast<const char*>(A.in);
         const char* U = reinterpret_cast<const char*>(A.U);
         const size_t ublk = (size_t)RECON * A.Vh * sizeof(T);   // bytes of one (mu, parity) link array
-        uint32_t issued = 0, a = 0, prev_col = 0xffffffffu;
-        for (uint32_t s = s_begin, k = 0; s < s_end; ++s, ++k) {
+        uint32_t issued = 0, a = 0, prev = NO_STEP;
+        for (uint32_t s = s_first, k = 0; s != NO_STEP; prev = s, s = next_step(s, A.chunk, A.steps), ++k) {
             const uint32_t col = s / A.Lz, z = s - col * A.Lz;
             const uint32_t yb = col % A.gy, t = A.t0 + col / A.gy, y0 = yb * RG;
-            if (k > 0) a += (col == prev_col) ? 1u : 3u;
-            prev_col = col;
+            if (k > 0) a += continues(prev, s, A.Lz) ? 1u : 3u;
             const uint32_t eph = (k & 1) ^ 1;
             const uint32_t row0 = y0 + A.Ly * (z + A.Lz * t);
-            const uint32_t rtp = y0 + A.Ly * (z + A.Lz * winc(t, A.Lt)), rtm = y0 + A.Ly * (z + A.Lz * wdec(t, A.Lt));
-            const uint32_t rzm = y0 + A.Ly * (wdec(z, A.Lz) + A.Lz * t);
-            // ---- U1: T+ rows, link t+ = U_t(x) on the output rows
-            mbar_wait(&empty_u[U_TP], eph);
-            if (lane == 0) mbar_expect_tx(&full_u[U_TP], RG * (rowB + lrowB));
-            __syncwarp();
-            if (lane == 0) bulk_g2s(tp, in + (size_t)rtp * rowB, RG * rowB, &full_u[U_TP]);
-            else if (lane == 1) bulk_g2s(links + (size_t)LK_TP * RG * lrowB, U + (size_t)(6 + A.par) * ublk + (size_t)row0 * lrowB, RG * lrowB, &full_u[U_TP]);
-            // ---- U2: T- rows, link t- = U_t(x - t^) on the t-1 rows of the other parity
-            mbar_wait(&empty_u[U_TM], eph);
-            if (lane == 0) mbar_expect_tx(&full_u[U_TM], RG * (rowB + lrowB));
-            __syncwarp();
-            if (lane == 0) bulk_g2s(tm, in + (size_t)rtm * rowB, RG * rowB, &full_u[U_TM]);
-            else if (lane == 1) bulk_g2s(links + (size_t)LK_TM * RG * lrowB, U + (size_t)(6 + 1 - A.par) * ublk + (size_t)rtm * lrowB, RG * lrowB, &full_u[U_TM]);
-            // ---- U3: link z- = U_z(x - z^) on the z-1 rows of the other parity
-            mbar_wait(&empty_u[U_ZM], eph);
-            if (lane == 0) {
-                mbar_expect_tx(&full_u[U_ZM], RG * lrowB);
-                bulk_g2s(links + (size_t)LK_ZM * RG * lrowB, U + (size_t)(4 + 1 - A.par) * ublk + (size_t)rzm * lrowB, RG * lrowB, &full_u[U_ZM]);
-            }
-            __syncwarp();
-            // ---- window planes up to sequence number a + 2 (one per step; three at a column start)
-            while (issued <= a + 2) {
-                const uint32_t d = issued - a;   // 0, 1, 2 = z-1, z, z+1
-                const uint32_t zz = d == 0 ? wdec(z, A.Lz) : (d == 1 ? z : winc(z, A.Lz));
-                const uint32_t w = issued % 3, use = issued / 3;
-                mbar_wait(&empty_w[w], (use & 1) ^ 1);
+            if (role == 0) {
+                // ---- U1: T+ rows, link t+ = U_t(x) on the output rows
+                const uint32_t rtp = y0 + A.Ly * (z + A.Lz * winc(t, A.Lt));
+                mbar_wait_relaxed(&empty_u[U_TP], eph);
+                if (lane == 0) mbar_expect_tx(&full_u[U_TP], RG * (rowB + lrowB));
+                __syncwarp();
+                if (lane == 0) bulk_g2s(tp, in + (size_t)rtp * rowB, RG * rowB, &full_u[U_TP]);
+                else if (lane == 1) bulk_g2s(links + (size_t)LK_TP * RG * lrowB, U + (size_t)(6 + A.par) * ublk + (size_t)row0 * lrowB, RG * lrowB, &full_u[U_TP]);
+                // ---- U3: link z- = U_z(x - z^) on the z-1 rows of the other parity
+                const uint32_t rzm = y0 + A.Ly * (wdec(z, A.Lz) + A.Lz * t);
+                mbar_wait_relaxed(&empty_u[U_ZM], eph);
                 if (lane == 0) {
-                    mbar_expect_tx(&full_w[w], RG * rowB);
-                    bulk_g2s(planes + (size_t)w * RG * rowB, in + (size_t)(y0 + A.Ly * (zz + A.Lz * t)) * rowB, RG * rowB, &full_w[w]);
+                    mbar_expect_tx(&full_u[U_ZM], RG * lrowB);
+                    bulk_g2s(links + (size_t)LK_ZM * RG * lrowB, U + (size_t)(4 + 1 - A.par) * ublk + (size_t)rzm * lrowB, RG * lrowB, &full_u[U_ZM]);
                 }
                 __syncwarp();
-                ++issued;
-            }
-            // ---- U4: halo rows y0-1, y0+RG of the centre plane; links y- = U_y(x - y^) (rows y0-1 .. y0+RG-2 of the
-            //      other parity), y+ = U_y(x)
-            {
+            } else if (role == 1) {
+                // ---- U2: T- rows, link t- = U_t(x - t^) on the t-1 rows of the other parity
+                const uint32_t rtm = y0 + A.Ly * (z + A.Lz * wdec(t, A.Lt));
+                mbar_wait_relaxed(&empty_u[U_TM], eph);
+                if (lane == 0) mbar_expect_tx(&full_u[U_TM], RG * (rowB + lrowB));
+                __syncwarp();
+                if (lane == 0) bulk_g2s(tm, in + (size_t)rtm * rowB, RG * rowB, &full_u[U_TM]);
+                else if (lane == 1) bulk_g2s(links + (size_t)LK_TM * RG * lrowB, U + (size_t)(6 + 1 - A.par) * ublk + (size_t)rtm * lrowB, RG * lrowB, &full_u[U_TM]);
+                // ---- window planes up to sequence number a + 2 (one per step; three at a column start)
+                while (issued <= a + 2) {
+                    const uint32_t d = issued - a;   // 0, 1, 2 = z-1, z, z+1
+                    const uint32_t zz = d == 0 ? wdec(z, A.Lz) : (d == 1 ? z : winc(z, A.Lz));
+                    const uint32_t w = issued % 3, use = issued / 3;
+                    mbar_wait_relaxed(&empty_w[w], (use & 1) ^ 1);
+                    if (lane == 0) {
+                        mbar_expect_tx(&full_w[w], RG * rowB);
+                        bulk_g2s(planes + (size_t)w * RG * rowB, in + (size_t)(y0 + A.Ly * (zz + A.Lz * t)) * rowB, RG * rowB, &full_w[w]);
+                    }
+                    __syncwarp();
+                    ++issued;
+                }
+            } else if (role == 2) {
+                // ---- U4: halo rows y0-1, y0+RG of the centre plane; links y- = U_y(x - y^) (rows y0-1 .. y0+RG-2 of
+                //      the other parity), y+ = U_y(x)
                 const bool lo = y0 == 0;
                 const uint32_t zt = A.Ly * (z + A.Lz * t);
                 const uint32_t rm = (lo ? A.Ly - 1 : y0 - 1) + zt, rp = (y0 + RG == A.Ly ? 0 : y0 + RG) + zt;
-                mbar_wait(&empty_u[U_Y], eph);
+                mbar_wait_relaxed(&empty_u[U_Y], eph);
                 if (lane == 0) mbar_expect_tx(&full_u[U_Y], 2 * rowB + 2 * RG * lrowB);
                 __syncwarp();
                 char* lym = links + (size_t)LK_YM * RG * lrowB;
@@ -191,23 +229,24 @@ __global__ void __launch_bounds__(MAXT, 1) hop_zm_kernel(const ZmArgs<T> A) {
                 else if (lane == 2) bulk_g2s(links + (size_t)LK_YP * RG * lrowB, U + (size_t)(2 + A.par) * ublk + (size_t)row0 * lrowB, RG * lrowB, &full_u[U_Y]);
                 else if (lane == 3) bulk_g2s(lym, uym + (size_t)rm * lrowB, lrowB, &full_u[U_Y]);   // row y0-1 (may wrap)
                 else if (lane == 4 && RG > 1) bulk_g2s(lym + lrowB, uym + (size_t)row0 * lrowB, (RG - 1) * lrowB, &full_u[U_Y]);
+            } else {
+                // ---- U5: links x- = U_x(x - x^) (same rows, other parity), x+ = U_x(x), z+ = U_z(x)
+                mbar_wait_relaxed(&empty_u[U_XZ], eph);
+                if (lane == 0) mbar_expect_tx(&full_u[U_XZ], 3 * RG * lrowB);
+                __syncwarp();
+                if (lane == 0) bulk_g2s(links + (size_t)LK_XM * RG * lrowB, U + (size_t)(0 + 1 - A.par) * ublk + (size_t)row0 * lrowB, RG * lrowB, &full_u[U_XZ]);
+                else if (lane == 1) bulk_g2s(links + (size_t)LK_XP * RG * lrowB, U + (size_t)(0 + A.par) * ublk + (size_t)row0 * lrowB, RG * lrowB, &full_u[U_XZ]);
+                else if (lane == 2) bulk_g2s(links + (size_t)LK_ZP * RG * lrowB, U + (size_t)(4 + A.par) * ublk + (size_t)row0 * lrowB, RG * lrowB, &full_u[U_XZ]);
             }
-            // ---- U5: links x- = U_x(x - x^) (same rows, other parity), x+ = U_x(x), z+ = U_z(x)
-            mbar_wait(&empty_u[U_XZ], eph);
-            if (lane == 0) mbar_expect_tx(&full_u[U_XZ], 3 * RG * lrowB);
-            __syncwarp();
-            if (lane == 0) bulk_g2s(links + (size_t)LK_XM * RG * lrowB, U + (size_t)(0 + 1 - A.par) * ublk + (size_t)row0 * lrowB, RG * lrowB, &full_u[U_XZ]);
-            else if (lane == 1) bulk_g2s(links + (size_t)LK_XP * RG * lrowB, U + (size_t)(0 + A.par) * ublk + (size_t)row0 * lrowB, RG * lrowB, &full_u[U_XZ]);
-            else if (lane == 2) bulk_g2s(links + (size_t)LK_ZP * RG * lrowB, U + (size_t)(4 + A.par) * ublk + (size_t)row0 * lrowB, RG * lrowB, &full_u[U_XZ]);
         }
     } else {
         // ================= consumers: thread i = (site s of the step, column r) ==========================
         const uint32_t i = threadIdx.x;
         const bool active = i < nct;
-        const uint32_t sidx = i / A.n, r = i - sidx * A.n;
-        const uint32_t j = sidx / A.Lxh, xh = sidx - j * A.Lxh;   // row inside the step, site inside the row
+        const uint32_t sidx = i / nr, r = i - sidx * nr;
+        const uint32_t j = sidx / Lxh, xh = sidx - j * Lxh;       // row inside the step, site inside the row
         const uint32_t lrowV = lrowB / 16;
-        const uint32_t e0 = xh * A.n + r;
+        const uint32_t e0 = xh * nr + r;
         const vec* const Pl = reinterpret_cast<const vec*>(planes);
         const vec* const Tp = reinterpret_cast<const vec*>(tp) + (size_t)j * NCH * rowV;
         const vec* const Tm = reinterpret_cast<const vec*>(tm) + (size_t)j * NCH * rowV;
@@ -221,18 +260,16 @@ __global__ void __launch_bounds__(MAXT, 1) hop_zm_kernel(const ZmArgs<T> A) {
             for (uint32_t row = blockIdx.x; row < A.zero_rows; row += gridDim.x)
                 for (uint32_t v = i; v < NCH * rowV; v += ncw * 32) A.out[(size_t)row * NCH * rowV + v] = z4;
         }
-        uint32_t a = 0, prev_col = 0xffffffffu;
-        for (uint32_t s = s_begin, k = 0; s < s_end; ++s, ++k) {
+        uint32_t a = 0, prev = NO_STEP;
+        for (uint32_t s = s_first, k = 0; s != NO_STEP; prev = s, s = next_step(s, A.chunk, A.steps), ++k) {
             const uint32_t col = s / A.Lz, z = s - col * A.Lz;
             const uint32_t yb = col % A.gy, t = A.t0 + col / A.gy, y0 = yb * RG;
-            if (k > 0) a += (col == prev_col) ? 1u : 3u;
-            prev_col = col;
-            const bool switch_next = (s + 1 < s_end) && ((s + 1) / A.Lz != col);
+            if (k > 0) a += continues(prev, s, A.Lz) ? 1u : 3u;
+            const uint32_t s_next = next_step(s, A.chunk, A.steps);
+            const bool switch_next = s_next != NO_STEP && !continues(s, s_next, A.Lz);
             const uint32_t ph = k & 1;
             const size_t own = (size_t)(y0 + A.Ly * (z + A.Lz * t) + j) * NCH * rowV;
             cx<T> acc[12];
-#pragma unroll
-            for (int q = 0; q < 12; ++q) { acc[q].re = 0; acc[q].im = 0; }
             if (EPI >= EPI_XPAY && active) {
 #pragma unroll
                 for (uint32_t c = 0; c < NCH; ++c) {
@@ -246,18 +283,18 @@ __global__ void __launch_bounds__(MAXT, 1) hop_zm_kernel(const ZmArgs<T> A) {
             const vec* const Pp = Pl + (size_t)wp * planeV + (size_t)j * NCH * rowV;
             // ---- t+
             mbar_wait(&full_u[U_TP], ph);
-            if (active) dir_smem<T, RECON, 3, true, DAG>(Tp, rowV, e0, Lk + LK_TP * lblk, A.Lxh, xh, acc);
+            if (active) dir_smem<T, RECON, 3, true, DAG, true>(Tp, rowV, e0, Lk + LK_TP * lblk, Lxh, xh, acc);
             __syncwarp();
             if (lane == 0) mbar_arrive(&empty_u[U_TP]);
             // ---- t-
             mbar_wait(&full_u[U_TM], ph);
-            if (active) dir_smem<T, RECON, 3, false, DAG>(Tm, rowV, e0, Lk + LK_TM * lblk, A.Lxh, xh, acc);
+            if (active) dir_smem<T, RECON, 3, false, DAG>(Tm, rowV, e0, Lk + LK_TM * lblk, Lxh, xh, acc);
             __syncwarp();
             if (lane == 0) mbar_arrive(&empty_u[U_TM]);
             // ---- z-
             mbar_wait(&full_u[U_ZM], ph);
             mbar_wait(&full_w[wm], (a / 3) & 1);
-            if (active) dir_smem<T, RECON, 2, false, DAG>(Pm, rowV, e0, Lk + LK_ZM * lblk, A.Lxh, xh, acc);
+            if (active) dir_smem<T, RECON, 2, false, DAG>(Pm, rowV, e0, Lk + LK_ZM * lblk, Lxh, xh, acc);
             __syncwarp();
             if (lane == 0) { mbar_arrive(&empty_u[U_ZM]); mbar_arrive(&empty_w[wm]); }
             // ---- y-, y+
@@ -266,8 +303,8 @@ __global__ void __launch_bounds__(MAXT, 1) hop_zm_kernel(const ZmArgs<T> A) {
             if (active) {
                 const vec* ym = j == 0 ? Hl : Pc - NCH * rowV;
                 const vec* yp = j == RG - 1 ? Hl + NCH * rowV : Pc + NCH * rowV;
-                dir_smem<T, RECON, 1, false, DAG>(ym, rowV, e0, Lk + LK_YM * lblk, A.Lxh, xh, acc);
-                dir_smem<T, RECON, 1, true, DAG>(yp, rowV, e0, Lk + LK_YP * lblk, A.Lxh, xh, acc);
+                dir_smem<T, RECON, 1, false, DAG>(ym, rowV, e0, Lk + LK_YM * lblk, Lxh, xh, acc);
+                dir_smem<T, RECON, 1, true, DAG>(yp, rowV, e0, Lk + LK_YP * lblk, Lxh, xh, acc);
             }
             __syncwarp();
             if (lane == 0) mbar_arrive(&empty_u[U_Y]);
@@ -278,11 +315,11 @@ __global__ void __launch_bounds__(MAXT, 1) hop_zm_kernel(const ZmArgs<T> A) {
             mbar_wait(&full_w[wp], ((a + 2) / 3) & 1);
             if (active) {
                 const uint32_t bb = (y0 + j + z + t + A.par) & 1;
-                const uint32_t xp = bb ? winc(xh, A.Lxh) : xh;   // xh of the +x neighbour
-                const uint32_t xm = bb ? xh : wdec(xh, A.Lxh);   // xh of the -x neighbour
-                dir_smem<T, RECON, 0, false, DAG>(Pc, rowV, xm * A.n + r, Lk + LK_XM * lblk, A.Lxh, xm, acc);
-                dir_smem<T, RECON, 0, true, DAG>(Pc, rowV, xp * A.n + r, Lk + LK_XP * lblk, A.Lxh, xh, acc);
-                dir_smem<T, RECON, 2, true, DAG>(Pp, rowV, e0, Lk + LK_ZP * lblk, A.Lxh, xh, acc);
+                const uint32_t xp = bb ? winc(xh, Lxh) : xh;   // xh of the +x neighbour
+                const uint32_t xm = bb ? xh : wdec(xh, Lxh);   // xh of the -x neighbour
+                dir_smem<T, RECON, 0, false, DAG>(Pc, rowV, xm * nr + r, Lk + LK_XM * lblk, Lxh, xm, acc);
+                dir_smem<T, RECON, 0, true, DAG>(Pc, rowV, xp * nr + r, Lk + LK_XP * lblk, Lxh, xh, acc);
+                dir_smem<T, RECON, 2, true, DAG>(Pp, rowV, e0, Lk + LK_ZP * lblk, Lxh, xh, acc);
             }
             __syncwarp();
             if (lane == 0) {
@@ -334,23 +371,23 @@ __global__ void __launch_bounds__(MAXT, 1) hop_zm_kernel(const ZmArgs<T> A) {
         }
         __syncthreads();
         const uint32_t nwarps = blockDim.x >> 5;
-        for (uint32_t item = warp; item < A.n * K; item += nwarps) {
+        for (uint32_t item = warp; item < nr * K; item += nwarps) {
             const uint32_t col = item / K, q = item - col * K;
             double v = 0.0;
-            for (uint32_t ss = lane; ss < A.S; ss += 32) v += red[q * nct + ss * A.n + col];
+            for (uint32_t ss = lane; ss < RG * Lxh; ss += 32) v += red[q * nct + ss * nr + col];
 #pragma unroll
             for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
             if (lane == 0) A.rb.partials[(size_t)item * gridDim.x + blockIdx.x] = v;
         }
         double* tot = red + K * nct;
-        volatile uint32_t* is_last = reinterpret_cast<volatile uint32_t*>(tot + A.n * K);
+        volatile uint32_t* is_last = reinterpret_cast<volatile uint32_t*>(tot + nr * K);
         __threadfence();
         __syncthreads();
         if (threadIdx.x == 0) *is_last = (atomicAdd(A.rb.ticket, 1u) == gridDim.x - 1) ? 1u : 0u;
         __syncthreads();
         if (*is_last == 0u) return;
         __threadfence();
-        for (uint32_t item = warp; item < A.n * K; item += nwarps) {
+        for (uint32_t item = warp; item < nr * K; item += nwarps) {
             const double* p = A.rb.partials + (size_t)item * gridDim.x;
             double v = 0.0;
             for (uint32_t g = lane; g < gridDim.x; g += 32) v += __ldcg(p + g);
@@ -359,7 +396,7 @@ __global__ void __launch_bounds__(MAXT, 1) hop_zm_kernel(const ZmArgs<T> A) {
             if (lane == 0) tot[item] = v;
         }
         __syncthreads();
-        if (threadIdx.x < A.n)
+        if (threadIdx.x < nr)
             wdblas::finalize_column<EPI == EPI_SIGMA ? wdblas::K_SIGMA : wdblas::K_OMEGA>(A.rb.scal, (int)threadIdx.x, tot + threadIdx.x * K);
         if (threadIdx.x == 0) *A.rb.ticket = 0u;
     }
@@ -382,24 +419,41 @@ bool pick_shape(const wd_ctx* c, int n, int max_threads, Shape* sh) {
         if (Ly % RG || RG > cap) continue;
         const uint32_t S = RG * Lxh;
         const uint32_t cthreads = ((S * n + 31) / 32) * 32;
-        if ((int)cthreads + 32 > max_threads) continue;
+        if ((int)cthreads + 128 > max_threads) continue;
         const size_t rowB = (size_t)Lxh * n * 16 * Vec<T>::NCH, lrowB = (size_t)Lxh * RECON * sizeof(T);
         const size_t smem = 128 + (5 * (size_t)RG + 2) * rowB + 8 * (size_t)RG * lrowB;
         if (smem > kSmemMax) continue;
         // the epilogue's reduction scratch (3 sums per consumer thread + totals) reuses the staging area
         if ((size_t)(3 * S * n + 3 * WD_MAX_RHS + 2) * sizeof(double) > smem - 128) continue;
-        sh->RG = RG; sh->S = S; sh->threads = cthreads + 32; sh->smem = smem;
+        sh->RG = RG; sh->S = S; sh->threads = cthreads + 128; sh->smem = smem;
         return true;
     }
     return false;
 }
 
-template <typename T, int RECON, bool DAG, int EPI, int MAXT>
+template <typename T, int RECON, bool DAG, int EPI, int MAXT, int LXH, int NR, int RGT>
 int launch_one(wd_ctx* c, const ZmArgs<T>& A, const Shape& sh, unsigned G) {
-    auto kern = hop_zm_kernel<T, RECON, DAG, EPI, MAXT>;
+    auto kern = hop_zm_kernel<T, RECON, DAG, EPI, MAXT, LXH, NR, RGT>;
     WD_CUDA_CHECK(c, wd_ensure_smem_attr(c, (const void*)kern, (int)kSmemMax));
     kern<<<G, sh.threads, sh.smem, c->stream>>>(A);
     return WD_OK;
+}
+
+template <typename T, int RECON, int MAXT, int LXH, int NR, int RGT>
+int launch_epi(wd_ctx* c, const ZmArgs<T>& A, const Shape& sh, unsigned G, int dag, int epi) {
+#define WD_ZM_CASE(D, E) return launch_one<T, RECON, D, E, MAXT, LXH, NR, RGT>(c, A, sh, G)
+    if (dag) {
+        if (epi == EPI_NONE) WD_ZM_CASE(true, EPI_NONE);
+        else if (epi == EPI_XPAY) WD_ZM_CASE(true, EPI_XPAY);
+        else if (epi == EPI_SIGMA) WD_ZM_CASE(true, EPI_SIGMA);
+        else WD_ZM_CASE(true, EPI_OMEGA);
+    } else {
+        if (epi == EPI_NONE) WD_ZM_CASE(false, EPI_NONE);
+        else if (epi == EPI_XPAY) WD_ZM_CASE(false, EPI_XPAY);
+        else if (epi == EPI_SIGMA) WD_ZM_CASE(false, EPI_SIGMA);
+        else WD_ZM_CASE(false, EPI_OMEGA);
+    }
+#undef WD_ZM_CASE
 }
 
 template <typename T, int RECON, int MAXT>
@@ -422,22 +476,30 @@ int launch_zm(wd_ctx* c, int dag, int n, int par, const wd_hop_ops& o, const T* 
     A.steps = A.gy * (A.Lt - A.t0) * A.Lz;
     A.zero_rows = c->bc == WD_BC_SF ? A.Ly * A.Lz : 0u;
     A.a = (T)o.a; A.b = (T)o.b;
-    const unsigned G = A.steps < (uint32_t)c->n_sm ? A.steps : (unsigned)c->n_sm;
-    int rc;
-#define WD_ZM_CASE(D, E) rc = launch_one<T, RECON, D, E, MAXT>(c, A, sh, G)
-    if (dag) {
-        if (o.epi == EPI_NONE) WD_ZM_CASE(true, EPI_NONE);
-        else if (o.epi == EPI_XPAY) WD_ZM_CASE(true, EPI_XPAY);
-        else if (o.epi == EPI_SIGMA) WD_ZM_CASE(true, EPI_SIGMA);
-        else WD_ZM_CASE(true, EPI_OMEGA);
-    } else {
-        if (o.epi == EPI_NONE) WD_ZM_CASE(false, EPI_NONE);
-        else if (o.epi == EPI_XPAY) WD_ZM_CASE(false, EPI_XPAY);
-        else if (o.epi == EPI_SIGMA) WD_ZM_CASE(false, EPI_SIGMA);
-        else WD_ZM_CASE(false, EPI_OMEGA);
+    // Chunk length: a divisor of gy * Lz, the step distance between the columns of t and t + 1, so that the CTAs
+    // working on t-neighbouring columns are at the same z at the same time and the T+- rows one of them copies are
+    // still in L2 when the other copies them as its centre plane (with chunks of steps/G = 14.9 steps the two were
+    // 6.5 steps = 150 MB of traffic apart at 24^4: ncu r02a, DRAM reads 271 MB against 168 MB algorithmic).  Among
+    // those: the smallest makespan, counting 1.5 steps for every window restart.
+    {
+        const uint32_t period = A.gy * A.Lz, G0 = (uint32_t)c->n_sm;
+        double best = 1e30;
+        A.chunk = 1;
+        for (uint32_t L = 1; L <= period; ++L) {
+            if (period % L) continue;
+            const uint32_t nch = (A.steps + L - 1) / L, waves = (nch + G0 - 1) / G0;
+            const double cost = waves * (L + 1.5 * (1 + (L - 1) / A.Lz));
+            if (cost < best) { best = cost; A.chunk = L; }
+        }
     }
-#undef WD_ZM_CASE
-    return rc;
+    const uint32_t nch = (A.steps + A.chunk - 1) / A.chunk;
+    const unsigned G = nch < (uint32_t)c->n_sm ? nch : (unsigned)c->n_sm;
+    // shapes with a compile-time geometry (the paper-shaped lattices of BASELINE.json at their n_rhs); any other
+    // shape runs the same kernel with run-time strides
+#define WD_ZM_GEOM(LXH, NR, RGT) if (A.Lxh == LXH && A.n == NR && A.RG == RGT) return launch_epi<T, RECON, MAXT, LXH, NR, RGT>(c, A, sh, G, dag, o.epi)
+    WD_ZM_GEOM(12, 5, 6);
+#undef WD_ZM_GEOM
+    return launch_epi<T, RECON, MAXT, 0, 0, 0>(c, A, sh, G, dag, o.epi);
 }
 
 }  // namespace
@@ -447,6 +509,6 @@ int launch_zm(wd_ctx* c, int dag, int n, int par, const wd_hop_ops& o, const T* 
 int wd_hop_zm_launch(wd_ctx* c, int prec, int recon, int dag, int n, int par, const wd_hop_ops& o) {
     if (c->order != WD_ORDER_LINEAR || c->RB != (uint32_t)(c->L[0] / 2)) return 1;  // needs the row-major layout
     if (prec != WD_F32) return 1;
-    if (recon == WD_LINK18) return launch_zm<float, 18, 416>(c, dag, n, par, o, c->d_U32[0]);
-    return launch_zm<float, 12, 416>(c, dag, n, par, o, c->d_U32[1]);
+    if (recon == WD_LINK18) return launch_zm<float, 18, 512>(c, dag, n, par, o, c->d_U32[0]);
+    return launch_zm<float, 12, 512>(c, dag, n, par, o, c->d_U32[1]);
 }

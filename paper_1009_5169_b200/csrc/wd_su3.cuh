@@ -110,9 +110,14 @@ __device__ __forceinline__ void project(const cx<T> (&psi)[12], cx<T> (&hs)[6]) 
 }
 
 // ---- acc += reconstruct(chi): upper = (chi0, chi1), lower from the same table ---------------------
-template <int MU, int SIGMA, typename T>
+// FIRST: acc is taken as zero (the first of the eight directions), which saves the 24 additions to 0.
+template <int MU, int SIGMA, bool FIRST = false, typename T>
 __device__ __forceinline__ void accumulate(cx<T> (&acc)[12], const cx<T> (&chi)[6]) {
     const T s = (T)SIGMA;
+    if (FIRST) {
+#pragma unroll
+        for (int k = 0; k < 12; ++k) { acc[k].re = 0; acc[k].im = 0; }
+    }
 #pragma unroll
     for (int a = 0; a < 3; ++a) {
         const cx<T> c0 = chi[a], c1 = chi[3 + a];
