@@ -164,7 +164,7 @@ __global__ void __launch_bounds__(MAXT, 1) hop_zm_kernel(const ZmArgs<T> A) {
         // itself takes 8 issuers in parallel at 85-92 GB/s per SM), and a step needs 13-14 copies, so the units are
         // dealt to FOUR producer warps, each walking the steps on its own and waiting only for its own buffers:
         //   P0: U1 {T+ rows, link t+}, U3 {link z-}      P1: U2 {T- rows, link t-}, window planes
-        //   P2: U4 {halo rows, links y-, y+}             P3: U5 {links x-, x+, z+}
+        //   P2: U4 {halo rows, link y-}                  P3: U4 {link y+}, U5 {links x-, x+, z+}
         const uint32_t role = warp - ncw;
         const char* in = reinterpret_cast<const char*>(A.in);
         const char* U = reinterpret_cast<const char*>(A.U);
@@ -214,23 +214,25 @@ __global__ void __launch_bounds__(MAXT, 1) hop_zm_kernel(const ZmArgs<T> A) {
                     ++issued;
                 }
             } else if (role == 2) {
-                // ---- U4: halo rows y0-1, y0+RG of the centre plane; links y- = U_y(x - y^) (rows y0-1 .. y0+RG-2 of
-                //      the other parity), y+ = U_y(x)
+                // ---- U4 (with P3): halo rows y0-1, y0+RG of the centre plane; link y- = U_y(x - y^) on rows y0-1 ..
+                //      y0+RG-2 of the other parity (one copy unless row y0-1 wraps around)
                 const bool lo = y0 == 0;
                 const uint32_t zt = A.Ly * (z + A.Lz * t);
                 const uint32_t rm = (lo ? A.Ly - 1 : y0 - 1) + zt, rp = (y0 + RG == A.Ly ? 0 : y0 + RG) + zt;
                 mbar_wait_relaxed(&empty_u[U_Y], eph);
-                if (lane == 0) mbar_expect_tx(&full_u[U_Y], 2 * rowB + 2 * RG * lrowB);
+                if (lane == 0) mbar_expect_tx(&full_u[U_Y], 2 * rowB + 2 * RG * lrowB);   // includes P3's y+ copy
                 __syncwarp();
                 char* lym = links + (size_t)LK_YM * RG * lrowB;
                 const char* uym = U + (size_t)(2 + 1 - A.par) * ublk;
                 if (lane == 0) bulk_g2s(halo, in + (size_t)rm * rowB, rowB, &full_u[U_Y]);
                 else if (lane == 1) bulk_g2s(halo + rowB, in + (size_t)rp * rowB, rowB, &full_u[U_Y]);
-                else if (lane == 2) bulk_g2s(links + (size_t)LK_YP * RG * lrowB, U + (size_t)(2 + A.par) * ublk + (size_t)row0 * lrowB, RG * lrowB, &full_u[U_Y]);
-                else if (lane == 3) bulk_g2s(lym, uym + (size_t)rm * lrowB, lrowB, &full_u[U_Y]);   // row y0-1 (may wrap)
-                else if (lane == 4 && RG > 1) bulk_g2s(lym + lrowB, uym + (size_t)row0 * lrowB, (RG - 1) * lrowB, &full_u[U_Y]);
+                else if (lane == 2) bulk_g2s(lym, uym + (size_t)rm * lrowB, (lo ? 1u : RG) * lrowB, &full_u[U_Y]);
+                else if (lane == 3 && lo && RG > 1) bulk_g2s(lym + lrowB, uym + (size_t)row0 * lrowB, (RG - 1) * lrowB, &full_u[U_Y]);
             } else {
+                // ---- link y+ = U_y(x) (part of U4: P2 has announced its bytes), then
                 // ---- U5: links x- = U_x(x - x^) (same rows, other parity), x+ = U_x(x), z+ = U_z(x)
+                mbar_wait_relaxed(&empty_u[U_Y], eph);
+                if (lane == 0) bulk_g2s(links + (size_t)LK_YP * RG * lrowB, U + (size_t)(2 + A.par) * ublk + (size_t)row0 * lrowB, RG * lrowB, &full_u[U_Y]);
                 mbar_wait_relaxed(&empty_u[U_XZ], eph);
                 if (lane == 0) mbar_expect_tx(&full_u[U_XZ], 3 * RG * lrowB);
                 __syncwarp();
