@@ -289,6 +289,46 @@ int orc_solve(const int dims[4], double kappa, int bc, int dag, int n_rhs, const
     return rc;
 }
 
+// The fallback route of orc_solve on its own (SURVEY.md §8(c.4) "fall back to CG on D^dag D x = D^dag phi"), exported so
+// that tests can pin it: same arguments and outputs as orc_solve, iters[r] = CG iterations.  (Export only: cgne_one is
+// unchanged.)
+int orc_solve_cgne(const int dims[4], double kappa, int bc, int dag, int n_rhs, const double* U,
+                   const double* B, double* X, double tol, int max_iter, double* relres, int* iters) {
+    Lattice lat;
+    if (!make_lattice(dims, bc, lat) || n_rhs < 0) return -1;
+    const long n = lat.V * 12;
+    int rc = 0;
+    std::vector<cplx> ax(n);
+    for (int r = 0; r < n_rhs; ++r) {
+        const cplx* b = reinterpret_cast<const cplx*>(B) + (long)r * n;
+        cplx* x = reinterpret_cast<cplx*>(X) + (long)r * n;
+        const int it = cgne_one(lat, kappa, dag, U, b, x, tol, max_iter);
+        apply_one(lat, kappa, dag, U, x, ax.data());
+        double num = 0.0;
+        for (long i = 0; i < n; ++i) num += std::norm(b[i] - ax[i]);
+        const double bn = norm2(n, b);
+        const double rr = bn > 0.0 ? std::sqrt(num / bn) : 0.0;
+        if (relres) relres[r] = rr;
+        if (iters) iters[r] = it;
+        if (!(rr <= 10 * tol)) rc = 1;
+    }
+    return rc;
+}
+
+// out = P_parity in: keeps the sites with (x+y+z+t) mod 2 == parity, zero elsewhere (the even/odd-
+// preconditioned-action variant has phi on even sites only).  in == out is allowed.
+int orc_project_parity(const int dims[4], int parity, int n_rhs, const double* in, double* out) {
+    if (parity != 0 && parity != 1) return -1;
+    const long Lx = dims[0], Ly = dims[1], Lz = dims[2], Lt = dims[3], V = Lx * Ly * Lz * Lt;
+    for (int r = 0; r < n_rhs; ++r)
+        for (long t = 0; t < Lt; ++t) for (long z = 0; z < Lz; ++z) for (long y = 0; y < Ly; ++y) for (long x = 0; x < Lx; ++x) {
+            const long s = x + Lx * (y + Ly * (z + Lz * t));
+            const bool keep = ((x + y + z + t) & 1) == parity;
+            for (int k = 0; k < 24; ++k) out[((long)r * V + s) * 24 + k] = keep ? in[((long)r * V + s) * 24 + k] : 0.0;
+        }
+    return 0;
+}
+
 // F += sum_i 2 kappa TA[ U_mu(x) W^(i)_mu(x) ]   ("F = F + f[x_i,y_i]").
 int orc_force(const int dims[4], double kappa, int bc, int n_rhs, const double* U, const double* X,
               const double* Y, double* F) {

@@ -40,6 +40,8 @@ def lib():
         L.orc_apply.argtypes = [ip, ctypes.c_double, ctypes.c_int, ctypes.c_int, ctypes.c_int, dp, dp, dp]
         L.orc_solve.argtypes = [ip, ctypes.c_double, ctypes.c_int, ctypes.c_int, ctypes.c_int, dp, dp, dp,
                                 ctypes.c_double, ctypes.c_int, dp, ip]
+        L.orc_solve_cgne.argtypes = L.orc_solve.argtypes
+        L.orc_project_parity.argtypes = [ip, ctypes.c_int, ctypes.c_int, dp, dp]
         L.orc_force.argtypes = [ip, ctypes.c_double, ctypes.c_int, ctypes.c_int, dp, dp, dp, dp]
         L.orc_dense_dim.argtypes = [ip, ctypes.c_int]
         L.orc_dense_dim.restype = ctypes.c_long
@@ -102,6 +104,51 @@ def solve(dims, kappa, bc, dag, U, B, tol=1e-14, max_iter=5000):
                          iters.ctypes.data_as(ctypes.POINTER(ctypes.c_int)))
     assert rc >= 0
     return X, relres, iters, rc
+
+
+def solve_cgne(dims, kappa, bc, dag, U, B, tol=1e-14, max_iter=100000):
+    """The CG-on-normal-equations fallback of `solve`, on its own.  Same returns as `solve`."""
+    U = _f64(U)
+    B = _f64(B)
+    n_rhs = B.shape[0]
+    X = np.zeros_like(B)
+    relres = np.zeros(n_rhs, dtype=np.float64)
+    iters = np.zeros(n_rhs, dtype=np.int32)
+    rc = lib().orc_solve_cgne(_dims(dims), float(kappa), int(bc), int(dag), n_rhs, _dp(U), _dp(B), _dp(X),
+                              float(tol), int(max_iter), _dp(relres),
+                              iters.ctypes.data_as(ctypes.POINTER(ctypes.c_int)))
+    assert rc >= 0
+    return X, relres, iters, rc
+
+
+def project_parity(dims, parity, psi) -> np.ndarray:
+    """P_parity psi: the sites with (x+y+z+t) mod 2 == parity kept, the others zero."""
+    psi = _f64(psi)
+    out = np.empty_like(psi)
+    rc = lib().orc_project_parity(_dims(dims), int(parity), psi.shape[0], _dp(psi), _dp(out))
+    assert rc == 0
+    return out
+
+
+def action(X) -> np.ndarray:
+    """Pseudo-fermion action per column, S_i = |x_i|^2 with x_i = D^-1 phi_i (eq. 2.2)."""
+    X = _f64(X)
+    return np.sum(X.reshape(X.shape[0], -1) ** 2, axis=1)
+
+
+def eo_md_force(dims, kappa, bc, U, Phi_e, tol=1e-14):
+    """Even/odd-preconditioned-action variant: phi lives on even sites,
+    S = sum_i |Dhat^-1 phi_i|^2 with Dhat = 1 - kappa^2 H_eo H_oe the Schur complement of D on the even sites.
+    Because D (x_e, kappa H_oe x_e) = (Dhat x_e, 0), Dhat^-1 phi_e = P_e D^-1 (phi_e, 0); so with
+        X = D^-1 (phi_e, 0),   Y = D^dag^-1 (P_e X),
+    S_i = |P_e x_i|^2 and dS = -2 Re(y^dag dD x): the SAME functional f[x, y] as the full action.  Composition of the
+    pinned pieces only.  Returns (X, Y, S per column, F)."""
+    Phi = project_parity(dims, 0, Phi_e)
+    X, r1, _, rc1 = solve(dims, kappa, bc, 0, U, Phi, tol=tol)
+    Xe = project_parity(dims, 0, X)
+    Y, r2, _, rc2 = solve(dims, kappa, bc, 1, U, Xe, tol=tol)
+    assert rc1 == 0 and rc2 == 0, (r1, r2)
+    return X, Y, action(Xe), force(dims, kappa, bc, U, X, Y)
 
 
 def force(dims, kappa, bc, U, X, Y, F=None) -> np.ndarray:

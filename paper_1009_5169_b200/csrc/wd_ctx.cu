@@ -71,7 +71,9 @@ struct WsMap {
 
 const int kReals[2] = {18, 12};
 const size_t kScalDoubles = 64 * WD_MAX_RHS;
-// per column: 3 values x the largest grid of any reducing kernel (BLAS1: 4 x SMs; hop with fused dots: V/2/32 + 1)
+// Reducing kernels write n * K partial sums per block, K <= 3, n <= WD_MAX_RHS.  Largest grids: BLAS1 4 x SMs;
+// staged hops one CTA per SM; the register hop with fused inner products always runs 32 sites per CTA
+// (wd_hop.cu launch_t), i.e. ceil(V/2 / 32) blocks, and checks its grid against this capacity.
 size_t partial_doubles(const wd_ctx* c) {
     const size_t blocks = (size_t)c->Vh / 32 + 1 > 4096 ? (size_t)c->Vh / 32 + 1 : 4096;
     return 3 * blocks * WD_MAX_RHS;
@@ -280,6 +282,7 @@ int wd_set_workspace(wd_ctx* ctx, void* ws_dev, size_t bytes) {
     for (int r = 0; r < 2; ++r) { ctx->d_U64[r] = (double*)(w + m.u64[r]); ctx->d_U32[r] = (float*)(w + m.u32[r]); }
     ctx->d_scal = (double*)(w + m.scal);
     ctx->d_partials = (double*)(w + m.partials);
+    ctx->partial_doubles = partial_doubles(ctx);
     ctx->d_totals = ctx->d_scal + 48 * WD_MAX_RHS;  // tail of the scalar block (kScalDoubles = 64 * WD_MAX_RHS)
     ctx->d_ticket = (unsigned int*)(w + m.ticket);
     ctx->d_solver = w + m.solver;
@@ -326,6 +329,12 @@ int wd_unpack(wd_ctx* ctx, int prec, int n_rhs, const void* native, double* cano
     return wd_layout_unpack(ctx, prec, n_rhs, native, canon);
 }
 
+static int check_solver_params(wd_ctx* ctx, double tol, int max_outer, int max_inner, double inner_tol) {
+    if (!(tol > 0.0) || max_outer < 1 || max_inner < 1 || !(inner_tol >= 0.0) || inner_tol >= 1.0)
+        return wd_fail(ctx, WD_EINVAL, "bad solver parameters");
+    return WD_OK;
+}
+
 static int check_op_args(wd_ctx* ctx, int op, int prec, int recon, int n_rhs, const void* a, const void* b) {
     if (!ctx) return WD_EINVAL;
     if (!a || !b || a == b) return wd_fail(ctx, WD_EINVAL, "null or aliased field pointer");
@@ -363,8 +372,8 @@ int wd_solve_block(wd_ctx* ctx, int op, int n_rhs, const double* Phi, double* X,
                    int max_inner, double inner_tol, int recon, wd_solve_info* info) {
     int rc = check_op_args(ctx, op, WD_F64, recon, n_rhs, Phi, X);
     if (rc) return rc;
-    if (!(tol > 0.0) || max_outer < 1 || max_inner < 1 || inner_tol < 0.0 || inner_tol >= 1.0)
-        return wd_fail(ctx, WD_EINVAL, "bad solver parameters");
+    rc = check_solver_params(ctx, tol, max_outer, max_inner, inner_tol);
+    if (rc) return rc;
     return wd_solve_impl(ctx, op == WD_OP_DDAG, n_rhs, Phi, X, tol, max_outer, max_inner,
                          inner_tol > 0.0 ? inner_tol : 1e-5, recon, info);
 }
@@ -382,7 +391,10 @@ int wd_md_force_host(wd_ctx* ctx, int n_rhs, const double* Phi_host, double* F_h
     if (!ctx) return WD_EINVAL;
     if (!Phi_host || !F_host) return wd_fail(ctx, WD_EINVAL, "null pointer");
     if (bad_n(ctx, n_rhs)) return wd_fail(ctx, WD_EINVAL, "n_rhs out of range");
+    if (recon != WD_LINK18 && recon != WD_LINK12) return wd_fail(ctx, WD_EINVAL, "bad link form");
     if (!ctx->have_gauge) return wd_fail(ctx, WD_ESTATE, "wd_set_gauge first");
+    int rcp = check_solver_params(ctx, tol, max_outer, max_inner, inner_tol);
+    if (rcp) return rcp;
     // staging lives at the END of the solver scratch (sized for max_rhs in wd_solver_scratch_bytes)
     const size_t full = wd_align_up(2 * wd_half_bytes(ctx, WD_F64, ctx->max_rhs));
     const size_t fbytes = wd_align_up(sizeof(double) * 4 * ctx->V * 18);

@@ -177,7 +177,7 @@ void launch_r(wd_ctx* c, const HopArgs<T>& A, int dag, int epi, unsigned G, unsi
 }
 
 template <typename T, int RECON>
-void launch_t(wd_ctx* c, int dag, int n, int par, const wd_hop_ops& o, const T* U) {
+int launch_t(wd_ctx* c, int dag, int n, int par, const wd_hop_ops& o, const T* U) {
     HopArgs<T> A;
     A.in = (const typename Vec<T>::type*)o.in;
     A.out = (typename Vec<T>::type*)o.out;
@@ -208,10 +208,16 @@ void launch_t(wd_ctx* c, int dag, int n, int par, const wd_hop_ops& o, const T* 
                 if ((s * n) % 32 == 0 && s * n >= 64) { sites = s; break; }
         if (f64) sites = 16;
     }
-    while (sites * n > (fused ? 512 : 1024)) sites >>= 1;
-    if (fused && (sites * n) % 32 != 0) sites = 32;  // the block reduction shuffles whole warps (n <= 16: 512 threads)
+    // fused reductions: exactly 32 sites per CTA.  B = 32 n is a multiple of 32 (the block reduction shuffles whole
+    // warps) and at most 512, and the grid is ceil(V/2 / 32) blocks, which is what the partial-sum buffer is sized
+    // for (wd_ctx.cu partial_doubles: n * K * G doubles are written); the option does not apply to these launches.
+    if (fused) sites = 32;
+    while (sites * n > (fused ? 512 : 1024) && sites > 1) sites >>= 1;
+    // the smallest compiled variant needs 128 (fp64) / 64 (fp32) registers per thread: keep one CTA within an SM
+    while ((long)sites * n * (f64 ? 128 : 64) > 65536 && sites > 1) sites >>= 1;
     const unsigned B = (unsigned)(sites * n);
     const unsigned G = (A.total + B - 1) / B;
+    if (fused && (size_t)G * 3 * WD_MAX_RHS > c->partial_doubles) return wd_fail(c, WD_EINVAL, "hop: reduction scratch too small for this grid");
     // largest compiled register budget that the option allows and that lets one CTA of B threads fit
     int regs = c->opt[f64 ? WD_OPT_HOP64_REGS : WD_OPT_HOP32_REGS];
     if (regs == 0) regs = f64 ? 168 : ((n <= 2 || RECON == 18) ? 128 : 64);  // 18-real links: 64 registers spill
@@ -228,6 +234,7 @@ void launch_t(wd_ctx* c, int dag, int n, int par, const wd_hop_ops& o, const T* 
     else if (o.epi == EPI_OMEGA)
         wdblas::finalize_partials_kernel<3, wdblas::K_OMEGA><<<3 * n, 256, 0, c->stream>>>(n, G, A.rb, c->d_totals);
     if (o.epi >= EPI_SIGMA) c->launches++;
+    return WD_OK;
 }
 
 }  // namespace
@@ -246,13 +253,15 @@ int wd_hop_launch_ex(wd_ctx* c, int prec, int recon, int dag, int n, int par, co
             return rc;
         }
     }
+    int rc;
     if (prec == WD_F64) {
-        if (recon == WD_LINK18) launch_t<double, 18>(c, dag, n, par, o, c->d_U64[0]);
-        else                    launch_t<double, 12>(c, dag, n, par, o, c->d_U64[1]);
+        if (recon == WD_LINK18) rc = launch_t<double, 18>(c, dag, n, par, o, c->d_U64[0]);
+        else                    rc = launch_t<double, 12>(c, dag, n, par, o, c->d_U64[1]);
     } else {
-        if (recon == WD_LINK18) launch_t<float, 18>(c, dag, n, par, o, c->d_U32[0]);
-        else                    launch_t<float, 12>(c, dag, n, par, o, c->d_U32[1]);
+        if (recon == WD_LINK18) rc = launch_t<float, 18>(c, dag, n, par, o, c->d_U32[0]);
+        else                    rc = launch_t<float, 12>(c, dag, n, par, o, c->d_U32[1]);
     }
+    if (rc) return rc;
     WD_LAUNCH_CHECK(c);
     return WD_OK;
 }

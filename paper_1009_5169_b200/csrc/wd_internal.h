@@ -50,6 +50,7 @@ struct wd_ctx {
     // solver scratch
     double* d_scal;        // per-RHS scalars (see wd_solve.cu)
     double* d_partials;    // block partial sums
+    size_t partial_doubles; // capacity of d_partials
     double* d_totals;      // 3 * WD_MAX_RHS item totals of the two-kernel reductions
     unsigned int* d_ticket;
     double* h_pinned;      // pinned host mirror for convergence polling (cudaMallocHost, small)

@@ -302,7 +302,8 @@ def test_solve_and_force_with_either_hop_kernel(impl, recon):
 
 
 def test_launch_options_change_speed_only():
-    """CTA shape, register budget and poll interval never change results; bad keys and values are rejected."""
+    """CTA shape, register budget and poll interval never change results; bad keys and values are rejected.
+    The CTA-shape and register options belong to the REGISTER kernel, so the sweep runs with WD_OPT_HOP_IMPL = 0."""
     pkg = _wd()
     dims, bc, n = (8, 4, 6, 10), wi.BC_SF, 5
     U = wi.gauge_field(dims, 0.3, 7, bc)
@@ -310,24 +311,75 @@ def test_launch_options_change_speed_only():
     ctx = make_ctx(dims, 0.13, bc, n, U)
     assert ctx.get_option(pkg.OPT_HOP_IMPL) == 2
     for prec, ks, kr, sites, regs in ((pkg.F32, pkg.OPT_HOP32_SITES, pkg.OPT_HOP32_REGS, (0, 7, 16, 32, 64, 1024), (0, 64, 128)),
-                                      (pkg.F64, pkg.OPT_HOP64_SITES, pkg.OPT_HOP64_REGS, (5, 16, 32, 64), (128, 168, 255))):
+                                      (pkg.F64, pkg.OPT_HOP64_SITES, pkg.OPT_HOP64_REGS, (5, 16, 32, 64, 1024), (128, 168, 255))):
         nat = ctx.pack(dev(psi), prec)
+        ctx.set_option(pkg.OPT_HOP_IMPL, 2)
         ref = ctx.apply(0, nat, n, prec, pkg.LINK12)
+        ctx.set_option(pkg.OPT_HOP_IMPL, 0)
         for s in sites:
             for r in regs:
                 ctx.set_option(ks, s)
                 ctx.set_option(kr, r)
                 assert torch.equal(ctx.apply(0, nat, n, prec, pkg.LINK12), ref), (prec, s, r)
+        ctx.set_option(ks, 0)
+        ctx.set_option(kr, 0)
     for key, val in ((99, 1), (pkg.OPT_HOP32_SITES, -1), (pkg.OPT_HOP32_REGS, 1000), (pkg.OPT_POLL_EVERY, 0),
                      (pkg.OPT_HOP_IMPL, 3)):
         with pytest.raises(pkg.WdError):
             ctx.set_option(key, val)
+    ctx.set_option(pkg.OPT_HOP_IMPL, 2)
     P = ctx.pack(dev(psi))
     ctx.set_option(pkg.OPT_POLL_EVERY, 1)
     X1, i1 = ctx.solve_block(pkg.OP_D, P, n)
     ctx.set_option(pkg.OPT_POLL_EVERY, 7)
     X7, i7 = ctx.solve_block(pkg.OP_D, P, n)
     assert torch.equal(X1, X7) and i1["inner_iters_total"] == i7["inner_iters_total"]
+    ctx.close()
+
+
+@pytest.mark.parametrize("n_rhs", [8, 12, 16])
+def test_register_kernel_solve_for_every_cta_shape(n_rhs):
+    """The register kernel's fused <rt,v> / <t,s>,<t,t> reductions (block partials + finalize kernel) for large
+    n_rhs and every CTA-shape / register option: the solve reaches the tolerance, X has the oracle's true residual and
+    equals the default kernel's X to solver accuracy.  (the partial-sum buffer was sized for 32 sites
+    per CTA while the launch picked 8 or 16 for n_rhs >= 8.)"""
+    pkg = _wd()
+    dims, bc = (8, 8, 8, 8), wi.BC_SF
+    kappa = 0.13
+    U = wi.gauge_field(dims, 0.3, 1, bc)
+    Phi = wi.spinor_field(dims, n_rhs, 1, bc)
+    ctx = make_ctx(dims, kappa, bc, n_rhs, U)
+    P = ctx.pack(dev(Phi))
+    Xd, _ = ctx.solve_block(pkg.OP_D, P, n_rhs, tol=1e-12)
+    Xdc = ctx.unpack(Xd, n_rhs).cpu().numpy()
+    ctx.set_option(pkg.OPT_HOP_IMPL, 0)
+    for sites, regs in ((0, 0), (8, 64), (16, 128), (64, 0)):
+        ctx.set_option(pkg.OPT_HOP32_SITES, sites)
+        ctx.set_option(pkg.OPT_HOP32_REGS, regs)
+        X, info = ctx.solve_block(pkg.OP_D, P, n_rhs, tol=1e-12)
+        assert info["converged"] and max(info["relres"]) <= 1e-12, (sites, regs, info)
+        Xc = ctx.unpack(X, n_rhs).cpu().numpy()
+        assert rel_per_rhs(orc.apply(dims, kappa, bc, 0, U, Xc), Phi).max() < 2e-12
+        assert rel_per_rhs(Xc, Xdc).max() < 1e-10
+    ctx.close()
+
+
+@pytest.mark.slow
+def test_register_kernel_fused_reductions_on_a_lattice_with_odd_half_row():
+    """18^4 (Lx/2 = 9 odd: chunk-major layout, the register kernel is the only hop) at n_rhs = 12: G = V/2/32 blocks
+    write 12 * 3 * G partial sums -- the case that overran the buffer in round 1 (ADVICE, high).  True residual with
+    the oracle's operator."""
+    pkg = _wd()
+    dims, bc, n = (18, 18, 18, 18), wi.BC_SF, 12
+    kappa = 0.13
+    U = wi.gauge_field(dims, 0.3, 1, bc)
+    Phi = wi.spinor_field(dims, n, 1, bc)
+    ctx = make_ctx(dims, kappa, bc, n, U)
+    P = ctx.pack(dev(Phi))
+    X, info = ctx.solve_block(pkg.OP_D, P, n, tol=1e-12)
+    assert info["converged"] and max(info["relres"]) <= 1e-12
+    Xc = ctx.unpack(X, n).cpu().numpy()
+    assert rel_per_rhs(orc.apply(dims, kappa, bc, 0, U, Xc), Phi).max() < 2e-12
     ctx.close()
 
 

@@ -394,3 +394,107 @@ def test_force_gauge_covariance():
     Fg = cview(orc.force(dims, kappa, bc, gauge_transform(U, g), rot(X), rot(Y)))
     expect = np.einsum("...ab,m...bc,...dc->m...ad", g, F, np.conj(g))
     assert relerr(Fg, expect) < 1e-14
+
+
+# ----------------------------------------------------------------------------- CG on the normal equations
+def test_cgne_fallback_matches_lu_inverse_and_bicgstab():
+    """`cgne_one` (the fallback route of orc_solve) pinned on its own: against the dense LU inverse and
+    numpy's solver on 2^3 x 4 (D and D^dag), and against the BiCGStab route on configs[0]."""
+    kappa = 0.13
+    U = wi.gauge_field(SMALL, 0.4, 1, wi.BC_SF)
+    phi = wi.spinor_field(SMALL, 3, 1, wi.BC_SF)
+    for dag in (0, 1):
+        A = orc.dense_matrix(SMALL, kappa, wi.BC_SF, dag, U)
+        b = cview(phi)[:, 1:].reshape(3, -1)
+        x_lu = orc.lu_solve(A, b)
+        x_np = np.linalg.solve(A, b.T).T
+        X, relres, iters, rc = orc.solve_cgne(SMALL, kappa, wi.BC_SF, dag, U, phi, tol=1e-14)
+        assert rc == 0 and relres.max() < 1e-13 and np.all(iters > 0)
+        assert np.all(X[:, 0] == 0.0)
+        assert relerr(cview(X)[:, 1:].reshape(3, -1), x_lu) < 1e-12
+        assert relerr(cview(X)[:, 1:].reshape(3, -1), x_np) < 1e-12
+    cfg, U, phi = wi.make_config(0)
+    dims, k, bc = cfg["dims"], cfg["kappa"], cfg["bc"]
+    for dag in (0, 1):
+        Xb, rb, _, rcb = orc.solve(dims, k, bc, dag, U, phi, tol=1e-14)
+        Xc, rcg, itc, rcc = orc.solve_cgne(dims, k, bc, dag, U, phi, tol=1e-14)
+        assert rcb == 0 and rcc == 0 and rb.max() < 1e-13 and rcg.max() < 1e-13
+        assert relerr(Xc, Xb) < 1e-12
+        assert np.all(itc < 100000)
+
+
+# ----------------------------------------------------------------------------- even/odd-preconditioned action (f1)
+def test_parity_projector():
+    dims = (4, 2, 6, 4)
+    psi = wi.spinor_field(dims, 2, 3, wi.BC_PERIODIC)
+    x, y, z, t = site_coords(dims)
+    par = (x + y + z + t) & 1
+    for p in (0, 1):
+        out = orc.project_parity(dims, p, psi)
+        assert np.array_equal(out[:, par == p], psi[:, par == p])
+        assert np.all(out[:, par != p] == 0.0)
+    assert np.array_equal(orc.project_parity(dims, 0, psi) + orc.project_parity(dims, 1, psi), psi)
+
+
+def schur_even_dense(dims, kappa, bc, U):
+    """Dhat = A_ee - A_eo A_oo^-1 A_oe of the dense dynamical block of D, and the even-site index set.  With
+    D = 1 - kappa H and H odd-even only, A_ee = A_oo = 1, so Dhat = 1 - kappa^2 H_eo H_oe."""
+    A = orc.dense_matrix(dims, kappa, bc, 0, U)
+    lx, ly, lz, lt = dims
+    x, y, z, t = site_coords(dims)
+    lo = 1 if bc == wi.BC_SF else 0
+    par = ((x + y + z + t) & 1)[lo:].reshape(-1)                     # per dynamical site, site-major like the matrix
+    idx = np.repeat(par, 12)
+    e, o = np.where(idx == 0)[0], np.where(idx == 1)[0]
+    Aee, Aeo, Aoe, Aoo = A[np.ix_(e, e)], A[np.ix_(e, o)], A[np.ix_(o, e)], A[np.ix_(o, o)]
+    assert np.abs(Aee - np.eye(len(e))).max() < 1e-15 and np.abs(Aoo - np.eye(len(o))).max() < 1e-15
+    return Aee - Aeo @ np.linalg.solve(Aoo, Aoe), e
+
+
+def eo_action_dense(dims, kappa, bc, U, phi):
+    Dhat, e = schur_even_dense(dims, kappa, bc, U)
+    lo = 1 if bc == wi.BC_SF else 0
+    b = cview(phi)[:, lo:].reshape(phi.shape[0], -1)[:, e]
+    x = np.linalg.solve(Dhat, b.T)
+    return float(np.sum(np.abs(x) ** 2)), x.T
+
+
+@pytest.mark.parametrize("bc", [wi.BC_SF, wi.BC_PERIODIC])
+def test_eo_preconditioned_action_and_its_force(bc):
+    """phi on even sites, S = sum |Dhat^-1 phi_i|^2, Dhat the even-site Schur complement.  The oracle's
+    route (X = D^-1 (phi_e, 0), Y = D^dag^-1 P_e X, the full-action functional f[x, y]) against the dense Schur
+    complement: x_e, S, and dS/deps = Re tr[Omega F] by central finite differences of the DENSE S."""
+    dims, kappa, n = SMALL, 0.13, 3
+    U = wi.gauge_field(dims, 0.4, 1, bc)
+    phi = wi.spinor_field(dims, n, 1, bc)
+    X, Y, S, F = orc.eo_md_force(dims, kappa, bc, U, phi)
+    S_dense, xe_dense = eo_action_dense(dims, kappa, bc, U, phi)
+    assert abs(S.sum() - S_dense) / S_dense < 1e-12
+    _, e = schur_even_dense(dims, kappa, bc, U)
+    lo = 1 if bc == wi.BC_SF else 0
+    assert relerr(cview(X)[:, lo:].reshape(n, -1)[:, e], xe_dense) < 1e-12
+    # the odd part of X is kappa H_oe x_e: D X must vanish on odd sites and equal phi on even sites
+    DX = orc.apply(dims, kappa, bc, 0, U, X)
+    assert relerr(DX, orc.project_parity(dims, 0, phi)) < 1e-12
+    Fc = cview(F)
+    eps = 1e-4
+    probes = [(0, (1, 0, 1, 0)), (1, (2, 1, 0, 1)), (2, (1, 1, 1, 1)), (3, (1, 0, 0, 1)), (3, (2, 1, 1, 0))]
+    for k, (mu, site) in enumerate(probes):
+        om = random_antihermitian_traceless(80 + k)
+        sp, _ = eo_action_dense(dims, kappa, bc, perturbed(U, mu, site, om, +eps), phi)
+        sm, _ = eo_action_dense(dims, kappa, bc, perturbed(U, mu, site, om, -eps), phi)
+        fd = (sp - sm) / (2 * eps)
+        an = np.real(np.trace(om @ Fc[(mu,) + site]))
+        assert abs(an) > 1e-4, "probe must be sensitive"
+        assert abs(fd - an) / abs(an) < 5e-7, (mu, site, fd, an)
+
+
+def test_refresh_gives_unit_action():
+    """Pseudo-fermion refresh phi = D eta: then x = D^-1 phi = eta and S = |eta|^2 exactly."""
+    cfg, U, _ = wi.make_config(0)
+    dims, k, bc = cfg["dims"], cfg["kappa"], cfg["bc"]
+    eta = wi.spinor_field(dims, 2, 9, bc)
+    phi = orc.apply(dims, k, bc, 0, U, eta)
+    X, rr, _, rc = orc.solve(dims, k, bc, 0, U, phi, tol=1e-14)
+    assert rc == 0 and relerr(X, eta) < 1e-12
+    assert np.allclose(orc.action(X), np.sum(eta.reshape(2, -1) ** 2, axis=1), rtol=1e-12)
