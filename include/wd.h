@@ -59,6 +59,8 @@ enum { WD_OP_D = 0, WD_OP_DDAG = 1 };
 enum { WD_F64 = 0, WD_F32 = 1 };
 enum { WD_LINK18 = 0, WD_LINK12 = 1 }; /* 18 reals per link, or rows 1-2 only */
 enum { WD_ORDER_LINEAR = 0, WD_ORDER_TILED = 1 };
+enum { WD_ACTION_FULL = 0, WD_ACTION_EO = 1 };   /* pseudo-fermion action on D (eq. 2.2) or on the even/odd Schur complement */
+enum { WD_PARITY_EVEN = 0, WD_PARITY_ODD = 1, WD_PARITY_BOTH = 2 };
 
 #define WD_MAX_RHS 16
 
@@ -166,6 +168,35 @@ int wd_force(wd_ctx* ctx, int n_rhs, const double* X_native_dev, const double* Y
 int wd_md_force_host(wd_ctx* ctx, int n_rhs, const double* Phi_canon_host, double* F_canon_host,
                      double tol, int max_outer, int max_inner, double inner_tol, int recon,
                      wd_solve_info* info2);
+
+/* One whole MD force evaluation from HOST buffers INCLUDING the gauge field (the links change between force
+ * evaluations of a trajectory): copies the canonical U (4 V 18 doubles) and Phi to the device, runs the
+ * gauge ingest (hot-path step a0) and then everything wd_md_force_host does.  U_canon_host should be pinned. */
+int wd_md_force_host_gauge(wd_ctx* ctx, int n_rhs, const double* U_canon_host, const double* Phi_canon_host,
+                           double* F_canon_host, double tol, int max_outer, int max_inner, double inner_tol, int recon,
+                           wd_solve_info* info2);
+
+/* The steps either side of the path in a molecular-dynamics step (PAPER.md:33-40 eq. 2.1-2.2, :60, :74).
+ *
+ * wd_refresh: pseudo-fermion heat bath.  variant = WD_ACTION_FULL: phi = D eta on the full lattice (then
+ *   S = sum_i |D^-1 phi_i|^2 = sum_i |eta_i|^2).  WD_ACTION_EO: the pseudo-fermions live on the even sites and the
+ *   action is written on Dhat = 1 - kappa^2 H_eo H_oe (the even/odd-preconditioned operator):
+ *   phi_e = Dhat eta_e, phi_o = 0 (the odd half of eta is ignored).  eta, phi: native fp64 full-lattice blocks, no overlap.
+ * wd_action: S_host[i] = |x_i|^2 over the sites selected by parity_sel (WD_PARITY_BOTH for the full action with
+ *   x = D^-1 phi; WD_PARITY_EVEN for the even/odd variant); one fused fp64 norm kernel, synchronises.
+ * wd_project_parity: native = P_parity native (the other parity's sites are zeroed), in place.
+ * wd_md_force: Algorithm 2 on DEVICE-resident native fields: X = A^-1 Phi, Y = A^dag^-1 X',
+ *   F += sum_i f[x_i, y_i], S_host[i] (nullable) = action per column.  WD_ACTION_FULL: A = D, X' = X.
+ *   WD_ACTION_EO: right-hand sides P_e Phi and X' = P_e X, i.e. x_e = Dhat^-1 phi_e, X = (x_e, kappa H_oe x_e) and Y
+ *   likewise, with the same force functional (reading R16).  X, Y: native fp64 outputs; F canonical,
+ *   accumulated; info2[0], info2[1] (nullable) describe the two solves.  Solver parameters as wd_solve_block.
+ * Errors: WD_EINVAL (null, n_rhs, enums), WD_ESTATE (no gauge), WD_ENOCONV. */
+int wd_refresh(wd_ctx* ctx, int variant, int n_rhs, const double* eta_native_dev, double* phi_native_dev);
+int wd_action(wd_ctx* ctx, int n_rhs, int parity_sel, const double* X_native_dev, double* S_host);
+int wd_project_parity(wd_ctx* ctx, int prec, int n_rhs, int parity, void* native_dev);
+int wd_md_force(wd_ctx* ctx, int variant, int n_rhs, const double* Phi_native_dev, double* X_native_dev,
+                double* Y_native_dev, double* F_canon_dev, double* S_host, double tol, int max_outer, int max_inner,
+                double inner_tol, int recon, wd_solve_info* info2);
 
 /* Per-class device timing for measurement (bench.py's roofline line).  wd_profile(ctx, 1) makes every
  * later hop / BLAS1 / force launch record a CUDA event pair on the context's stream (a few

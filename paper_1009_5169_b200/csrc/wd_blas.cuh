@@ -22,6 +22,7 @@ enum {
     S_PHI2,       // |phi_i|^2 over the full lattice
     S_SCALE,      // |R_i| used to normalise the inner right-hand side
     S_OUT_CONV,   // 1 if column met the outer tolerance
+    S_ACTION,     // |x_i|^2 of wd_action (pseudo-fermion action per column)
     S_ROWS
 };
 // global (not per-column) slots after the table
@@ -29,7 +30,7 @@ enum { G_DONE = S_ROWS * WD_MAX_RHS, G_ITERS, G_OUT_DONE, G_TOL2, G_INTOL2, G_CO
 
 __device__ __forceinline__ double& SC(double* scal, int row, int r) { return scal[row * WD_MAX_RHS + r]; }
 
-enum Kind { K_SIGMA, K_OMEGA, K_RHO, K_PHI2, K_OUT_R2, K_INIT_RHO };
+enum Kind { K_SIGMA, K_OMEGA, K_RHO, K_PHI2, K_OUT_R2, K_INIT_RHO, K_ACTION };
 
 struct RedBuf {
     double* scal;
@@ -98,6 +99,8 @@ __device__ void finalize_column(double* scal, int r, const double* tot) {
         SC(scal, S_BETA_RE, r) = beta.re; SC(scal, S_BETA_IM, r) = beta.im;
     } else if (KIND == K_PHI2) {
         SC(scal, S_PHI2, r) = tot[0];
+    } else if (KIND == K_ACTION) {
+        SC(scal, S_ACTION, r) = tot[0];
     } else if (KIND == K_OUT_R2) {  // tot = |R_i|^2 of the fp64 even/odd system
         SC(scal, S_OUT_R2, r) = tot[0];
         const double phi2 = SC(scal, S_PHI2, r);

@@ -386,13 +386,15 @@ int wd_force(wd_ctx* ctx, int n_rhs, const double* X, const double* Y, double* F
     return wd_force_impl(ctx, n_rhs, X, Y, F);
 }
 
-int wd_md_force_host(wd_ctx* ctx, int n_rhs, const double* Phi_host, double* F_host, double tol, int max_outer,
-                     int max_inner, double inner_tol, int recon, wd_solve_info* info2) {
+static int md_force_host_common(wd_ctx* ctx, int n_rhs, const double* U_host, const double* Phi_host, double* F_host,
+                                double tol, int max_outer, int max_inner, double inner_tol, int recon,
+                                wd_solve_info* info2) {
     if (!ctx) return WD_EINVAL;
     if (!Phi_host || !F_host) return wd_fail(ctx, WD_EINVAL, "null pointer");
     if (bad_n(ctx, n_rhs)) return wd_fail(ctx, WD_EINVAL, "n_rhs out of range");
     if (recon != WD_LINK18 && recon != WD_LINK12) return wd_fail(ctx, WD_EINVAL, "bad link form");
-    if (!ctx->have_gauge) return wd_fail(ctx, WD_ESTATE, "wd_set_gauge first");
+    if (!U_host && !ctx->have_gauge) return wd_fail(ctx, WD_ESTATE, "wd_set_gauge first");
+    if (U_host && !ctx->have_ws) return wd_fail(ctx, WD_ESTATE, "wd_set_workspace first");
     int rcp = check_solver_params(ctx, tol, max_outer, max_inner, inner_tol);
     if (rcp) return rcp;
     // staging lives at the END of the solver scratch (sized for max_rhs in wd_solver_scratch_bytes)
@@ -404,21 +406,74 @@ int wd_md_force_host(wd_ctx* ctx, int n_rhs, const double* Phi_host, double* F_h
     double* dX = (double*)(end - fbytes - 2 * full);
     double* dPhi = (double*)(end - fbytes - 3 * full);
     double* dCanon = (double*)(end - fbytes - 4 * full);
+    if (U_host) {   // a0: the canonical links go through dF (same size), which is cleared afterwards
+        WD_CUDA_CHECK(ctx, cudaMemcpyAsync(dF, U_host, sizeof(double) * 4 * ctx->V * 18, cudaMemcpyHostToDevice, ctx->stream));
+        int rcg = wd_layout_gauge(ctx, dF);
+        if (rcg) return rcg;
+        ctx->have_gauge = true;
+    }
     const size_t cbytes = sizeof(double) * 24 * ctx->V * n_rhs;
     WD_CUDA_CHECK(ctx, cudaMemcpyAsync(dCanon, Phi_host, cbytes, cudaMemcpyHostToDevice, ctx->stream));
     int rc = wd_layout_pack(ctx, WD_F64, n_rhs, dCanon, dPhi);
     if (rc) return rc;
     WD_CUDA_CHECK(ctx, cudaMemsetAsync(dF, 0, sizeof(double) * 4 * ctx->V * 18, ctx->stream));
     const double itol = inner_tol > 0.0 ? inner_tol : 1e-5;
-    int rc1 = wd_solve_impl(ctx, 0, n_rhs, dPhi, dX, tol, max_outer, max_inner, itol, recon, info2 ? &info2[0] : nullptr);
-    if (rc1 != WD_OK && rc1 != WD_ENOCONV) return rc1;
-    int rc2 = wd_solve_impl(ctx, 1, n_rhs, dX, dY, tol, max_outer, max_inner, itol, recon, info2 ? &info2[1] : nullptr);
-    if (rc2 != WD_OK && rc2 != WD_ENOCONV) return rc2;
-    rc = wd_force_impl(ctx, n_rhs, dX, dY, dF);
-    if (rc) return rc;
+    rc = wd_md_force_impl(ctx, WD_ACTION_FULL, n_rhs, dPhi, dX, dY, dF, nullptr, dCanon, tol, max_outer, max_inner, itol,
+                          recon, info2);
+    if (rc != WD_OK && rc != WD_ENOCONV) return rc;
     WD_CUDA_CHECK(ctx, cudaMemcpyAsync(F_host, dF, sizeof(double) * 4 * ctx->V * 18, cudaMemcpyDeviceToHost, ctx->stream));
     WD_CUDA_CHECK(ctx, cudaStreamSynchronize(ctx->stream));
-    return (rc1 == WD_OK && rc2 == WD_OK) ? WD_OK : WD_ENOCONV;
+    return rc;
+}
+
+int wd_md_force_host(wd_ctx* ctx, int n_rhs, const double* Phi_host, double* F_host, double tol, int max_outer,
+                     int max_inner, double inner_tol, int recon, wd_solve_info* info2) {
+    return md_force_host_common(ctx, n_rhs, nullptr, Phi_host, F_host, tol, max_outer, max_inner, inner_tol, recon, info2);
+}
+
+int wd_md_force_host_gauge(wd_ctx* ctx, int n_rhs, const double* U_host, const double* Phi_host, double* F_host, double tol,
+                           int max_outer, int max_inner, double inner_tol, int recon, wd_solve_info* info2) {
+    if (ctx && !U_host) return wd_fail(ctx, WD_EINVAL, "null pointer");
+    return md_force_host_common(ctx, n_rhs, U_host, Phi_host, F_host, tol, max_outer, max_inner, inner_tol, recon, info2);
+}
+
+int wd_refresh(wd_ctx* ctx, int variant, int n_rhs, const double* eta, double* phi) {
+    int rc = check_op_args(ctx, WD_OP_D, WD_F64, WD_LINK18, n_rhs, eta, phi);
+    if (rc) return rc;
+    if (variant != WD_ACTION_FULL && variant != WD_ACTION_EO) return wd_fail(ctx, WD_EINVAL, "bad action variant");
+    return wd_refresh_impl(ctx, variant, n_rhs, eta, phi);
+}
+
+int wd_action(wd_ctx* ctx, int n_rhs, int parity_sel, const double* X, double* S_host) {
+    if (!ctx) return WD_EINVAL;
+    if (!X || !S_host) return wd_fail(ctx, WD_EINVAL, "null pointer");
+    if (bad_n(ctx, n_rhs)) return wd_fail(ctx, WD_EINVAL, "n_rhs out of range");
+    if (parity_sel < WD_PARITY_EVEN || parity_sel > WD_PARITY_BOTH) return wd_fail(ctx, WD_EINVAL, "bad parity selection");
+    if (!ctx->have_ws) return wd_fail(ctx, WD_ESTATE, "wd_set_workspace first");
+    return wd_action_impl(ctx, n_rhs, parity_sel, X, S_host);
+}
+
+int wd_project_parity(wd_ctx* ctx, int prec, int n_rhs, int parity, void* native) {
+    if (!ctx) return WD_EINVAL;
+    if (!native || bad_n(ctx, n_rhs) || (prec != WD_F64 && prec != WD_F32) || (parity != 0 && parity != 1))
+        return wd_fail(ctx, WD_EINVAL, "wd_project_parity: bad argument");
+    return wd_project_parity_impl(ctx, prec, n_rhs, parity, native);
+}
+
+int wd_md_force(wd_ctx* ctx, int variant, int n_rhs, const double* Phi, double* X, double* Y, double* F, double* S_host,
+                double tol, int max_outer, int max_inner, double inner_tol, int recon, wd_solve_info* info2) {
+    int rc = check_op_args(ctx, WD_OP_D, WD_F64, recon, n_rhs, Phi, X);
+    if (rc) return rc;
+    if (!Y || !F || Y == X || (const double*)Y == Phi) return wd_fail(ctx, WD_EINVAL, "null or aliased field pointer");
+    if (variant != WD_ACTION_FULL && variant != WD_ACTION_EO) return wd_fail(ctx, WD_EINVAL, "bad action variant");
+    rc = check_solver_params(ctx, tol, max_outer, max_inner, inner_tol);
+    if (rc) return rc;
+    // scratch for the projected right-hand sides of the even/odd variant: the host path's canonical staging block
+    const size_t full = wd_align_up(2 * wd_half_bytes(ctx, WD_F64, ctx->max_rhs));
+    const size_t fbytes = wd_align_up(sizeof(double) * 4 * ctx->V * 18);
+    double* tmp = (double*)(ctx->d_solver + ctx->solver_bytes - fbytes - 4 * full);
+    return wd_md_force_impl(ctx, variant, n_rhs, Phi, X, Y, F, S_host, tmp, tol, max_outer, max_inner,
+                            inner_tol > 0.0 ? inner_tol : 1e-5, recon, info2);
 }
 
 }  // extern "C"

@@ -174,3 +174,11 @@ int wd_solve_impl(wd_ctx* c, int dag, int n, const double* Phi, double* X, doubl
 
 // wd_force.cu
 int wd_force_impl(wd_ctx* c, int n, const double* X, const double* Y, double* F);
+
+// wd_md.cu
+int wd_action_impl(wd_ctx* c, int n, int parity_sel, const double* X, double* S_host);
+int wd_project_parity_impl(wd_ctx* c, int prec, int n, int parity, void* native);
+int wd_refresh_impl(wd_ctx* c, int variant, int n, const double* eta, double* phi);
+int wd_md_force_impl(wd_ctx* c, int variant, int n, const double* Phi, double* X, double* Y, double* F, double* S_host,
+                     double* tmp, double tol, int max_outer, int max_inner, double inner_tol, int recon,
+                     wd_solve_info* info2);

@@ -26,6 +26,8 @@ OP_D, OP_DDAG = 0, 1
 F64, F32 = 0, 1
 LINK18, LINK12 = 0, 1
 ORDER_LINEAR, ORDER_TILED = 0, 1
+ACTION_FULL, ACTION_EO = 0, 1
+PARITY_EVEN, PARITY_ODD, PARITY_BOTH = 0, 1, 2
 MAX_RHS = 16
 OPT_HOP32_SITES, OPT_HOP64_SITES, OPT_HOP32_REGS, OPT_HOP64_REGS, OPT_POLL_EVERY, OPT_HOP_IMPL, OPT_ALTERNATE_SWEEP, OPT_HOP_ROWS = 0, 1, 2, 3, 4, 5, 6, 7
 PROF_NAMES = ("hop32", "hop64", "blas", "force", "layout")
@@ -34,7 +36,8 @@ PROF_N = len(PROF_NAMES)
 # every symbol include/wd.h declares (tests check that the library exports each one)
 SYMBOLS = ["wd_create", "wd_destroy", "wd_site_order", "wd_workspace_bytes", "wd_set_workspace",
            "wd_set_option", "wd_get_option", "wd_set_gauge", "wd_native_bytes", "wd_pack", "wd_unpack", "wd_apply", "wd_hop",
-           "wd_solve_block", "wd_force", "wd_md_force_host", "wd_profile", "wd_profile_read", "wd_launch_count", "wd_strerror",
+           "wd_solve_block", "wd_force", "wd_md_force_host", "wd_md_force_host_gauge", "wd_refresh", "wd_action",
+           "wd_project_parity", "wd_md_force", "wd_profile", "wd_profile_read", "wd_launch_count", "wd_strerror",
            "wd_last_error", "wd_version"]
 
 
@@ -89,6 +92,11 @@ def lib():
     L.wd_solve_block.argtypes = [vp, ci, ci, vp, vp, cd, ci, ci, cd, ci, ctypes.POINTER(SolveInfo)]
     L.wd_force.argtypes = [vp, ci, vp, vp, vp]
     L.wd_md_force_host.argtypes = [vp, ci, vp, vp, cd, ci, ci, cd, ci, ctypes.POINTER(SolveInfo)]
+    L.wd_md_force_host_gauge.argtypes = [vp, ci, vp, vp, vp, cd, ci, ci, cd, ci, ctypes.POINTER(SolveInfo)]
+    L.wd_refresh.argtypes = [vp, ci, ci, vp, vp]
+    L.wd_action.argtypes = [vp, ci, ci, vp, ctypes.POINTER(cd)]
+    L.wd_project_parity.argtypes = [vp, ci, ci, ci, vp]
+    L.wd_md_force.argtypes = [vp, ci, ci, vp, vp, vp, vp, ctypes.POINTER(cd), cd, ci, ci, cd, ci, ctypes.POINTER(SolveInfo)]
     L.wd_profile.argtypes = [vp, ci]
     L.wd_profile_read.argtypes = [vp, ctypes.POINTER(cd), ctypes.POINTER(ctypes.c_longlong)]
     L.wd_launch_count.argtypes = [vp]
@@ -99,7 +107,8 @@ def lib():
     L.wd_last_error.restype = ctypes.c_char_p
     L.wd_version.restype = ctypes.c_char_p
     for name in ("wd_create", "wd_destroy", "wd_site_order", "wd_set_option", "wd_get_option", "wd_set_workspace", "wd_set_gauge", "wd_pack",
-                 "wd_unpack", "wd_apply", "wd_hop", "wd_solve_block", "wd_force", "wd_md_force_host", "wd_profile",
+                 "wd_unpack", "wd_apply", "wd_hop", "wd_solve_block", "wd_force", "wd_md_force_host", "wd_md_force_host_gauge", "wd_refresh", "wd_action",
+           "wd_project_parity", "wd_md_force", "wd_profile",
                  "wd_profile_read"):
         getattr(L, name).restype = ci
     _lib = L
@@ -239,6 +248,56 @@ class Context:
                                      int(max_inner), float(inner_tol), int(recon), infos)
         self._check(rc)
         return F_host, [infos[0].as_dict(), infos[1].as_dict()]
+
+    def md_force_host_gauge(self, U_host, Phi_host, F_host=None, tol=1e-12, max_outer=20, max_inner=1000, inner_tol=0.0,
+                            recon=LINK18):
+        """Whole MD force evaluation from HOST canonical tensors including the gauge field (upload + ingest)."""
+        lx, ly, lz, lt = self.dims
+        assert (not Phi_host.is_cuda) and Phi_host.dtype == torch.float64 and Phi_host.is_contiguous()
+        assert (not U_host.is_cuda) and U_host.dtype == torch.float64 and U_host.is_contiguous()
+        assert tuple(U_host.shape) == (4, lt, lz, ly, lx, 3, 3, 2), U_host.shape
+        n = int(Phi_host.shape[0])
+        if F_host is None:
+            F_host = torch.empty((4, lt, lz, ly, lx, 3, 3, 2), dtype=torch.float64).pin_memory()
+        infos = (SolveInfo * 2)()
+        rc = self.L.wd_md_force_host_gauge(self._h, n, self._ptr(U_host), self._ptr(Phi_host), self._ptr(F_host), float(tol),
+                                           int(max_outer), int(max_inner), float(inner_tol), int(recon), infos)
+        self._check(rc)
+        return F_host, [infos[0].as_dict(), infos[1].as_dict()]
+
+    def refresh(self, eta_native, n_rhs, variant=ACTION_FULL, out=None):
+        """phi = D eta (ACTION_FULL) or phi_e = Dhat eta_e, phi_o = 0 (ACTION_EO); native fp64 blocks."""
+        if out is None:
+            out = torch.empty_like(eta_native)
+        self._check(self.L.wd_refresh(self._h, int(variant), int(n_rhs), self._ptr(eta_native), self._ptr(out)))
+        return out
+
+    def action(self, X_native, n_rhs, parity_sel=PARITY_BOTH):
+        """Per-column |x_i|^2 over the selected sites, as a list of floats (synchronises)."""
+        S = (ctypes.c_double * int(n_rhs))()
+        self._check(self.L.wd_action(self._h, int(n_rhs), int(parity_sel), self._ptr(X_native), S))
+        return [S[i] for i in range(int(n_rhs))]
+
+    def project_parity(self, native, n_rhs, parity, prec=F64):
+        """In place: zero the sites of the other parity."""
+        self._check(self.L.wd_project_parity(self._h, int(prec), int(n_rhs), int(parity), self._ptr(native)))
+        return native
+
+    def md_force(self, Phi_native, n_rhs, variant=ACTION_FULL, F=None, tol=1e-12, max_outer=20, max_inner=1000,
+                 inner_tol=0.0, recon=LINK18, want_action=True):
+        """Algorithm 2 on device-resident fields: returns (X, Y, F, S per column or None, [info_X, info_Y])."""
+        lx, ly, lz, lt = self.dims
+        if F is None:
+            F = torch.zeros((4, lt, lz, ly, lx, 3, 3, 2), dtype=torch.float64, device=self.device)
+        X = torch.empty_like(Phi_native)
+        Y = torch.empty_like(Phi_native)
+        S = (ctypes.c_double * int(n_rhs))() if want_action else None
+        infos = (SolveInfo * 2)()
+        rc = self.L.wd_md_force(self._h, int(variant), int(n_rhs), self._ptr(Phi_native), self._ptr(X), self._ptr(Y),
+                                self._ptr(F), S, float(tol), int(max_outer), int(max_inner), float(inner_tol), int(recon),
+                                infos)
+        self._check(rc)
+        return X, Y, F, ([S[i] for i in range(int(n_rhs))] if want_action else None), [infos[0].as_dict(), infos[1].as_dict()]
 
     def profile(self, enable=True):
         self._check(self.L.wd_profile(self._h, 1 if enable else 0))

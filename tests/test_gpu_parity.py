@@ -25,6 +25,17 @@ def rel_per_rhs(a, b):
     return np.linalg.norm(a - b, axis=1) / np.maximum(np.linalg.norm(b, axis=1), 1e-300)
 
 
+def force_close(F, Fr, tol):
+    """Relative Frobenius norm over the whole field AND the largest per-link deviation relative to the typical
+    link norm (a wrong coefficient or operand on a few links would hide in the global norm)."""
+    assert np.linalg.norm(F - Fr) / np.linalg.norm(Fr) < tol
+    d = np.sqrt(((F - Fr) ** 2).sum(axis=(-1, -2, -3)))     # per link [mu][T][Lz][Ly][Lx]
+    n = np.sqrt((Fr ** 2).sum(axis=(-1, -2, -3)))
+    scale = np.sqrt((n ** 2).mean())
+    assert d.max() < 10 * tol * scale, (d.max(), scale)
+    assert np.all(d[n == 0.0] == 0.0)                         # exact zeros (SF boundary links) stay exact
+
+
 def dev(a):
     return torch.from_numpy(np.ascontiguousarray(a)).cuda()
 
@@ -157,7 +168,7 @@ def _solve_force_case(cfg_idx, n_rhs=None, recon=0):
     assert res.max() < 2e-12, res
     assert rel_per_rhs(Xc, Xr).max() < 1e-9
     assert rel_per_rhs(Yc, Yr).max() < 1e-9
-    assert np.linalg.norm(F - Fr) / np.linalg.norm(Fr) < 1e-9
+    force_close(F, Fr, 1e-9)
     ctx.close()
     return ix, iy
 
@@ -191,9 +202,9 @@ def test_force_accumulates_and_matches_oracle_on_random_fields():
     ctx = make_ctx(dims, kappa, bc, n, U)
     Xn, Yn = ctx.pack(dev(X)), ctx.pack(dev(Y))
     F = ctx.force(Xn, Yn, n)
-    assert np.linalg.norm(F.cpu().numpy() - Fr) / np.linalg.norm(Fr) < 1e-13
+    force_close(F.cpu().numpy(), Fr, 1e-13)
     F = ctx.force(Xn, Yn, n, F=F)  # accumulate a second time
-    assert np.linalg.norm(F.cpu().numpy() - 2 * Fr) / np.linalg.norm(Fr) < 1e-13
+    force_close(F.cpu().numpy(), 2 * Fr, 1e-13)
     ctx.close()
 
 
@@ -297,7 +308,7 @@ def test_solve_and_force_with_either_hop_kernel(impl, recon):
     assert ix["converged"] and iy["converged"]
     assert rel_per_rhs(ctx.unpack(X, n).cpu().numpy(), Xr).max() < 1e-9
     assert rel_per_rhs(ctx.unpack(Y, n).cpu().numpy(), Yr).max() < 1e-9
-    assert np.linalg.norm(F - Fr) / np.linalg.norm(Fr) < 1e-9
+    force_close(F, Fr, 1e-9)
     ctx.close()
 
 
@@ -383,39 +394,197 @@ def test_register_kernel_fused_reductions_on_a_lattice_with_odd_half_row():
     ctx.close()
 
 
-def test_full_size_bench_configuration_properties():
-    """BASELINE.json configs[4] at n_rhs = 5, exactly as bench.py runs it (24^4 SF, 12-real inner links, default
-    launch options = staged hop kernel).  The oracle cannot solve this size in test time, so: D-apply parity on
-    the whole lattice (the oracle's apply is cheap), and for the solves the properties that pin X and Y at any size --
-    the TRUE residuals |Phi - D X| / |Phi| and |X - D^dag Y| / |X| recomputed with the oracle's operator -- plus the
-    force's exact symmetries (anti-hermitian, traceless, zero on links touching the SF boundary)."""
+# ---- the measured configuration: BASELINE.json configs[4] (24^4 SF), exactly as bench.py runs it -----------------
+_ORACLE_24 = {}
+
+
+def oracle_24(ncol):
+    """The oracle's X = D^-1 Phi, Y = D^dag^-1 X for the first `ncol` columns of configs[4] (about 10 s per column and
+    solve on 16 cores), cached for the tests below.  Column i of the seeded right-hand sides does not depend on n_rhs."""
+    if "U" not in _ORACLE_24:
+        cfg, U, Phi = wi.make_config(4, 12)
+        _ORACLE_24.update(cfg=cfg, U=U, Phi=Phi, X={}, Y={})
+    cfg, U, Phi = _ORACLE_24["cfg"], _ORACLE_24["U"], _ORACLE_24["Phi"]
+    dims, kappa, bc = cfg["dims"], cfg["kappa"], cfg["bc"]
+    for i in range(ncol):
+        if i not in _ORACLE_24["X"]:
+            X, rr, _, rc = orc.solve(dims, kappa, bc, 0, U, Phi[i:i + 1], tol=1e-14)
+            assert rc == 0 and rr.max() < 1e-13
+            Y, rr, _, rc = orc.solve(dims, kappa, bc, 1, U, X, tol=1e-14)
+            assert rc == 0 and rr.max() < 1e-13
+            _ORACLE_24["X"][i], _ORACLE_24["Y"][i] = X[0], Y[0]
+    Xr = np.stack([_ORACLE_24["X"][i] for i in range(ncol)])
+    Yr = np.stack([_ORACLE_24["Y"][i] for i in range(ncol)])
+    return cfg, U, Phi, Xr, Yr
+
+
+@pytest.mark.slow
+def test_full_size_bench_configuration_elementwise():
+    """configs[4] at n_rhs = 5 with bench.py's launch configuration (default options: z-march hop, 18-real inner
+    links): D and D^dag apply in fp64 (18- and 12-real) and fp32 (18 and 12) against the oracle on the whole lattice;
+    X, Y, F element by element against the oracle's own solves; wd_force alone against the oracle's force applied to
+    the GPU's X, Y (isolates the force kernel at full size)."""
     pkg = _wd()
-    cfg, U, Phi = wi.make_config(4, 5)
-    dims, kappa, bc, n = cfg["dims"], cfg["kappa"], cfg["bc"], 5
+    n = 5
+    cfg, U, Phi12, Xr, Yr = oracle_24(n)
+    Phi = np.ascontiguousarray(Phi12[:n])
+    dims, kappa, bc = cfg["dims"], cfg["kappa"], cfg["bc"]
     ctx = make_ctx(dims, kappa, bc, n, U)
     assert ctx.get_option(pkg.OPT_HOP_IMPL) == 2
     P = ctx.pack(dev(Phi))
-    ref = orc.apply(dims, kappa, bc, 0, U, Phi)
-    out = ctx.unpack(ctx.apply(pkg.OP_D, P, n), n).cpu().numpy()
-    assert rel_per_rhs(out, ref).max() < 1e-13
     P32 = ctx.pack(dev(Phi), pkg.F32)
-    ref32 = orc.apply(dims, kappa, bc, 0, U.astype(np.float32).astype(np.float64), Phi.astype(np.float32).astype(np.float64))
-    out32 = ctx.unpack(ctx.apply(pkg.OP_D, P32, n, pkg.F32, pkg.LINK12), n, pkg.F32).cpu().numpy()
-    assert rel_per_rhs(out32, ref32).max() < 1e-5
+    U32, Phi32 = U.astype(np.float32).astype(np.float64), Phi.astype(np.float32).astype(np.float64)
+    for op in (pkg.OP_D, pkg.OP_DDAG):
+        ref = orc.apply(dims, kappa, bc, op, U, Phi)
+        for recon in (pkg.LINK18, pkg.LINK12):
+            out = ctx.unpack(ctx.apply(op, P, n, pkg.F64, recon), n).cpu().numpy()
+            assert rel_per_rhs(out, ref).max() < 1e-13, (op, recon)
+        ref32 = orc.apply(dims, kappa, bc, op, U32, Phi32)
+        for recon in (pkg.LINK18, pkg.LINK12):
+            out32 = ctx.unpack(ctx.apply(op, P32, n, pkg.F32, recon), n, pkg.F32).cpu().numpy()
+            assert rel_per_rhs(out32, ref32).max() < 1e-5, (op, recon)
     del ref, out, ref32, out32
-    X, ix = ctx.solve_block(pkg.OP_D, P, n, tol=1e-12, recon=pkg.LINK12)
-    Y, iy = ctx.solve_block(pkg.OP_DDAG, X, n, tol=1e-12, recon=pkg.LINK12)
+    X, ix = ctx.solve_block(pkg.OP_D, P, n, tol=1e-12)
+    Y, iy = ctx.solve_block(pkg.OP_DDAG, X, n, tol=1e-12)
     assert ix["converged"] and iy["converged"]
     Xc = ctx.unpack(X, n).cpu().numpy()
     Yc = ctx.unpack(Y, n).cpu().numpy()
     assert rel_per_rhs(orc.apply(dims, kappa, bc, 0, U, Xc), Phi).max() < 2e-12
     assert rel_per_rhs(orc.apply(dims, kappa, bc, 1, U, Yc), Xc).max() < 2e-12
     assert np.all(Xc[:, 0] == 0.0) and np.all(Yc[:, 0] == 0.0)          # SF: the stored t = 0 slice stays zero
+    assert rel_per_rhs(Xc, Xr).max() < 1e-9
+    assert rel_per_rhs(Yc, Yr).max() < 1e-9
     F = ctx.force(X, Y, n).cpu().numpy()                                  # [mu][T][Lz][Ly][Lx][3][3][2]
+    force_close(F, orc.force(dims, kappa, bc, U, Xc, Yc), 1e-13)          # the force kernel alone
+    force_close(F, orc.force(dims, kappa, bc, U, Xr, Yr), 1e-9)           # the whole path
     Fm = F[..., 0] + 1j * F[..., 1]
     scale = np.abs(Fm).max()
-    assert scale > 0
     assert np.abs(Fm + np.conj(np.swapaxes(Fm, -1, -2))).max() < 1e-13 * scale   # anti-hermitian
     assert np.abs(np.trace(Fm, axis1=-2, axis2=-1)).max() < 1e-12 * scale        # traceless
     assert np.all(F[:, 0] == 0.0) and np.all(F[3, -1] == 0.0)                     # links touching t = 0 / t = T
+    ctx.close()
+
+
+@pytest.mark.slow
+@pytest.mark.parametrize("n_rhs", [1, 2, 8, 12])
+def test_full_size_rhs_sweep_parity(n_rhs):
+    """configs[4]'s n_rhs sweep (bench.py --rhs-sweep): fp32 and fp64 D apply on all columns against the oracle, and
+    the blocked solve with column 0 against the oracle's solve (n_rhs <= 2 runs the register kernel in the chunk-major
+    layout, n_rhs >= 3 the staged kernels in the row-major layout)."""
+    pkg = _wd()
+    cfg, U, Phi12, Xr, _ = oracle_24(1)
+    Phi = np.ascontiguousarray(Phi12[:n_rhs])
+    dims, kappa, bc = cfg["dims"], cfg["kappa"], cfg["bc"]
+    ctx = make_ctx(dims, kappa, bc, n_rhs, U)
+    P = ctx.pack(dev(Phi))
+    out = ctx.unpack(ctx.apply(pkg.OP_D, P, n_rhs), n_rhs).cpu().numpy()
+    assert rel_per_rhs(out, orc.apply(dims, kappa, bc, 0, U, Phi)).max() < 1e-13
+    P32 = ctx.pack(dev(Phi), pkg.F32)
+    ref32 = orc.apply(dims, kappa, bc, 0, U.astype(np.float32).astype(np.float64), Phi.astype(np.float32).astype(np.float64))
+    for recon in (pkg.LINK18, pkg.LINK12):
+        out32 = ctx.unpack(ctx.apply(pkg.OP_D, P32, n_rhs, pkg.F32, recon), n_rhs, pkg.F32).cpu().numpy()
+        assert rel_per_rhs(out32, ref32).max() < 1e-5, recon
+    del out, out32, ref32
+    X, ix = ctx.solve_block(pkg.OP_D, P, n_rhs, tol=1e-12)
+    assert ix["converged"] and max(ix["relres"]) <= 1e-12
+    Xc = ctx.unpack(X, n_rhs).cpu().numpy()
+    assert rel_per_rhs(orc.apply(dims, kappa, bc, 0, U, Xc), Phi).max() < 2e-12
+    assert rel_per_rhs(Xc[:1], Xr).max() < 1e-9
+    ctx.close()
+
+
+def test_apply_16_configuration():
+    """configs[3] (16^4 SF, n_rhs = 5; bench.py --apply-sweep): D and D^dag, fp32 / fp64 x 18 / 12 reals."""
+    pkg = _wd()
+    cfg, U, Phi = wi.make_config(3)
+    dims, kappa, bc, n = cfg["dims"], cfg["kappa"], cfg["bc"], cfg["n_rhs"]
+    ctx = make_ctx(dims, kappa, bc, n, U)
+    P, P32 = ctx.pack(dev(Phi)), ctx.pack(dev(Phi), pkg.F32)
+    U32, Phi32 = U.astype(np.float32).astype(np.float64), Phi.astype(np.float32).astype(np.float64)
+    for op in (pkg.OP_D, pkg.OP_DDAG):
+        ref, ref32 = orc.apply(dims, kappa, bc, op, U, Phi), orc.apply(dims, kappa, bc, op, U32, Phi32)
+        for recon in (pkg.LINK18, pkg.LINK12):
+            assert rel_per_rhs(ctx.unpack(ctx.apply(op, P, n, pkg.F64, recon), n).cpu().numpy(), ref).max() < 1e-13
+            assert rel_per_rhs(ctx.unpack(ctx.apply(op, P32, n, pkg.F32, recon), n, pkg.F32).cpu().numpy(), ref32).max() < 1e-5
+    ctx.close()
+
+
+# ---- f1: the steps either side of the path (SURVEY.md 8(f1)) ------------------------------------------------------
+@pytest.mark.parametrize("cfg_idx", [0, 1])
+def test_refresh_and_action(cfg_idx):
+    """wd_refresh (phi = D eta; even/odd variant phi_e = Dhat eta_e) and wd_action against the oracle."""
+    pkg = _wd()
+    cfg, U, _ = wi.make_config(cfg_idx)
+    dims, kappa, bc, n = cfg["dims"], cfg["kappa"], cfg["bc"], cfg["n_rhs"]
+    eta = wi.spinor_field(dims, n, 9, bc)
+    ctx = make_ctx(dims, kappa, bc, n, U)
+    E = ctx.pack(dev(eta))
+    phi = ctx.unpack(ctx.refresh(E, n), n).cpu().numpy()
+    assert rel_per_rhs(phi, orc.apply(dims, kappa, bc, 0, U, eta)).max() < 1e-13
+    # action of x = eta: S_i = |eta_i|^2, all sites / even sites / odd sites
+    S = np.array(ctx.action(E, n))
+    assert np.allclose(S, orc.action(eta), rtol=1e-13)
+    Se = np.array(ctx.action(E, n, pkg.PARITY_EVEN))
+    So = np.array(ctx.action(E, n, pkg.PARITY_ODD))
+    assert np.allclose(Se, orc.action(orc.project_parity(dims, 0, eta)), rtol=1e-13)
+    assert np.allclose(So, orc.action(orc.project_parity(dims, 1, eta)), rtol=1e-13)
+    # even/odd variant: phi_e = Dhat eta_e = P_e D (eta_e, kappa H_oe eta_e); the oracle gets it as the even part of
+    # D applied to D^-1-free data: Dhat eta_e = eta_e - kappa^2 H_eo H_oe eta_e with H = (1 - D) / kappa
+    eta_e = orc.project_parity(dims, 0, eta)
+    H1 = (eta_e - orc.apply(dims, kappa, bc, 0, U, eta_e)) / kappa          # H eta_e (lives on odd sites)
+    H2 = (H1 - orc.apply(dims, kappa, bc, 0, U, H1)) / kappa                # H H eta_e (even sites)
+    ref = eta_e - kappa ** 2 * H2
+    phi_eo = ctx.unpack(ctx.refresh(E, n, pkg.ACTION_EO), n).cpu().numpy()
+    assert rel_per_rhs(phi_eo, ref).max() < 1e-13
+    assert np.all(orc.project_parity(dims, 1, phi_eo) == 0.0)
+    # project_parity in place
+    Q = E.clone()
+    ctx.project_parity(Q, n, 1)
+    assert np.array_equal(ctx.unpack(Q, n).cpu().numpy(), orc.project_parity(dims, 1, eta))
+    ctx.close()
+
+
+@pytest.mark.parametrize("cfg_idx", [0, 1])
+def test_md_force_full_and_even_odd_action_variants(cfg_idx):
+    """wd_md_force: Algorithm 2 in one call on device fields.  Full action: equals the oracle's X, Y, F and S = |x|^2.
+    Even/odd-preconditioned action (phi on even sites): equals the oracle's composition (pinned by finite differences
+    of the dense Schur-complement action in tests/test_oracle_pins.py)."""
+    pkg = _wd()
+    cfg, U, Phi = wi.make_config(cfg_idx)
+    dims, kappa, bc, n = cfg["dims"], cfg["kappa"], cfg["bc"], cfg["n_rhs"]
+    ctx = make_ctx(dims, kappa, bc, n, U)
+    P = ctx.pack(dev(Phi))
+    # full
+    Xr, rr, _, rc = orc.solve(dims, kappa, bc, 0, U, Phi, tol=1e-14)
+    assert rc == 0 and rr.max() < 1e-13
+    Yr, rr, _, rc = orc.solve(dims, kappa, bc, 1, U, Xr, tol=1e-14)
+    assert rc == 0 and rr.max() < 1e-13
+    X, Y, F, S, infos = ctx.md_force(P, n, pkg.ACTION_FULL)
+    assert infos[0]["converged"] and infos[1]["converged"]
+    assert rel_per_rhs(ctx.unpack(X, n).cpu().numpy(), Xr).max() < 1e-9
+    assert rel_per_rhs(ctx.unpack(Y, n).cpu().numpy(), Yr).max() < 1e-9
+    force_close(F.cpu().numpy(), orc.force(dims, kappa, bc, U, Xr, Yr), 1e-9)
+    assert np.allclose(S, orc.action(Xr), rtol=1e-9)
+    # even/odd
+    Xe, Ye, Se, Fe = orc.eo_md_force(dims, kappa, bc, U, Phi)
+    X, Y, F, S, infos = ctx.md_force(P, n, pkg.ACTION_EO)
+    assert infos[0]["converged"] and infos[1]["converged"]
+    assert rel_per_rhs(ctx.unpack(X, n).cpu().numpy(), Xe).max() < 1e-9
+    assert rel_per_rhs(ctx.unpack(Y, n).cpu().numpy(), Ye).max() < 1e-9
+    force_close(F.cpu().numpy(), Fe, 1e-9)
+    assert np.allclose(S, Se, rtol=1e-9)
+    ctx.close()
+
+
+def test_md_force_host_gauge_matches_device_path():
+    pkg = _wd()
+    cfg, U, Phi = wi.make_config(0)
+    dims, kappa, bc, n = cfg["dims"], cfg["kappa"], cfg["bc"], cfg["n_rhs"]
+    ctx = make_ctx(dims, kappa, bc, n, wi.unit_gauge(dims))   # a different gauge field first: the call must replace it
+    Fh, infos = ctx.md_force_host_gauge(torch.from_numpy(U).pin_memory(), torch.from_numpy(Phi).pin_memory())
+    assert infos[0]["converged"] and infos[1]["converged"]
+    P = ctx.pack(dev(Phi))
+    X, _ = ctx.solve_block(pkg.OP_D, P, n)
+    Y, _ = ctx.solve_block(pkg.OP_DDAG, X, n)
+    assert np.array_equal(Fh.numpy(), ctx.force(X, Y, n).cpu().numpy())
     ctx.close()
