@@ -4,7 +4,8 @@
 A "step" is one MD force evaluation (Algorithm 2): the blocked mixed-precision solve
 D X = Phi, the blocked solve D^dag Y = X (both to a true fp64 relative residual of 1e-12) and the
 force accumulation F += sum_i f[x_i, y_i], over all n_rhs pseudo-fermion fields, all in the CUDA
-kernels of libwd.so through its C ABI.  Workload at N = 1: BASELINE.json configs[4] at n_rhs = 5
+kernels of libwd.so through its C ABI (inner fp32 links: 18 reals by default, --recon 12 for the compressed
+form).  Workload at N = 1: BASELINE.json configs[4] at n_rhs = 5
 (24^3 x 24 SF lattice, eps 0.4, kappa 0.135) -- the largest single-GPU config and the only one whose
 working set (about 0.65 GB of solver vectors + 96 MB of fp32 links) is far outside the 126 MB L2,
 so no L2 flush is needed between steps.  N > 1: independent replicas (the path has no exchange step,
@@ -39,14 +40,16 @@ def parse_args():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", type=int, default=4, help="index into BASELINE.json configs")
     ap.add_argument("--n-rhs", type=int, default=5)
-    ap.add_argument("--recon", type=int, default=12, choices=(12, 18), help="inner fp32 link form")
+    ap.add_argument("--recon", type=int, default=18, choices=(12, 18), help="inner fp32 link form")
     ap.add_argument("--impl", default="ours", choices=("ours", "reference"))
     ap.add_argument("--hop-impl", type=int, default=-1, choices=(-1, 0, 1),
                     help="WD_OPT_HOP_IMPL: 0 register kernel, 1 shared-memory-staged kernel, -1 library default")
     ap.add_argument("--rhs-sweep", action="store_true", help="configs[4]: blocked solve at n_rhs = 1, 2, 5, 8, 12")
     ap.add_argument("--apply-sweep", action="store_true", help="configs[3]: D, D^dag apply on 16^4, fp32/fp64 x 18/12 reals")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cpu-baseline-full", action="store_true", help="time the oracle on the WHOLE workload (minutes)")
     ap.add_argument("--no-hop-sweep", action="store_true")
+    ap.add_argument("--no-config2", action="store_true", help="skip the configs[2] (12^4) force-evaluation time")
     return ap.parse_args()
 
 
@@ -58,42 +61,90 @@ def workload_name(cfg, n):
 # ------------------------------------------------------------------------------------------------
 # the oracle, timed on the host cores (cpu_baseline leg and --impl reference arm)
 # ------------------------------------------------------------------------------------------------
-# rough cost of one 1-RHS MD force evaluation of the oracle on 8 cores, seconds, by lattice size
-_ORACLE_SAMPLES = [(24, 90.0), (16, 14.0), (12, 3.5), (8, 0.6)]
+def pick_oracle_lattice(cfg, budget_s):
+    """Largest L in (workload's L, 16, 12, 8) whose 1-RHS oracle force evaluation is expected to fit `budget_s` on this
+    box: calibrated by timing the 8^4 case and scaling by (L/8)^4 x 1.6 (iteration counts and cache misses grow with L)."""
+    t8, _ = oracle_force_eval(cfg, 8, 1)
+    Lw = cfg["dims"][0]
+    for L in sorted({Lw, 16, 12, 8}, reverse=True):
+        if L <= Lw and (L == 8 or t8 * (L / 8.0) ** 4 * 1.6 <= budget_s):
+            return L
+    return 8
 
 
-def oracle_sample_time(cfg_full, n_full, L):
-    """Time the oracle, as it stands, on a bounded sample of the workload: ONE right-hand side on an
-    L^3 x L SF lattice drawn from the same link/RHS distribution (eps, kappa, seed of the workload).
-    Returns (seconds, site*rhs of the sample, iterations)."""
+def oracle_force_eval(cfg, L, n_cols):
+    """The oracle, as it stands, on `n_cols` right-hand sides of an L^4 SF lattice drawn from the workload's link / RHS
+    distribution (its eps, kappa, seed; L = the workload's own lattice when it fits the time budget): both solves to
+    TOL + force.  Returns (seconds, (iterations D, iterations D^dag) of column 0)."""
     import wd_inputs as wi
     from oracle import wd_oracle as orc
     dims = (L, L, L, L)
-    U = wi.gauge_field(dims, cfg_full["eps"], cfg_full["seed"], cfg_full["bc"])
-    Phi = wi.spinor_field(dims, 1, cfg_full["seed"], cfg_full["bc"])
-    k, bc = cfg_full["kappa"], cfg_full["bc"]
+    U = wi.gauge_field(dims, cfg["eps"], cfg["seed"], cfg["bc"])
+    Phi = wi.spinor_field(dims, n_cols, cfg["seed"], cfg["bc"])
+    k, bc = cfg["kappa"], cfg["bc"]
     t0 = time.perf_counter()
     X, r1, it1, _ = orc.solve(dims, k, bc, 0, U, Phi, tol=TOL)
     Y, r2, it2, _ = orc.solve(dims, k, bc, 1, U, X, tol=TOL)
     orc.force(dims, k, bc, U, X, Y)
-    dt = time.perf_counter() - t0
-    return dt, L ** 4, (int(it1[0]), int(it2[0]))
+    return time.perf_counter() - t0, (int(it1[0]), int(it2[0]))
 
 
-def oracle_value(cfg_full, n_full, L):
-    """force_eval/s of the full workload extrapolated from the sample by site*rhs count."""
-    dt, units, iters = oracle_sample_time(cfg_full, n_full, L)
-    lx, ly, lz, lt = cfg_full["dims"]
-    full_units = lx * ly * lz * lt * n_full
-    est_full = dt * full_units / units
-    sample = (f"oracle (fp64, unpreconditioned BiCGStab, OpenMP over sites) on 1 RHS of a {L}^4 SF lattice of the "
-              f"same distribution: 2 solves to {TOL:g} + force took {dt:.2f} s ({iters[0]}+{iters[1]} iterations); "
-              f"scaled by site*rhs count x{full_units / units:.1f} to the full workload")
-    return 1.0 / est_full, sample, dt
+def oracle_apply_rate(cfg, n, threads=None):
+    """site*RHS/s of the oracle's D apply on the workload's own lattice and n_rhs."""
+    import wd_inputs as wi
+    from oracle import wd_oracle as orc
+    dims = cfg["dims"]
+    U = wi.gauge_field(dims, cfg["eps"], cfg["seed"], cfg["bc"])
+    Phi = wi.spinor_field(dims, n, cfg["seed"], cfg["bc"])
+    full = orc.max_threads()
+    if threads:
+        orc.set_threads(threads)
+    orc.apply(dims, cfg["kappa"], cfg["bc"], 0, U, Phi)
+    t0 = time.perf_counter()
+    reps = 2
+    for _ in range(reps):
+        orc.apply(dims, cfg["kappa"], cfg["bc"], 0, U, Phi)
+    dt = (time.perf_counter() - t0) / reps
+    orc.set_threads(full)
+    lx, ly, lz, lt = dims
+    return lx * ly * lz * lt * n / dt
+
+
+def cpu_baseline(cfg, n, full=False):
+    """cpu_baseline leg: ONE column of the workload's own lattice (the oracle solves column by column, so the block
+    costs n_rhs times that: no extrapolation over lattice size), all host cores; plus the oracle's D-apply rate on the
+    full block with all cores and with one thread, and a single-thread force evaluation on a stated smaller lattice."""
+    from oracle import wd_oracle as orc
+    Lw = cfg["dims"][0]
+    cores = orc.max_threads()
+    if full:
+        L, ncol = Lw, n
+    else:
+        L, ncol = pick_oracle_lattice(cfg, 40.0), 1
+    dt, iters = oracle_force_eval(cfg, L, ncol)
+    orc.set_threads(1)
+    Ls = 8 if Lw >= 8 else Lw
+    dt1, it1 = oracle_force_eval(cfg, Ls, 1)
+    orc.set_threads(cores)
+    scale = (Lw / float(L)) ** 4 * n / ncol
+    how = ("the whole workload" if full else
+           f"1 of the {n} right-hand sides (the oracle works column by column, so the block costs {n} x that)" +
+           ("" if L == Lw else f" on a {L}^4 lattice of the same distribution, scaled by site count x{(Lw / float(L)) ** 4:.2f} "
+                               "(iteration counts grow slowly with L: this flatters the oracle)"))
+    sample = (f"oracle (fp64, unpreconditioned BiCGStab, OpenMP over sites), {cores} threads: 2 solves to {TOL:g} + force on {how}: "
+              f"{dt:.2f} s ({iters[0]}+{iters[1]} iterations for column 0)")
+    return {"value": 1.0 / (dt * scale), "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample,
+            "apply_site_rhs_per_s_all_cores": oracle_apply_rate(cfg, n),
+            "apply_site_rhs_per_s_1_thread": oracle_apply_rate(cfg, n, threads=1),
+            "single_thread": {"lattice": f"{Ls}^4 SF, 1 RHS", "seconds_per_force_eval": round(dt1, 2),
+                              "iterations": list(it1)}}
 
 
 def run_reference(args):
-    """--impl reference: the oracle on the host cores (rank 0 only)."""
+    """--impl reference: the oracle on the host cores (rank 0 only).  Each step is a bounded sample: ONE right-hand side
+    on the largest lattice of the workload's distribution that fits the time budget of this --steps/--warmup.  The line
+    reports what was RUN (`value`, `ms_per_step`, `config.workload` are the sample's) and, separately, the estimate for
+    the full workload (`scaled_to_full_workload`)."""
     from paper_1009_5169_b200 import replicas as rp
     if not rp.reference_arm_runs_here(rp.env_world()[1]):
         return
@@ -101,23 +152,31 @@ def run_reference(args):
     from oracle import wd_oracle as orc
     cfg = dict(wi.CONFIGS[args.config])
     n = args.n_rhs
-    budget = 200.0 / max(1, args.steps + args.warmup)
-    L = next((l for l, cost in _ORACLE_SAMPLES if cost <= budget and l <= cfg["dims"][0]), 8)
+    L = pick_oracle_lattice(cfg, 150.0 / max(1, args.steps + args.warmup))
     for _ in range(args.warmup):
-        oracle_value(cfg, n, L)
-    times, sample = [], ""
+        oracle_force_eval(cfg, L, 1)
+    times, iters = [], (0, 0)
     t0 = time.perf_counter()
     for _ in range(args.steps):
-        v, sample, dt = oracle_value(cfg, n, L)
-        times.append(1.0 / v)
+        dt, iters = oracle_force_eval(cfg, L, 1)
+        times.append(dt)
     total = time.perf_counter() - t0
     value = args.steps / sum(times)
     cores = orc.max_threads()
+    lx, ly, lz, lt = cfg["dims"]
+    scale = lx * ly * lz * lt * n / float(L ** 4)
+    scfg = dict(cfg, dims=(L, L, L, L))
+    sample = (f"each step = the oracle (fp64, unpreconditioned BiCGStab, OpenMP over sites) on 1 RHS of a {L}^4 SF lattice of the "
+              f"workload's distribution: 2 solves to {TOL:g} + force, {sum(times) / len(times):.2f} s ({iters[0]}+{iters[1]} "
+              f"iterations); value, ms_per_step and config.workload describe THIS sample")
     line = {
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": 1e3 / value, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": workload_name(cfg, n), "l2": "n/a (CPU)"},
+        "config": {"workload": workload_name(scfg, 1), "full_workload": workload_name(cfg, n), "l2": "n/a (CPU)",
+                   "sample_of_full_workload": f"1/{scale:.1f} of its site*RHS count"},
+        "scaled_to_full_workload": {"value": value / scale, "unit": UNIT,
+                                    "note": "by site*RHS count; iteration counts grow slowly with L, so this flatters the oracle"},
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0, "wall_s": total,
@@ -184,14 +243,15 @@ class ClockSampler:
 # ------------------------------------------------------------------------------------------------
 # standalone hop (dslash) measurement: BASELINE.json metric "multi-RHS Wilson dslash GFLOP/s & HBM GB/s"
 # ------------------------------------------------------------------------------------------------
-def hop_bytes_per_launch(Vh, n, s, R, extra_operands=0.0):
-    """Algorithmic bytes of one hop launch on one output parity: per output
-    site*RHS 24 reals in + 24 out, +24 per extra operand the fused epilogue reads (xpay operand,
-    left operand of a fused inner product), and 8 links of R reals per site."""
-    return Vh * (n * (48 + 24 * extra_operands) * s + 8 * R * s)
+def hop_bytes_per_launch(Vh, n, s, R, extra_operands=0.0, interior=1.0):
+    """Algorithmic bytes of one hop launch on one output parity: per output site*RHS 24 reals in +
+    24 out, +24 per extra operand the fused epilogue reads (xpay operand, left operand of a fused inner product), and
+    8 links of R reals per site.  `interior` = (T-1)/T with Schroedinger-functional boundaries: the kernels skip the
+    frozen t = 0 slice, so everything READ is counted on interior sites only; the output is written on all sites."""
+    return Vh * (n * (24 * interior + 24 + 24 * extra_operands * interior) * s + 8 * R * s * interior)
 
 
-def hop_sweep(pkg, ctx, torch, n, peak_gbs, reps=50, only=None):
+def hop_sweep(pkg, ctx, torch, n, peak_gbs, reps=50, only=None, interior=1.0):
     """wd_hop back to back on native half-lattice blocks, fp32/fp64 x 18/12-real links; CUDA events
     on the launching stream.  Fields rotate through enough copies to exceed 2x L2 (L2-cold)."""
     res = {}
@@ -217,7 +277,7 @@ def hop_sweep(pkg, ctx, torch, n, peak_gbs, reps=50, only=None):
             e1.record()
             torch.cuda.synchronize()
             us = e0.elapsed_time(e1) * 1e3 / reps
-            b = hop_bytes_per_launch(Vh, n, s, R)
+            b = hop_bytes_per_launch(Vh, n, s, R, interior=interior)
             gbs = b / us * 1e-3
             res[f"{pname}_r{R}"] = {"us": round(us, 2), "gbs": round(gbs, 1), "frac_hbm": round(gbs / peak_gbs, 4),
                                     "gflops": round(1320.0 * Vh * n / us * 1e-3, 1),
@@ -250,7 +310,7 @@ def rhs_sweep(pkg, wi, torch, peak_gbs, R, recon):
         torch.cuda.synchronize()
         ms = e0.elapsed_time(e1) / reps
         del P, X
-        hop = hop_sweep(pkg, ctx, torch, n, peak_gbs, reps=30, only=("f32", R))
+        hop = hop_sweep(pkg, ctx, torch, n, peak_gbs, reps=30, only=("f32", R), interior=(dims[3] - 1) / dims[3])
         out[str(n)] = {"solve_ms": round(ms, 3), "ms_per_rhs": round(ms / n, 3), "inner_iters": info["inner_iters_total"],
                        "us_per_inner_iter": round(ms * 1e3 / max(1, info["inner_iters_total"]), 1),
                        "max_relres": max(info["relres"]), "hop_f32": hop[f"f32_r{R}"]}
@@ -297,6 +357,31 @@ def apply_sweep(pkg, wi, torch, peak_gbs, reps=50):
         del bufs, out
     ctx.close()
     return res
+
+
+def config2_time(pkg, wi, torch, recon):
+    """BASELINE.json configs[2]: full MD force evaluation (two blocked solves + force) on the 12^4 SF lattice, 5 RHS.
+    L2-resident and launch-bound: an absolute time only, no roofline claim."""
+    cfg, U, Phi = wi.make_config(2)
+    dims, kappa, bc, n = cfg["dims"], cfg["kappa"], cfg["bc"], cfg["n_rhs"]
+    ctx = pkg.Context(dims, kappa, bc=bc, max_rhs=n)
+    ctx.set_gauge(torch.from_numpy(U).cuda())
+    P = ctx.pack(torch.from_numpy(Phi).cuda())
+    for _ in range(2):
+        X, Y, F, S, infos = ctx.md_force(P, n, recon=recon, want_action=False)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    e0.record()
+    reps = 5
+    for _ in range(reps):
+        X, Y, F, S, infos = ctx.md_force(P, n, recon=recon, want_action=False)
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / reps
+    ctx.close()
+    return {"ms_per_force_eval": round(ms, 3), "inner_iters": [infos[0]["inner_iters_total"], infos[1]["inner_iters_total"]],
+            "outer_steps": [infos[0]["outer_steps"], infos[1]["outer_steps"]],
+            "max_relres": max(max(infos[0]["relres"]), max(infos[1]["relres"]))}
 
 
 # ------------------------------------------------------------------------------------------------
@@ -380,18 +465,42 @@ def run_ours(args):
     ms_step = ms_total / args.steps
     value = rp.job_throughput(world, args.steps, ms_total)
 
-    # ---- e2e: host buffers through the one-call C-ABI entry, copies inside the timed region ------
-    ctx.md_force_host(Phi_host, F_host, tol=TOL, recon=recon)
+    # ---- e2e: host buffers through the one-call C-ABI entry, copies inside the timed region --------
+    # The links change between the force evaluations of a trajectory, so the end-to-end step uploads
+    # and ingests the gauge field too (wd_md_force_host_gauge); the Phi-only form is reported beside it.
+    U_host = torch.from_numpy(U).pin_memory()
+    ctx.md_force_host_gauge(U_host, Phi_host, F_host, tol=TOL, recon=recon)
     barrier()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        ctx.md_force_host_gauge(U_host, Phi_host, F_host, tol=TOL, recon=recon)
+    barrier()
+    e2e_ms = max_over_ranks((time.perf_counter() - t0) * 1e3)
+    e2e_value = rp.job_throughput(world, args.steps, e2e_ms)
     t0 = time.perf_counter()
     for _ in range(args.steps):
         ctx.md_force_host(Phi_host, F_host, tol=TOL, recon=recon)
     barrier()
-    e2e_ms = max_over_ranks((time.perf_counter() - t0) * 1e3)
-    e2e_value = rp.job_throughput(world, args.steps, e2e_ms)
+    e2e_phi_ms = max_over_ranks((time.perf_counter() - t0) * 1e3)
     clocks = sampler.stop()
     f_check = float(F_host.abs().sum())
     assert np.isfinite(f_check) and f_check > 0.0
+    # a0 alone: gauge upload (pinned host -> device) + ingest kernel
+    Ud = torch.empty(U_host.shape, dtype=torch.float64, device=ctx.device)
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    for _ in range(3):
+        Ud.copy_(U_host, non_blocking=True)
+        ctx.set_gauge(Ud)
+    torch.cuda.synchronize()
+    a0_ms = (time.perf_counter() - t0) * 1e3 / 3
+    e0.record()
+    for _ in range(3):
+        ctx.set_gauge(Ud)
+    e1.record()
+    torch.cuda.synchronize()
+    a0_ingest_ms = e0.elapsed_time(e1) / 3
+    del Ud
 
     # ---- per-class device time of one more step (event pairs inside the library) -----------------
     ctx.profile(True)
@@ -405,25 +514,38 @@ def run_ours(args):
     tot_prof = sum(v[0] for v in prof.values())
     # the four fp32 hop launches of one BiCGStab iteration: plain, xpay + <rt, v> (2 extra operands), plain,
     # xpay + <t, s>, <t, t> (1 extra operand): 0.75 extra operands per launch on average
-    hop_bytes = hop_bytes_per_launch(Vh, n, 4, R, extra_operands=0.75)
+    interior = (dims[3] - 1) / dims[3] if bc == wi.BC_SF else 1.0
+    hop_bytes = hop_bytes_per_launch(Vh, n, 4, R, extra_operands=0.75, interior=interior)
     hop_us = hop_ms * 1e3 / max(1, hop_cnt)
     achieved = hop_bytes / (hop_us * 1e-6) * 1e-9 if hop_cnt else 0.0
-    staged = ctx.get_option(pkg.OPT_HOP_IMPL) == 1 and (dims[0] // 2) % 2 == 0
-    kname = f"hop_tma_kernel<float,{R}>" if staged else f"hop_kernel<float,{R}>"
-    traffic = None
-    try:  # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu --set full capture
-        tr = json.load(open(os.path.join(ROOT, "profiles", "r01b_hop_traffic.json.txt")))
-        if tr.get("kernel") == kname and tr.get("workload") == workload_name(dict(wi.CONFIGS[args.config]), n):
-            traffic = tr["dram_bytes_per_launch"]
+    # which kernel the library's dispatch picks (wd_hop.cu wd_hop_launch_ex): z-march (impl 2) or row-group ring (impl 1)
+    # where the layout is row-major (linear site order, Lx/2 even, max_rhs >= 3) and n_rhs >= 3, else the register kernel
+    impl = ctx.get_option(pkg.OPT_HOP_IMPL)
+    staged = impl >= 1 and (dims[0] // 2) % 2 == 0 and n >= 3
+    kname = (f"hop_zm_kernel<float,{R}>" if impl == 2 else f"hop_tma_kernel<float,{R}>") if staged else f"hop_kernel<float,{R}>"
+    # dram__bytes_read.sum + dram__bytes_write.sum per launch from an ncu --set full capture of THIS kernel source: the
+    # committed record carries the sha256 of the kernel's source file and is ignored when the source has changed since
+    traffic, traffic_note = None, "no capture on record for this kernel source"
+    try:
+        import hashlib
+        tr = json.load(open(os.path.join(ROOT, "profiles", "r02_hop_traffic.json.txt")))
+        src = {"hop_zm_kernel": "wd_hop_zm.cu", "hop_tma_kernel": "wd_hop_tma.cu", "hop_kernel": "wd_hop.cu"}[kname.split("<")[0]]
+        sha = hashlib.sha256(open(os.path.join(ROOT, "paper_1009_5169_b200", "csrc", src), "rb").read()).hexdigest()
+        if tr.get("kernel") == kname and tr.get("source_sha256") == sha and \
+                tr.get("workload") == workload_name(dict(wi.CONFIGS[args.config]), n):
+            traffic, traffic_note = tr["dram_bytes_per_launch"], tr.get("how", "")
+        elif tr.get("source_sha256") != sha:
+            traffic_note = "the capture on record is of an older kernel source"
     except Exception:
         pass
     roofline = {"bound": "hbm", "kernel": f"{kname} (fp32 multi-RHS Wilson hop inside the inner solver, 2 of 4 launches per iteration with "
                                           "fused xpay + inner-product epilogues)",
                 "achieved": round(achieved, 1), "peak": peak_gbs, "unit": "GB/s", "frac": round(achieved / peak_gbs, 4),
-                "peak_source": peak_src, "traffic": traffic, "bytes_per_launch": hop_bytes,
+                "peak_source": peak_src, "traffic": traffic, "traffic_note": traffic_note, "bytes_per_launch": hop_bytes,
+                "bytes_counted": f"interior sites only for everything read ((T-1)/T = {interior:.4f}), all sites for the output",
                 "avg_launch_us": round(hop_us, 2), "launches_in_step": hop_cnt,
                 "share_of_step": round(hop_ms / tot_prof, 4) if tot_prof else None,
-                "gflops": round(1320.0 * Vh * n / hop_us * 1e-3, 1) if hop_cnt else None}
+                "gflops": round(1320.0 * Vh * n * interior / hop_us * 1e-3, 1) if hop_cnt else None}
     breakdown = {k: {"ms": round(v[0], 3), "launch_groups": v[1]} for k, v in prof.items()}
 
     line = {
@@ -434,7 +556,11 @@ def run_ours(args):
                    "tol": TOL, "l2": "no flush: solver working set >> 126 MB L2", "parallelism": f"replicas x{world}"},
         "clocks": clocks,
         "e2e": {"value": e2e_value, "unit": UNIT, "ms_per_step": e2e_ms / args.steps,
-                "h2d_bytes_per_step": Phi_host.numel() * 8, "d2h_bytes_per_step": F_host.numel() * 8},
+                "h2d_bytes_per_step": (Phi_host.numel() + U_host.numel()) * 8, "d2h_bytes_per_step": F_host.numel() * 8,
+                "includes": "gauge upload + ingest (a0), Phi upload + pack, both solves, force, F download",
+                "phi_only_ms_per_step": e2e_phi_ms / args.steps},
+        "a0_gauge": {"upload_plus_ingest_ms": round(a0_ms, 3), "ingest_kernel_ms": round(a0_ingest_ms, 3),
+                     "h2d_bytes": U_host.numel() * 8},
         "gpu_launches": int(launches),
         "roofline": roofline,
         "solver": {"outer_steps": [ix["outer_steps"], iy["outer_steps"]],
@@ -444,17 +570,17 @@ def run_ours(args):
         "breakdown_ms": breakdown,
     }
     if rank == 0 and not args.no_hop_sweep:
-        line["hop"] = hop_sweep(pkg, ctx, torch, n, peak_gbs)
+        line["hop"] = hop_sweep(pkg, ctx, torch, n, peak_gbs, interior=interior)
     ctx.close()
     del ctx, P, X, Y, F
     if rank == 0 and args.rhs_sweep:
         line["rhs_sweep"] = rhs_sweep(pkg, wi, torch, peak_gbs, R, recon)
     if rank == 0 and args.apply_sweep:
         line["apply_16"] = apply_sweep(pkg, wi, torch, peak_gbs)
+    if rank == 0 and not args.no_config2:
+        line["config2_12x12x12x12"] = config2_time(pkg, wi, torch, recon)
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        from oracle import wd_oracle as orc
-        v, sample, _ = oracle_value(dict(wi.CONFIGS[args.config]), n, 16 if dims[0] >= 16 else dims[0])
-        line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": orc.max_threads(), "kind": "oracle", "sample": sample}
+        line["cpu_baseline"] = cpu_baseline(dict(wi.CONFIGS[args.config]), n, full=args.cpu_baseline_full)
     if world > 1:
         dist.barrier()
         dist.destroy_process_group()
