@@ -106,9 +106,21 @@ int wd_site_order(wd_ctx* ctx, int order, const int tile[4]);
  *   WD_OPT_ALTERNATE_SWEEP  1 (default): consecutive kernels of the inner solver sweep the vectors in opposite
  *       directions, so that what one kernel wrote last is still in L2 when the next reads it first; 0: off.
  *   WD_OPT_POLL_EVERY   inner iterations enqueued between two convergence polls of the solver (>= 1).
+ *   WD_OPT_SOLVER       the route wd_solve_block (and everything built on it) takes to the SAME result X = A^-1 Phi
+ *       within tol; iteration counts differ.
+ *       WD_SOLVER_DC_F32 (default): fp64 defect correction around an fp32-storage BiCGStab (reading R11).
+ *       WD_SOLVER_RELIABLE_H16: one continuous BiCGStab sequence per column with the vectors STORED in 16 bits
+ *       (fp16 mantissas + one fp32 scale per spinor, arithmetic in fp32) and fp64 reliable updates in place of
+ *       restarts ("tuning techniques described in [4]"); inner_tol is then the
+ *       reliable-update threshold delta (0 = default 0.01), max_outer bounds the number of updates and max_inner the
+ *       total number of iterations.  Needs the z-march hop kernel (linear site order, Lx/2 even, n_rhs >= 3,
+ *       Lx/2 * n_rhs a multiple of 4); elsewhere the default solver runs.
  * Errors: WD_EINVAL (null, unknown key, value out of range). */
 enum { WD_OPT_HOP32_SITES = 0, WD_OPT_HOP64_SITES = 1, WD_OPT_HOP32_REGS = 2, WD_OPT_HOP64_REGS = 3,
-       WD_OPT_POLL_EVERY = 4, WD_OPT_HOP_IMPL = 5, WD_OPT_ALTERNATE_SWEEP = 6, WD_OPT_HOP_ROWS = 7, WD_OPT_N = 8 };
+       WD_OPT_POLL_EVERY = 4, WD_OPT_HOP_IMPL = 5, WD_OPT_ALTERNATE_SWEEP = 6, WD_OPT_HOP_ROWS = 7, WD_OPT_SOLVER = 8,
+       WD_OPT_N = 9 };
+/* values of WD_OPT_SOLVER */
+enum { WD_SOLVER_DC_F32 = 0, WD_SOLVER_RELIABLE_H16 = 1, WD_SOLVER_N = 2 };
 int wd_set_option(wd_ctx* ctx, int key, int value);
 int wd_get_option(const wd_ctx* ctx, int key, int* value_host);
 

@@ -23,14 +23,17 @@ enum {
     S_SCALE,      // |R_i| used to normalise the inner right-hand side
     S_OUT_CONV,   // 1 if column met the outer tolerance
     S_ACTION,     // |x_i|^2 of wd_action (pseudo-fermion action per column)
+    S_RHO_PREV_RE, S_RHO_PREV_IM,  // rho of the previous iteration (reliable updates: beta is recomputed after r is replaced)
+    S_RMAX2,      // largest recursive |r_i|^2 since the last reliable update
     S_ROWS
 };
 // global (not per-column) slots after the table
-enum { G_DONE = S_ROWS * WD_MAX_RHS, G_ITERS, G_OUT_DONE, G_TOL2, G_INTOL2, G_COUNT };
+enum { G_DONE = S_ROWS * WD_MAX_RHS, G_ITERS, G_OUT_DONE, G_TOL2, G_INTOL2, G_DELTA2, G_UPDATES, G_COUNT };
 
 __device__ __forceinline__ double& SC(double* scal, int row, int r) { return scal[row * WD_MAX_RHS + r]; }
 
-enum Kind { K_SIGMA, K_OMEGA, K_RHO, K_PHI2, K_OUT_R2, K_INIT_RHO, K_ACTION };
+enum Kind { K_SIGMA, K_OMEGA, K_RHO, K_PHI2, K_OUT_R2, K_INIT_RHO, K_ACTION,
+            K_RHO_REL, K_OUT_R2_REL, K_REPLACE };   // reliable-update solver (wd_solve_h16.cu)
 
 struct RedBuf {
     double* scal;
@@ -74,6 +77,7 @@ __device__ void finalize_column(double* scal, int r, const double* tot) {
             SC(scal, S_OMEGA_RE, r) = 1.0;  SC(scal, S_OMEGA_IM, r) = 0.0;
             SC(scal, S_BETA_RE, r) = 0.0;   SC(scal, S_BETA_IM, r) = 0.0;
             SC(scal, S_RNORM2, r) = tot[2];
+            SC(scal, S_RMAX2, r) = tot[2];
             // S_FLAG was set by the outer residual kernel (1 = column already converged)
             if (!frozen && !(tot[2] > 0.0)) SC(scal, S_FLAG, r) = 1.0;
             return;
@@ -97,6 +101,55 @@ __device__ void finalize_column(double* scal, int r, const double* tot) {
         }
         SC(scal, S_RHO_RE, r) = rho1.re; SC(scal, S_RHO_IM, r) = rho1.im;
         SC(scal, S_BETA_RE, r) = beta.re; SC(scal, S_BETA_IM, r) = beta.im;
+    } else if (KIND == K_RHO_REL) {  // tot = <rt, r>, |r|^2 after the x, r update of the reliable-update solver
+        if (frozen) {
+            SC(scal, S_BETA_RE, r) = 0.0; SC(scal, S_BETA_IM, r) = 0.0;
+            return;
+        }
+        SC(scal, S_RNORM2, r) = tot[2];
+        const cd rho1 = {tot[0], tot[1]};
+        const cd rho = {SC(scal, S_RHO_RE, r), SC(scal, S_RHO_IM, r)};
+        const cd alpha = {SC(scal, S_ALPHA_RE, r), SC(scal, S_ALPHA_IM, r)};
+        const cd omega = {SC(scal, S_OMEGA_RE, r), SC(scal, S_OMEGA_IM, r)};
+        cd beta = {0.0, 0.0};
+        if (tot[2] <= SC(scal, S_THR2, r)) {
+            SC(scal, S_FLAG, r) = 1.0;   // converged by the recursive residual: the next reliable update checks the true one
+        } else if (!(tot[2] == tot[2]) || (omega.re == 0.0 && omega.im == 0.0) || (rho1.re == 0.0 && rho1.im == 0.0)) {
+            SC(scal, S_FLAG, r) = 2.0;   // breakdown or NaN: frozen until the next reliable update restarts the column
+        } else {
+            beta = cmul(cdiv(rho1, rho), cdiv(alpha, omega));
+        }
+        SC(scal, S_RHO_PREV_RE, r) = rho.re; SC(scal, S_RHO_PREV_IM, r) = rho.im;
+        SC(scal, S_RHO_RE, r) = rho1.re; SC(scal, S_RHO_IM, r) = rho1.im;
+        SC(scal, S_BETA_RE, r) = beta.re; SC(scal, S_BETA_IM, r) = beta.im;
+        if (tot[2] > SC(scal, S_RMAX2, r)) SC(scal, S_RMAX2, r) = tot[2];
+    } else if (KIND == K_REPLACE) {  // tot = <rt, r'>, |r'|^2 with r' the true residual that replaced r
+        SC(scal, S_RNORM2, r) = tot[2];
+        SC(scal, S_RMAX2, r) = tot[2];
+        if (frozen) return;            // converged columns (S_FLAG set by K_OUT_R2_REL) stay frozen
+        const cd rho1 = {tot[0], tot[1]};
+        const cd rho = {SC(scal, S_RHO_PREV_RE, r), SC(scal, S_RHO_PREV_IM, r)};
+        const cd alpha = {SC(scal, S_ALPHA_RE, r), SC(scal, S_ALPHA_IM, r)};
+        const cd omega = {SC(scal, S_OMEGA_RE, r), SC(scal, S_OMEGA_IM, r)};
+        cd beta = {0.0, 0.0};
+        const bool bad = (omega.re == 0.0 && omega.im == 0.0) || (rho.re == 0.0 && rho.im == 0.0) || (rho1.re == 0.0 && rho1.im == 0.0);
+        if (!bad) beta = cmul(cdiv(rho1, rho), cdiv(alpha, omega));
+        else { SC(scal, S_OMEGA_RE, r) = 1.0; SC(scal, S_OMEGA_IM, r) = 0.0; SC(scal, S_ALPHA_RE, r) = 1.0; SC(scal, S_ALPHA_IM, r) = 0.0; }
+        // after a breakdown the column restarts: beta = 0 makes p = r'; (alpha, omega reset; v is multiplied by beta = 0)
+        SC(scal, S_RHO_RE, r) = rho1.re; SC(scal, S_RHO_IM, r) = rho1.im;
+        SC(scal, S_BETA_RE, r) = beta.re; SC(scal, S_BETA_IM, r) = beta.im;
+    } else if (KIND == K_OUT_R2_REL) {  // tot = |R_i|^2, the TRUE fp64 residual of the even/odd system
+        SC(scal, S_OUT_R2, r) = tot[0];
+        const double phi2 = SC(scal, S_PHI2, r);
+        const double tol2 = scal[G_TOL2];
+        const bool conv = tot[0] <= tol2 * phi2;
+        SC(scal, S_OUT_CONV, r) = conv ? 1.0 : 0.0;
+        SC(scal, S_FLAG, r) = conv ? 1.0 : 0.0;   // a column frozen on its recursive residual or a breakdown goes on if not converged
+        if (scal[G_UPDATES] == 0.0) {             // first call: the normalisation of the low-precision system is fixed here
+            SC(scal, S_SCALE, r) = sqrt(tot[0]);
+            // recursive target: half of what the tolerance needs, in units of the scale
+            SC(scal, S_THR2, r) = tot[0] > 0.0 ? 0.25 * tol2 * phi2 / tot[0] : 0.0;
+        }
     } else if (KIND == K_PHI2) {
         SC(scal, S_PHI2, r) = tot[0];
     } else if (KIND == K_ACTION) {
@@ -127,6 +180,26 @@ __device__ void finalize_global(double* scal, int n) {
         bool all = true;
         for (int r = 0; r < n; ++r) all = all && (SC(scal, S_OUT_CONV, r) != 0.0);
         scal[G_OUT_DONE] = all ? 1.0 : 0.0;
+    } else if (KIND == K_RHO_REL) {
+        // the iteration kernels turn into no-ops when every column is frozen OR a column asks for a reliable update
+        // (its recursive residual fell below delta times the largest one since the last update)
+        bool all = true, rel = false;
+        for (int r = 0; r < n; ++r) {
+            const bool fr = SC(scal, S_FLAG, r) != 0.0;
+            all = all && fr;
+            rel = rel || (!fr && SC(scal, S_RNORM2, r) < scal[G_DELTA2] * SC(scal, S_RMAX2, r));
+        }
+        scal[G_DONE] = (all || rel) ? 1.0 : 0.0;
+        scal[G_ITERS] += 1.0;
+    } else if (KIND == K_OUT_R2_REL) {
+        bool all = true;
+        for (int r = 0; r < n; ++r) all = all && (SC(scal, S_OUT_CONV, r) != 0.0);
+        scal[G_OUT_DONE] = all ? 1.0 : 0.0;
+        scal[G_UPDATES] += 1.0;
+    } else if (KIND == K_REPLACE) {
+        bool all = true;
+        for (int r = 0; r < n; ++r) all = all && (SC(scal, S_FLAG, r) != 0.0);
+        scal[G_DONE] = all ? 1.0 : 0.0;
     }
 }
 

@@ -206,6 +206,9 @@ int wd_set_option(wd_ctx* ctx, int key, int value) {
         case WD_OPT_HOP_ROWS:
             if (value < 0 || value > 1024) return wd_fail(ctx, WD_EINVAL, "rows per group out of range");
             break;
+        case WD_OPT_SOLVER:
+            if (value < 0 || value >= WD_SOLVER_N) return wd_fail(ctx, WD_EINVAL, "unknown solver");
+            break;
         case WD_OPT_POLL_EVERY:
             if (value < 1 || value > 1024) return wd_fail(ctx, WD_EINVAL, "poll interval out of range");
             break;
@@ -374,8 +377,7 @@ int wd_solve_block(wd_ctx* ctx, int op, int n_rhs, const double* Phi, double* X,
     if (rc) return rc;
     rc = check_solver_params(ctx, tol, max_outer, max_inner, inner_tol);
     if (rc) return rc;
-    return wd_solve_impl(ctx, op == WD_OP_DDAG, n_rhs, Phi, X, tol, max_outer, max_inner,
-                         inner_tol > 0.0 ? inner_tol : 1e-5, recon, info);
+    return wd_solve_impl(ctx, op == WD_OP_DDAG, n_rhs, Phi, X, tol, max_outer, max_inner, inner_tol, recon, info);
 }
 
 int wd_force(wd_ctx* ctx, int n_rhs, const double* X, const double* Y, double* F) {
@@ -417,7 +419,7 @@ static int md_force_host_common(wd_ctx* ctx, int n_rhs, const double* U_host, co
     int rc = wd_layout_pack(ctx, WD_F64, n_rhs, dCanon, dPhi);
     if (rc) return rc;
     WD_CUDA_CHECK(ctx, cudaMemsetAsync(dF, 0, sizeof(double) * 4 * ctx->V * 18, ctx->stream));
-    const double itol = inner_tol > 0.0 ? inner_tol : 1e-5;
+    const double itol = inner_tol;
     rc = wd_md_force_impl(ctx, WD_ACTION_FULL, n_rhs, dPhi, dX, dY, dF, nullptr, dCanon, tol, max_outer, max_inner, itol,
                           recon, info2);
     if (rc != WD_OK && rc != WD_ENOCONV) return rc;
@@ -473,7 +475,7 @@ int wd_md_force(wd_ctx* ctx, int variant, int n_rhs, const double* Phi, double* 
     const size_t fbytes = wd_align_up(sizeof(double) * 4 * ctx->V * 18);
     double* tmp = (double*)(ctx->d_solver + ctx->solver_bytes - fbytes - 4 * full);
     return wd_md_force_impl(ctx, variant, n_rhs, Phi, X, Y, F, S_host, tmp, tol, max_outer, max_inner,
-                            inner_tol > 0.0 ? inner_tol : 1e-5, recon, info2);
+                            inner_tol, recon, info2);
 }
 
 }  // extern "C"

@@ -244,6 +244,12 @@ int wd_hop_launch_ex(wd_ctx* c, int prec, int recon, int dag, int n, int par, co
     if (o.epi >= EPI_SIGMA && prec != WD_F32) return wd_fail(c, WD_EINVAL, "fused reductions are fp32 only");
     // staged kernel where it applies (row-major layout) and pays: with 1-2 columns a group of rows gives it too few
     // consumer threads (24^4 fp32: 41 us against 33 us at n = 2; 71 against 76 at n = 5; 146 against 151 at n = 12)
+    if (o.storage == 1) {   // 16-bit storage: served by the z-march kernel only
+        const int rc = n >= 3 ? wd_hop_zm_launch(c, prec, recon, dag, n, par, o) : 1;
+        if (rc > 0) return wd_fail(c, WD_EINVAL, "hop: the 16-bit storage format needs the z-march kernel (row-major layout, n_rhs >= 3)");
+        if (rc == WD_OK) WD_LAUNCH_CHECK(c);
+        return rc;
+    }
     if (c->opt[WD_OPT_HOP_IMPL] >= 1 && n >= 3) {
         int rc = 1;
         if (c->opt[WD_OPT_HOP_IMPL] == 2) rc = wd_hop_zm_launch(c, prec, recon, dag, n, par, o);
@@ -274,5 +280,6 @@ int wd_hop_launch(wd_ctx* c, int prec, int recon, int dag, int n, int par, const
     o.epi = in2 ? EPI_XPAY : EPI_NONE;
     o.check_done = false;
     o.rev = 0;
+    o.storage = 0;
     return wd_hop_launch_ex(c, prec, recon, dag, n, par, o);
 }

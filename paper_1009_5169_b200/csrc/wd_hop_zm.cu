@@ -25,6 +25,7 @@
 // r fastest: conflict-free 128-bit shared-memory reads, results bit for bit those of the register kernel
 // (wd_hop.cu accumulates the directions in the same order).
 #include "wd_blas.cuh"
+#include "wd_h16.cuh"
 #include "wd_su3.cuh"
 #include "wd_tma.cuh"
 
@@ -101,7 +102,7 @@ __device__ __forceinline__ void lds_link(const float4* __restrict__ L, uint32_t 
     }
 }
 
-template <typename T, int RECON, int MU, bool FWD, bool DAG, bool FIRST = false>
+template <typename T, int RECON, int ST, int MU, bool FWD, bool DAG, bool FIRST = false>
 __device__ __forceinline__ void dir_smem(const typename Vec<T>::type* sp, uint32_t stride, uint32_t e,
                                          const typename Vec<T>::type* L, uint32_t S, uint32_t site, cx<T> (&acc)[12]) {
     if (WD_ZM_ABLATE == 1) {
@@ -113,11 +114,16 @@ __device__ __forceinline__ void dir_smem(const typename Vec<T>::type* sp, uint32
     }
     constexpr int SIGMA = (FWD ? 1 : -1) * (DAG ? -1 : 1);
     cx<T> psi[12], hs[6], chi[6], u[9];
-    lds_spinor(sp, stride, e, psi);
+    [[maybe_unused]] T scale = 1;
+    if (ST) scale = wdh::h16_load_raw(sp, stride, e, psi); else lds_spinor(sp, stride, e, psi);
     lds_link<RECON>(L, S, site, u);
     if (RECON == 12) rebuild_row3(u);
     project<MU, SIGMA>(psi, hs);
     su3_mul<!FWD>(u, hs, chi);
+    if (ST) {
+#pragma unroll
+        for (int q = 0; q < 6; ++q) { chi[q].re *= scale; chi[q].im *= scale; }
+    }
     accumulate<MU, SIGMA, FIRST>(acc, chi);
 }
 
@@ -127,7 +133,8 @@ __device__ __forceinline__ void dir_smem(const typename Vec<T>::type* sp, uint32
 // LXH, NR, RGT: Lx/2, n_rhs and rows per step as compile-time constants (0 = taken from the arguments).  With all
 // three fixed every shared-memory operand address is one per-thread base register plus an immediate; with run-time
 // strides the kernel spent 220 integer instructions per step and ~40 registers on addresses (ncu r02b).
-template <typename T, int RECON, bool DAG, int EPI, int MAXT, int LXH, int NR, int RGT>
+// ST = 1: spinor blocks (in, out, in2, in3) are in the 16-bit storage format of wd_h16.cuh (arithmetic stays fp32).
+template <typename T, int RECON, bool DAG, int EPI, int MAXT, int LXH, int NR, int RGT, int ST>
 __global__ void __launch_bounds__(MAXT, 1) hop_zm_kernel(const ZmArgs<T> A) {
     typedef typename Vec<T>::type vec;
     constexpr uint32_t NCH = Vec<T>::NCH;
@@ -139,7 +146,8 @@ __global__ void __launch_bounds__(MAXT, 1) hop_zm_kernel(const ZmArgs<T> A) {
     uint64_t* full_w = empty_u + NUNIT;                      // [3]
     uint64_t* empty_w = full_w + 3;                          // [3]
     const uint32_t RG = RGT ? (uint32_t)RGT : A.RG, rowV = Lxh * nr;
-    const uint32_t rowB = rowV * 16 * NCH;                               // bytes of one spinor row (all chunks)
+    const uint32_t rowS = ST ? wdh::h16_row_vecs(rowV) : NCH * rowV;     // 16-byte units of one spinor row (all chunks)
+    const uint32_t rowB = rowS * 16;                                     // bytes of one spinor row
     const uint32_t lrowB = Lxh * RECON * (uint32_t)sizeof(T);            // bytes of one row of one link array
     char* const base = reinterpret_cast<char*>(smem) + 128;
     char* const planes = base;
@@ -250,17 +258,17 @@ __global__ void __launch_bounds__(MAXT, 1) hop_zm_kernel(const ZmArgs<T> A) {
         const uint32_t lrowV = lrowB / 16;
         const uint32_t e0 = xh * nr + r;
         const vec* const Pl = reinterpret_cast<const vec*>(planes);
-        const vec* const Tp = reinterpret_cast<const vec*>(tp) + (size_t)j * NCH * rowV;
-        const vec* const Tm = reinterpret_cast<const vec*>(tm) + (size_t)j * NCH * rowV;
+        const vec* const Tp = reinterpret_cast<const vec*>(tp) + (size_t)j * rowS;
+        const vec* const Tm = reinterpret_cast<const vec*>(tm) + (size_t)j * rowS;
         const vec* const Hl = reinterpret_cast<const vec*>(halo);
         const vec* const Lk = reinterpret_cast<const vec*>(links) + (size_t)j * lrowV;
         const uint32_t lblk = RG * lrowV;    // 16-byte units of one link block
-        const uint32_t planeV = RG * NCH * rowV;
+        const uint32_t planeV = RG * rowS;
         // SF: the stored t = 0 slice of the output stays zero
         if (A.zero_rows) {
             const vec z4 = {};
             for (uint32_t row = blockIdx.x; row < A.zero_rows; row += gridDim.x)
-                for (uint32_t v = i; v < NCH * rowV; v += ncw * 32) A.out[(size_t)row * NCH * rowV + v] = z4;
+                for (uint32_t v = i; v < rowS; v += ncw * 32) A.out[(size_t)row * rowS + v] = z4;
         }
         uint32_t a = 0, prev = NO_STEP;
         for (uint32_t s = s_first, k = 0; s != NO_STEP; prev = s, s = next_step(s, A.chunk, A.steps), ++k) {
@@ -270,58 +278,58 @@ __global__ void __launch_bounds__(MAXT, 1) hop_zm_kernel(const ZmArgs<T> A) {
             const uint32_t s_next = next_step(s, A.chunk, A.steps);
             const bool switch_next = s_next != NO_STEP && !continues(s, s_next, A.Lz);
             const uint32_t ph = k & 1;
-            const size_t own = (size_t)(y0 + A.Ly * (z + A.Lz * t) + j) * NCH * rowV;
+            const size_t own = (size_t)(y0 + A.Ly * (z + A.Lz * t) + j) * rowS;
             cx<T> acc[12];
             if (EPI >= EPI_XPAY && active) {
 #pragma unroll
-                for (uint32_t c = 0; c < NCH; ++c) {
+                for (uint32_t c = 0; c < (ST ? 3u : NCH); ++c) {
                     asm volatile("prefetch.global.L2 [%0];" ::"l"(A.in2 + own + c * rowV + e0));
                     if (EPI == EPI_SIGMA) asm volatile("prefetch.global.L2 [%0];" ::"l"(A.in3 + own + c * rowV + e0));
                 }
             }
             const uint32_t wm = a % 3, wc = (a + 1) % 3, wp = (a + 2) % 3;
-            const vec* const Pm = Pl + (size_t)wm * planeV + (size_t)j * NCH * rowV;
-            const vec* const Pc = Pl + (size_t)wc * planeV + (size_t)j * NCH * rowV;
-            const vec* const Pp = Pl + (size_t)wp * planeV + (size_t)j * NCH * rowV;
+            const vec* const Pm = Pl + (size_t)wm * planeV + (size_t)j * rowS;
+            const vec* const Pc = Pl + (size_t)wc * planeV + (size_t)j * rowS;
+            const vec* const Pp = Pl + (size_t)wp * planeV + (size_t)j * rowS;
             // ---- t+
             mbar_wait(&full_u[U_TP], ph);
-            if (active) dir_smem<T, RECON, 3, true, DAG, true>(Tp, rowV, e0, Lk + LK_TP * lblk, Lxh, xh, acc);
+            if (active) dir_smem<T, RECON, ST, 3, true, DAG, true>(Tp, rowV, e0, Lk + LK_TP * lblk, Lxh, xh, acc);
             __syncwarp();
             if (lane == 0) mbar_arrive(&empty_u[U_TP]);
             // ---- t-
             mbar_wait(&full_u[U_TM], ph);
-            if (active) dir_smem<T, RECON, 3, false, DAG>(Tm, rowV, e0, Lk + LK_TM * lblk, Lxh, xh, acc);
+            if (active) dir_smem<T, RECON, ST, 3, false, DAG>(Tm, rowV, e0, Lk + LK_TM * lblk, Lxh, xh, acc);
             __syncwarp();
             if (lane == 0) mbar_arrive(&empty_u[U_TM]);
             // ---- z-
             mbar_wait(&full_u[U_ZM], ph);
             mbar_wait(&full_w[wm], (a / 3) & 1);
-            if (active) dir_smem<T, RECON, 2, false, DAG>(Pm, rowV, e0, Lk + LK_ZM * lblk, Lxh, xh, acc);
+            if (active) dir_smem<T, RECON, ST, 2, false, DAG>(Pm, rowV, e0, Lk + LK_ZM * lblk, Lxh, xh, acc);
             __syncwarp();
             if (lane == 0) { mbar_arrive(&empty_u[U_ZM]); mbar_arrive(&empty_w[wm]); }
             // ---- y-, y+
             mbar_wait(&full_u[U_Y], ph);
             mbar_wait(&full_w[wc], ((a + 1) / 3) & 1);
             if (active) {
-                const vec* ym = j == 0 ? Hl : Pc - NCH * rowV;
-                const vec* yp = j == RG - 1 ? Hl + NCH * rowV : Pc + NCH * rowV;
-                dir_smem<T, RECON, 1, false, DAG>(ym, rowV, e0, Lk + LK_YM * lblk, Lxh, xh, acc);
-                dir_smem<T, RECON, 1, true, DAG>(yp, rowV, e0, Lk + LK_YP * lblk, Lxh, xh, acc);
+                const vec* ym = j == 0 ? Hl : Pc - rowS;
+                const vec* yp = j == RG - 1 ? Hl + rowS : Pc + rowS;
+                dir_smem<T, RECON, ST, 1, false, DAG>(ym, rowV, e0, Lk + LK_YM * lblk, Lxh, xh, acc);
+                dir_smem<T, RECON, ST, 1, true, DAG>(yp, rowV, e0, Lk + LK_YP * lblk, Lxh, xh, acc);
             }
             __syncwarp();
             if (lane == 0) mbar_arrive(&empty_u[U_Y]);
             // ---- x-, x+, z+
             [[maybe_unused]] cx<T> qv[12];
-            if (EPI >= EPI_XPAY && active) load_spinor(A.in2 + own, rowV, e0, qv);
+            if (EPI >= EPI_XPAY && active) { if (ST) wdh::h16_load<true>(A.in2 + own, rowV, e0, qv); else load_spinor(A.in2 + own, rowV, e0, qv); }
             mbar_wait(&full_u[U_XZ], ph);
             mbar_wait(&full_w[wp], ((a + 2) / 3) & 1);
             if (active) {
                 const uint32_t bb = (y0 + j + z + t + A.par) & 1;
                 const uint32_t xp = bb ? winc(xh, Lxh) : xh;   // xh of the +x neighbour
                 const uint32_t xm = bb ? xh : wdec(xh, Lxh);   // xh of the -x neighbour
-                dir_smem<T, RECON, 0, false, DAG>(Pc, rowV, xm * nr + r, Lk + LK_XM * lblk, Lxh, xm, acc);
-                dir_smem<T, RECON, 0, true, DAG>(Pc, rowV, xp * nr + r, Lk + LK_XP * lblk, Lxh, xh, acc);
-                dir_smem<T, RECON, 2, true, DAG>(Pp, rowV, e0, Lk + LK_ZP * lblk, Lxh, xh, acc);
+                dir_smem<T, RECON, ST, 0, false, DAG>(Pc, rowV, xm * nr + r, Lk + LK_XM * lblk, Lxh, xm, acc);
+                dir_smem<T, RECON, ST, 0, true, DAG>(Pc, rowV, xp * nr + r, Lk + LK_XP * lblk, Lxh, xh, acc);
+                dir_smem<T, RECON, ST, 2, true, DAG>(Pp, rowV, e0, Lk + LK_ZP * lblk, Lxh, xh, acc);
             }
             __syncwarp();
             if (lane == 0) {
@@ -348,7 +356,7 @@ __global__ void __launch_bounds__(MAXT, 1) hop_zm_kernel(const ZmArgs<T> A) {
                     }
                 }
                 if (EPI == EPI_SIGMA) {  // <r~, v> with v = acc
-                    load_spinor(A.in3 + own, rowV, e0, qv);
+                    if (ST) wdh::h16_load<true>(A.in3 + own, rowV, e0, qv); else load_spinor(A.in3 + own, rowV, e0, qv);
                     T s0 = 0, s1 = 0;
 #pragma unroll
                     for (int q = 0; q < 12; ++q) {
@@ -357,7 +365,7 @@ __global__ void __launch_bounds__(MAXT, 1) hop_zm_kernel(const ZmArgs<T> A) {
                     }
                     dsum[0] += (double)s0; dsum[1] += (double)s1;
                 }
-                store_spinor(A.out + own, rowV, e0, acc);
+                if (ST) wdh::h16_store(A.out + own, rowV, e0, acc); else store_spinor(A.out + own, rowV, e0, acc);
             }
         }
     }
@@ -413,7 +421,7 @@ struct Shape {
 };
 
 // largest row group (a divisor of Ly) whose CTA fits the thread budget and whose buffers fit shared memory
-template <typename T, int RECON>
+template <typename T, int RECON, int ST>
 bool pick_shape(const wd_ctx* c, int n, int max_threads, Shape* sh) {
     const uint32_t Lxh = c->L[0] / 2, Ly = c->L[1];
     const uint32_t cap = c->opt[WD_OPT_HOP_ROWS] > 0 ? (uint32_t)c->opt[WD_OPT_HOP_ROWS] : Ly;
@@ -422,7 +430,8 @@ bool pick_shape(const wd_ctx* c, int n, int max_threads, Shape* sh) {
         const uint32_t S = RG * Lxh;
         const uint32_t cthreads = ((S * n + 31) / 32) * 32;
         if ((int)cthreads + 128 > max_threads) continue;
-        const size_t rowB = (size_t)Lxh * n * 16 * Vec<T>::NCH, lrowB = (size_t)Lxh * RECON * sizeof(T);
+        const size_t rowB = ST ? (size_t)wdh::h16_row_vecs(Lxh * n) * 16 : (size_t)Lxh * n * 16 * Vec<T>::NCH;
+        const size_t lrowB = (size_t)Lxh * RECON * sizeof(T);
         const size_t smem = 128 + (5 * (size_t)RG + 2) * rowB + 8 * (size_t)RG * lrowB;
         if (smem > kSmemMax) continue;
         // the epilogue's reduction scratch (3 sums per consumer thread + totals) reuses the staging area
@@ -433,17 +442,17 @@ bool pick_shape(const wd_ctx* c, int n, int max_threads, Shape* sh) {
     return false;
 }
 
-template <typename T, int RECON, bool DAG, int EPI, int MAXT, int LXH, int NR, int RGT>
+template <typename T, int RECON, bool DAG, int EPI, int MAXT, int LXH, int NR, int RGT, int ST>
 int launch_one(wd_ctx* c, const ZmArgs<T>& A, const Shape& sh, unsigned G) {
-    auto kern = hop_zm_kernel<T, RECON, DAG, EPI, MAXT, LXH, NR, RGT>;
+    auto kern = hop_zm_kernel<T, RECON, DAG, EPI, MAXT, LXH, NR, RGT, ST>;
     WD_CUDA_CHECK(c, wd_ensure_smem_attr(c, (const void*)kern, (int)kSmemMax));
     kern<<<G, sh.threads, sh.smem, c->stream>>>(A);
     return WD_OK;
 }
 
-template <typename T, int RECON, int MAXT, int LXH, int NR, int RGT>
+template <typename T, int RECON, int MAXT, int LXH, int NR, int RGT, int ST>
 int launch_epi(wd_ctx* c, const ZmArgs<T>& A, const Shape& sh, unsigned G, int dag, int epi) {
-#define WD_ZM_CASE(D, E) return launch_one<T, RECON, D, E, MAXT, LXH, NR, RGT>(c, A, sh, G)
+#define WD_ZM_CASE(D, E) return launch_one<T, RECON, D, E, MAXT, LXH, NR, RGT, ST>(c, A, sh, G)
     if (dag) {
         if (epi == EPI_NONE) WD_ZM_CASE(true, EPI_NONE);
         else if (epi == EPI_XPAY) WD_ZM_CASE(true, EPI_XPAY);
@@ -458,10 +467,11 @@ int launch_epi(wd_ctx* c, const ZmArgs<T>& A, const Shape& sh, unsigned G, int d
 #undef WD_ZM_CASE
 }
 
-template <typename T, int RECON, int MAXT>
+template <typename T, int RECON, int MAXT, int ST>
 int launch_zm(wd_ctx* c, int dag, int n, int par, const wd_hop_ops& o, const T* U) {
     Shape sh;
-    if (!pick_shape<T, RECON>(c, n, MAXT, &sh)) return 1;
+    if (ST && ((c->L[0] / 2) * n) % 4 != 0) return 1;   // the H16 scale chunk must keep rows 16-byte aligned
+    if (!pick_shape<T, RECON, ST>(c, n, MAXT, &sh)) return 1;
     ZmArgs<T> A;
     A.in = (const typename Vec<T>::type*)o.in;
     A.out = (typename Vec<T>::type*)o.out;
@@ -498,10 +508,10 @@ int launch_zm(wd_ctx* c, int dag, int n, int par, const wd_hop_ops& o, const T* 
     const unsigned G = nch < (uint32_t)c->n_sm ? nch : (unsigned)c->n_sm;
     // shapes with a compile-time geometry (the paper-shaped lattices of BASELINE.json at their n_rhs); any other
     // shape runs the same kernel with run-time strides
-#define WD_ZM_GEOM(LXH, NR, RGT) if (A.Lxh == LXH && A.n == NR && A.RG == RGT) return launch_epi<T, RECON, MAXT, LXH, NR, RGT>(c, A, sh, G, dag, o.epi)
+#define WD_ZM_GEOM(LXH, NR, RGT) if (A.Lxh == LXH && A.n == NR && A.RG == RGT) return launch_epi<T, RECON, MAXT, LXH, NR, RGT, ST>(c, A, sh, G, dag, o.epi)
     WD_ZM_GEOM(12, 5, 6);
 #undef WD_ZM_GEOM
-    return launch_epi<T, RECON, MAXT, 0, 0, 0>(c, A, sh, G, dag, o.epi);
+    return launch_epi<T, RECON, MAXT, 0, 0, 0, ST>(c, A, sh, G, dag, o.epi);
 }
 
 }  // namespace
@@ -511,6 +521,10 @@ int launch_zm(wd_ctx* c, int dag, int n, int par, const wd_hop_ops& o, const T* 
 int wd_hop_zm_launch(wd_ctx* c, int prec, int recon, int dag, int n, int par, const wd_hop_ops& o) {
     if (c->order != WD_ORDER_LINEAR || c->RB != (uint32_t)(c->L[0] / 2)) return 1;  // needs the row-major layout
     if (prec != WD_F32) return 1;
-    if (recon == WD_LINK18) return launch_zm<float, 18, 512>(c, dag, n, par, o, c->d_U32[0]);
-    return launch_zm<float, 12, 512>(c, dag, n, par, o, c->d_U32[1]);
+    if (o.storage == 1) {
+        if (recon == WD_LINK18) return launch_zm<float, 18, 512, 1>(c, dag, n, par, o, c->d_U32[0]);
+        return launch_zm<float, 12, 512, 1>(c, dag, n, par, o, c->d_U32[1]);
+    }
+    if (recon == WD_LINK18) return launch_zm<float, 18, 512, 0>(c, dag, n, par, o, c->d_U32[0]);
+    return launch_zm<float, 12, 512, 0>(c, dag, n, par, o, c->d_U32[1]);
 }

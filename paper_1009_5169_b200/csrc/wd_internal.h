@@ -153,6 +153,7 @@ struct wd_hop_ops {
     int epi;
     bool check_done;
     int rev;  // 1: sweep the sites from the top (L2 reuse between consecutive kernels)
+    int storage = 0;  // 1: spinor blocks in the 16-bit H16 format (wd_h16.cuh); z-march kernel only
 };
 int wd_hop_launch_ex(wd_ctx* c, int prec, int recon, int dag, int n, int par, const wd_hop_ops& o);
 // wd_hop_tma.cu: the shared-memory-staged (bulk copy + mbarrier) form; > 0 = not applicable, use the plain kernel
@@ -171,6 +172,12 @@ int wd_layout_unpack(wd_ctx* c, int prec, int n, const void* native, double* can
 size_t wd_solver_scratch_bytes(const wd_ctx* c);
 int wd_solve_impl(wd_ctx* c, int dag, int n, const double* Phi, double* X, double tol, int max_outer,
                   int max_inner, double inner_tol, int recon, wd_solve_info* info);
+int wd_solve_dc(wd_ctx* c, int dag, int n, const double* Phi, double* X, double tol, int max_outer,
+                int max_inner, double inner_tol, int recon, wd_solve_info* info);
+// wd_solve_h16.cu
+bool wd_solve_h16_applies(const wd_ctx* c, int n);
+int wd_solve_h16(wd_ctx* c, int dag, int n, const double* Phi, double* X, double tol, int max_updates, int max_iters,
+                 double delta, int recon, wd_solve_info* info);
 
 // wd_force.cu
 int wd_force_impl(wd_ctx* c, int n, const double* X, const double* Y, double* F);

@@ -208,8 +208,17 @@ size_t wd_solver_scratch_bytes(const wd_ctx* c) {
     return b;
 }
 
+// Solver dispatch (WD_OPT_SOLVER).  inner_tol = 0 picks each solver's default.
 int wd_solve_impl(wd_ctx* c, int dag, int n, const double* Phi, double* X, double tol, int max_outer,
                   int max_inner, double inner_tol, int recon, wd_solve_info* info) {
+    const int solver = c->opt[WD_OPT_SOLVER];
+    if (solver == WD_SOLVER_RELIABLE_H16 && wd_solve_h16_applies(c, n))
+        return wd_solve_h16(c, dag, n, Phi, X, tol, max_outer, max_inner, inner_tol > 0.0 ? inner_tol : 0.01, recon, info);
+    return wd_solve_dc(c, dag, n, Phi, X, tol, max_outer, max_inner, inner_tol > 0.0 ? inner_tol : 1e-5, recon, info);
+}
+
+int wd_solve_dc(wd_ctx* c, int dag, int n, const double* Phi, double* X, double tol, int max_outer,
+                int max_inner, double inner_tol, int recon, wd_solve_info* info) {
     const auto t_begin = std::chrono::steady_clock::now();
     cudaStream_t st = c->stream;
     const long Vh = c->Vh;

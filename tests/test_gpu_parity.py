@@ -588,3 +588,57 @@ def test_md_force_host_gauge_matches_device_path():
     Y, _ = ctx.solve_block(pkg.OP_DDAG, X, n)
     assert np.array_equal(Fh.numpy(), ctx.force(X, Y, n).cpu().numpy())
     ctx.close()
+
+
+# ---- f3: 16-bit storage + reliable updates -------------------------------------------------------
+@pytest.mark.parametrize("case", [(1, 5, wi.BC_SF), (1, 3, wi.BC_PERIODIC), (3, 5, wi.BC_SF)])
+def test_reliable_update_h16_solver_matches_oracle(case):
+    """WD_OPT_SOLVER = WD_SOLVER_RELIABLE_H16: vectors stored in 16 bits, fp32 arithmetic, fp64 reliable updates.  Same
+    tolerances as the default solver: true residual <= 1e-12 (recomputed with the oracle's operator), X, Y within 1e-9 of
+    the oracle, F within 1e-9; iteration counts reported beside the default solver's."""
+    pkg = _wd()
+    idx, n, bc = case
+    cfg = dict(wi.CONFIGS[idx])
+    dims, kappa = cfg["dims"], cfg["kappa"]
+    U = wi.gauge_field(dims, cfg["eps"], cfg["seed"], bc)
+    Phi = wi.spinor_field(dims, n, cfg["seed"], bc)
+    ctx = make_ctx(dims, kappa, bc, n, U)
+    P = ctx.pack(dev(Phi))
+    X0, i0 = ctx.solve_block(pkg.OP_D, P, n, tol=1e-12)
+    ctx.set_option(pkg.OPT_SOLVER, pkg.SOLVER_RELIABLE_H16)
+    X, ix = ctx.solve_block(pkg.OP_D, P, n, tol=1e-12)
+    Y, iy = ctx.solve_block(pkg.OP_DDAG, X, n, tol=1e-12)
+    assert ix["converged"] and iy["converged"] and max(ix["relres"]) <= 1e-12 and max(iy["relres"]) <= 1e-12
+    assert ix["outer_steps"] >= 2, "the 16-bit solver must have taken reliable updates (else the default solver ran)"
+    assert ix["inner_iters_total"] <= 1.5 * i0["inner_iters_total"] + 5
+    Xc, Yc = ctx.unpack(X, n).cpu().numpy(), ctx.unpack(Y, n).cpu().numpy()
+    assert rel_per_rhs(orc.apply(dims, kappa, bc, 0, U, Xc), Phi).max() < 2e-12
+    assert rel_per_rhs(orc.apply(dims, kappa, bc, 1, U, Yc), Xc).max() < 2e-12
+    assert rel_per_rhs(Xc, ctx.unpack(X0, n).cpu().numpy()).max() < 1e-10
+    if idx == 1:
+        Xr, rr, _, rc = orc.solve(dims, kappa, bc, 0, U, Phi, tol=1e-14)
+        assert rc == 0 and rr.max() < 1e-13
+        Yr, rr, _, rc = orc.solve(dims, kappa, bc, 1, U, Xr, tol=1e-14)
+        assert rc == 0 and rr.max() < 1e-13
+        assert rel_per_rhs(Xc, Xr).max() < 1e-9 and rel_per_rhs(Yc, Yr).max() < 1e-9
+        force_close(ctx.force(X, Y, n).cpu().numpy(), orc.force(dims, kappa, bc, U, Xr, Yr), 1e-9)
+    ctx.close()
+
+
+@pytest.mark.slow
+def test_reliable_update_h16_solver_full_size():
+    """The same at configs[4] (24^4, n_rhs = 5): all columns' true residuals, column 0 against the oracle's solve."""
+    pkg = _wd()
+    n = 5
+    cfg, U, Phi12, Xr, Yr = oracle_24(1)
+    Phi = np.ascontiguousarray(Phi12[:n])
+    dims, kappa, bc = cfg["dims"], cfg["kappa"], cfg["bc"]
+    ctx = make_ctx(dims, kappa, bc, n, U)
+    ctx.set_option(pkg.OPT_SOLVER, pkg.SOLVER_RELIABLE_H16)
+    P = ctx.pack(dev(Phi))
+    X, ix = ctx.solve_block(pkg.OP_D, P, n, tol=1e-12)
+    assert ix["converged"] and ix["outer_steps"] >= 2
+    Xc = ctx.unpack(X, n).cpu().numpy()
+    assert rel_per_rhs(orc.apply(dims, kappa, bc, 0, U, Xc), Phi).max() < 2e-12
+    assert rel_per_rhs(Xc[:1], Xr).max() < 1e-9
+    ctx.close()
