@@ -115,12 +115,19 @@ int wd_site_order(wd_ctx* ctx, int order, const int tile[4]);
  *       reliable-update threshold delta (0 = default 0.01), max_outer bounds the number of updates and max_inner the
  *       total number of iterations.  Needs the z-march hop kernel (linear site order, Lx/2 even, n_rhs >= 3,
  *       Lx/2 * n_rhs a multiple of 4); elsewhere the default solver runs.
+ *       WD_SOLVER_GL_FLEX: the paper's case D1 (Table 1): fp64 Global BiCGStab (one alpha, beta, omega for the
+ *       whole block, Frobenius inner products) in flexible form, preconditioned by the fp32 BiCGStab per column;
+ *       max_outer bounds its iterations (two preconditioner calls each), info.outer_steps counts preconditioner calls.
+ *       WD_SOLVER_GL_F64: case B, the same without preconditioner (all fp64; info.inner_iters_total = its iterations).
+ *       WD_SOLVER_BL_F64: case C, fp64 Block BiCGStab (ref. [7] of the paper): n_rhs x n_rhs coefficient matrices from the
+ *       Gram matrices of the block vectors, one Krylov space shared by the columns; max_inner bounds its iterations.
  * Errors: WD_EINVAL (null, unknown key, value out of range). */
 enum { WD_OPT_HOP32_SITES = 0, WD_OPT_HOP64_SITES = 1, WD_OPT_HOP32_REGS = 2, WD_OPT_HOP64_REGS = 3,
        WD_OPT_POLL_EVERY = 4, WD_OPT_HOP_IMPL = 5, WD_OPT_ALTERNATE_SWEEP = 6, WD_OPT_HOP_ROWS = 7, WD_OPT_SOLVER = 8,
        WD_OPT_N = 9 };
 /* values of WD_OPT_SOLVER */
-enum { WD_SOLVER_DC_F32 = 0, WD_SOLVER_RELIABLE_H16 = 1, WD_SOLVER_N = 2 };
+enum { WD_SOLVER_DC_F32 = 0, WD_SOLVER_RELIABLE_H16 = 1, WD_SOLVER_GL_FLEX = 2, WD_SOLVER_GL_F64 = 3, WD_SOLVER_BL_F64 = 4,
+       WD_SOLVER_N = 5 };
 int wd_set_option(wd_ctx* ctx, int key, int value);
 int wd_get_option(const wd_ctx* ctx, int key, int* value_host);
 

@@ -25,15 +25,20 @@ enum {
     S_ACTION,     // |x_i|^2 of wd_action (pseudo-fermion action per column)
     S_RHO_PREV_RE, S_RHO_PREV_IM,  // rho of the previous iteration (reliable updates: beta is recomputed after r is replaced)
     S_RMAX2,      // largest recursive |r_i|^2 since the last reliable update
+    S_T0, S_T1, S_T2,  // per-column totals of the global (Frobenius) inner products of the blocked outer solvers
+    S_GL_CONV,    // column met the tolerance (blocked outer solvers)
     S_ROWS
 };
 // global (not per-column) slots after the table
-enum { G_DONE = S_ROWS * WD_MAX_RHS, G_ITERS, G_OUT_DONE, G_TOL2, G_INTOL2, G_DELTA2, G_UPDATES, G_COUNT };
+enum { G_DONE = S_ROWS * WD_MAX_RHS, G_ITERS, G_OUT_DONE, G_TOL2, G_INTOL2, G_DELTA2, G_UPDATES,
+       G_GL_RHO_RE, G_GL_RHO_IM, G_GL_ALPHA_RE, G_GL_ALPHA_IM, G_GL_OMEGA_RE, G_GL_OMEGA_IM, G_GL_BETA_RE, G_GL_BETA_IM, G_GL_BREAK,
+       G_COUNT };
 
 __device__ __forceinline__ double& SC(double* scal, int row, int r) { return scal[row * WD_MAX_RHS + r]; }
 
 enum Kind { K_SIGMA, K_OMEGA, K_RHO, K_PHI2, K_OUT_R2, K_INIT_RHO, K_ACTION,
-            K_RHO_REL, K_OUT_R2_REL, K_REPLACE };   // reliable-update solver (wd_solve_h16.cu)
+            K_RHO_REL, K_OUT_R2_REL, K_REPLACE,     // reliable-update solver (wd_solve_h16.cu)
+            K_GL_INIT, K_GL_SIGMA, K_GL_S, K_GL_OMEGA, K_GL_RHO, K_PREC_PREP };   // blocked outer solvers (wd_solve_gl.cu)
 
 struct RedBuf {
     double* scal;
@@ -150,6 +155,22 @@ __device__ void finalize_column(double* scal, int r, const double* tot) {
             // recursive target: half of what the tolerance needs, in units of the scale
             SC(scal, S_THR2, r) = tot[0] > 0.0 ? 0.25 * tol2 * phi2 / tot[0] : 0.0;
         }
+    } else if (KIND == K_GL_INIT || KIND == K_GL_S || KIND == K_GL_RHO) {
+        // per-column part of a global inner product; the residual norm of the column is tot[0] (INIT, S) or tot[2] (RHO)
+        const double r2 = KIND == K_GL_RHO ? tot[2] : tot[0];
+        SC(scal, S_T0, r) = tot[0];
+        if (KIND == K_GL_RHO) { SC(scal, S_T1, r) = tot[1]; SC(scal, S_T2, r) = tot[2]; }
+        SC(scal, S_OUT_R2, r) = r2;
+        SC(scal, S_GL_CONV, r) = r2 <= scal[G_TOL2] * SC(scal, S_PHI2, r) ? 1.0 : 0.0;
+    } else if (KIND == K_GL_SIGMA) {
+        SC(scal, S_T0, r) = tot[0]; SC(scal, S_T1, r) = tot[1];
+    } else if (KIND == K_GL_OMEGA) {
+        SC(scal, S_T0, r) = tot[0]; SC(scal, S_T1, r) = tot[1]; SC(scal, S_T2, r) = tot[2];
+    } else if (KIND == K_PREC_PREP) {  // tot = |in_i|^2: the inner solver works on in_i / |in_i|
+        SC(scal, S_SCALE, r) = sqrt(tot[0]);
+        SC(scal, S_FLAG, r) = tot[0] > 0.0 ? 0.0 : 1.0;
+        SC(scal, S_THR2, r) = scal[G_INTOL2];
+        SC(scal, S_OUT_CONV, r) = 0.0;
     } else if (KIND == K_PHI2) {
         SC(scal, S_PHI2, r) = tot[0];
     } else if (KIND == K_ACTION) {
@@ -200,6 +221,42 @@ __device__ void finalize_global(double* scal, int n) {
         bool all = true;
         for (int r = 0; r < n; ++r) all = all && (SC(scal, S_FLAG, r) != 0.0);
         scal[G_DONE] = all ? 1.0 : 0.0;
+    } else if (KIND == K_GL_INIT || KIND == K_GL_S || KIND == K_GL_RHO || KIND == K_GL_SIGMA || KIND == K_GL_OMEGA) {
+        // Frobenius inner products = sums over the columns (PAPER.md:72 Gl-BiCGStab, ref. [6])
+        double t0 = 0.0, t1 = 0.0, t2 = 0.0;
+        bool all = true;
+        for (int r = 0; r < n; ++r) {
+            t0 += SC(scal, S_T0, r); t1 += SC(scal, S_T1, r); t2 += SC(scal, S_T2, r);
+            all = all && (SC(scal, S_GL_CONV, r) != 0.0);
+        }
+        if (KIND == K_GL_INIT) {          // rho = <R~, R>_F with R~ = R
+            scal[G_GL_RHO_RE] = t0; scal[G_GL_RHO_IM] = 0.0;
+            scal[G_GL_ALPHA_RE] = 1.0; scal[G_GL_ALPHA_IM] = 0.0; scal[G_GL_OMEGA_RE] = 1.0; scal[G_GL_OMEGA_IM] = 0.0;
+            scal[G_GL_BETA_RE] = 0.0; scal[G_GL_BETA_IM] = 0.0; scal[G_GL_BREAK] = 0.0;
+            scal[G_OUT_DONE] = all ? 1.0 : 0.0;
+        } else if (KIND == K_GL_SIGMA) {  // alpha = rho / <R~, V>_F
+            const cd sigma = {t0, t1};
+            cd alpha = {0.0, 0.0};
+            if (sigma.re == 0.0 && sigma.im == 0.0) scal[G_GL_BREAK] = 1.0;
+            else alpha = cdiv({scal[G_GL_RHO_RE], scal[G_GL_RHO_IM]}, sigma);
+            scal[G_GL_ALPHA_RE] = alpha.re; scal[G_GL_ALPHA_IM] = alpha.im;
+        } else if (KIND == K_GL_S) {
+            scal[G_OUT_DONE] = all ? 1.0 : 0.0;
+        } else if (KIND == K_GL_OMEGA) {  // omega = <T, S>_F / <T, T>_F
+            cd omega = {0.0, 0.0};
+            if (t2 > 0.0) omega = {t0 / t2, t1 / t2};
+            else scal[G_GL_BREAK] = 1.0;
+            scal[G_GL_OMEGA_RE] = omega.re; scal[G_GL_OMEGA_IM] = omega.im;
+        } else {                          // K_GL_RHO: rho' = <R~, R>_F, beta = (rho'/rho)(alpha/omega)
+            const cd rho1 = {t0, t1}, rho = {scal[G_GL_RHO_RE], scal[G_GL_RHO_IM]};
+            const cd alpha = {scal[G_GL_ALPHA_RE], scal[G_GL_ALPHA_IM]}, omega = {scal[G_GL_OMEGA_RE], scal[G_GL_OMEGA_IM]};
+            cd beta = {0.0, 0.0};
+            if ((rho.re == 0.0 && rho.im == 0.0) || (omega.re == 0.0 && omega.im == 0.0)) scal[G_GL_BREAK] = 1.0;
+            else beta = cmul(cdiv(rho1, rho), cdiv(alpha, omega));
+            scal[G_GL_RHO_RE] = rho1.re; scal[G_GL_RHO_IM] = rho1.im;
+            scal[G_GL_BETA_RE] = beta.re; scal[G_GL_BETA_IM] = beta.im;
+            scal[G_OUT_DONE] = all ? 1.0 : 0.0;
+        }
     }
 }
 

@@ -174,6 +174,11 @@ int wd_solve_impl(wd_ctx* c, int dag, int n, const double* Phi, double* X, doubl
                   int max_inner, double inner_tol, int recon, wd_solve_info* info);
 int wd_solve_dc(wd_ctx* c, int dag, int n, const double* Phi, double* X, double tol, int max_outer,
                 int max_inner, double inner_tol, int recon, wd_solve_info* info);
+int wd_inner_solve_f32(wd_ctx* c, int dag, int n, int recon, int max_inner, const double2* R64, double2* Xacc);
+// wd_solve_gl.cu
+int wd_solve_gl(wd_ctx* c, int flex, int dag, int n, const double* Phi, double* X, double tol, int max_outer, int max_inner,
+                double inner_tol, int recon, wd_solve_info* info);
+int wd_solve_bl(wd_ctx* c, int dag, int n, const double* Phi, double* X, double tol, int max_iters, wd_solve_info* info);
 // wd_solve_h16.cu
 bool wd_solve_h16_applies(const wd_ctx* c, int n);
 int wd_solve_h16(wd_ctx* c, int dag, int n, const double* Phi, double* X, double tol, int max_updates, int max_iters,

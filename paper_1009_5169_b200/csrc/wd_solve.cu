@@ -203,15 +203,91 @@ size_t wd_solver_scratch_bytes(const wd_ctx* c) {
     size_t b = 0;
     b += 3 * wd_align_up(wd_half_bytes(c, WD_F64, n));      // phihat, tmp_o, R/W
     b += 7 * wd_align_up(wd_half_bytes(c, WD_F32, n));      // x, r, p, v, t, rt, tmp_o
+    b += 8 * wd_align_up(wd_half_bytes(c, WD_F64, n));      // blocked outer solvers (wd_solve_gl.cu): Rt, P, V, S, T, Ph, Sh, Pnew
     b += 4 * wd_align_up(2 * wd_half_bytes(c, WD_F64, n));  // host path: canonical Phi, native Phi, X, Y
     b += wd_align_up(sizeof(double) * 4 * c->V * 18);       // host path: F
     return b;
+}
+
+// The fp32 inner solver on its own: E_i = BiCGStab_fp32(R_i / scale_i) for the columns whose S_FLAG is 0, to a recursive
+// residual of S_THR2 (relative to the unit-norm right-hand side), then Xacc_i += scale_i E_i.  S_SCALE, S_FLAG, S_THR2 and
+// S_OUT_CONV are set on the device by the caller's preceding reduction.  Uses the seven fp32 slots of the solver scratch.
+int wd_inner_solve_f32(wd_ctx* c, int dag, int n, int recon, int max_inner, const double2* R64, double2* Xacc) {
+    cudaStream_t st = c->stream;
+    const long Vh = c->Vh;
+    const size_t sb64 = wd_align_up(wd_half_bytes(c, WD_F64, c->max_rhs)), sb32 = wd_align_up(wd_half_bytes(c, WD_F32, c->max_rhs));
+    char* w = c->d_solver + 3 * sb64;
+    float4* x32 = (float4*)w;   w += sb32;
+    float4* r32 = (float4*)w;   w += sb32;
+    float4* p32 = (float4*)w;   w += sb32;
+    float4* v32 = (float4*)w;   w += sb32;
+    float4* t32 = (float4*)w;   w += sb32;
+    float4* rt32 = (float4*)w;  w += sb32;
+    float4* tmp32 = (float4*)w; w += sb32;
+    const double kap = c->kappa;
+    RedBuf rb{c->d_scal, c->d_partials, c->d_ticket};
+    const long nv32 = 6 * Vh * n;
+    const Launch L32 = blas_cfg(c, nv32, n);
+    double* hp = c->h_pinned;
+    int rc;
+    {
+        { wd_prof_scope pr__(c, WD_PROF_BLAS); demote_kernel<<<L32.G, L32.B, 0, st>>>(Vh, (long)c->RB, n, rb, R64, r32, rt32, x32, p32, v32); }
+        WD_LAUNCH_CHECK(c);
+        // One iteration = 3 BLAS1 kernels + 4 hops; sigma and omega are reduced inside the even-parity hops.
+        // Kernels turn into no-ops once the device-side done flag is set, so iterations are enqueued
+        // poll_every at a time and the host only looks at the flag in between.
+        const int poll_every = c->opt[WD_OPT_POLL_EVERY];
+        // Consecutive kernels sweep the vectors in opposite directions: what one kernel wrote last (and the
+        // 126 MB L2 still holds) is what the next one reads first.
+        int sweep_dir = 0;
+        auto sweep = [&]() { sweep_dir ^= c->opt[WD_OPT_ALTERNATE_SWEEP] ? 1 : 0; return sweep_dir; };
+        wd_hop_ops o;
+        o.check_done = true;
+        for (int it = 1; it <= max_inner; ++it) {
+            { wd_prof_scope pr__(c, WD_PROF_BLAS); p_update_kernel<float><<<L32.G, L32.B, 0, st>>>(nv32, n, sweep(), c->d_scal, r32, p32, v32); }
+            WD_LAUNCH_CHECK(c);
+            // v = Ahat p, sigma = <rt, v> -> alpha
+            o.in = p32; o.out = tmp32; o.in2 = nullptr; o.in3 = nullptr; o.a = 0.0; o.b = 1.0; o.epi = 0;
+            o.rev = sweep();
+            rc = wd_hop_launch_ex(c, WD_F32, recon, dag, n, 1, o);
+            if (rc) return rc;
+            o.in = tmp32; o.out = v32; o.in2 = p32; o.in3 = rt32; o.a = 1.0; o.b = -kap * kap; o.epi = 2;
+            o.rev = sweep();
+            rc = wd_hop_launch_ex(c, WD_F32, recon, dag, n, 0, o);
+            if (rc) return rc;
+            { wd_prof_scope pr__(c, WD_PROF_BLAS); s_update_kernel<float><<<L32.G, L32.B, 0, st>>>(nv32, n, sweep(), c->d_scal, r32, v32); }
+            WD_LAUNCH_CHECK(c);
+            // t = Ahat s, <t, s>, <t, t> -> omega
+            o.in = r32; o.out = tmp32; o.in2 = nullptr; o.in3 = nullptr; o.a = 0.0; o.b = 1.0; o.epi = 0;
+            o.rev = sweep();
+            rc = wd_hop_launch_ex(c, WD_F32, recon, dag, n, 1, o);
+            if (rc) return rc;
+            o.in = tmp32; o.out = t32; o.in2 = r32; o.in3 = nullptr; o.a = 1.0; o.b = -kap * kap; o.epi = 3;
+            o.rev = sweep();
+            rc = wd_hop_launch_ex(c, WD_F32, recon, dag, n, 0, o);
+            if (rc) return rc;
+            { wd_prof_scope pr__(c, WD_PROF_BLAS); xr_update_kernel<float><<<L32.G, L32.B, 0, st>>>(nv32, n, sweep(), rb, x32, p32, r32, t32, rt32); }
+            WD_LAUNCH_CHECK(c);
+            if (it % poll_every == 0 || it == max_inner) {
+                WD_CUDA_CHECK(c, cudaMemcpyAsync(hp + G_COUNT, c->d_scal + G_DONE, sizeof(double), cudaMemcpyDeviceToHost, st));
+                WD_CUDA_CHECK(c, cudaStreamSynchronize(st));
+                if (hp[G_COUNT] != 0.0) break;
+            }
+        }
+        { wd_prof_scope pr__(c, WD_PROF_BLAS); promote_kernel<<<L32.G, L32.B, 0, st>>>(Vh, (long)c->RB, n, c->d_scal, x32, Xacc); }
+        WD_LAUNCH_CHECK(c);
+    }
+    return WD_OK;
 }
 
 // Solver dispatch (WD_OPT_SOLVER).  inner_tol = 0 picks each solver's default.
 int wd_solve_impl(wd_ctx* c, int dag, int n, const double* Phi, double* X, double tol, int max_outer,
                   int max_inner, double inner_tol, int recon, wd_solve_info* info) {
     const int solver = c->opt[WD_OPT_SOLVER];
+    if (solver == WD_SOLVER_GL_FLEX || solver == WD_SOLVER_GL_F64)
+        return wd_solve_gl(c, solver == WD_SOLVER_GL_FLEX, dag, n, Phi, X, tol, max_outer, max_inner, inner_tol > 0.0 ? inner_tol : 1e-5,
+                           recon, info);
+    if (solver == WD_SOLVER_BL_F64) return wd_solve_bl(c, dag, n, Phi, X, tol, max_inner, info);
     if (solver == WD_SOLVER_RELIABLE_H16 && wd_solve_h16_applies(c, n))
         return wd_solve_h16(c, dag, n, Phi, X, tol, max_outer, max_inner, inner_tol > 0.0 ? inner_tol : 0.01, recon, info);
     return wd_solve_dc(c, dag, n, Phi, X, tol, max_outer, max_inner, inner_tol > 0.0 ? inner_tol : 1e-5, recon, info);
@@ -277,52 +353,9 @@ int wd_solve_dc(wd_ctx* c, int dag, int n, const double* Phi, double* X, double 
         if (outer >= max_outer) break;
         ++outer;
 
-        // inner fp32 BiCGStab on the normalised residual
-        { wd_prof_scope pr__(c, WD_PROF_BLAS); demote_kernel<<<L32.G, L32.B, 0, st>>>(Vh, (long)c->RB, n, rb, R64, r32, rt32, x32, p32, v32); }
-        WD_LAUNCH_CHECK(c);
-        // One iteration = 3 BLAS1 kernels + 4 hops; sigma and omega are reduced inside the even-parity hops.
-        // Kernels turn into no-ops once the device-side done flag is set, so iterations are enqueued
-        // poll_every at a time and the host only looks at the flag in between.
-        const int poll_every = c->opt[WD_OPT_POLL_EVERY];
-        // Consecutive kernels sweep the vectors in opposite directions: what one kernel wrote last (and the
-        // 126 MB L2 still holds) is what the next one reads first.
-        int sweep_dir = 0;
-        auto sweep = [&]() { sweep_dir ^= c->opt[WD_OPT_ALTERNATE_SWEEP] ? 1 : 0; return sweep_dir; };
-        wd_hop_ops o;
-        o.check_done = true;
-        for (int it = 1; it <= max_inner; ++it) {
-            { wd_prof_scope pr__(c, WD_PROF_BLAS); p_update_kernel<float><<<L32.G, L32.B, 0, st>>>(nv32, n, sweep(), c->d_scal, r32, p32, v32); }
-            WD_LAUNCH_CHECK(c);
-            // v = Ahat p, sigma = <rt, v> -> alpha
-            o.in = p32; o.out = tmp32; o.in2 = nullptr; o.in3 = nullptr; o.a = 0.0; o.b = 1.0; o.epi = 0;
-            o.rev = sweep();
-            rc = wd_hop_launch_ex(c, WD_F32, recon, dag, n, 1, o);
-            if (rc) return rc;
-            o.in = tmp32; o.out = v32; o.in2 = p32; o.in3 = rt32; o.a = 1.0; o.b = -kap * kap; o.epi = 2;
-            o.rev = sweep();
-            rc = wd_hop_launch_ex(c, WD_F32, recon, dag, n, 0, o);
-            if (rc) return rc;
-            { wd_prof_scope pr__(c, WD_PROF_BLAS); s_update_kernel<float><<<L32.G, L32.B, 0, st>>>(nv32, n, sweep(), c->d_scal, r32, v32); }
-            WD_LAUNCH_CHECK(c);
-            // t = Ahat s, <t, s>, <t, t> -> omega
-            o.in = r32; o.out = tmp32; o.in2 = nullptr; o.in3 = nullptr; o.a = 0.0; o.b = 1.0; o.epi = 0;
-            o.rev = sweep();
-            rc = wd_hop_launch_ex(c, WD_F32, recon, dag, n, 1, o);
-            if (rc) return rc;
-            o.in = tmp32; o.out = t32; o.in2 = r32; o.in3 = nullptr; o.a = 1.0; o.b = -kap * kap; o.epi = 3;
-            o.rev = sweep();
-            rc = wd_hop_launch_ex(c, WD_F32, recon, dag, n, 0, o);
-            if (rc) return rc;
-            { wd_prof_scope pr__(c, WD_PROF_BLAS); xr_update_kernel<float><<<L32.G, L32.B, 0, st>>>(nv32, n, sweep(), rb, x32, p32, r32, t32, rt32); }
-            WD_LAUNCH_CHECK(c);
-            if (it % poll_every == 0 || it == max_inner) {
-                WD_CUDA_CHECK(c, cudaMemcpyAsync(hp + G_COUNT, c->d_scal + G_DONE, sizeof(double), cudaMemcpyDeviceToHost, st));
-                WD_CUDA_CHECK(c, cudaStreamSynchronize(st));
-                if (hp[G_COUNT] != 0.0) break;
-            }
-        }
-        { wd_prof_scope pr__(c, WD_PROF_BLAS); promote_kernel<<<L32.G, L32.B, 0, st>>>(Vh, (long)c->RB, n, c->d_scal, x32, (double2*)XE); }
-        WD_LAUNCH_CHECK(c);
+        // inner fp32 BiCGStab on the normalised residual, X_e,i += |R_i| E_i
+        rc = wd_inner_solve_f32(c, dag, n, recon, max_inner, R64, (double2*)XE);
+        if (rc) return rc;
     }
 
     // X_o = Phi_o + kappa H_oe X_e

@@ -642,3 +642,43 @@ def test_reliable_update_h16_solver_full_size():
     assert rel_per_rhs(orc.apply(dims, kappa, bc, 0, U, Xc), Phi).max() < 2e-12
     assert rel_per_rhs(Xc[:1], Xr).max() < 1e-9
     ctx.close()
+
+
+# ---- f2: the paper's blocked Krylov solvers as outer solvers (Table 1) ------
+@pytest.mark.parametrize("case", [(1, 5, wi.BC_SF), (1, 3, wi.BC_PERIODIC), (0, 5, wi.BC_SF)])
+def test_blocked_krylov_outer_solvers_match_oracle(case):
+    """WD_SOLVER_GL_FLEX (case D1: fp64 Global BiCGStab, flexible, fp32 BiCGStab preconditioner), WD_SOLVER_GL_F64 (case B)
+    and WD_SOLVER_BL_F64 (case C, n x n coefficient matrices): the same X, Y as the oracle at the default solver's
+    tolerances.  Qualitative claims of the paper checked on the synthetic field: the preconditioner is called about three
+    times, and Gl-BiCGStab needs about as many iterations as BiCGStab per column."""
+    pkg = _wd()
+    idx, n, bc = case
+    cfg = dict(wi.CONFIGS[idx])
+    dims, kappa = cfg["dims"], cfg["kappa"]
+    U = wi.gauge_field(dims, cfg["eps"], cfg["seed"], bc)
+    Phi = wi.spinor_field(dims, n, cfg["seed"], bc)
+    Xr, rr, _, rc = orc.solve(dims, kappa, bc, 0, U, Phi, tol=1e-14)
+    assert rc == 0 and rr.max() < 1e-13
+    Yr, rr, _, rc = orc.solve(dims, kappa, bc, 1, U, Xr, tol=1e-14)
+    assert rc == 0 and rr.max() < 1e-13
+    ctx = make_ctx(dims, kappa, bc, n, U)
+    P = ctx.pack(dev(Phi))
+    _, i0 = ctx.solve_block(pkg.OP_D, P, n, tol=1e-12)
+    ctx.set_option(pkg.OPT_POLL_EVERY, 1)
+    iters = {}
+    for solver in (pkg.SOLVER_GL_FLEX, pkg.SOLVER_GL_F64, pkg.SOLVER_BL_F64):
+        ctx.set_option(pkg.OPT_SOLVER, solver)
+        X, ix = ctx.solve_block(pkg.OP_D, P, n, tol=1e-12, max_outer=500)
+        Y, iy = ctx.solve_block(pkg.OP_DDAG, X, n, tol=1e-12, max_outer=500)
+        assert ix["converged"] and iy["converged"], solver
+        Xc, Yc = ctx.unpack(X, n).cpu().numpy(), ctx.unpack(Y, n).cpu().numpy()
+        assert rel_per_rhs(orc.apply(dims, kappa, bc, 0, U, Xc), Phi).max() < 2e-12, solver
+        assert rel_per_rhs(orc.apply(dims, kappa, bc, 1, U, Yc), Xc).max() < 2e-12, solver
+        assert rel_per_rhs(Xc, Xr).max() < 1e-9 and rel_per_rhs(Yc, Yr).max() < 1e-9, solver
+        force_close(ctx.force(X, Y, n).cpu().numpy(), orc.force(dims, kappa, bc, U, Xr, Yr), 1e-9)
+        iters[solver] = ix
+    assert 2 <= iters[pkg.SOLVER_GL_FLEX]["outer_steps"] <= 4          # preconditioner calls
+    per_column = i0["inner_iters_total"]
+    assert abs(iters[pkg.SOLVER_GL_F64]["inner_iters_total"] - per_column) <= 0.25 * per_column + 2
+    assert iters[pkg.SOLVER_BL_F64]["inner_iters_total"] <= 1.25 * per_column + 2
+    ctx.close()
