@@ -46,6 +46,8 @@ def parse_args():
                     help="WD_OPT_HOP_IMPL: 0 register kernel, 1 shared-memory-staged kernel, -1 library default")
     ap.add_argument("--rhs-sweep", action="store_true", help="configs[4]: blocked solve at n_rhs = 1, 2, 5, 8, 12")
     ap.add_argument("--apply-sweep", action="store_true", help="configs[3]: D, D^dag apply on 16^4, fp32/fp64 x 18/12 reals")
+    ap.add_argument("--shard-rhs", action="store_true",
+                    help="N > 1: deal the n_rhs columns of ONE problem to the ranks (gauge replicated, allReduce of F): strong scaling")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-baseline-full", action="store_true", help="time the oracle on the WHOLE workload (minutes)")
     ap.add_argument("--no-hop-sweep", action="store_true")
@@ -588,10 +590,62 @@ def run_ours(args):
         print(json.dumps(line))
 
 
+def run_sharded(args):
+    """--shard-rhs: the RHS-sharded multi-GPU form (paper_1009_5169_b200/sharded.py): one
+    problem, its columns dealt to the ranks, one allReduce(sum) of F per force evaluation.  Total work is fixed: strong
+    scaling.  The default N > 1 mode stays "replicas" (north_star: no sharding for the headline)."""
+    import torch
+    import torch.distributed as dist
+
+    import paper_1009_5169_b200 as pkg
+    import wd_inputs as wi
+    from paper_1009_5169_b200 import replicas as rp
+    from paper_1009_5169_b200 import sharded as sh
+    world, rank, local = rp.env_world()
+    torch.cuda.set_device(local)
+    if world > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    cfg = dict(wi.CONFIGS[args.config])
+    n = args.n_rhs
+    dims, kappa, bc = cfg["dims"], cfg["kappa"], cfg["bc"]
+    recon = pkg.LINK12 if args.recon == 12 else pkg.LINK18
+    dev = f"cuda:{local}"
+    sc = sh.ShardedContext(pkg, dist, dims, kappa, bc, n, world, rank, dev)
+    sc.set_gauge(torch.from_numpy(wi.gauge_field(dims, cfg["eps"], cfg["seed"], bc)).cuda())
+    P = sc.pack_local(torch.from_numpy(wi.spinor_field(dims, n, cfg["seed"], bc)).cuda())
+    for _ in range(max(args.warmup, 3)):
+        F, S, infos = sc.md_force(P, recon=recon, tol=TOL)
+    rp.barrier(dist, world)
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(args.steps):
+        F, S, infos = sc.md_force(P, recon=recon, tol=TOL)
+    e1.record()
+    rp.barrier(dist, world)
+    torch.cuda.synchronize()
+    ms = rp.max_over_ranks(dist, torch, world, e0.elapsed_time(e1), sc.device)
+    line = {"metric": METRIC, "value": args.steps / (ms * 1e-3), "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": max(args.warmup, 3), "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "strong",
+            "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": workload_name(cfg, n), "parallelism": f"rhs-sharded x{world}: columns i mod {world}, gauge replicated, "
+                       "allReduce(sum) of F", "columns_of_rank0": sh.columns_of_rank(n, world, 0), "tol": TOL},
+            "exchange_bytes_per_step": 4 * 18 * 8 * dims[0] * dims[1] * dims[2] * dims[3], "action": S}
+    sc.close()
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+    if rank == 0:
+        print(json.dumps(line))
+
+
 def main():
     args = parse_args()
     if args.impl == "reference":
         run_reference(args)
+    elif args.shard_rhs:
+        run_sharded(args)
     else:
         run_ours(args)
 
