@@ -682,3 +682,33 @@ def test_blocked_krylov_outer_solvers_match_oracle(case):
     assert abs(iters[pkg.SOLVER_GL_F64]["inner_iters_total"] - per_column) <= 0.25 * per_column + 2
     assert iters[pkg.SOLVER_BL_F64]["inner_iters_total"] <= 1.25 * per_column + 2
     ctx.close()
+
+
+def test_no_out_of_bounds_writes_guard_bands():
+    """compute-sanitizer is closed on this GPU pool (profiles/r02_sanitizer.md), so out-of-bounds WRITES of the hop
+    kernels (register, row-group ring, z-march; fp32 / fp64 / 16-bit storage via the reliable solver) are looked for with
+    guard bands: every output lives inside a larger allocation whose surroundings hold a bit pattern that must survive."""
+    pkg = _wd()
+    for dims, bc, n in (((8, 4, 6, 4), wi.BC_SF, 5), ((12, 8, 4, 6), wi.BC_PERIODIC, 4), ((8, 8, 8, 8), wi.BC_SF, 16)):
+        U = wi.gauge_field(dims, 0.3, 7, bc)
+        psi = wi.spinor_field(dims, n, 11, bc)
+        ctx = make_ctx(dims, 0.13, bc, n, U)
+        for prec, dt in ((pkg.F64, torch.float64), (pkg.F32, torch.float32)):
+            nat = ctx.pack(dev(psi), prec)
+            numel, guard = nat.numel(), 4096
+            for impl in (0, 1, 2):
+                ctx.set_option(pkg.OPT_HOP_IMPL, impl)
+                for recon in (pkg.LINK18, pkg.LINK12):
+                    big = torch.full((numel + 2 * guard,), -12345.0, dtype=dt, device="cuda")
+                    ctx.apply(pkg.OP_D, nat, n, prec, recon, out=big[guard:guard + numel])
+                    assert bool((big[:guard] == -12345.0).all()) and bool((big[guard + numel:] == -12345.0).all()), (dims, prec, impl, recon)
+                    assert bool(torch.isfinite(big[guard:guard + numel]).all())
+        ctx.set_option(pkg.OPT_HOP_IMPL, 2)
+        P = ctx.pack(dev(psi))
+        for solver in (pkg.SOLVER_DC_F32, pkg.SOLVER_RELIABLE_H16):
+            ctx.set_option(pkg.OPT_SOLVER, solver)
+            big = torch.full((P.numel() + 8192,), -12345.0, dtype=torch.float64, device="cuda")
+            X, info = ctx.solve_block(pkg.OP_D, P, n, out=big[4096:4096 + P.numel()])
+            assert info["converged"]
+            assert bool((big[:4096] == -12345.0).all()) and bool((big[4096 + P.numel():] == -12345.0).all()), (dims, solver)
+        ctx.close()
