@@ -56,7 +56,14 @@ typedef struct wd_ctx wd_ctx; /* opaque; created by wd_create, freed by wd_destr
 enum { WD_OK = 0, WD_EINVAL = -1, WD_ENOMEM = -2, WD_ECUDA = -3, WD_ENOCONV = -4, WD_ESTATE = -5 };
 enum { WD_BC_PERIODIC = 0, WD_BC_SF = 1 }; /* time direction; space is always periodic, theta=0 */
 enum { WD_OP_D = 0, WD_OP_DDAG = 1 };
-enum { WD_F64 = 0, WD_F32 = 1 };
+/* WD_F32P: fp32 in the x-paired native form "P32" -- two sites of a lattice row (Lx/4 apart within their parity) share
+ * every 128-bit element, one complex number each, so that one thread works on both with the packed fp32 instructions of
+ * sm_100 (csrc/wd_f2.cuh).  It is the form the fp32 inner solver computes in (wd_solve_block) and is
+ * accepted by wd_native_bytes, wd_pack, wd_unpack, wd_hop and wd_apply so that it can be tested and timed on its own;
+ * results are bit for bit those of WD_F32.  Needs the row-major layout (linear site order, Lx/2 even, max_rhs >= 3) and
+ * a (lattice, n_rhs) shape the z-march hop kernel serves; elsewhere those calls return WD_EINVAL and the solver
+ * computes in WD_F32. */
+enum { WD_F64 = 0, WD_F32 = 1, WD_F32P = 2 };
 enum { WD_LINK18 = 0, WD_LINK12 = 1 }; /* 18 reals per link, or rows 1-2 only */
 enum { WD_ORDER_LINEAR = 0, WD_ORDER_TILED = 1 };
 enum { WD_ACTION_FULL = 0, WD_ACTION_EO = 1 };   /* pseudo-fermion action on D (eq. 2.2) or on the even/odd Schur complement */
@@ -121,10 +128,15 @@ int wd_site_order(wd_ctx* ctx, int order, const int tile[4]);
  *       WD_SOLVER_GL_F64: case B, the same without preconditioner (all fp64; info.inner_iters_total = its iterations).
  *       WD_SOLVER_BL_F64: case C, fp64 Block BiCGStab (ref. [7] of the paper): n_rhs x n_rhs coefficient matrices from the
  *       Gram matrices of the block vectors, one Krylov space shared by the columns; max_inner bounds its iterations.
+ *   WD_OPT_PAIRED       1: the fp32 inner solver computes in the x-paired form WD_F32P (two sites per thread, packed
+ *       fp32 instructions) wherever the z-march hop kernel serves the shape; 0 (default): plain WD_F32.  Same iterates
+ *       up to the summation order of the inner products.  (Measured at 24^4, n_rhs = 5: 64 us against 59 us per hop --
+ *       the hop is bound by shared-memory bandwidth, which pairing does not change, and has half the warps to hide
+ *       latency with.)
  * Errors: WD_EINVAL (null, unknown key, value out of range). */
 enum { WD_OPT_HOP32_SITES = 0, WD_OPT_HOP64_SITES = 1, WD_OPT_HOP32_REGS = 2, WD_OPT_HOP64_REGS = 3,
        WD_OPT_POLL_EVERY = 4, WD_OPT_HOP_IMPL = 5, WD_OPT_ALTERNATE_SWEEP = 6, WD_OPT_HOP_ROWS = 7, WD_OPT_SOLVER = 8,
-       WD_OPT_N = 9 };
+       WD_OPT_PAIRED = 9, WD_OPT_N = 10 };
 /* values of WD_OPT_SOLVER */
 enum { WD_SOLVER_DC_F32 = 0, WD_SOLVER_RELIABLE_H16 = 1, WD_SOLVER_GL_FLEX = 2, WD_SOLVER_GL_F64 = 3, WD_SOLVER_BL_F64 = 4,
        WD_SOLVER_N = 5 };

@@ -32,6 +32,7 @@ void build_tables(wd_ctx* c) {
     c->RB = (c->order == WD_ORDER_LINEAR && (c->L[0] / 2) % 2 == 0 && c->max_rhs >= 3) ? (uint32_t)(c->L[0] / 2) : (uint32_t)Vh;
     c->rb_lg = 0;
     while ((1u << c->rb_lg) < c->RB) ++c->rb_lg;
+    c->paired_ok = c->RB == (uint32_t)(c->L[0] / 2) && c->RB % 2 == 0;
     c->h_site_of.assign(2 * Vh, -1);
     c->h_nbr.assign(2 * Vh * WD_NDIR, 0);
     std::vector<int32_t> idx_of(V);
@@ -66,7 +67,7 @@ void build_tables(wd_ctx* c) {
 }
 
 struct WsMap {
-    size_t site_of, nbr, u64[2], u32[2], scal, partials, ticket, solver, total;
+    size_t site_of, nbr, u64[2], u32[2], u32p[2], scal, partials, ticket, solver, total;
 };
 
 const int kReals[2] = {18, 12};
@@ -86,6 +87,7 @@ WsMap ws_map(const wd_ctx* c) {
     m.nbr = o;     o += wd_align_up(sizeof(int32_t) * 2 * c->Vh * WD_NDIR);
     for (int r = 0; r < 2; ++r) { m.u64[r] = o; o += wd_align_up(sizeof(double) * 4 * c->V * kReals[r]); }
     for (int r = 0; r < 2; ++r) { m.u32[r] = o; o += wd_align_up(sizeof(float) * 4 * c->V * kReals[r]); }
+    for (int r = 0; r < 2; ++r) { m.u32p[r] = o; if (c->paired_ok) o += wd_align_up(sizeof(float) * 4 * c->V * kReals[r]); }
     m.scal = o;     o += wd_align_up(sizeof(double) * kScalDoubles);
     m.partials = o; o += wd_align_up(sizeof(double) * partial_doubles(c));
     m.ticket = o;   o += wd_align_up(256);
@@ -159,6 +161,7 @@ int wd_create(wd_ctx** out, const int dims[4], double kappa, int time_bc, int ma
     c->opt[WD_OPT_POLL_EVERY] = 4;
     c->opt[WD_OPT_HOP_IMPL] = 2;
     c->opt[WD_OPT_ALTERNATE_SWEEP] = 1;
+    c->opt[WD_OPT_PAIRED] = 0;
     c->prof_on = false;
     c->prof_used = 0;
     c->h_pinned = nullptr;
@@ -201,6 +204,7 @@ int wd_set_option(wd_ctx* ctx, int key, int value) {
             if (value < 0 || value > 2) return wd_fail(ctx, WD_EINVAL, "hop implementation is 0, 1 or 2");
             break;
         case WD_OPT_ALTERNATE_SWEEP:
+        case WD_OPT_PAIRED:
             if (value != 0 && value != 1) return wd_fail(ctx, WD_EINVAL, "this option is 0 or 1");
             break;
         case WD_OPT_HOP_ROWS:
@@ -283,6 +287,7 @@ int wd_set_workspace(wd_ctx* ctx, void* ws_dev, size_t bytes) {
     ctx->d_site_of = (int32_t*)(w + m.site_of);
     ctx->d_nbr = (int32_t*)(w + m.nbr);
     for (int r = 0; r < 2; ++r) { ctx->d_U64[r] = (double*)(w + m.u64[r]); ctx->d_U32[r] = (float*)(w + m.u32[r]); }
+    for (int r = 0; r < 2; ++r) ctx->d_U32P[r] = ctx->paired_ok ? (float*)(w + m.u32p[r]) : nullptr;
     ctx->d_scal = (double*)(w + m.scal);
     ctx->d_partials = (double*)(w + m.partials);
     ctx->partial_doubles = partial_doubles(ctx);
@@ -312,22 +317,24 @@ int wd_set_gauge(wd_ctx* ctx, const double* U) {
 }
 
 size_t wd_native_bytes(const wd_ctx* ctx, int prec, int n_rhs) {
-    if (!ctx || n_rhs < 0 || (prec != WD_F64 && prec != WD_F32)) return 0;
+    if (!ctx || n_rhs < 0 || !wd_is_prec(prec) || (prec == WD_F32P && !ctx->paired_ok)) return 0;
     return 2 * wd_half_bytes(ctx, prec, n_rhs);
 }
 
 int wd_pack(wd_ctx* ctx, int prec, int n_rhs, const double* canon, void* native) {
     if (!ctx) return WD_EINVAL;
-    if (!canon || !native || bad_n(ctx, n_rhs) || (prec != WD_F64 && prec != WD_F32))
+    if (!canon || !native || bad_n(ctx, n_rhs) || !wd_is_prec(prec))
         return wd_fail(ctx, WD_EINVAL, "wd_pack: bad argument");
+    if (prec == WD_F32P && !ctx->paired_ok) return wd_fail(ctx, WD_EINVAL, "wd_pack: WD_F32P needs the row-major layout");
     if (!ctx->have_ws) return wd_fail(ctx, WD_ESTATE, "wd_set_workspace first");
     return wd_layout_pack(ctx, prec, n_rhs, canon, native);
 }
 
 int wd_unpack(wd_ctx* ctx, int prec, int n_rhs, const void* native, double* canon) {
     if (!ctx) return WD_EINVAL;
-    if (!canon || !native || bad_n(ctx, n_rhs) || (prec != WD_F64 && prec != WD_F32))
+    if (!canon || !native || bad_n(ctx, n_rhs) || !wd_is_prec(prec))
         return wd_fail(ctx, WD_EINVAL, "wd_unpack: bad argument");
+    if (prec == WD_F32P && !ctx->paired_ok) return wd_fail(ctx, WD_EINVAL, "wd_unpack: WD_F32P needs the row-major layout");
     if (!ctx->have_ws) return wd_fail(ctx, WD_ESTATE, "wd_set_workspace first");
     return wd_layout_unpack(ctx, prec, n_rhs, native, canon);
 }
@@ -343,7 +350,8 @@ static int check_op_args(wd_ctx* ctx, int op, int prec, int recon, int n_rhs, co
     if (!a || !b || a == b) return wd_fail(ctx, WD_EINVAL, "null or aliased field pointer");
     if (bad_n(ctx, n_rhs)) return wd_fail(ctx, WD_EINVAL, "n_rhs out of range");
     if (op != WD_OP_D && op != WD_OP_DDAG) return wd_fail(ctx, WD_EINVAL, "bad op");
-    if (prec != WD_F64 && prec != WD_F32) return wd_fail(ctx, WD_EINVAL, "bad precision");
+    if (!wd_is_prec(prec)) return wd_fail(ctx, WD_EINVAL, "bad precision");
+    if (prec == WD_F32P && !ctx->paired_ok) return wd_fail(ctx, WD_EINVAL, "WD_F32P needs the row-major layout");
     if (recon != WD_LINK18 && recon != WD_LINK12) return wd_fail(ctx, WD_EINVAL, "bad link form");
     if (!ctx->have_gauge) return wd_fail(ctx, WD_ESTATE, "wd_set_gauge first");
     return WD_OK;

@@ -244,6 +244,14 @@ int wd_hop_launch_ex(wd_ctx* c, int prec, int recon, int dag, int n, int par, co
     if (o.epi >= EPI_SIGMA && prec != WD_F32) return wd_fail(c, WD_EINVAL, "fused reductions are fp32 only");
     // staged kernel where it applies (row-major layout) and pays: with 1-2 columns a group of rows gives it too few
     // consumer threads (24^4 fp32: 41 us against 33 us at n = 2; 71 against 76 at n = 5; 146 against 151 at n = 12)
+    if (prec == WD_F32P || o.storage == 2) {   // P32 (two sites per thread): served by the z-march kernel only
+        wd_hop_ops o2 = o;
+        o2.storage = 2;
+        const int rc = wd_hop_zm_launch(c, WD_F32, recon, dag, n, par, o2);
+        if (rc > 0) return wd_fail(c, WD_EINVAL, "hop: WD_F32P needs the z-march kernel (row-major layout, a shape that fits shared memory)");
+        if (rc == WD_OK) WD_LAUNCH_CHECK(c);
+        return rc;
+    }
     if (o.storage == 1) {   // 16-bit storage: served by the z-march kernel only
         const int rc = n >= 3 ? wd_hop_zm_launch(c, prec, recon, dag, n, par, o) : 1;
         if (rc > 0) return wd_fail(c, WD_EINVAL, "hop: the 16-bit storage format needs the z-march kernel (row-major layout, n_rhs >= 3)");

@@ -25,6 +25,7 @@
 // r fastest: conflict-free 128-bit shared-memory reads, results bit for bit those of the register kernel
 // (wd_hop.cu accumulates the directions in the same order).
 #include "wd_blas.cuh"
+#include "wd_f2.cuh"
 #include "wd_h16.cuh"
 #include "wd_su3.cuh"
 #include "wd_tma.cuh"
@@ -127,6 +128,38 @@ __device__ __forceinline__ void dir_smem(const typename Vec<T>::type* sp, uint32
     accumulate<MU, SIGMA, FIRST>(acc, chi);
 }
 
+// ---- the same for two sites per thread (ST = 2: P32 operands, wd_f2.cuh) ---------------------------------------
+// sp: spinor row in shared memory, cs = H * n elements per complex, e = element of the neighbour pair; L: link row,
+// lp = pair whose link is used.  SWAP (x hops only): the neighbour pair has its lanes exchanged -- the forward hop
+// exchanges the projected half spinor (the link is the output pair's own), the backward hop multiplies in the
+// neighbour's lane order (its link sits with it) and exchanges the result.
+template <int RECON, int MU, bool FWD, bool DAG, bool FIRST = false, bool SWAP = false>
+__device__ __forceinline__ void dir_pair(const ulonglong2* sp, uint32_t cs, uint32_t e, const ulonglong2* L, uint32_t H, uint32_t lp,
+                                         wdp::cx2 (&acc)[12], bool swp = false) {
+    if (WD_ZM_ABLATE == 1) {
+        if (FIRST) {
+#pragma unroll
+            for (int q = 0; q < 12; ++q) { acc[q].re = wdp::zero2(); acc[q].im = wdp::zero2(); }
+        }
+        return;
+    }
+    constexpr int SIGMA = (FWD ? 1 : -1) * (DAG ? -1 : 1);
+    wdp::cx2 psi[12], hs[6], chi[6], u[9];
+    wdp::ld_spinor(sp, cs, e, psi);
+    wdp::ld_link<RECON>(L, H, lp, u);
+    wdp::project<MU, SIGMA>(psi, hs);
+    if (SWAP && FWD) {
+#pragma unroll
+        for (int q = 0; q < 6; ++q) { hs[q].re = wdp::swap_if(swp, hs[q].re); hs[q].im = wdp::swap_if(swp, hs[q].im); }
+    }
+    wdp::su3_mul<!FWD>(u, hs, chi);
+    if (SWAP && !FWD) {
+#pragma unroll
+        for (int q = 0; q < 6; ++q) { chi[q].re = wdp::swap_if(swp, chi[q].re); chi[q].im = wdp::swap_if(swp, chi[q].im); }
+    }
+    wdp::accumulate<MU, SIGMA, FIRST>(acc, chi);
+}
+
 // ---- the kernel -------------------------------------------------------------------------------------------
 // block = consumer warps (S * n threads, rounded up) + four producer warps; grid = min(steps, SMs).
 // dynamic smem: 128 B of mbarriers | planes 3 x RG rows | T+ | T- | halo 2 rows | links 8 x RG link rows
@@ -146,7 +179,8 @@ __global__ void __launch_bounds__(MAXT, 1) hop_zm_kernel(const ZmArgs<T> A) {
     uint64_t* full_w = empty_u + NUNIT;                      // [3]
     uint64_t* empty_w = full_w + 3;                          // [3]
     const uint32_t RG = RGT ? (uint32_t)RGT : A.RG, rowV = Lxh * nr;
-    const uint32_t rowS = ST ? wdh::h16_row_vecs(rowV) : NCH * rowV;     // 16-byte units of one spinor row (all chunks)
+    const uint32_t rowS = ST == 1 ? wdh::h16_row_vecs(rowV) : NCH * rowV;   // 16-byte units of one spinor row (all chunks)
+    const uint32_t SW = ST == 2 ? Lxh / 2 : Lxh;                            // thread-sites per row (ST = 2: site pairs)
     const uint32_t rowB = rowS * 16;                                     // bytes of one spinor row
     const uint32_t lrowB = Lxh * RECON * (uint32_t)sizeof(T);            // bytes of one row of one link array
     char* const base = reinterpret_cast<char*>(smem) + 128;
@@ -155,7 +189,7 @@ __global__ void __launch_bounds__(MAXT, 1) hop_zm_kernel(const ZmArgs<T> A) {
     char* const tm = tp + (size_t)RG * rowB;
     char* const halo = tm + (size_t)RG * rowB;
     char* const links = halo + (size_t)2 * rowB;
-    const uint32_t nct = RG * Lxh * nr, ncw = (nct + 31) >> 5;
+    const uint32_t nct = RG * SW * nr, ncw = (nct + 31) >> 5;
     const uint32_t warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     if (threadIdx.x == 0) {
         for (uint32_t u = 0; u < NUNIT; ++u) { mbar_init(&full_u[u], 1); mbar_init(&empty_u[u], ncw); }
@@ -249,6 +283,136 @@ __global__ void __launch_bounds__(MAXT, 1) hop_zm_kernel(const ZmArgs<T> A) {
                 else if (lane == 2) bulk_g2s(links + (size_t)LK_ZP * RG * lrowB, U + (size_t)(4 + A.par) * ublk + (size_t)row0 * lrowB, RG * lrowB, &full_u[U_XZ]);
             }
         }
+    } else if constexpr (ST == 2) {
+        // ================= consumers, two sites per thread: thread i = (row j, pair p, column r) =========
+        typedef ulonglong2 pv;
+        using namespace wdp;
+        const uint32_t i = threadIdx.x;
+        const bool active = i < nct;
+        const uint32_t H = SW, cs = H * nr;                       // pairs per row, elements per complex of a row
+        const uint32_t sidx = i / nr, r = i - sidx * nr;
+        const uint32_t j = sidx / H, p = sidx - j * H;
+        const uint32_t lrowV = lrowB / 16;
+        const uint32_t e0 = p * nr + r;
+        const pv* const Pl = reinterpret_cast<const pv*>(planes);
+        const pv* const Tp = reinterpret_cast<const pv*>(tp) + (size_t)j * rowS;
+        const pv* const Tm = reinterpret_cast<const pv*>(tm) + (size_t)j * rowS;
+        const pv* const Hl = reinterpret_cast<const pv*>(halo);
+        const pv* const Lk = reinterpret_cast<const pv*>(links) + (size_t)j * lrowV;
+        const uint32_t lblk = RG * lrowV;
+        const uint32_t planeV = RG * rowS;
+        if (A.zero_rows) {
+            const vec z4 = {};
+            for (uint32_t row = blockIdx.x; row < A.zero_rows; row += gridDim.x)
+                for (uint32_t v = i; v < rowS; v += ncw * 32) A.out[(size_t)row * rowS + v] = z4;
+        }
+        const f2 a2 = mk2(A.a, A.a), b2 = mk2(A.b, A.b);
+        uint32_t a = 0, prev = NO_STEP;
+        for (uint32_t s = s_first, k = 0; s != NO_STEP; prev = s, s = next_step(s, A.chunk, A.steps), ++k) {
+            const uint32_t col = s / A.Lz, z = s - col * A.Lz;
+            const uint32_t yb = col % A.gy, t = A.t0 + col / A.gy, y0 = yb * RG;
+            if (k > 0) a += continues(prev, s, A.Lz) ? 1u : 3u;
+            const uint32_t s_next = next_step(s, A.chunk, A.steps);
+            const bool switch_next = s_next != NO_STEP && !continues(s, s_next, A.Lz);
+            const uint32_t ph = k & 1;
+            const size_t own = (size_t)(y0 + A.Ly * (z + A.Lz * t) + j) * rowS;
+            cx2 acc[12];
+            if (EPI >= EPI_XPAY && active) {
+#pragma unroll
+                for (uint32_t c = 0; c < 12; ++c) {
+                    asm volatile("prefetch.global.L2 [%0];" ::"l"(A.in2 + own + c * cs + e0));
+                    if (EPI == EPI_SIGMA) asm volatile("prefetch.global.L2 [%0];" ::"l"(A.in3 + own + c * cs + e0));
+                }
+            }
+            const uint32_t wm = a % 3, wc = (a + 1) % 3, wp = (a + 2) % 3;
+            const pv* const Pm = Pl + (size_t)wm * planeV + (size_t)j * rowS;
+            const pv* const Pc = Pl + (size_t)wc * planeV + (size_t)j * rowS;
+            const pv* const Pp = Pl + (size_t)wp * planeV + (size_t)j * rowS;
+            // ---- t+
+            mbar_wait(&full_u[U_TP], ph);
+            if (active) dir_pair<RECON, 3, true, DAG, true>(Tp, cs, e0, Lk + LK_TP * lblk, H, p, acc);
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&empty_u[U_TP]);
+            // ---- t-
+            mbar_wait(&full_u[U_TM], ph);
+            if (active) dir_pair<RECON, 3, false, DAG>(Tm, cs, e0, Lk + LK_TM * lblk, H, p, acc);
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&empty_u[U_TM]);
+            // ---- z-
+            mbar_wait(&full_u[U_ZM], ph);
+            mbar_wait(&full_w[wm], (a / 3) & 1);
+            if (active) dir_pair<RECON, 2, false, DAG>(Pm, cs, e0, Lk + LK_ZM * lblk, H, p, acc);
+            __syncwarp();
+            if (lane == 0) { mbar_arrive(&empty_u[U_ZM]); mbar_arrive(&empty_w[wm]); }
+            // ---- y-, y+
+            mbar_wait(&full_u[U_Y], ph);
+            mbar_wait(&full_w[wc], ((a + 1) / 3) & 1);
+            if (active) {
+                const pv* ym = j == 0 ? Hl : Pc - rowS;
+                const pv* yp = j == RG - 1 ? Hl + rowS : Pc + rowS;
+                dir_pair<RECON, 1, false, DAG>(ym, cs, e0, Lk + LK_YM * lblk, H, p, acc);
+                dir_pair<RECON, 1, true, DAG>(yp, cs, e0, Lk + LK_YP * lblk, H, p, acc);
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&empty_u[U_Y]);
+            // ---- x-, x+, z+
+            mbar_wait(&full_u[U_XZ], ph);
+            mbar_wait(&full_w[wp], ((a + 2) / 3) & 1);
+            if (active) {
+                // rows with bb = 1 have their +x neighbour one pair up and their -x neighbour in the same pair; bb = 0
+                // the other way round.  A step past the half row lands on the pair at the other end, lanes exchanged.
+                const uint32_t bb = (y0 + j + z + t + A.par) & 1;
+                const uint32_t pp = bb ? (p + 1 == H ? 0u : p + 1) : p;
+                const uint32_t pm = bb ? p : (p == 0 ? H - 1 : p - 1);
+                const bool swp_p = bb && p + 1 == H, swp_m = !bb && p == 0;
+                dir_pair<RECON, 0, false, DAG, false, true>(Pc, cs, pm * nr + r, Lk + LK_XM * lblk, H, pm, acc, swp_m);
+                dir_pair<RECON, 0, true, DAG, false, true>(Pc, cs, pp * nr + r, Lk + LK_XP * lblk, H, p, acc, swp_p);
+                dir_pair<RECON, 2, true, DAG>(Pp, cs, e0, Lk + LK_ZP * lblk, H, p, acc);
+            }
+            __syncwarp();
+            if (lane == 0) {
+                mbar_arrive(&empty_u[U_XZ]);
+                if (switch_next) { mbar_arrive(&empty_w[wc]); mbar_arrive(&empty_w[wp]); }
+            }
+            // ---- epilogue and store
+            if (active) {
+                [[maybe_unused]] cx2 qv[12];
+                if (EPI >= EPI_XPAY) {
+                    ldg_spinor(reinterpret_cast<const pv*>(A.in2) + own, cs, e0, qv);
+#pragma unroll
+                    for (int q = 0; q < 12; ++q) {
+                        acc[q].re = fma2(b2, acc[q].re, mul2(a2, qv[q].re));
+                        acc[q].im = fma2(b2, acc[q].im, mul2(a2, qv[q].im));
+                    }
+                    if (EPI == EPI_OMEGA) {  // <t, s>, <t, t> with t = acc, s = qv
+                        f2 s0 = zero2(), s1 = zero2(), s2 = zero2();
+#pragma unroll
+                        for (int q = 0; q < 12; ++q) {
+                            s0 = fma2(acc[q].re, qv[q].re, s0);  s0 = fma2(acc[q].im, qv[q].im, s0);
+                            s1 = fma2(acc[q].re, qv[q].im, s1);  s1 = fma2(neg2(acc[q].im), qv[q].re, s1);
+                            s2 = fma2(acc[q].re, acc[q].re, s2); s2 = fma2(acc[q].im, acc[q].im, s2);
+                        }
+                        float lo, hi;
+                        un2(s0, lo, hi); dsum[0] += (double)lo + (double)hi;
+                        un2(s1, lo, hi); dsum[1] += (double)lo + (double)hi;
+                        un2(s2, lo, hi); dsum[2] += (double)lo + (double)hi;
+                    }
+                }
+                if (EPI == EPI_SIGMA) {  // <r~, v> with v = acc
+                    ldg_spinor(reinterpret_cast<const pv*>(A.in3) + own, cs, e0, qv);
+                    f2 s0 = zero2(), s1 = zero2();
+#pragma unroll
+                    for (int q = 0; q < 12; ++q) {
+                        s0 = fma2(qv[q].re, acc[q].re, s0);  s0 = fma2(qv[q].im, acc[q].im, s0);
+                        s1 = fma2(qv[q].re, acc[q].im, s1);  s1 = fma2(neg2(qv[q].im), acc[q].re, s1);
+                    }
+                    float lo, hi;
+                    un2(s0, lo, hi); dsum[0] += (double)lo + (double)hi;
+                    un2(s1, lo, hi); dsum[1] += (double)lo + (double)hi;
+                }
+                st_spinor(reinterpret_cast<pv*>(A.out) + own, cs, e0, acc);
+            }
+        }
     } else {
         // ================= consumers: thread i = (site s of the step, column r) ==========================
         const uint32_t i = threadIdx.x;
@@ -282,7 +446,7 @@ __global__ void __launch_bounds__(MAXT, 1) hop_zm_kernel(const ZmArgs<T> A) {
             cx<T> acc[12];
             if (EPI >= EPI_XPAY && active) {
 #pragma unroll
-                for (uint32_t c = 0; c < (ST ? 3u : NCH); ++c) {
+                for (uint32_t c = 0; c < (ST == 1 ? 3u : NCH); ++c) {
                     asm volatile("prefetch.global.L2 [%0];" ::"l"(A.in2 + own + c * rowV + e0));
                     if (EPI == EPI_SIGMA) asm volatile("prefetch.global.L2 [%0];" ::"l"(A.in3 + own + c * rowV + e0));
                 }
@@ -384,7 +548,7 @@ __global__ void __launch_bounds__(MAXT, 1) hop_zm_kernel(const ZmArgs<T> A) {
         for (uint32_t item = warp; item < nr * K; item += nwarps) {
             const uint32_t col = item / K, q = item - col * K;
             double v = 0.0;
-            for (uint32_t ss = lane; ss < RG * Lxh; ss += 32) v += red[q * nct + ss * nr + col];
+            for (uint32_t ss = lane; ss < RG * SW; ss += 32) v += red[q * nct + ss * nr + col];
 #pragma unroll
             for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
             if (lane == 0) A.rb.partials[(size_t)item * gridDim.x + blockIdx.x] = v;
@@ -428,9 +592,9 @@ bool pick_shape(const wd_ctx* c, int n, int max_threads, Shape* sh) {
     for (uint32_t RG = Ly; RG >= 1; --RG) {
         if (Ly % RG || RG > cap) continue;
         const uint32_t S = RG * Lxh;
-        const uint32_t cthreads = ((S * n + 31) / 32) * 32;
+        const uint32_t cthreads = (((ST == 2 ? S / 2 : S) * n + 31) / 32) * 32;   // ST = 2: one thread per site pair
         if ((int)cthreads + 128 > max_threads) continue;
-        const size_t rowB = ST ? (size_t)wdh::h16_row_vecs(Lxh * n) * 16 : (size_t)Lxh * n * 16 * Vec<T>::NCH;
+        const size_t rowB = ST == 1 ? (size_t)wdh::h16_row_vecs(Lxh * n) * 16 : (size_t)Lxh * n * 16 * Vec<T>::NCH;
         const size_t lrowB = (size_t)Lxh * RECON * sizeof(T);
         const size_t smem = 128 + (5 * (size_t)RG + 2) * rowB + 8 * (size_t)RG * lrowB;
         if (smem > kSmemMax) continue;
@@ -470,7 +634,7 @@ int launch_epi(wd_ctx* c, const ZmArgs<T>& A, const Shape& sh, unsigned G, int d
 template <typename T, int RECON, int MAXT, int ST>
 int launch_zm(wd_ctx* c, int dag, int n, int par, const wd_hop_ops& o, const T* U) {
     Shape sh;
-    if (ST && ((c->L[0] / 2) * n) % 4 != 0) return 1;   // the H16 scale chunk must keep rows 16-byte aligned
+    if (ST == 1 && ((c->L[0] / 2) * n) % 4 != 0) return 1;   // the H16 scale chunk must keep rows 16-byte aligned
     if (!pick_shape<T, RECON, ST>(c, n, MAXT, &sh)) return 1;
     ZmArgs<T> A;
     A.in = (const typename Vec<T>::type*)o.in;
@@ -516,6 +680,20 @@ int launch_zm(wd_ctx* c, int dag, int n, int par, const wd_hop_ops& o, const T* 
 
 }  // namespace
 
+bool wd_hop_zm_serves(const wd_ctx* c, int recon, int n, int storage) {
+    if (c->order != WD_ORDER_LINEAR || c->RB != (uint32_t)(c->L[0] / 2)) return false;
+    Shape sh;
+    if (storage == 2) {
+        if (!c->paired_ok) return false;
+        return recon == WD_LINK18 ? pick_shape<float, 18, 2>(c, n, 320, &sh) : pick_shape<float, 12, 2>(c, n, 320, &sh);
+    }
+    if (storage == 1) {
+        if (((c->L[0] / 2) * n) % 4 != 0) return false;
+        return recon == WD_LINK18 ? pick_shape<float, 18, 1>(c, n, 512, &sh) : pick_shape<float, 12, 1>(c, n, 512, &sh);
+    }
+    return recon == WD_LINK18 ? pick_shape<float, 18, 0>(c, n, 512, &sh) : pick_shape<float, 12, 0>(c, n, 512, &sh);
+}
+
 // Returns WD_OK if launched, a positive value if this lattice / option set is not served by this kernel (tiled site
 // order, fp64, nothing fits): the caller then tries wd_hop_tma.cu's kernel and then the register kernel.
 int wd_hop_zm_launch(wd_ctx* c, int prec, int recon, int dag, int n, int par, const wd_hop_ops& o) {
@@ -524,6 +702,11 @@ int wd_hop_zm_launch(wd_ctx* c, int prec, int recon, int dag, int n, int par, co
     if (o.storage == 1) {
         if (recon == WD_LINK18) return launch_zm<float, 18, 512, 1>(c, dag, n, par, o, c->d_U32[0]);
         return launch_zm<float, 12, 512, 1>(c, dag, n, par, o, c->d_U32[1]);
+    }
+    if (o.storage == 2) {   // P32: two sites per thread (wd_f2.cuh); 320 threads leave the consumers ~200 registers
+        if (!c->paired_ok) return 1;
+        if (recon == WD_LINK18) return launch_zm<float, 18, 320, 2>(c, dag, n, par, o, c->d_U32P[0]);
+        return launch_zm<float, 12, 320, 2>(c, dag, n, par, o, c->d_U32P[1]);
     }
     if (recon == WD_LINK18) return launch_zm<float, 18, 512, 0>(c, dag, n, par, o, c->d_U32[0]);
     return launch_zm<float, 12, 512, 0>(c, dag, n, par, o, c->d_U32[1]);

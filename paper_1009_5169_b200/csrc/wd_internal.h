@@ -47,6 +47,9 @@ struct wd_ctx {
     int32_t* d_nbr;
     double* d_U64[2];  // [recon] native fp64 links  [mu][parity][R][Vh]
     float* d_U32[2];   // [recon] native fp32 links
+    // P32, the x-paired fp32 form (wd_f2.cuh): available in the row-major layout (RB = Lx/2, which is even there)
+    bool paired_ok;
+    float* d_U32P[2];  // [recon] P32 links (null unless paired_ok)
     // solver scratch
     double* d_scal;        // per-RHS scalars (see wd_solve.cu)
     double* d_partials;    // block partial sums
@@ -102,8 +105,9 @@ static inline size_t wd_align_up(size_t x, size_t a = 256) { return (x + a - 1) 
 
 // size in bytes of a native HALF-lattice block
 static inline size_t wd_half_bytes(const wd_ctx* c, int prec, int n) {
-    return (size_t)c->Vh * 24 * (prec == WD_F64 ? 8 : 4) * (size_t)n;
+    return (size_t)c->Vh * 24 * (prec == WD_F64 ? 8 : 4) * (size_t)n;   // WD_F32 and WD_F32P: 4 bytes per real
 }
+static inline bool wd_is_prec(int prec) { return prec == WD_F64 || prec == WD_F32 || prec == WD_F32P; }
 
 static inline int wd_fail(wd_ctx* c, int code, const char* msg) {
     if (c) c->err = msg;
@@ -153,13 +157,15 @@ struct wd_hop_ops {
     int epi;
     bool check_done;
     int rev;  // 1: sweep the sites from the top (L2 reuse between consecutive kernels)
-    int storage = 0;  // 1: spinor blocks in the 16-bit H16 format (wd_h16.cuh); z-march kernel only
+    int storage = 0;  // 1: spinor blocks in the 16-bit H16 format (wd_h16.cuh); 2: P32 (wd_f2.cuh); z-march kernel only
 };
 int wd_hop_launch_ex(wd_ctx* c, int prec, int recon, int dag, int n, int par, const wd_hop_ops& o);
 // wd_hop_tma.cu: the shared-memory-staged (bulk copy + mbarrier) form; > 0 = not applicable, use the plain kernel
 int wd_hop_tma_launch(wd_ctx* c, int prec, int recon, int dag, int n, int par, const wd_hop_ops& o);
 // wd_hop_zm.cu: the z-marching sliding-window form (fp32); > 0 = not applicable
 int wd_hop_zm_launch(wd_ctx* c, int prec, int recon, int dag, int n, int par, const wd_hop_ops& o);
+// does the z-march kernel serve this (n_rhs, link form, storage) on this context's lattice?
+bool wd_hop_zm_serves(const wd_ctx* c, int recon, int n, int storage);
 int wd_hop_launch(wd_ctx* c, int prec, int recon, int dag, int n, int par, const void* in, void* out,
                   const void* in2, double a, double b);
 

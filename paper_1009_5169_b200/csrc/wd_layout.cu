@@ -17,7 +17,8 @@ namespace {
 
 __global__ void gauge_ingest_kernel(const double* __restrict__ U, const int32_t* __restrict__ site_of, long V,
                                     long Vh, long RB, double* __restrict__ u64_18, double* __restrict__ u64_12,
-                                    float* __restrict__ u32_18, float* __restrict__ u32_12) {
+                                    float* __restrict__ u32_18, float* __restrict__ u32_12,
+                                    float* __restrict__ p32_18, float* __restrict__ p32_12) {
     const long tid = (long)blockIdx.x * blockDim.x + threadIdx.x;
     if (tid >= 4 * 2 * Vh) return;
     const long h = tid % Vh;
@@ -52,9 +53,23 @@ __global__ void gauge_ingest_kernel(const double* __restrict__ U, const int32_t*
         }
     fa[16 * RB + 2 * o] = (float)v[16];
     fa[16 * RB + 2 * o + 1] = (float)v[17];
+    if (p32_18) {   // P32 (wd_f2.cuh): float4 (A.re, B.re, A.im, B.im) of complex c at index c * H + pair, H = RB / 2
+        const long H = RB / 2, pr = o % H, lane = o / H;
+        float* pa = p32_18 + blk * 18 * Vh + lb * 18 * RB;
+        float* pb = p32_12 + blk * 12 * Vh + lb * 12 * RB;
+#pragma unroll
+        for (int c = 0; c < 9; ++c) {
+            pa[(c * H + pr) * 4 + lane] = (float)v[2 * c];
+            pa[(c * H + pr) * 4 + 2 + lane] = (float)v[2 * c + 1];
+            if (c < 6) {
+                pb[(c * H + pr) * 4 + lane] = (float)v[2 * c];
+                pb[(c * H + pr) * 4 + 2 + lane] = (float)v[2 * c + 1];
+            }
+        }
+    }
 }
 
-template <typename T>
+template <typename T, bool PAIRED = false>
 __global__ void pack_kernel(const double* __restrict__ canon, const int32_t* __restrict__ site_of,
                             const int32_t* __restrict__ nbr, long V, long Vh, long RB, int n, T* __restrict__ native) {
     const long tid = (long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -78,6 +93,15 @@ __global__ void pack_kernel(const double* __restrict__ canon, const int32_t* __r
             dst[e] = v[2 * k];
             dst[e + 1] = v[2 * k + 1];
         }
+    } else if (PAIRED) {   // P32: complex k of pair (o % H) at element ((lb*12 + k)*H + pair)*n + r, lane o / H
+        float* dst = (float*)native;
+        const long H = RB / 2, pr = o % H, lane = o / H;
+#pragma unroll
+        for (int k = 0; k < 12; ++k) {
+            const long e = ((long)p * 6 * Vh * n + ((lb * 12 + k) * H + pr) * n + r) * 4;
+            dst[e + lane] = (float)v[2 * k];
+            dst[e + 2 + lane] = (float)v[2 * k + 1];
+        }
     } else {
         float* dst = (float*)native;
 #pragma unroll
@@ -89,7 +113,7 @@ __global__ void pack_kernel(const double* __restrict__ canon, const int32_t* __r
     }
 }
 
-template <typename T>
+template <typename T, bool PAIRED = false>
 __global__ void unpack_kernel(const T* __restrict__ native, const int32_t* __restrict__ site_of, long V, long Vh,
                               long RB, int n, double* __restrict__ canon) {
     const long tid = (long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -109,6 +133,15 @@ __global__ void unpack_kernel(const T* __restrict__ native, const int32_t* __res
             dst[2 * k] = src[e];
             dst[2 * k + 1] = src[e + 1];
         }
+    } else if (PAIRED) {
+        const float* src = (const float*)native;
+        const long H = RB / 2, pr = o % H, lane = o / H;
+#pragma unroll
+        for (int k = 0; k < 12; ++k) {
+            const long e = ((long)p * 6 * Vh * n + ((lb * 12 + k) * H + pr) * n + r) * 4;
+            dst[2 * k] = (double)src[e + lane];
+            dst[2 * k + 1] = (double)src[e + 2 + lane];
+        }
     } else {
         const float* src = (const float*)native;
 #pragma unroll
@@ -127,7 +160,7 @@ int wd_layout_gauge(wd_ctx* c, const double* U) {
     const int B = 128;
     wd_prof_scope prof(c, WD_PROF_LAYOUT);
     gauge_ingest_kernel<<<(unsigned)((total + B - 1) / B), B, 0, c->stream>>>(
-        U, c->d_site_of, c->V, c->Vh, (long)c->RB, c->d_U64[0], c->d_U64[1], c->d_U32[0], c->d_U32[1]);
+        U, c->d_site_of, c->V, c->Vh, (long)c->RB, c->d_U64[0], c->d_U64[1], c->d_U32[0], c->d_U32[1], c->d_U32P[0], c->d_U32P[1]);
     WD_LAUNCH_CHECK(c);
     return WD_OK;
 }
@@ -139,6 +172,8 @@ int wd_layout_pack(wd_ctx* c, int prec, int n, const double* canon, void* native
     wd_prof_scope prof(c, WD_PROF_LAYOUT);
     if (prec == WD_F64)
         pack_kernel<double><<<G, B, 0, c->stream>>>(canon, c->d_site_of, c->d_nbr, c->V, c->Vh, (long)c->RB, n, (double*)native);
+    else if (prec == WD_F32P)
+        pack_kernel<float, true><<<G, B, 0, c->stream>>>(canon, c->d_site_of, c->d_nbr, c->V, c->Vh, (long)c->RB, n, (float*)native);
     else
         pack_kernel<float><<<G, B, 0, c->stream>>>(canon, c->d_site_of, c->d_nbr, c->V, c->Vh, (long)c->RB, n, (float*)native);
     WD_LAUNCH_CHECK(c);
@@ -152,6 +187,8 @@ int wd_layout_unpack(wd_ctx* c, int prec, int n, const void* native, double* can
     wd_prof_scope prof(c, WD_PROF_LAYOUT);
     if (prec == WD_F64)
         unpack_kernel<double><<<G, B, 0, c->stream>>>((const double*)native, c->d_site_of, c->V, c->Vh, (long)c->RB, n, canon);
+    else if (prec == WD_F32P)
+        unpack_kernel<float, true><<<G, B, 0, c->stream>>>((const float*)native, c->d_site_of, c->V, c->Vh, (long)c->RB, n, canon);
     else
         unpack_kernel<float><<<G, B, 0, c->stream>>>((const float*)native, c->d_site_of, c->V, c->Vh, (long)c->RB, n, canon);
     WD_LAUNCH_CHECK(c);

@@ -17,10 +17,16 @@ using namespace wdblas;
 
 namespace {
 
-template <typename T>
+// 128-bit element -> its two complex numbers (re, im, re, im).  PAIRED: the element is in the P32 form of wd_f2.cuh,
+// (A.re, B.re, A.im, B.im); both lanes belong to the same column, so the per-column scalars apply to both.
+template <typename T, bool PAIRED>
 __device__ __forceinline__ void to_arr(const typename V<T>::type& v, T (&a)[2 * V<T>::NC]);
-template <> __device__ __forceinline__ void to_arr<float>(const float4& v, float (&a)[4]) { a[0] = v.x; a[1] = v.y; a[2] = v.z; a[3] = v.w; }
-__device__ __forceinline__ float4 from_arr(const float (&a)[4]) { return make_float4(a[0], a[1], a[2], a[3]); }
+template <> __device__ __forceinline__ void to_arr<float, false>(const float4& v, float (&a)[4]) { a[0] = v.x; a[1] = v.y; a[2] = v.z; a[3] = v.w; }
+template <> __device__ __forceinline__ void to_arr<float, true>(const float4& v, float (&a)[4]) { a[0] = v.x; a[1] = v.z; a[2] = v.y; a[3] = v.w; }
+template <bool PAIRED>
+__device__ __forceinline__ float4 from_arr(const float (&a)[4]) {
+    return PAIRED ? make_float4(a[0], a[2], a[1], a[3]) : make_float4(a[0], a[1], a[2], a[3]);
+}
 
 #define WD_BLAS_PROLOGUE(T)                                                        \
     typedef typename V<T>::type vec;                                               \
@@ -31,7 +37,7 @@ __device__ __forceinline__ float4 from_arr(const float (&a)[4]) { return make_fl
     const long cnt = i0 < nvec ? (nvec - 1 - i0) / stride + 1 : 0;
 
 // P = R + beta (P - omega V)
-template <typename T>
+template <typename T, bool PAIRED>
 __global__ void p_update_kernel(long nvec, int n, int rev, const double* __restrict__ scal, const typename V<T>::type* __restrict__ R,
                                 typename V<T>::type* __restrict__ P, const typename V<T>::type* __restrict__ Vv) {
     if (scal[G_DONE] != 0.0) return;
@@ -41,7 +47,7 @@ __global__ void p_update_kernel(long nvec, int n, int rev, const double* __restr
     for (long k = 0; k < cnt; ++k) {
         const long i = i0 + (rev ? cnt - 1 - k : k) * stride;  // rev: sweep from the top, see wd_solve_impl
         T a[2 * NC], p[2 * NC], v[2 * NC];
-        to_arr<T>(R[i], a); to_arr<T>(P[i], p); to_arr<T>(Vv[i], v);
+        to_arr<T, PAIRED>(R[i], a); to_arr<T, PAIRED>(P[i], p); to_arr<T, PAIRED>(Vv[i], v);
 #pragma unroll
         for (int c = 0; c < NC; ++c) {
             const T tr = p[2 * c] - (wr * v[2 * c] - wi * v[2 * c + 1]);
@@ -49,12 +55,12 @@ __global__ void p_update_kernel(long nvec, int n, int rev, const double* __restr
             p[2 * c] = a[2 * c] + (br * tr - bi * ti);
             p[2 * c + 1] = a[2 * c + 1] + (br * ti + bi * tr);
         }
-        P[i] = from_arr(p);
+        P[i] = from_arr<PAIRED>(p);
     }
 }
 
 // S = R - alpha V   (in place on R)
-template <typename T>
+template <typename T, bool PAIRED>
 __global__ void s_update_kernel(long nvec, int n, int rev, const double* __restrict__ scal, typename V<T>::type* __restrict__ R,
                                 const typename V<T>::type* __restrict__ Vv) {
     if (scal[G_DONE] != 0.0) return;
@@ -63,18 +69,18 @@ __global__ void s_update_kernel(long nvec, int n, int rev, const double* __restr
     for (long k = 0; k < cnt; ++k) {
         const long i = i0 + (rev ? cnt - 1 - k : k) * stride;  // rev: sweep from the top, see wd_solve_impl
         T a[2 * NC], v[2 * NC];
-        to_arr<T>(R[i], a); to_arr<T>(Vv[i], v);
+        to_arr<T, PAIRED>(R[i], a); to_arr<T, PAIRED>(Vv[i], v);
 #pragma unroll
         for (int c = 0; c < NC; ++c) {
             a[2 * c] -= ar * v[2 * c] - ai * v[2 * c + 1];
             a[2 * c + 1] -= ar * v[2 * c + 1] + ai * v[2 * c];
         }
-        R[i] = from_arr(a);
+        R[i] = from_arr<PAIRED>(a);
     }
 }
 
 // X += alpha P + omega S;  R = S - omega T;  <Rt, R>, |R|^2  ->  rho, beta, convergence flags
-template <typename T>
+template <typename T, bool PAIRED>
 __global__ void xr_update_kernel(long nvec, int n, int rev, RedBuf rb, typename V<T>::type* __restrict__ X,
                                  const typename V<T>::type* __restrict__ P, typename V<T>::type* __restrict__ R,
                                  const typename V<T>::type* __restrict__ Tt, const typename V<T>::type* __restrict__ Rt) {
@@ -87,7 +93,7 @@ __global__ void xr_update_kernel(long nvec, int n, int rev, RedBuf rb, typename 
     for (long k = 0; k < cnt; ++k) {
         const long i = i0 + (rev ? cnt - 1 - k : k) * stride;  // rev: sweep from the top, see wd_solve_impl
         T x[2 * NC], p[2 * NC], sv[2 * NC], t[2 * NC], q[2 * NC];
-        to_arr<T>(X[i], x); to_arr<T>(P[i], p); to_arr<T>(R[i], sv); to_arr<T>(Tt[i], t); to_arr<T>(Rt[i], q);
+        to_arr<T, PAIRED>(X[i], x); to_arr<T, PAIRED>(P[i], p); to_arr<T, PAIRED>(R[i], sv); to_arr<T, PAIRED>(Tt[i], t); to_arr<T, PAIRED>(Rt[i], q);
 #pragma unroll
         for (int c = 0; c < NC; ++c) {
             x[2 * c] += (ar * p[2 * c] - ai * p[2 * c + 1]) + (wr * sv[2 * c] - wi * sv[2 * c + 1]);
@@ -99,8 +105,8 @@ __global__ void xr_update_kernel(long nvec, int n, int rev, RedBuf rb, typename 
             s[1] += (double)q[2 * c] * ri - (double)q[2 * c + 1] * rr;
             s[2] += (double)rr * rr + (double)ri * ri;
         }
-        X[i] = from_arr(x);
-        R[i] = from_arr(sv);
+        X[i] = from_arr<PAIRED>(x);
+        R[i] = from_arr<PAIRED>(sv);
     }
     reduce_finalize<3, K_RHO>(s, n, rb);
 }
@@ -132,6 +138,8 @@ __global__ void outer_resid_kernel(long nvec, int n, RedBuf rb, const double2* _
 
 // inner start: b = R_i / |R_i| in fp32 -> r, rt;  x = p = v = 0;  rho = <b, b>.
 // fp64 vec index ((block*12 + k)*RB + o)*n + r, k < 12  <->  fp32 vec index ((block*6 + k/2)*RB + o)*n + r, components 2*(k%2)..
+// PAIRED: the fp32 side is P32 (wd_f2.cuh): vec index ((block*12 + k)*H + p)*n + r = complex k of sites o = p and p + H, H = RB/2.
+template <bool PAIRED>
 __global__ void demote_kernel(long Vh, long RB, int n, RedBuf rb, const double2* __restrict__ R64, float4* __restrict__ r32,
                               float4* __restrict__ rt32, float4* __restrict__ x32, float4* __restrict__ p32,
                               float4* __restrict__ v32) {
@@ -144,8 +152,15 @@ __global__ void demote_kernel(long Vh, long RB, int n, RedBuf rb, const double2*
     const double inv = (frozen || !(sc > 0.0)) ? 0.0 : 1.0 / sc;
     double s[3] = {0.0, 0.0, 0.0};
     for (long i = (long)blockIdx.x * blockDim.x + threadIdx.x; i < nvec; i += stride) {
-        const long c = i / half, rem = i - c * half;
-        const double2 a = R64[(2 * c) * half + rem], b = R64[(2 * c + 1) * half + rem];
+        double2 a, b;
+        if (PAIRED) {   // i = bk * (half/2) + rem, bk = block*12 + k:  lane A at fp64 index bk*half + rem, lane B half/2 further
+            const long bk = i / (half / 2), rem = i - bk * (half / 2);
+            const double2 sa = R64[bk * half + rem], sb = R64[bk * half + half / 2 + rem];
+            a = make_double2(sa.x, sb.x); b = make_double2(sa.y, sb.y);
+        } else {
+            const long c = i / half, rem = i - c * half;
+            a = R64[(2 * c) * half + rem]; b = R64[(2 * c + 1) * half + rem];
+        }
         const float4 f = make_float4((float)(a.x * inv), (float)(a.y * inv), (float)(b.x * inv), (float)(b.y * inv));
         r32[i] = f;
         rt32[i] = f;
@@ -158,6 +173,7 @@ __global__ void demote_kernel(long Vh, long RB, int n, RedBuf rb, const double2*
 }
 
 // X_i += |R_i| E_i  (fp32 -> fp64)
+template <bool PAIRED>
 __global__ void promote_kernel(long Vh, long RB, int n, const double* __restrict__ scal, const float4* __restrict__ e32,
                                double2* __restrict__ X64) {
     const int r = threadIdx.x % n;
@@ -165,12 +181,20 @@ __global__ void promote_kernel(long Vh, long RB, int n, const double* __restrict
     const long nvec = 6 * Vh * n, half = RB * n;  // i / half = block * 6 + c  <->  fp64 chunks 2 (block * 6 + c), + 1
     const double sc = scal[S_OUT_CONV * WD_MAX_RHS + r] != 0.0 ? 0.0 : scal[S_SCALE * WD_MAX_RHS + r];
     for (long i = (long)blockIdx.x * blockDim.x + threadIdx.x; i < nvec; i += stride) {
-        const long c = i / half, rem = i - c * half;
         const float4 f = e32[i];
-        double2 a = X64[(2 * c) * half + rem], b = X64[(2 * c + 1) * half + rem];
-        a.x += sc * f.x; a.y += sc * f.y; b.x += sc * f.z; b.y += sc * f.w;
-        X64[(2 * c) * half + rem] = a;
-        X64[(2 * c + 1) * half + rem] = b;
+        if (PAIRED) {
+            const long bk = i / (half / 2), rem = i - bk * (half / 2);
+            double2 a = X64[bk * half + rem], b = X64[bk * half + half / 2 + rem];
+            a.x += sc * f.x; b.x += sc * f.y; a.y += sc * f.z; b.y += sc * f.w;
+            X64[bk * half + rem] = a;
+            X64[bk * half + half / 2 + rem] = b;
+        } else {
+            const long c = i / half, rem = i - c * half;
+            double2 a = X64[(2 * c) * half + rem], b = X64[(2 * c + 1) * half + rem];
+            a.x += sc * f.x; a.y += sc * f.y; b.x += sc * f.z; b.y += sc * f.w;
+            X64[(2 * c) * half + rem] = a;
+            X64[(2 * c + 1) * half + rem] = b;
+        }
     }
 }
 
@@ -231,7 +255,13 @@ int wd_inner_solve_f32(wd_ctx* c, int dag, int n, int recon, int max_inner, cons
     double* hp = c->h_pinned;
     int rc;
     {
-        { wd_prof_scope pr__(c, WD_PROF_BLAS); demote_kernel<<<L32.G, L32.B, 0, st>>>(Vh, (long)c->RB, n, rb, R64, r32, rt32, x32, p32, v32); }
+        // P32 (two sites per thread, packed fp32 instructions: wd_f2.cuh) wherever the z-march kernel serves it
+        const bool paired = c->opt[WD_OPT_PAIRED] != 0 && c->opt[WD_OPT_HOP_IMPL] == 2 && n >= 3 && wd_hop_zm_serves(c, recon, n, 2);
+        {
+            wd_prof_scope pr__(c, WD_PROF_BLAS);
+            if (paired) demote_kernel<true><<<L32.G, L32.B, 0, st>>>(Vh, (long)c->RB, n, rb, R64, r32, rt32, x32, p32, v32);
+            else demote_kernel<false><<<L32.G, L32.B, 0, st>>>(Vh, (long)c->RB, n, rb, R64, r32, rt32, x32, p32, v32);
+        }
         WD_LAUNCH_CHECK(c);
         // One iteration = 3 BLAS1 kernels + 4 hops; sigma and omega are reduced inside the even-parity hops.
         // Kernels turn into no-ops once the device-side done flag is set, so iterations are enqueued
@@ -243,8 +273,13 @@ int wd_inner_solve_f32(wd_ctx* c, int dag, int n, int recon, int max_inner, cons
         auto sweep = [&]() { sweep_dir ^= c->opt[WD_OPT_ALTERNATE_SWEEP] ? 1 : 0; return sweep_dir; };
         wd_hop_ops o;
         o.check_done = true;
+        o.storage = paired ? 2 : 0;
         for (int it = 1; it <= max_inner; ++it) {
-            { wd_prof_scope pr__(c, WD_PROF_BLAS); p_update_kernel<float><<<L32.G, L32.B, 0, st>>>(nv32, n, sweep(), c->d_scal, r32, p32, v32); }
+            {
+                wd_prof_scope pr__(c, WD_PROF_BLAS);
+                if (paired) p_update_kernel<float, true><<<L32.G, L32.B, 0, st>>>(nv32, n, sweep(), c->d_scal, r32, p32, v32);
+                else p_update_kernel<float, false><<<L32.G, L32.B, 0, st>>>(nv32, n, sweep(), c->d_scal, r32, p32, v32);
+            }
             WD_LAUNCH_CHECK(c);
             // v = Ahat p, sigma = <rt, v> -> alpha
             o.in = p32; o.out = tmp32; o.in2 = nullptr; o.in3 = nullptr; o.a = 0.0; o.b = 1.0; o.epi = 0;
@@ -255,7 +290,11 @@ int wd_inner_solve_f32(wd_ctx* c, int dag, int n, int recon, int max_inner, cons
             o.rev = sweep();
             rc = wd_hop_launch_ex(c, WD_F32, recon, dag, n, 0, o);
             if (rc) return rc;
-            { wd_prof_scope pr__(c, WD_PROF_BLAS); s_update_kernel<float><<<L32.G, L32.B, 0, st>>>(nv32, n, sweep(), c->d_scal, r32, v32); }
+            {
+                wd_prof_scope pr__(c, WD_PROF_BLAS);
+                if (paired) s_update_kernel<float, true><<<L32.G, L32.B, 0, st>>>(nv32, n, sweep(), c->d_scal, r32, v32);
+                else s_update_kernel<float, false><<<L32.G, L32.B, 0, st>>>(nv32, n, sweep(), c->d_scal, r32, v32);
+            }
             WD_LAUNCH_CHECK(c);
             // t = Ahat s, <t, s>, <t, t> -> omega
             o.in = r32; o.out = tmp32; o.in2 = nullptr; o.in3 = nullptr; o.a = 0.0; o.b = 1.0; o.epi = 0;
@@ -266,7 +305,11 @@ int wd_inner_solve_f32(wd_ctx* c, int dag, int n, int recon, int max_inner, cons
             o.rev = sweep();
             rc = wd_hop_launch_ex(c, WD_F32, recon, dag, n, 0, o);
             if (rc) return rc;
-            { wd_prof_scope pr__(c, WD_PROF_BLAS); xr_update_kernel<float><<<L32.G, L32.B, 0, st>>>(nv32, n, sweep(), rb, x32, p32, r32, t32, rt32); }
+            {
+                wd_prof_scope pr__(c, WD_PROF_BLAS);
+                if (paired) xr_update_kernel<float, true><<<L32.G, L32.B, 0, st>>>(nv32, n, sweep(), rb, x32, p32, r32, t32, rt32);
+                else xr_update_kernel<float, false><<<L32.G, L32.B, 0, st>>>(nv32, n, sweep(), rb, x32, p32, r32, t32, rt32);
+            }
             WD_LAUNCH_CHECK(c);
             if (it % poll_every == 0 || it == max_inner) {
                 WD_CUDA_CHECK(c, cudaMemcpyAsync(hp + G_COUNT, c->d_scal + G_DONE, sizeof(double), cudaMemcpyDeviceToHost, st));
@@ -274,7 +317,11 @@ int wd_inner_solve_f32(wd_ctx* c, int dag, int n, int recon, int max_inner, cons
                 if (hp[G_COUNT] != 0.0) break;
             }
         }
-        { wd_prof_scope pr__(c, WD_PROF_BLAS); promote_kernel<<<L32.G, L32.B, 0, st>>>(Vh, (long)c->RB, n, c->d_scal, x32, Xacc); }
+        {
+            wd_prof_scope pr__(c, WD_PROF_BLAS);
+            if (paired) promote_kernel<true><<<L32.G, L32.B, 0, st>>>(Vh, (long)c->RB, n, c->d_scal, x32, Xacc);
+            else promote_kernel<false><<<L32.G, L32.B, 0, st>>>(Vh, (long)c->RB, n, c->d_scal, x32, Xacc);
+        }
         WD_LAUNCH_CHECK(c);
     }
     return WD_OK;

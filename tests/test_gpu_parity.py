@@ -287,6 +287,69 @@ def test_staged_hop_kernel_matches_oracle_and_register_kernel(dims, bc, n_rhs):
     ctx.close()
 
 
+PAIRED_CASES = [
+    # dims, bc, n_rhs: row-major layout (Lx/2 even); Lx/4 = 1 (a pair is the whole half row), 2, 3; n_rhs odd and even
+    ((4, 4, 4, 4), wi.BC_SF, 5),
+    ((8, 4, 6, 4), wi.BC_PERIODIC, 3),
+    ((12, 8, 4, 6), wi.BC_SF, 5),
+    ((8, 8, 8, 8), wi.BC_SF, 16),
+    ((8, 6, 4, 4), wi.BC_SF, 7),
+    ((4, 10, 2, 6), wi.BC_PERIODIC, 4),
+    ((16, 4, 4, 4), wi.BC_PERIODIC, 3),
+]
+
+
+@pytest.mark.parametrize("dims,bc,n_rhs", PAIRED_CASES)
+def test_paired_fp32_form_matches_oracle_and_plain_fp32(dims, bc, n_rhs):
+    """WD_F32P (two sites per thread, packed fp32 instructions): pack/unpack round trip, D and D^dag apply and the
+    single-parity hop against the oracle at the fp32 tolerance, and bit for bit the plain fp32 kernels' result (each
+    lane runs the scalar kernel's operations in the same order)."""
+    pkg = _wd()
+    kappa = 0.13
+    U = wi.gauge_field(dims, 0.4, 7, bc)
+    psi = wi.spinor_field(dims, n_rhs, 11, bc)
+    ctx = make_ctx(dims, kappa, bc, n_rhs, U)
+    natp = ctx.pack(dev(psi), pkg.F32P)
+    nat = ctx.pack(dev(psi), pkg.F32)
+    assert torch.equal(ctx.unpack(natp, n_rhs, pkg.F32P), ctx.unpack(nat, n_rhs, pkg.F32))
+    assert not torch.equal(natp, nat)
+    for op in (0, 1):
+        ref32 = orc.apply(dims, kappa, bc, op, U.astype(np.float32).astype(np.float64),
+                          psi.astype(np.float32).astype(np.float64))
+        for recon in (pkg.LINK18, pkg.LINK12):
+            a = ctx.unpack(ctx.apply(op, nat, n_rhs, pkg.F32, recon), n_rhs, pkg.F32)
+            b = ctx.unpack(ctx.apply(op, natp, n_rhs, pkg.F32P, recon), n_rhs, pkg.F32P)
+            assert torch.equal(a, b), (op, recon)
+            assert rel_per_rhs(b.cpu().numpy(), ref32).max() < 1e-5, (op, recon)
+    half = nat.numel() // 2
+    for par in (0, 1):
+        h = ctx.hop(pkg.OP_D, nat[(1 - par) * half:(2 - par) * half], n_rhs, par, pkg.F32, pkg.LINK18)
+        hp = ctx.hop(pkg.OP_D, natp[(1 - par) * half:(2 - par) * half], n_rhs, par, pkg.F32P, pkg.LINK18)
+        full, fullp = torch.zeros_like(nat), torch.zeros_like(natp)
+        full[par * half:(par + 1) * half] = h
+        fullp[par * half:(par + 1) * half] = hp
+        assert torch.equal(ctx.unpack(full, n_rhs, pkg.F32), ctx.unpack(fullp, n_rhs, pkg.F32P)), par
+    ctx.close()
+
+
+@pytest.mark.parametrize("paired", [0, 1])
+def test_solver_with_and_without_the_paired_form(paired):
+    """WD_OPT_PAIRED switches the inner solver between WD_F32P and WD_F32: the same X to solver accuracy."""
+    pkg = _wd()
+    cfg, U, Phi = wi.make_config(1)
+    dims, kappa, bc, n = cfg["dims"], cfg["kappa"], cfg["bc"], cfg["n_rhs"]
+    Xr, rr, _, rc = orc.solve(dims, kappa, bc, 0, U, Phi, tol=1e-14)
+    assert rc == 0 and rr.max() < 1e-13
+    ctx = make_ctx(dims, kappa, bc, n, U)
+    assert ctx.get_option(pkg.OPT_PAIRED) == 0
+    ctx.set_option(pkg.OPT_PAIRED, paired)
+    for recon in (pkg.LINK18, pkg.LINK12):
+        X, ix = ctx.solve_block(pkg.OP_D, ctx.pack(dev(Phi)), n, tol=1e-12, recon=recon)
+        assert ix["converged"] and max(ix["relres"]) < 1e-12
+        assert rel_per_rhs(ctx.unpack(X, n).cpu().numpy(), Xr).max() < 1e-9
+    ctx.close()
+
+
 @pytest.mark.parametrize("impl", [0, 1, 2])
 @pytest.mark.parametrize("recon", [0, 1])
 def test_solve_and_force_with_either_hop_kernel(impl, recon):
