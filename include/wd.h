@@ -133,10 +133,13 @@ int wd_site_order(wd_ctx* ctx, int order, const int tile[4]);
  *       up to the summation order of the inner products.  (Measured at 24^4, n_rhs = 5: 64 us against 59 us per hop --
  *       the hop is bound by shared-memory bandwidth, which pairing does not change, and has half the warps to hide
  *       latency with.)
+ *   WD_OPT_GRAPH        1 (default): the fp32 inner solver replays each block of WD_OPT_POLL_EVERY iterations (7 kernels
+ *       each, plus the read-back of the convergence flag) as one CUDA graph, captured the second time a (operator, n_rhs,
+ *       link form) combination is solved; 0: plain stream launches.  Identical results; off while wd_profile is on.
  * Errors: WD_EINVAL (null, unknown key, value out of range). */
 enum { WD_OPT_HOP32_SITES = 0, WD_OPT_HOP64_SITES = 1, WD_OPT_HOP32_REGS = 2, WD_OPT_HOP64_REGS = 3,
        WD_OPT_POLL_EVERY = 4, WD_OPT_HOP_IMPL = 5, WD_OPT_ALTERNATE_SWEEP = 6, WD_OPT_HOP_ROWS = 7, WD_OPT_SOLVER = 8,
-       WD_OPT_PAIRED = 9, WD_OPT_N = 10 };
+       WD_OPT_PAIRED = 9, WD_OPT_GRAPH = 10, WD_OPT_N = 11 };
 /* values of WD_OPT_SOLVER */
 enum { WD_SOLVER_DC_F32 = 0, WD_SOLVER_RELIABLE_H16 = 1, WD_SOLVER_GL_FLEX = 2, WD_SOLVER_GL_F64 = 3, WD_SOLVER_BL_F64 = 4,
        WD_SOLVER_N = 5 };

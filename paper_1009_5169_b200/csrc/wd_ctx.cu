@@ -100,6 +100,12 @@ bool bad_n(const wd_ctx* c, int n) { return n < 1 || n > c->max_rhs; }
 
 }  // namespace
 
+void wd_graphs_clear(wd_ctx* c) {
+    for (wd_graph_entry& g : c->graphs)
+        if (g.exec) cudaGraphExecDestroy(g.exec);
+    c->graphs.clear();
+}
+
 extern "C" {
 
 const char* wd_version(void) { return "wd 0.1 (sm_100a)"; }
@@ -162,6 +168,8 @@ int wd_create(wd_ctx** out, const int dims[4], double kappa, int time_bc, int ma
     c->opt[WD_OPT_HOP_IMPL] = 2;
     c->opt[WD_OPT_ALTERNATE_SWEEP] = 1;
     c->opt[WD_OPT_PAIRED] = 0;
+    c->opt[WD_OPT_GRAPH] = 1;
+    c->cap_stream = nullptr;
     c->prof_on = false;
     c->prof_used = 0;
     c->h_pinned = nullptr;
@@ -183,6 +191,8 @@ int wd_create(wd_ctx** out, const int dims[4], double kappa, int time_bc, int ma
 
 int wd_destroy(wd_ctx* ctx) {
     if (!ctx) return WD_EINVAL;
+    wd_graphs_clear(ctx);
+    if (ctx->cap_stream) cudaStreamDestroy(ctx->cap_stream);
     if (ctx->h_pinned) cudaFreeHost(ctx->h_pinned);
     for (cudaEvent_t e : ctx->prof_ev) cudaEventDestroy(e);
     delete ctx;
@@ -205,6 +215,7 @@ int wd_set_option(wd_ctx* ctx, int key, int value) {
             break;
         case WD_OPT_ALTERNATE_SWEEP:
         case WD_OPT_PAIRED:
+        case WD_OPT_GRAPH:
             if (value != 0 && value != 1) return wd_fail(ctx, WD_EINVAL, "this option is 0 or 1");
             break;
         case WD_OPT_HOP_ROWS:
@@ -220,6 +231,7 @@ int wd_set_option(wd_ctx* ctx, int key, int value) {
             return wd_fail(ctx, WD_EINVAL, "unknown option");
     }
     ctx->opt[key] = value;
+    wd_graphs_clear(ctx);   // captured launch shapes may depend on any of them
     return WD_OK;
 }
 
@@ -281,6 +293,7 @@ int wd_set_workspace(wd_ctx* ctx, void* ws_dev, size_t bytes) {
     if (((uintptr_t)ws_dev) & 255) return wd_fail(ctx, WD_EINVAL, "workspace must be 256-byte aligned");
     const WsMap m = ws_map(ctx);
     if (bytes < m.total) return wd_fail(ctx, WD_EINVAL, "workspace too small");
+    wd_graphs_clear(ctx);
     char* w = (char*)ws_dev;
     ctx->ws = w;
     ctx->ws_bytes = bytes;

@@ -53,11 +53,15 @@ __device__ __forceinline__ void st_spinor(ulonglong2* __restrict__ row, uint32_t
 #pragma unroll
     for (int k = 0; k < 12; ++k) row[k * cs + e] = to_vec(psi[k]);
 }
-// link of pair p of a P32 link row; H pairs per complex.  RECON == 12: row 3 rebuilt as in wd_su3.cuh rebuild_row3.
+// link of pair p of a P32 link row; H pairs per complex: the RECON / 2 stored complex numbers
 template <int RECON>
-__device__ __forceinline__ void ld_link(const ulonglong2* __restrict__ row, uint32_t H, uint32_t p, cx2 (&u)[9]) {
+__device__ __forceinline__ void ld_link_raw(const ulonglong2* __restrict__ row, uint32_t H, uint32_t p, cx2 (&u)[9]) {
 #pragma unroll
     for (int c = 0; c < RECON / 2; ++c) u[c] = from_vec(row[c * H + p]);
+}
+// RECON == 12: row 3 rebuilt as in wd_su3.cuh rebuild_row3
+template <int RECON>
+__device__ __forceinline__ void finish_link(cx2 (&u)[9]) {
     if (RECON == 12) {
 #pragma unroll
         for (int k = 0; k < 3; ++k) {
@@ -74,6 +78,11 @@ __device__ __forceinline__ void ld_link(const ulonglong2* __restrict__ row, uint
             u[6 + k].im = im;
         }
     }
+}
+template <int RECON>
+__device__ __forceinline__ void ld_link(const ulonglong2* __restrict__ row, uint32_t H, uint32_t p, cx2 (&u)[9]) {
+    ld_link_raw<RECON>(row, H, p, u);
+    finish_link<RECON>(u);
 }
 
 // ---- spin projection (1 - SIGMA gamma_MU) psi -> hs[0..2] = h0, hs[3..5] = h1 (wd_su3.cuh project, per lane) ----

@@ -129,13 +129,26 @@ __device__ __forceinline__ void dir_smem(const typename Vec<T>::type* sp, uint32
 }
 
 // ---- the same for two sites per thread (ST = 2: P32 operands, wd_f2.cuh) ---------------------------------------
+// The operands of one direction: the neighbour pair's spinor and the link, as loaded (12-real links before the rebuild).
+// The consumers keep TWO of these: the loads of direction d + 1 are issued before the arithmetic of direction d, so that
+// with six consumer warps per SM the shared-memory pipe and the FMA pipe work at the same time.
+struct PairOps {
+    wdp::cx2 psi[12];
+    wdp::cx2 u[9];
+};
 // sp: spinor row in shared memory, cs = H * n elements per complex, e = element of the neighbour pair; L: link row,
-// lp = pair whose link is used.  SWAP (x hops only): the neighbour pair has its lanes exchanged -- the forward hop
-// exchanges the projected half spinor (the link is the output pair's own), the backward hop multiplies in the
-// neighbour's lane order (its link sits with it) and exchanges the result.
+// lp = pair whose link is used.
+template <int RECON>
+__device__ __forceinline__ void pair_load(PairOps& o, const ulonglong2* sp, uint32_t cs, uint32_t e, const ulonglong2* L, uint32_t H, uint32_t lp) {
+    if (WD_ZM_ABLATE == 1) return;
+    wdp::ld_spinor(sp, cs, e, o.psi);
+    wdp::ld_link_raw<RECON>(L, H, lp, o.u);
+}
+// SWAP (x hops only): the neighbour pair has its lanes exchanged -- the forward hop exchanges the projected half spinor
+// (the link is the output pair's own), the backward hop multiplies in the neighbour's lane order (its link sits with it)
+// and exchanges the result.
 template <int RECON, int MU, bool FWD, bool DAG, bool FIRST = false, bool SWAP = false>
-__device__ __forceinline__ void dir_pair(const ulonglong2* sp, uint32_t cs, uint32_t e, const ulonglong2* L, uint32_t H, uint32_t lp,
-                                         wdp::cx2 (&acc)[12], bool swp = false) {
+__device__ __forceinline__ void pair_compute(PairOps& o, wdp::cx2 (&acc)[12], bool swp = false) {
     if (WD_ZM_ABLATE == 1) {
         if (FIRST) {
 #pragma unroll
@@ -144,15 +157,14 @@ __device__ __forceinline__ void dir_pair(const ulonglong2* sp, uint32_t cs, uint
         return;
     }
     constexpr int SIGMA = (FWD ? 1 : -1) * (DAG ? -1 : 1);
-    wdp::cx2 psi[12], hs[6], chi[6], u[9];
-    wdp::ld_spinor(sp, cs, e, psi);
-    wdp::ld_link<RECON>(L, H, lp, u);
-    wdp::project<MU, SIGMA>(psi, hs);
+    wdp::cx2 hs[6], chi[6];
+    wdp::finish_link<RECON>(o.u);
+    wdp::project<MU, SIGMA>(o.psi, hs);
     if (SWAP && FWD) {
 #pragma unroll
         for (int q = 0; q < 6; ++q) { hs[q].re = wdp::swap_if(swp, hs[q].re); hs[q].im = wdp::swap_if(swp, hs[q].im); }
     }
-    wdp::su3_mul<!FWD>(u, hs, chi);
+    wdp::su3_mul<!FWD>(o.u, hs, chi);
     if (SWAP && !FWD) {
 #pragma unroll
         for (int q = 0; q < 6; ++q) { chi[q].re = wdp::swap_if(swp, chi[q].re); chi[q].im = wdp::swap_if(swp, chi[q].im); }
@@ -200,7 +212,78 @@ __global__ void __launch_bounds__(MAXT, 1) hop_zm_kernel(const ZmArgs<T> A) {
     const uint32_t s_first = blockIdx.x * A.chunk;   // < steps: the grid has at most ceil(steps / chunk) CTAs
     [[maybe_unused]] double dsum[3] = {0.0, 0.0, 0.0};
 
-    if (warp >= ncw) {
+    if (ST == 2 && warp >= ncw) {
+        // ================= producer warps, P32 form: TWO warps (the consumers, two sites per thread with the next
+        // direction's operands in flight, need ~250 registers: 256 threads per CTA).  A thread can start a bulk copy
+        // only every ~280 ns, so every copy of a step has a lane of its own; the waits follow the order in which the
+        // consumers release the buffers.
+        //   P0: U1 {T+ rows, link t+}, U2 {T- rows, link t-}, U3 {link z-}, window planes      P1: U4, U5
+        const uint32_t role = warp - ncw;
+        const char* in = reinterpret_cast<const char*>(A.in);
+        const char* U = reinterpret_cast<const char*>(A.U);
+        const size_t ublk = (size_t)RECON * A.Vh * sizeof(T);
+        uint32_t issued = 0, a = 0, prev = NO_STEP;
+        for (uint32_t s = s_first, k = 0; s != NO_STEP; prev = s, s = next_step(s, A.chunk, A.steps), ++k) {
+            const uint32_t col = s / A.Lz, z = s - col * A.Lz;
+            const uint32_t yb = col % A.gy, t = A.t0 + col / A.gy, y0 = yb * RG;
+            if (k > 0) a += continues(prev, s, A.Lz) ? 1u : 3u;
+            const uint32_t eph = (k & 1) ^ 1;
+            const uint32_t row0 = y0 + A.Ly * (z + A.Lz * t);
+            if (role == 0) {
+                const uint32_t rtp = y0 + A.Ly * (z + A.Lz * winc(t, A.Lt));
+                const uint32_t rtm = y0 + A.Ly * (z + A.Lz * wdec(t, A.Lt));
+                const uint32_t rzm = y0 + A.Ly * (wdec(z, A.Lz) + A.Lz * t);
+                mbar_wait_relaxed(&empty_u[U_TP], eph);
+                if (lane == 0) mbar_expect_tx(&full_u[U_TP], RG * (rowB + lrowB));
+                __syncwarp();
+                if (lane == 0) bulk_g2s(tp, in + (size_t)rtp * rowB, RG * rowB, &full_u[U_TP]);
+                else if (lane == 1) bulk_g2s(links + (size_t)LK_TP * RG * lrowB, U + (size_t)(6 + A.par) * ublk + (size_t)row0 * lrowB, RG * lrowB, &full_u[U_TP]);
+                mbar_wait_relaxed(&empty_u[U_TM], eph);
+                if (lane == 2) mbar_expect_tx(&full_u[U_TM], RG * (rowB + lrowB));
+                __syncwarp();
+                if (lane == 2) bulk_g2s(tm, in + (size_t)rtm * rowB, RG * rowB, &full_u[U_TM]);
+                else if (lane == 3) bulk_g2s(links + (size_t)LK_TM * RG * lrowB, U + (size_t)(6 + 1 - A.par) * ublk + (size_t)rtm * lrowB, RG * lrowB, &full_u[U_TM]);
+                mbar_wait_relaxed(&empty_u[U_ZM], eph);
+                if (lane == 4) {
+                    mbar_expect_tx(&full_u[U_ZM], RG * lrowB);
+                    bulk_g2s(links + (size_t)LK_ZM * RG * lrowB, U + (size_t)(4 + 1 - A.par) * ublk + (size_t)rzm * lrowB, RG * lrowB, &full_u[U_ZM]);
+                }
+                __syncwarp();
+                while (issued <= a + 2) {
+                    const uint32_t d = issued - a;   // 0, 1, 2 = z-1, z, z+1
+                    const uint32_t zz = d == 0 ? wdec(z, A.Lz) : (d == 1 ? z : winc(z, A.Lz));
+                    const uint32_t w = issued % 3, use = issued / 3;
+                    mbar_wait_relaxed(&empty_w[w], (use & 1) ^ 1);
+                    if (lane == 5 + d) {
+                        mbar_expect_tx(&full_w[w], RG * rowB);
+                        bulk_g2s(planes + (size_t)w * RG * rowB, in + (size_t)(y0 + A.Ly * (zz + A.Lz * t)) * rowB, RG * rowB, &full_w[w]);
+                    }
+                    __syncwarp();
+                    ++issued;
+                }
+            } else {
+                const bool lo = y0 == 0;
+                const uint32_t zt = A.Ly * (z + A.Lz * t);
+                const uint32_t rm = (lo ? A.Ly - 1 : y0 - 1) + zt, rp = (y0 + RG == A.Ly ? 0 : y0 + RG) + zt;
+                mbar_wait_relaxed(&empty_u[U_Y], eph);
+                if (lane == 0) mbar_expect_tx(&full_u[U_Y], 2 * rowB + 2 * RG * lrowB);
+                __syncwarp();
+                char* lym = links + (size_t)LK_YM * RG * lrowB;
+                const char* uym = U + (size_t)(2 + 1 - A.par) * ublk;
+                if (lane == 0) bulk_g2s(halo, in + (size_t)rm * rowB, rowB, &full_u[U_Y]);
+                else if (lane == 1) bulk_g2s(halo + rowB, in + (size_t)rp * rowB, rowB, &full_u[U_Y]);
+                else if (lane == 2) bulk_g2s(lym, uym + (size_t)rm * lrowB, (lo ? 1u : RG) * lrowB, &full_u[U_Y]);
+                else if (lane == 3 && lo && RG > 1) bulk_g2s(lym + lrowB, uym + (size_t)row0 * lrowB, (RG - 1) * lrowB, &full_u[U_Y]);
+                else if (lane == 4) bulk_g2s(links + (size_t)LK_YP * RG * lrowB, U + (size_t)(2 + A.par) * ublk + (size_t)row0 * lrowB, RG * lrowB, &full_u[U_Y]);
+                mbar_wait_relaxed(&empty_u[U_XZ], eph);
+                if (lane == 5) mbar_expect_tx(&full_u[U_XZ], 3 * RG * lrowB);
+                __syncwarp();
+                if (lane == 5) bulk_g2s(links + (size_t)LK_XM * RG * lrowB, U + (size_t)(0 + 1 - A.par) * ublk + (size_t)row0 * lrowB, RG * lrowB, &full_u[U_XZ]);
+                else if (lane == 6) bulk_g2s(links + (size_t)LK_XP * RG * lrowB, U + (size_t)(0 + A.par) * ublk + (size_t)row0 * lrowB, RG * lrowB, &full_u[U_XZ]);
+                else if (lane == 7) bulk_g2s(links + (size_t)LK_ZP * RG * lrowB, U + (size_t)(4 + A.par) * ublk + (size_t)row0 * lrowB, RG * lrowB, &full_u[U_XZ]);
+            }
+        }
+    } else if (warp >= ncw) {
         // ================= producer warps ================================================================
         // One thread can start a bulk copy only every ~280 ns (measured: _work/ubench/tma_stream2.cu; the copy engine
         // itself takes 8 issuers in parallel at 85-92 GB/s per SM), and a step needs 13-14 copies, so the units are
@@ -328,46 +411,59 @@ __global__ void __launch_bounds__(MAXT, 1) hop_zm_kernel(const ZmArgs<T> A) {
             const pv* const Pm = Pl + (size_t)wm * planeV + (size_t)j * rowS;
             const pv* const Pc = Pl + (size_t)wc * planeV + (size_t)j * rowS;
             const pv* const Pp = Pl + (size_t)wp * planeV + (size_t)j * rowS;
-            // ---- t+
+            // rows with bb = 1 have their +x neighbour one pair up and their -x neighbour in the same pair; bb = 0 the
+            // other way round.  A step past the half row lands on the pair at the other end, lanes exchanged.
+            const uint32_t bb = (y0 + j + z + t + A.par) & 1;
+            const uint32_t pp = bb ? (p + 1 == H ? 0u : p + 1) : p;
+            const uint32_t pm = bb ? p : (p == 0 ? H - 1 : p - 1);
+            const bool swp_p = bb && p + 1 == H, swp_m = !bb && p == 0;
+            const pv* const ym = j == 0 ? Hl : Pc - rowS;
+            const pv* const yp = j == RG - 1 ? Hl + rowS : Pc + rowS;
+            PairOps oa, ob;
+            // direction order t+, t-, z-, y-, y+, x-, x+, z+ (that of every hop kernel); loads one direction ahead
             mbar_wait(&full_u[U_TP], ph);
-            if (active) dir_pair<RECON, 3, true, DAG, true>(Tp, cs, e0, Lk + LK_TP * lblk, H, p, acc);
+            if (active) pair_load<RECON>(oa, Tp, cs, e0, Lk + LK_TP * lblk, H, p);
+            mbar_wait(&full_u[U_TM], ph);
+            if (active) {
+                pair_load<RECON>(ob, Tm, cs, e0, Lk + LK_TM * lblk, H, p);
+                pair_compute<RECON, 3, true, DAG, true>(oa, acc);
+            }
             __syncwarp();
             if (lane == 0) mbar_arrive(&empty_u[U_TP]);
-            // ---- t-
-            mbar_wait(&full_u[U_TM], ph);
-            if (active) dir_pair<RECON, 3, false, DAG>(Tm, cs, e0, Lk + LK_TM * lblk, H, p, acc);
-            __syncwarp();
-            if (lane == 0) mbar_arrive(&empty_u[U_TM]);
-            // ---- z-
             mbar_wait(&full_u[U_ZM], ph);
             mbar_wait(&full_w[wm], (a / 3) & 1);
-            if (active) dir_pair<RECON, 2, false, DAG>(Pm, cs, e0, Lk + LK_ZM * lblk, H, p, acc);
+            if (active) {
+                pair_load<RECON>(oa, Pm, cs, e0, Lk + LK_ZM * lblk, H, p);
+                pair_compute<RECON, 3, false, DAG>(ob, acc);
+            }
             __syncwarp();
-            if (lane == 0) { mbar_arrive(&empty_u[U_ZM]); mbar_arrive(&empty_w[wm]); }
-            // ---- y-, y+
+            if (lane == 0) mbar_arrive(&empty_u[U_TM]);
             mbar_wait(&full_u[U_Y], ph);
             mbar_wait(&full_w[wc], ((a + 1) / 3) & 1);
             if (active) {
-                const pv* ym = j == 0 ? Hl : Pc - rowS;
-                const pv* yp = j == RG - 1 ? Hl + rowS : Pc + rowS;
-                dir_pair<RECON, 1, false, DAG>(ym, cs, e0, Lk + LK_YM * lblk, H, p, acc);
-                dir_pair<RECON, 1, true, DAG>(yp, cs, e0, Lk + LK_YP * lblk, H, p, acc);
+                pair_load<RECON>(ob, ym, cs, e0, Lk + LK_YM * lblk, H, p);
+                pair_compute<RECON, 2, false, DAG>(oa, acc);
             }
             __syncwarp();
-            if (lane == 0) mbar_arrive(&empty_u[U_Y]);
-            // ---- x-, x+, z+
+            if (lane == 0) { mbar_arrive(&empty_u[U_ZM]); mbar_arrive(&empty_w[wm]); }
+            if (active) {
+                pair_load<RECON>(oa, yp, cs, e0, Lk + LK_YP * lblk, H, p);
+                pair_compute<RECON, 1, false, DAG>(ob, acc);
+            }
             mbar_wait(&full_u[U_XZ], ph);
             mbar_wait(&full_w[wp], ((a + 2) / 3) & 1);
             if (active) {
-                // rows with bb = 1 have their +x neighbour one pair up and their -x neighbour in the same pair; bb = 0
-                // the other way round.  A step past the half row lands on the pair at the other end, lanes exchanged.
-                const uint32_t bb = (y0 + j + z + t + A.par) & 1;
-                const uint32_t pp = bb ? (p + 1 == H ? 0u : p + 1) : p;
-                const uint32_t pm = bb ? p : (p == 0 ? H - 1 : p - 1);
-                const bool swp_p = bb && p + 1 == H, swp_m = !bb && p == 0;
-                dir_pair<RECON, 0, false, DAG, false, true>(Pc, cs, pm * nr + r, Lk + LK_XM * lblk, H, pm, acc, swp_m);
-                dir_pair<RECON, 0, true, DAG, false, true>(Pc, cs, pp * nr + r, Lk + LK_XP * lblk, H, p, acc, swp_p);
-                dir_pair<RECON, 2, true, DAG>(Pp, cs, e0, Lk + LK_ZP * lblk, H, p, acc);
+                pair_load<RECON>(ob, Pc, cs, pm * nr + r, Lk + LK_XM * lblk, H, pm);
+                pair_compute<RECON, 1, true, DAG>(oa, acc);
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&empty_u[U_Y]);
+            if (active) {
+                pair_load<RECON>(oa, Pc, cs, pp * nr + r, Lk + LK_XP * lblk, H, p);
+                pair_compute<RECON, 0, false, DAG, false, true>(ob, acc, swp_m);
+                pair_load<RECON>(ob, Pp, cs, e0, Lk + LK_ZP * lblk, H, p);
+                pair_compute<RECON, 0, true, DAG, false, true>(oa, acc, swp_p);
+                pair_compute<RECON, 2, true, DAG>(ob, acc);
             }
             __syncwarp();
             if (lane == 0) {
@@ -593,14 +689,15 @@ bool pick_shape(const wd_ctx* c, int n, int max_threads, Shape* sh) {
         if (Ly % RG || RG > cap) continue;
         const uint32_t S = RG * Lxh;
         const uint32_t cthreads = (((ST == 2 ? S / 2 : S) * n + 31) / 32) * 32;   // ST = 2: one thread per site pair
-        if ((int)cthreads + 128 > max_threads) continue;
+        const uint32_t pthreads = ST == 2 ? 64 : 128;   // producer warps: two in the P32 form, else four
+        if ((int)(cthreads + pthreads) > max_threads) continue;
         const size_t rowB = ST == 1 ? (size_t)wdh::h16_row_vecs(Lxh * n) * 16 : (size_t)Lxh * n * 16 * Vec<T>::NCH;
         const size_t lrowB = (size_t)Lxh * RECON * sizeof(T);
         const size_t smem = 128 + (5 * (size_t)RG + 2) * rowB + 8 * (size_t)RG * lrowB;
         if (smem > kSmemMax) continue;
         // the epilogue's reduction scratch (3 sums per consumer thread + totals) reuses the staging area
         if ((size_t)(3 * S * n + 3 * WD_MAX_RHS + 2) * sizeof(double) > smem - 128) continue;
-        sh->RG = RG; sh->S = S; sh->threads = cthreads + 128; sh->smem = smem;
+        sh->RG = RG; sh->S = S; sh->threads = cthreads + pthreads; sh->smem = smem;
         return true;
     }
     return false;
@@ -685,7 +782,7 @@ bool wd_hop_zm_serves(const wd_ctx* c, int recon, int n, int storage) {
     Shape sh;
     if (storage == 2) {
         if (!c->paired_ok) return false;
-        return recon == WD_LINK18 ? pick_shape<float, 18, 2>(c, n, 320, &sh) : pick_shape<float, 12, 2>(c, n, 320, &sh);
+        return recon == WD_LINK18 ? pick_shape<float, 18, 2>(c, n, 256, &sh) : pick_shape<float, 12, 2>(c, n, 256, &sh);
     }
     if (storage == 1) {
         if (((c->L[0] / 2) * n) % 4 != 0) return false;
@@ -703,10 +800,10 @@ int wd_hop_zm_launch(wd_ctx* c, int prec, int recon, int dag, int n, int par, co
         if (recon == WD_LINK18) return launch_zm<float, 18, 512, 1>(c, dag, n, par, o, c->d_U32[0]);
         return launch_zm<float, 12, 512, 1>(c, dag, n, par, o, c->d_U32[1]);
     }
-    if (o.storage == 2) {   // P32: two sites per thread (wd_f2.cuh); 320 threads leave the consumers ~200 registers
+    if (o.storage == 2) {   // P32: two sites per thread (wd_f2.cuh); 256 threads leave the consumers 255 registers
         if (!c->paired_ok) return 1;
-        if (recon == WD_LINK18) return launch_zm<float, 18, 320, 2>(c, dag, n, par, o, c->d_U32P[0]);
-        return launch_zm<float, 12, 320, 2>(c, dag, n, par, o, c->d_U32P[1]);
+        if (recon == WD_LINK18) return launch_zm<float, 18, 256, 2>(c, dag, n, par, o, c->d_U32P[0]);
+        return launch_zm<float, 12, 256, 2>(c, dag, n, par, o, c->d_U32P[1]);
     }
     if (recon == WD_LINK18) return launch_zm<float, 18, 512, 0>(c, dag, n, par, o, c->d_U32[0]);
     return launch_zm<float, 12, 512, 0>(c, dag, n, par, o, c->d_U32[1]);

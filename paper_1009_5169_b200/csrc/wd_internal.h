@@ -15,6 +15,13 @@
 // Bit 31 of nbr[.][0] marks a site that is not dynamical (SF: the stored t=0 slice).
 #define WD_SITE_FROZEN 0x80000000u
 
+// A block of inner-solver iterations captured once as a CUDA graph and replayed (wd_solve.cu).
+struct wd_graph_entry {
+    unsigned long long key;
+    cudaGraphExec_t exec;   // null: the block has run once in stream order (function attributes are set), not yet captured
+    long long launches;     // kernel launches one replay stands for
+};
+
 struct wd_ctx {
     int L[4];
     long V, Vh;
@@ -61,6 +68,10 @@ struct wd_ctx {
     size_t solver_bytes;
 
     int opt[WD_OPT_N];  // tunables (wd_set_option)
+
+    // CUDA graphs of the inner solver's iteration blocks; dropped whenever an option or the workspace changes
+    std::vector<wd_graph_entry> graphs;
+    cudaStream_t cap_stream;   // the library's own stream to capture on (the caller's may be the legacy default stream)
 
     long long launches;
     std::string err;
@@ -168,6 +179,9 @@ int wd_hop_zm_launch(wd_ctx* c, int prec, int recon, int dag, int n, int par, co
 bool wd_hop_zm_serves(const wd_ctx* c, int recon, int n, int storage);
 int wd_hop_launch(wd_ctx* c, int prec, int recon, int dag, int n, int par, const void* in, void* out,
                   const void* in2, double a, double b);
+
+// wd_ctx.cu
+void wd_graphs_clear(wd_ctx* c);
 
 // wd_layout.cu
 int wd_layout_gauge(wd_ctx* c, const double* U);

@@ -411,6 +411,35 @@ def test_launch_options_change_speed_only():
     ctx.close()
 
 
+@pytest.mark.parametrize("poll", [1, 3, 4])
+def test_graph_replay_of_iteration_blocks_changes_nothing(poll):
+    """WD_OPT_GRAPH: blocks of WD_OPT_POLL_EVERY inner iterations replayed as a CUDA graph (captured at the second
+    sight of an (operator, n_rhs, link form, sweep phase) combination) give bit for bit the stream-order X, for even and
+    odd block lengths (an odd block flips the sweep direction the next block starts with: two graphs), D and D^dag,
+    with the launch counter still counting every kernel."""
+    pkg = _wd()
+    cfg, U, Phi = wi.make_config(1)
+    dims, kappa, bc, n = cfg["dims"], cfg["kappa"], cfg["bc"], cfg["n_rhs"]
+    ctx = make_ctx(dims, kappa, bc, n, U)
+    assert ctx.get_option(pkg.OPT_GRAPH) == 1
+    ctx.set_option(pkg.OPT_POLL_EVERY, poll)
+    P = ctx.pack(dev(Phi))
+    for op in (pkg.OP_D, pkg.OP_DDAG):
+        ctx.set_option(pkg.OPT_GRAPH, 0)
+        l0 = ctx.launch_count()
+        X0, i0 = ctx.solve_block(op, P, n, tol=1e-12)
+        l_plain = ctx.launch_count() - l0
+        X0 = X0.clone()
+        ctx.set_option(pkg.OPT_GRAPH, 1)
+        for rep in range(3):   # first solve: mostly stream order + capture; later ones replay
+            l0 = ctx.launch_count()
+            X1, i1 = ctx.solve_block(op, P, n, tol=1e-12)
+            assert ctx.launch_count() - l0 == l_plain
+            assert torch.equal(X0, X1), (op, rep)
+            assert i1["inner_iters_total"] == i0["inner_iters_total"] and i1["converged"]
+    ctx.close()
+
+
 @pytest.mark.parametrize("n_rhs", [8, 12, 16])
 def test_register_kernel_solve_for_every_cta_shape(n_rhs):
     """The register kernel's fused <rt,v> / <t,s>,<t,t> reductions (block partials + finalize kernel) for large
