@@ -51,6 +51,7 @@ def parse_args():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-baseline-full", action="store_true", help="time the oracle on the WHOLE workload (minutes)")
     ap.add_argument("--no-hop-sweep", action="store_true")
+    ap.add_argument("--hop-only", action="store_true", help="only the standalone hop table (wd_hop back to back), one JSON line")
     ap.add_argument("--no-config2", action="store_true", help="skip the configs[2] (12^4) force-evaluation time")
     return ap.parse_args()
 
@@ -258,19 +259,25 @@ def hop_sweep(pkg, ctx, torch, n, peak_gbs, reps=50, only=None, interior=1.0):
     on the launching stream.  Fields rotate through enough copies to exceed 2x L2 (L2-cold)."""
     res = {}
     Vh = ctx.V // 2
-    for prec, pname, s in ((pkg.F32, "f32", 4), (pkg.F64, "f64", 8)):
+    precs = [(pkg.F32, "f32", 4), (pkg.F64, "f64", 8)]
+    if ctx.native_numel(pkg.F32P, n) > 0:
+        precs.insert(1, (pkg.F32P, "f32p", 4))   # two sites per thread, packed fp32 instructions (wd.h WD_F32P)
+    for prec, pname, s in precs:
         if only and only[0] != pname:
             continue
         half = ctx.native_numel(prec, n) // 2
-        dt = torch.float32 if prec == pkg.F32 else torch.float64
+        dt = torch.float64 if prec == pkg.F64 else torch.float32
         nbuf = max(2, int(2 * 130e6 / (half * s)) + 1)
         bufs = [torch.randn(half, dtype=dt, device=ctx.device) for _ in range(nbuf)]
         out = [torch.empty(half, dtype=dt, device=ctx.device) for _ in range(2)]
         for recon, R in ((pkg.LINK18, 18), (pkg.LINK12, 12)):
             if only and only[1] != R:
                 continue
-            for i in range(5):
-                ctx.hop(pkg.OP_D, bufs[i % nbuf], n, 0, prec, recon, out=out[i % 2])
+            try:
+                for i in range(5):
+                    ctx.hop(pkg.OP_D, bufs[i % nbuf], n, 0, prec, recon, out=out[i % 2])
+            except pkg.WdError:
+                continue   # WD_F32P: the z-march kernel does not serve this shape
             e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             torch.cuda.synchronize()
             e0.record()
@@ -426,6 +433,13 @@ def run_ours(args):
     if args.hop_impl >= 0:
         ctx.set_option(pkg.OPT_HOP_IMPL, args.hop_impl)
     ctx.set_gauge(torch.from_numpy(U).cuda())
+    if args.hop_only:
+        interior = (dims[3] - 1) / dims[3] if bc == wi.BC_SF else 1.0
+        print(json.dumps({"hop": hop_sweep(pkg, ctx, torch, n, peak_gbs, interior=interior), "workload": workload_name(cfg, n),
+                          "nvcc_defines": os.environ.get("WD_NVCC_DEFINES", ""), "peak_gbs": peak_gbs,
+                          "note": "wd_hop back to back (50 launches per entry, L2-cold rotation), CUDA events"}))
+        ctx.close()
+        return
     Phi_host = torch.from_numpy(Phi).pin_memory()
     P = ctx.pack(Phi_host.cuda())
     X = torch.empty_like(P)
@@ -527,7 +541,7 @@ def run_ours(args):
     kname = (f"hop_zm_kernel<float,{R}>" if impl == 2 else f"hop_tma_kernel<float,{R}>") if staged else f"hop_kernel<float,{R}>"
     # dram__bytes_read.sum + dram__bytes_write.sum per launch from an ncu --set full capture of THIS kernel source: the
     # committed record carries the sha256 of the kernel's source file and is ignored when the source has changed since
-    traffic, traffic_note = None, "no capture on record for this kernel source"
+    traffic, traffic_note, ncu_us = None, "no capture on record for this kernel source", None
     try:
         import hashlib
         tr = json.load(open(os.path.join(ROOT, "profiles", "r02_hop_traffic.json.txt")))
@@ -536,6 +550,7 @@ def run_ours(args):
         if tr.get("kernel") == kname and tr.get("source_sha256") == sha and \
                 tr.get("workload") == workload_name(dict(wi.CONFIGS[args.config]), n):
             traffic, traffic_note = tr["dram_bytes_per_launch"], tr.get("how", "")
+            ncu_us = tr.get("ncu_us_per_launch")
         elif tr.get("source_sha256") != sha:
             traffic_note = "the capture on record is of an older kernel source"
     except Exception:
@@ -546,6 +561,12 @@ def run_ours(args):
                 "peak_source": peak_src, "traffic": traffic, "traffic_note": traffic_note, "bytes_per_launch": hop_bytes,
                 "bytes_counted": f"interior sites only for everything read ((T-1)/T = {interior:.4f}), all sites for the output",
                 "avg_launch_us": round(hop_us, 2), "launches_in_step": hop_cnt,
+                "timing": "CUDA event pairs on the library's stream around the two hop launches of every application of the "
+                          "even/odd operator (one kernel-to-kernel gap inside each pair), CUDA graphs off for that step",
+                # the same four launches timed alone by ncu (gpu__time_duration of the committed full capture; cold caches,
+                # no neighbours on the stream): context for how much of avg_launch_us is gap between dependent kernels
+                "ncu_isolated": None if not ncu_us else {"avg_launch_us": round(sum(ncu_us) / len(ncu_us), 2),
+                                                         "frac": round(hop_bytes / (sum(ncu_us) / len(ncu_us) * 1e-6) * 1e-9 / peak_gbs, 4)},
                 "share_of_step": round(hop_ms / tot_prof, 4) if tot_prof else None,
                 "gflops": round(1320.0 * Vh * n * interior / hop_us * 1e-3, 1) if hop_cnt else None}
     breakdown = {k: {"ms": round(v[0], 3), "launch_groups": v[1]} for k, v in prof.items()}
@@ -555,6 +576,7 @@ def run_ours(args):
         "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
         "data": "synthetic",
         "config": {"workload": workload_name(cfg, n), "inner_links": f"{R}-real fp32", "outer": "fp64 defect correction",
+                   "launch": "inner iterations replayed as CUDA graphs, 4 per graph" if ctx.get_option(pkg.OPT_GRAPH) else "stream order",
                    "tol": TOL, "l2": "no flush: solver working set >> 126 MB L2", "parallelism": f"replicas x{world}"},
         "clocks": clocks,
         "e2e": {"value": e2e_value, "unit": UNIT, "ms_per_step": e2e_ms / args.steps,

@@ -2,6 +2,9 @@
 
     python -m paper_1009_5169_b200.build [--force]
 
+WD_NVCC_DEFINES (environment) adds -D flags for measurement builds, e.g. the ablation switches of csrc/wd_hop_zm.cu:
+    WD_NVCC_DEFINES="-DWD_ZM_ABLATE=1" python -m paper_1009_5169_b200.build --force     (and --force again without it afterwards)
+
 The .so is git-ignored but travels to the GPU box with the gpurun snapshot.
 """
 from __future__ import annotations
@@ -36,7 +39,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
     for s in SOURCES:
         o = os.path.join(HERE, "build", s.replace(".cu", ".o"))
         objs.append(o)
-        cmd = [nvcc] + [f for f in NVCC_FLAGS if not f.startswith("--use_fast_math")] + \
+        cmd = [nvcc] + [f for f in NVCC_FLAGS if not f.startswith("--use_fast_math")] + os.environ.get("WD_NVCC_DEFINES", "").split() + \
               (["-Xptxas", "-v"] if verbose else []) + ["-c", os.path.join(CSRC, s), "-o", o]
         procs.append((s, subprocess.Popen(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)))
     failed = False

@@ -171,6 +171,7 @@ int wd_create(wd_ctx** out, const int dims[4], double kappa, int time_bc, int ma
     c->opt[WD_OPT_GRAPH] = 1;
     c->cap_stream = nullptr;
     c->prof_on = false;
+    c->prof_depth = 0;
     c->prof_used = 0;
     c->h_pinned = nullptr;
     if (cudaMallocHost((void**)&c->h_pinned, sizeof(double) * kScalDoubles) != cudaSuccess) {

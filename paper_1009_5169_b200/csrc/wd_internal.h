@@ -81,6 +81,7 @@ struct wd_ctx {
 
     // optional per-class device timing (wd_profile): CUDA event pairs around the classed launches
     bool prof_on;
+    int prof_depth;                     // open wd_prof_scope brackets: only the outermost records events
     std::vector<cudaEvent_t> prof_ev;   // pairs (begin, end)
     std::vector<int> prof_cls;          // class of pair i
     size_t prof_used;                   // pairs used since the last wd_profile_read
@@ -91,7 +92,7 @@ struct wd_prof_scope {
     wd_ctx* c;
     long idx;
     wd_prof_scope(wd_ctx* ctx, int cls) : c(ctx), idx(-1) {
-        if (!c->prof_on) return;
+        if (c->prof_depth++ > 0 || !c->prof_on) return;
         if (c->prof_used == c->prof_cls.size()) {
             cudaEvent_t a, b;
             if (cudaEventCreate(&a) != cudaSuccess || cudaEventCreate(&b) != cudaSuccess) return;
@@ -104,6 +105,7 @@ struct wd_prof_scope {
         cudaEventRecord(c->prof_ev[2 * idx], c->stream);
     }
     ~wd_prof_scope() {
+        --c->prof_depth;
         if (idx >= 0) cudaEventRecord(c->prof_ev[2 * idx + 1], c->stream);
     }
 };

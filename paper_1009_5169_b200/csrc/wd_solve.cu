@@ -282,15 +282,20 @@ int wd_inner_solve_f32(wd_ctx* c, int dag, int n, int recon, int max_inner, cons
                 else p_update_kernel<float, false><<<L32.G, L32.B, 0, c->stream>>>(nv32, n, sweep(), c->d_scal, r32, p32, v32);
             }
             WD_LAUNCH_CHECK(c);
-            // v = Ahat p, sigma = <rt, v> -> alpha
-            o.in = p32; o.out = tmp32; o.in2 = nullptr; o.in3 = nullptr; o.a = 0.0; o.b = 1.0; o.epi = 0;
-            o.rev = sweep();
-            int rc2 = wd_hop_launch_ex(c, WD_F32, recon, dag, n, 1, o);
-            if (rc2) return rc2;
-            o.in = tmp32; o.out = v32; o.in2 = p32; o.in3 = rt32; o.a = 1.0; o.b = -kap * kap; o.epi = 2;
-            o.rev = sweep();
-            rc2 = wd_hop_launch_ex(c, WD_F32, recon, dag, n, 0, o);
-            if (rc2) return rc2;
+            // v = Ahat p, sigma = <rt, v> -> alpha.  (wd_profile: one event pair brackets the two hop launches of an
+            // application of Ahat, so that the per-launch average carries one kernel-to-kernel gap, not two.)
+            int rc2;
+            {
+                wd_prof_scope pr__(c, WD_PROF_HOP32);
+                o.in = p32; o.out = tmp32; o.in2 = nullptr; o.in3 = nullptr; o.a = 0.0; o.b = 1.0; o.epi = 0;
+                o.rev = sweep();
+                rc2 = wd_hop_launch_ex(c, WD_F32, recon, dag, n, 1, o);
+                if (rc2) return rc2;
+                o.in = tmp32; o.out = v32; o.in2 = p32; o.in3 = rt32; o.a = 1.0; o.b = -kap * kap; o.epi = 2;
+                o.rev = sweep();
+                rc2 = wd_hop_launch_ex(c, WD_F32, recon, dag, n, 0, o);
+                if (rc2) return rc2;
+            }
             {
                 wd_prof_scope pr__(c, WD_PROF_BLAS);
                 if (paired) s_update_kernel<float, true><<<L32.G, L32.B, 0, c->stream>>>(nv32, n, sweep(), c->d_scal, r32, v32);
@@ -298,14 +303,17 @@ int wd_inner_solve_f32(wd_ctx* c, int dag, int n, int recon, int max_inner, cons
             }
             WD_LAUNCH_CHECK(c);
             // t = Ahat s, <t, s>, <t, t> -> omega
-            o.in = r32; o.out = tmp32; o.in2 = nullptr; o.in3 = nullptr; o.a = 0.0; o.b = 1.0; o.epi = 0;
-            o.rev = sweep();
-            rc2 = wd_hop_launch_ex(c, WD_F32, recon, dag, n, 1, o);
-            if (rc2) return rc2;
-            o.in = tmp32; o.out = t32; o.in2 = r32; o.in3 = nullptr; o.a = 1.0; o.b = -kap * kap; o.epi = 3;
-            o.rev = sweep();
-            rc2 = wd_hop_launch_ex(c, WD_F32, recon, dag, n, 0, o);
-            if (rc2) return rc2;
+            {
+                wd_prof_scope pr__(c, WD_PROF_HOP32);
+                o.in = r32; o.out = tmp32; o.in2 = nullptr; o.in3 = nullptr; o.a = 0.0; o.b = 1.0; o.epi = 0;
+                o.rev = sweep();
+                rc2 = wd_hop_launch_ex(c, WD_F32, recon, dag, n, 1, o);
+                if (rc2) return rc2;
+                o.in = tmp32; o.out = t32; o.in2 = r32; o.in3 = nullptr; o.a = 1.0; o.b = -kap * kap; o.epi = 3;
+                o.rev = sweep();
+                rc2 = wd_hop_launch_ex(c, WD_F32, recon, dag, n, 0, o);
+                if (rc2) return rc2;
+            }
             {
                 wd_prof_scope pr__(c, WD_PROF_BLAS);
                 if (paired) xr_update_kernel<float, true><<<L32.G, L32.B, 0, c->stream>>>(nv32, n, sweep(), rb, x32, p32, r32, t32, rt32);
