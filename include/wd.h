@@ -181,7 +181,7 @@ int wd_hop(wd_ctx* ctx, int op, int prec, int recon, int n_rhs, int out_parity, 
  * even/odd preconditioning, fp64 defect-correction outer loop around an fp32
  * BiCGStab run in lock-step over the columns with per-column scalars.  Stops
  * when every column has |phi_i - A x_i| <= tol |phi_i| in fp64 (true residual), or after
- * max_outer outer steps of at most max_inner inner iterations each; inner_tol (0 = default 1e-5)
+ * max_outer outer steps of at most max_inner inner iterations each; inner_tol (0 = default 3e-7)
  * is the relative reduction asked of each inner call; recon picks the inner (fp32) link form,
  * the fp64 outer operator always uses 18 reals.  Returns WD_ENOCONV if tol was not met: X then
  * holds the best iterate and info is still filled.  info may be NULL. */

@@ -411,7 +411,9 @@ int wd_solve_impl(wd_ctx* c, int dag, int n, const double* Phi, double* X, doubl
     if (solver == WD_SOLVER_BL_F64) return wd_solve_bl(c, dag, n, Phi, X, tol, max_inner, info);
     if (solver == WD_SOLVER_RELIABLE_H16 && wd_solve_h16_applies(c, n))
         return wd_solve_h16(c, dag, n, Phi, X, tol, max_outer, max_inner, inner_tol > 0.0 ? inner_tol : 0.01, recon, info);
-    return wd_solve_dc(c, dag, n, Phi, X, tol, max_outer, max_inner, inner_tol > 0.0 ? inner_tol : 1e-5, recon, info);
+    // default: the fp32 recurrence is run down to 3e-7, about what fp32 can deliver, so that TWO inner solves reach
+    // 1e-12 (at 1e-5 it takes three: an fp64 residual, a demotion and a promotion more per solve; reading R12)
+    return wd_solve_dc(c, dag, n, Phi, X, tol, max_outer, max_inner, inner_tol > 0.0 ? inner_tol : 3e-7, recon, info);
 }
 
 int wd_solve_dc(wd_ctx* c, int dag, int n, const double* Phi, double* X, double tol, int max_outer,
