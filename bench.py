@@ -562,7 +562,8 @@ def run_ours(args):
                 "bytes_counted": f"interior sites only for everything read ((T-1)/T = {interior:.4f}), all sites for the output",
                 "avg_launch_us": round(hop_us, 2), "launches_in_step": hop_cnt,
                 "timing": "CUDA event pairs on the library's stream around the two hop launches of every application of the "
-                          "even/odd operator (one kernel-to-kernel gap inside each pair), CUDA graphs off for that step",
+                          "even/odd operator (one kernel-to-kernel gap inside each pair); in the graph-replayed blocks the pairs "
+                          "are event-record nodes of the graph, read back after every replay",
                 # the same four launches timed alone by ncu (gpu__time_duration of the committed full capture; cold caches,
                 # no neighbours on the stream): context for how much of avg_launch_us is gap between dependent kernels
                 "ncu_isolated": None if not ncu_us else {"avg_launch_us": round(sum(ncu_us) / len(ncu_us), 2),

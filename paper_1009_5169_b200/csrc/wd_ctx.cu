@@ -101,8 +101,10 @@ bool bad_n(const wd_ctx* c, int n) { return n < 1 || n > c->max_rhs; }
 }  // namespace
 
 void wd_graphs_clear(wd_ctx* c) {
-    for (wd_graph_entry& g : c->graphs)
+    for (wd_graph_entry& g : c->graphs) {
         if (g.exec) cudaGraphExecDestroy(g.exec);
+        for (cudaEvent_t e : g.ev) cudaEventDestroy(e);
+    }
     c->graphs.clear();
 }
 
@@ -172,6 +174,8 @@ int wd_create(wd_ctx** out, const int dims[4], double kappa, int time_bc, int ma
     c->cap_stream = nullptr;
     c->prof_on = false;
     c->prof_depth = 0;
+    c->prof_graph = nullptr;
+    for (int k = 0; k < 8; ++k) { c->prof_acc_ms[k] = 0.0; c->prof_acc_cnt[k] = 0; }
     c->prof_used = 0;
     c->h_pinned = nullptr;
     if (cudaMallocHost((void**)&c->h_pinned, sizeof(double) * kScalDoubles) != cudaSuccess) {
@@ -244,6 +248,7 @@ int wd_get_option(const wd_ctx* ctx, int key, int* value) {
 
 int wd_profile(wd_ctx* ctx, int enable) {
     if (!ctx) return WD_EINVAL;
+    if (ctx->prof_on != (enable != 0)) wd_graphs_clear(ctx);   // graphs with and without event nodes differ
     ctx->prof_on = enable != 0;
     return WD_OK;
 }
@@ -260,6 +265,12 @@ int wd_profile_read(wd_ctx* ctx, double* ms, long long* count) {
         count[ctx->prof_cls[i]] += 1;
     }
     ctx->prof_used = 0;
+    for (int k = 0; k < WD_PROF_N; ++k) {   // what the graph replays recorded (wd_solve.cu)
+        ms[k] += ctx->prof_acc_ms[k];
+        count[k] += ctx->prof_acc_cnt[k];
+        ctx->prof_acc_ms[k] = 0.0;
+        ctx->prof_acc_cnt[k] = 0;
+    }
     return WD_OK;
 }
 

@@ -20,6 +20,10 @@ struct wd_graph_entry {
     unsigned long long key;
     cudaGraphExec_t exec;   // null: the block has run once in stream order (function attributes are set), not yet captured
     long long launches;     // kernel launches one replay stands for
+    // wd_profile on: the event pairs recorded as nodes of this graph (begin, end, class); every replay re-records them
+    // and the solver adds their times up before the next replay
+    std::vector<cudaEvent_t> ev;
+    std::vector<int> cls;
 };
 
 struct wd_ctx {
@@ -83,6 +87,9 @@ struct wd_ctx {
     bool prof_on;
     int prof_depth;                     // open wd_prof_scope brackets: only the outermost records events
     std::vector<cudaEvent_t> prof_ev;   // pairs (begin, end)
+    wd_graph_entry* prof_graph;         // set while a graph is being captured: brackets record into its own event list
+    double prof_acc_ms[8];              // time per class accumulated from graph replays since the last wd_profile_read
+    long long prof_acc_cnt[8];
     std::vector<int> prof_cls;          // class of pair i
     size_t prof_used;                   // pairs used since the last wd_profile_read
 };
@@ -91,8 +98,19 @@ struct wd_ctx {
 struct wd_prof_scope {
     wd_ctx* c;
     long idx;
-    wd_prof_scope(wd_ctx* ctx, int cls) : c(ctx), idx(-1) {
+    cudaEvent_t g_end;
+    wd_prof_scope(wd_ctx* ctx, int cls) : c(ctx), idx(-1), g_end(nullptr) {
         if (c->prof_depth++ > 0 || !c->prof_on) return;
+        if (c->prof_graph) {   // capturing: the records become event-record nodes of the graph, readable from outside
+            cudaEvent_t a, b;
+            if (cudaEventCreate(&a) != cudaSuccess || cudaEventCreate(&b) != cudaSuccess) return;
+            c->prof_graph->ev.push_back(a);
+            c->prof_graph->ev.push_back(b);
+            c->prof_graph->cls.push_back(cls);
+            cudaEventRecordWithFlags(a, c->stream, cudaEventRecordExternal);
+            g_end = b;
+            return;
+        }
         if (c->prof_used == c->prof_cls.size()) {
             cudaEvent_t a, b;
             if (cudaEventCreate(&a) != cudaSuccess || cudaEventCreate(&b) != cudaSuccess) return;
@@ -106,6 +124,7 @@ struct wd_prof_scope {
     }
     ~wd_prof_scope() {
         --c->prof_depth;
+        if (g_end) cudaEventRecordWithFlags(g_end, c->stream, cudaEventRecordExternal);
         if (idx >= 0) cudaEventRecord(c->prof_ev[2 * idx + 1], c->stream);
     }
 };

@@ -336,19 +336,21 @@ int wd_inner_solve_f32(wd_ctx* c, int dag, int n, int recon, int max_inner, cons
         // lattices).  A block is a function of (operator, n_rhs, link form, the sweep direction it starts with) and of
         // the options, which clear the cache when they change.  First sight of a key: stream order (this also sets the
         // kernels' function attributes outside any capture); second: capture on the library's own stream, then replay.
-        const bool use_graph = c->opt[WD_OPT_GRAPH] != 0 && !c->prof_on;
+        const bool use_graph = c->opt[WD_OPT_GRAPH] != 0;
         for (int it = 0; it < max_inner;) {
             const int blk = poll_every < max_inner - it ? poll_every : max_inner - it;
             const int start_dir = sweep_dir;
             bool launched = false;
+            unsigned long long graph_key = 0;
             if (use_graph && blk == poll_every) {
-                const unsigned long long key = (unsigned long long)dag | ((unsigned long long)n << 1) | ((unsigned long long)recon << 8) |
-                                               ((unsigned long long)start_dir << 9) | ((unsigned long long)(paired ? 1 : 0) << 10);
+                const unsigned long long key = graph_key = (unsigned long long)dag | ((unsigned long long)n << 1) | ((unsigned long long)recon << 8) |
+                                               ((unsigned long long)start_dir << 9) | ((unsigned long long)(paired ? 1 : 0) << 10) |
+                                               ((unsigned long long)(c->prof_on ? 1 : 0) << 11);
                 wd_graph_entry* ge = nullptr;
                 for (wd_graph_entry& g : c->graphs)
                     if (g.key == key) ge = &g;
                 if (ge == nullptr) {
-                    c->graphs.push_back(wd_graph_entry{key, nullptr, 0});
+                    c->graphs.push_back(wd_graph_entry{key, nullptr, 0, {}, {}});
                 } else {
                     if (ge->exec == nullptr) {
                         if (!c->cap_stream) WD_CUDA_CHECK(c, cudaStreamCreateWithFlags(&c->cap_stream, cudaStreamNonBlocking));
@@ -356,7 +358,9 @@ int wd_inner_solve_f32(wd_ctx* c, int dag, int n, int recon, int max_inner, cons
                         const long long l0 = c->launches;
                         WD_CUDA_CHECK(c, cudaStreamBeginCapture(c->cap_stream, cudaStreamCaptureModeRelaxed));
                         c->stream = c->cap_stream;
+                        c->prof_graph = ge;
                         rc = enqueue_block(blk);
+                        c->prof_graph = nullptr;
                         c->stream = user;
                         cudaGraph_t graph = nullptr;
                         const cudaError_t e = cudaStreamEndCapture(c->cap_stream, &graph);
@@ -389,6 +393,18 @@ int wd_inner_solve_f32(wd_ctx* c, int dag, int n, int recon, int max_inner, cons
             }
             it += blk;
             WD_CUDA_CHECK(c, cudaStreamSynchronize(c->stream));
+            if (launched && c->prof_on) {   // the replay's event pairs: add them up before the next replay re-records them
+                for (wd_graph_entry& g : c->graphs) {
+                    if (g.key != graph_key) continue;
+                    for (size_t e = 0; e < g.cls.size(); ++e) {
+                        float t = 0.f;
+                        if (cudaEventElapsedTime(&t, g.ev[2 * e], g.ev[2 * e + 1]) == cudaSuccess) {
+                            c->prof_acc_ms[g.cls[e]] += t;
+                            c->prof_acc_cnt[g.cls[e]] += 1;
+                        }
+                    }
+                }
+            }
             if (hp[G_COUNT] != 0.0) break;
         }
         {
