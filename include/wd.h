@@ -136,10 +136,15 @@ int wd_site_order(wd_ctx* ctx, int order, const int tile[4]);
  *   WD_OPT_GRAPH        1 (default): the fp32 inner solver replays each block of WD_OPT_POLL_EVERY iterations (7 kernels
  *       each, plus the read-back of the convergence flag) as one CUDA graph, captured the second time a (operator, n_rhs,
  *       link form) combination is solved; 0: plain stream launches.  Identical results; off while wd_profile is on.
+ *   WD_OPT_MERGE        1 (default): the fp32 inner solver folds the p-update of iteration k+1 into the x,r-update of
+ *       iteration k (one 8-stream kernel instead of a 7- and a 4-stream one: 23 instead of 25 vector passes per
+ *       iteration, 6 instead of 7 kernels); the rho it needs comes from the second hop's epilogue as
+ *       <rt,s> - omega <rt,t>.  Where the z-march hop kernel serves the shape; 0: the textbook order.  The iterates
+ *       agree to rounding, the result to tol.
  * Errors: WD_EINVAL (null, unknown key, value out of range). */
 enum { WD_OPT_HOP32_SITES = 0, WD_OPT_HOP64_SITES = 1, WD_OPT_HOP32_REGS = 2, WD_OPT_HOP64_REGS = 3,
        WD_OPT_POLL_EVERY = 4, WD_OPT_HOP_IMPL = 5, WD_OPT_ALTERNATE_SWEEP = 6, WD_OPT_HOP_ROWS = 7, WD_OPT_SOLVER = 8,
-       WD_OPT_PAIRED = 9, WD_OPT_GRAPH = 10, WD_OPT_N = 11 };
+       WD_OPT_PAIRED = 9, WD_OPT_GRAPH = 10, WD_OPT_MERGE = 11, WD_OPT_N = 12 };
 /* values of WD_OPT_SOLVER */
 enum { WD_SOLVER_DC_F32 = 0, WD_SOLVER_RELIABLE_H16 = 1, WD_SOLVER_GL_FLEX = 2, WD_SOLVER_GL_F64 = 3, WD_SOLVER_BL_F64 = 4,
        WD_SOLVER_N = 5 };

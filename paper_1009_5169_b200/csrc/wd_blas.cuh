@@ -37,6 +37,7 @@ enum { G_DONE = S_ROWS * WD_MAX_RHS, G_ITERS, G_OUT_DONE, G_TOL2, G_INTOL2, G_DE
 __device__ __forceinline__ double& SC(double* scal, int row, int r) { return scal[row * WD_MAX_RHS + r]; }
 
 enum Kind { K_SIGMA, K_OMEGA, K_RHO, K_PHI2, K_OUT_R2, K_INIT_RHO, K_ACTION,
+            K_OMEGA_RHO, K_RNORM,                  // merged-update schedule of the fp32 solver (wd_solve.cu)
             K_RHO_REL, K_OUT_R2_REL, K_REPLACE,     // reliable-update solver (wd_solve_h16.cu)
             K_GL_INIT, K_GL_SIGMA, K_GL_S, K_GL_OMEGA, K_GL_RHO, K_PREC_PREP };   // blocked outer solvers (wd_solve_gl.cu)
 
@@ -75,6 +76,32 @@ __device__ void finalize_column(double* scal, int r, const double* tot) {
         if (!frozen && tot[2] > 0.0) omega = {tot[0] / tot[2], tot[1] / tot[2]};
         SC(scal, S_OMEGA_RE, r) = omega.re;
         SC(scal, S_OMEGA_IM, r) = omega.im;
+    } else if (KIND == K_OMEGA_RHO) {
+        // tot = <t,s> (2), <t,t>, <rt,s> (2), <rt,t> (2): omega as above, and the NEXT rho without waiting for the new r,
+        // rho' = <rt, s - omega t> = <rt,s> - omega <rt,t>, so that beta is known before the merged x, r, p update runs
+        cd omega = {0.0, 0.0}, beta = {0.0, 0.0};
+        if (!frozen && tot[2] > 0.0) omega = {tot[0] / tot[2], tot[1] / tot[2]};
+        SC(scal, S_OMEGA_RE, r) = omega.re;
+        SC(scal, S_OMEGA_IM, r) = omega.im;
+        if (!frozen) {
+            const cd wt = cmul(omega, {tot[5], tot[6]});
+            const cd rho1 = {tot[3] - wt.re, tot[4] - wt.im};
+            const cd rho = {SC(scal, S_RHO_RE, r), SC(scal, S_RHO_IM, r)};
+            const cd alpha = {SC(scal, S_ALPHA_RE, r), SC(scal, S_ALPHA_IM, r)};
+            if (!(rho1.re == rho1.re) || !(rho1.im == rho1.im) || (omega.re == 0.0 && omega.im == 0.0) ||
+                (rho1.re == 0.0 && rho1.im == 0.0) || (rho.re == 0.0 && rho.im == 0.0)) {
+                SC(scal, S_FLAG, r) = 2.0;  // breakdown or NaN: the merged update still forms x and r; the outer loop restarts
+            } else {
+                beta = cmul(cdiv(rho1, rho), cdiv(alpha, omega));
+            }
+            SC(scal, S_RHO_RE, r) = rho1.re; SC(scal, S_RHO_IM, r) = rho1.im;
+        }
+        SC(scal, S_BETA_RE, r) = beta.re; SC(scal, S_BETA_IM, r) = beta.im;
+    } else if (KIND == K_RNORM) {  // tot = |r|^2 after the merged x, r, p update: convergence only
+        if (frozen) return;
+        SC(scal, S_RNORM2, r) = tot[0];
+        if (tot[0] <= SC(scal, S_THR2, r)) SC(scal, S_FLAG, r) = 1.0;
+        else if (!(tot[0] == tot[0])) SC(scal, S_FLAG, r) = 2.0;
     } else if (KIND == K_RHO || KIND == K_INIT_RHO) {  // tot = <rt, r>, |r|^2
         if (KIND == K_INIT_RHO) {
             SC(scal, S_RHO_RE, r) = tot[0]; SC(scal, S_RHO_IM, r) = tot[1];
@@ -192,11 +219,11 @@ __device__ void finalize_column(double* scal, int r, const double* tot) {
 
 template <int KIND>
 __device__ void finalize_global(double* scal, int n) {
-    if (KIND == K_RHO || KIND == K_INIT_RHO) {
+    if (KIND == K_RHO || KIND == K_INIT_RHO || KIND == K_RNORM) {
         bool all = true;
         for (int r = 0; r < n; ++r) all = all && (SC(scal, S_FLAG, r) != 0.0);
         scal[G_DONE] = all ? 1.0 : 0.0;
-        if (KIND == K_RHO) scal[G_ITERS] += 1.0;
+        if (KIND != K_INIT_RHO) scal[G_ITERS] += 1.0;
     } else if (KIND == K_OUT_R2) {
         bool all = true;
         for (int r = 0; r < n; ++r) all = all && (SC(scal, S_OUT_CONV, r) != 0.0);

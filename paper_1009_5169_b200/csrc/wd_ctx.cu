@@ -171,6 +171,7 @@ int wd_create(wd_ctx** out, const int dims[4], double kappa, int time_bc, int ma
     c->opt[WD_OPT_ALTERNATE_SWEEP] = 1;
     c->opt[WD_OPT_PAIRED] = 0;
     c->opt[WD_OPT_GRAPH] = 1;
+    c->opt[WD_OPT_MERGE] = 1;
     c->cap_stream = nullptr;
     c->prof_on = false;
     c->prof_depth = 0;
@@ -221,6 +222,7 @@ int wd_set_option(wd_ctx* ctx, int key, int value) {
         case WD_OPT_ALTERNATE_SWEEP:
         case WD_OPT_PAIRED:
         case WD_OPT_GRAPH:
+        case WD_OPT_MERGE:
             if (value != 0 && value != 1) return wd_fail(ctx, WD_EINVAL, "this option is 0 or 1");
             break;
         case WD_OPT_HOP_ROWS:

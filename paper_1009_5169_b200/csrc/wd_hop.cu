@@ -244,6 +244,12 @@ int wd_hop_launch_ex(wd_ctx* c, int prec, int recon, int dag, int n, int par, co
     if (o.epi >= EPI_SIGMA && prec != WD_F32) return wd_fail(c, WD_EINVAL, "fused reductions are fp32 only");
     // staged kernel where it applies (row-major layout) and pays: with 1-2 columns a group of rows gives it too few
     // consumer threads (24^4 fp32: 41 us against 33 us at n = 2; 71 against 76 at n = 5; 146 against 151 at n = 12)
+    if (o.epi == 4) {   // xpay + <t,s>, <t,t>, <rt,s>, <rt,t> (merged-update schedule): plain fp32 operands, z-march kernel only
+        const int rc = (prec == WD_F32 && o.storage == 0 && n >= 3) ? wd_hop_zm_launch(c, prec, recon, dag, n, par, o) : 1;
+        if (rc > 0) return wd_fail(c, WD_EINVAL, "hop: the seven-sum epilogue needs the z-march kernel");
+        if (rc == WD_OK) WD_LAUNCH_CHECK(c);
+        return rc;
+    }
     if (prec == WD_F32P || o.storage == 2) {   // P32 (two sites per thread): served by the z-march kernel only
         wd_hop_ops o2 = o;
         o2.storage = 2;

@@ -44,7 +44,9 @@ namespace {
 #define mbar_expect_tx(b, n) ((void)0)
 #endif
 
-enum { EPI_NONE = 0, EPI_XPAY = 1, EPI_SIGMA = 2, EPI_OMEGA = 3 };
+// EPI_OMEGA_RHO (plain fp32 operands only): EPI_OMEGA plus <in3, in2> and <in3, out>, i.e. <rt,s> and <rt,t> for the merged-update
+// schedule of the solver (7 sums per column)
+enum { EPI_NONE = 0, EPI_XPAY = 1, EPI_SIGMA = 2, EPI_OMEGA = 3, EPI_OMEGA_RHO = 4 };
 enum { U_TP = 0, U_TM = 1, U_ZM = 2, U_Y = 3, U_XZ = 4, NUNIT = 5 };
 // link blocks in shared memory, in consumption order
 enum { LK_TP = 0, LK_TM = 1, LK_ZM = 2, LK_YM = 3, LK_YP = 4, LK_XM = 5, LK_XP = 6, LK_ZP = 7 };
@@ -210,7 +212,7 @@ __global__ void __launch_bounds__(MAXT, 1) hop_zm_kernel(const ZmArgs<T> A) {
     }
     __syncthreads();
     const uint32_t s_first = blockIdx.x * A.chunk;   // < steps: the grid has at most ceil(steps / chunk) CTAs
-    [[maybe_unused]] double dsum[3] = {0.0, 0.0, 0.0};
+    [[maybe_unused]] double dsum[EPI == EPI_OMEGA_RHO ? 7 : 3] = {};
 
     if (ST == 2 && warp >= ncw) {
         // ================= producer warps, P32 form: TWO warps (the consumers, two sites per thread with the next
@@ -544,7 +546,7 @@ __global__ void __launch_bounds__(MAXT, 1) hop_zm_kernel(const ZmArgs<T> A) {
 #pragma unroll
                 for (uint32_t c = 0; c < (ST == 1 ? 3u : NCH); ++c) {
                     asm volatile("prefetch.global.L2 [%0];" ::"l"(A.in2 + own + c * rowV + e0));
-                    if (EPI == EPI_SIGMA) asm volatile("prefetch.global.L2 [%0];" ::"l"(A.in3 + own + c * rowV + e0));
+                    if (EPI == EPI_SIGMA || EPI == EPI_OMEGA_RHO) asm volatile("prefetch.global.L2 [%0];" ::"l"(A.in3 + own + c * rowV + e0));
                 }
             }
             const uint32_t wm = a % 3, wc = (a + 1) % 3, wp = (a + 2) % 3;
@@ -604,7 +606,7 @@ __global__ void __launch_bounds__(MAXT, 1) hop_zm_kernel(const ZmArgs<T> A) {
                         acc[q].re = fma(A.b, acc[q].re, A.a * qv[q].re);
                         acc[q].im = fma(A.b, acc[q].im, A.a * qv[q].im);
                     }
-                    if (EPI == EPI_OMEGA) {  // <t, s>, <t, t> with t = acc, s = qv
+                    if (EPI == EPI_OMEGA || EPI == EPI_OMEGA_RHO) {  // <t, s>, <t, t> with t = acc, s = qv
                         T s0 = 0, s1 = 0, s2 = 0;
 #pragma unroll
                         for (int q = 0; q < 12; ++q) {
@@ -613,6 +615,23 @@ __global__ void __launch_bounds__(MAXT, 1) hop_zm_kernel(const ZmArgs<T> A) {
                             s2 = fma(acc[q].re, acc[q].re, s2); s2 = fma(acc[q].im, acc[q].im, s2);
                         }
                         dsum[0] += (double)s0; dsum[1] += (double)s1; dsum[2] += (double)s2;
+                    }
+                    if constexpr (EPI == EPI_OMEGA_RHO && ST == 0) {  // <rt, s>, <rt, t> with rt = in3, two components at a time
+                        T s3 = 0, s4 = 0, s5 = 0, s6 = 0;
+#pragma unroll
+                        for (int c = 0; c < 6; ++c) {
+                            const float4 w = __ldg(A.in3 + own + c * rowV + e0);
+                            const cx<T> g0 = {w.x, w.y}, g1 = {w.z, w.w};
+                            s3 = fma(g0.re, qv[2 * c].re, s3);  s3 = fma(g0.im, qv[2 * c].im, s3);
+                            s4 = fma(g0.re, qv[2 * c].im, s4);  s4 = fma(-g0.im, qv[2 * c].re, s4);
+                            s5 = fma(g0.re, acc[2 * c].re, s5); s5 = fma(g0.im, acc[2 * c].im, s5);
+                            s6 = fma(g0.re, acc[2 * c].im, s6); s6 = fma(-g0.im, acc[2 * c].re, s6);
+                            s3 = fma(g1.re, qv[2 * c + 1].re, s3);  s3 = fma(g1.im, qv[2 * c + 1].im, s3);
+                            s4 = fma(g1.re, qv[2 * c + 1].im, s4);  s4 = fma(-g1.im, qv[2 * c + 1].re, s4);
+                            s5 = fma(g1.re, acc[2 * c + 1].re, s5); s5 = fma(g1.im, acc[2 * c + 1].im, s5);
+                            s6 = fma(g1.re, acc[2 * c + 1].im, s6); s6 = fma(-g1.im, acc[2 * c + 1].re, s6);
+                        }
+                        dsum[3] += (double)s3; dsum[4] += (double)s4; dsum[5] += (double)s5; dsum[6] += (double)s6;
                     }
                 }
                 if (EPI == EPI_SIGMA) {  // <r~, v> with v = acc
@@ -632,7 +651,7 @@ __global__ void __launch_bounds__(MAXT, 1) hop_zm_kernel(const ZmArgs<T> A) {
     if (EPI >= EPI_SIGMA) {
         // per-column sums of this CTA -> one partial per (column, value); the last CTA adds the partials in a fixed
         // order and runs the scalar recurrence (as wd_hop_tma.cu)
-        constexpr int K = EPI == EPI_SIGMA ? 2 : 3;
+        constexpr int K = EPI == EPI_SIGMA ? 2 : (EPI == EPI_OMEGA_RHO ? 7 : 3);
         __syncthreads();  // every bulk copy has been consumed: the staging area is free
         double* red = reinterpret_cast<double*>(base);
         if (threadIdx.x < nct) {
@@ -667,7 +686,7 @@ __global__ void __launch_bounds__(MAXT, 1) hop_zm_kernel(const ZmArgs<T> A) {
         }
         __syncthreads();
         if (threadIdx.x < nr)
-            wdblas::finalize_column<EPI == EPI_SIGMA ? wdblas::K_SIGMA : wdblas::K_OMEGA>(A.rb.scal, (int)threadIdx.x, tot + threadIdx.x * K);
+            wdblas::finalize_column<EPI == EPI_SIGMA ? wdblas::K_SIGMA : (EPI == EPI_OMEGA_RHO ? wdblas::K_OMEGA_RHO : wdblas::K_OMEGA)>(A.rb.scal, (int)threadIdx.x, tot + threadIdx.x * K);
         if (threadIdx.x == 0) *A.rb.ticket = 0u;
     }
 }
@@ -696,7 +715,7 @@ bool pick_shape(const wd_ctx* c, int n, int max_threads, Shape* sh) {
         const size_t smem = 128 + (5 * (size_t)RG + 2) * rowB + 8 * (size_t)RG * lrowB;
         if (smem > kSmemMax) continue;
         // the epilogue's reduction scratch (3 sums per consumer thread + totals) reuses the staging area
-        if ((size_t)(3 * S * n + 3 * WD_MAX_RHS + 2) * sizeof(double) > smem - 128) continue;
+        if ((size_t)(7 * S * n + 7 * WD_MAX_RHS + 2) * sizeof(double) > smem - 128) continue;
         sh->RG = RG; sh->S = S; sh->threads = cthreads + pthreads; sh->smem = smem;
         return true;
     }
@@ -714,6 +733,13 @@ int launch_one(wd_ctx* c, const ZmArgs<T>& A, const Shape& sh, unsigned G) {
 template <typename T, int RECON, int MAXT, int LXH, int NR, int RGT, int ST>
 int launch_epi(wd_ctx* c, const ZmArgs<T>& A, const Shape& sh, unsigned G, int dag, int epi) {
 #define WD_ZM_CASE(D, E) return launch_one<T, RECON, D, E, MAXT, LXH, NR, RGT, ST>(c, A, sh, G)
+    if (epi == EPI_OMEGA_RHO) {
+        if constexpr (ST == 0) {
+            if (dag) WD_ZM_CASE(true, EPI_OMEGA_RHO);
+            else WD_ZM_CASE(false, EPI_OMEGA_RHO);
+        }
+        return 1;
+    }
     if (dag) {
         if (epi == EPI_NONE) WD_ZM_CASE(true, EPI_NONE);
         else if (epi == EPI_XPAY) WD_ZM_CASE(true, EPI_XPAY);

@@ -111,6 +111,44 @@ __global__ void xr_update_kernel(long nvec, int n, int rev, RedBuf rb, typename 
     reduce_finalize<3, K_RHO>(s, n, rb);
 }
 
+// The merged update (WD_OPT_MERGE): X += alpha P + omega S;  R = S - omega T;  P = R + beta (P - omega V);  |R|^2.
+// beta = (rho'/rho)(alpha/omega) is already on the device: rho' = <Rt,S> - omega <Rt,T> came out of the epilogue of the
+// hop that made T (K_OMEGA_RHO), so the new P can be formed in the same pass as the new R.  5 reads + 3 writes.
+template <typename T, bool PAIRED>
+__global__ void xrp_update_kernel(long nvec, int n, int rev, RedBuf rb, typename V<T>::type* __restrict__ X,
+                                  typename V<T>::type* __restrict__ P, typename V<T>::type* __restrict__ R,
+                                  const typename V<T>::type* __restrict__ Tt, const typename V<T>::type* __restrict__ Vv) {
+    if (rb.scal[G_DONE] != 0.0) return;
+    WD_BLAS_PROLOGUE(T)
+    const double* scal = rb.scal;
+    const T ar = (T)scal[S_ALPHA_RE * WD_MAX_RHS + r], ai = (T)scal[S_ALPHA_IM * WD_MAX_RHS + r];
+    const T wr = (T)scal[S_OMEGA_RE * WD_MAX_RHS + r], wi = (T)scal[S_OMEGA_IM * WD_MAX_RHS + r];
+    const T br = (T)scal[S_BETA_RE * WD_MAX_RHS + r], bi = (T)scal[S_BETA_IM * WD_MAX_RHS + r];
+    double s[1] = {0.0};
+    for (long k = 0; k < cnt; ++k) {
+        const long i = i0 + (rev ? cnt - 1 - k : k) * stride;
+        T x[2 * NC], p[2 * NC], sv[2 * NC], t[2 * NC], v[2 * NC];
+        to_arr<T, PAIRED>(X[i], x); to_arr<T, PAIRED>(P[i], p); to_arr<T, PAIRED>(R[i], sv); to_arr<T, PAIRED>(Tt[i], t); to_arr<T, PAIRED>(Vv[i], v);
+#pragma unroll
+        for (int c = 0; c < NC; ++c) {
+            x[2 * c] += (ar * p[2 * c] - ai * p[2 * c + 1]) + (wr * sv[2 * c] - wi * sv[2 * c + 1]);
+            x[2 * c + 1] += (ar * p[2 * c + 1] + ai * p[2 * c]) + (wr * sv[2 * c + 1] + wi * sv[2 * c]);
+            const T rr = sv[2 * c] - (wr * t[2 * c] - wi * t[2 * c + 1]);
+            const T ri = sv[2 * c + 1] - (wr * t[2 * c + 1] + wi * t[2 * c]);
+            const T tr = p[2 * c] - (wr * v[2 * c] - wi * v[2 * c + 1]);
+            const T ti = p[2 * c + 1] - (wr * v[2 * c + 1] + wi * v[2 * c]);
+            sv[2 * c] = rr; sv[2 * c + 1] = ri;
+            p[2 * c] = rr + (br * tr - bi * ti);
+            p[2 * c + 1] = ri + (br * ti + bi * tr);
+            s[0] += (double)rr * rr + (double)ri * ri;
+        }
+        X[i] = from_arr<PAIRED>(x);
+        R[i] = from_arr<PAIRED>(sv);
+        P[i] = from_arr<PAIRED>(p);
+    }
+    reduce_finalize<1, K_RNORM>(s, n, rb);
+}
+
 // |phi_i|^2 over a full-lattice fp64 block
 __global__ void norm2_kernel(long nvec, int n, RedBuf rb, const double2* __restrict__ A) {
     const long stride = (long)gridDim.x * blockDim.x;
@@ -139,7 +177,8 @@ __global__ void outer_resid_kernel(long nvec, int n, RedBuf rb, const double2* _
 // inner start: b = R_i / |R_i| in fp32 -> r, rt;  x = p = v = 0;  rho = <b, b>.
 // fp64 vec index ((block*12 + k)*RB + o)*n + r, k < 12  <->  fp32 vec index ((block*6 + k/2)*RB + o)*n + r, components 2*(k%2)..
 // PAIRED: the fp32 side is P32 (wd_f2.cuh): vec index ((block*12 + k)*H + p)*n + r = complex k of sites o = p and p + H, H = RB/2.
-template <bool PAIRED>
+// P_IS_R (merged-update schedule): p starts as r, because no p-update precedes the first hop there.
+template <bool PAIRED, bool P_IS_R = false>
 __global__ void demote_kernel(long Vh, long RB, int n, RedBuf rb, const double2* __restrict__ R64, float4* __restrict__ r32,
                               float4* __restrict__ rt32, float4* __restrict__ x32, float4* __restrict__ p32,
                               float4* __restrict__ v32) {
@@ -165,7 +204,7 @@ __global__ void demote_kernel(long Vh, long RB, int n, RedBuf rb, const double2*
         r32[i] = f;
         rt32[i] = f;
         const float4 z = make_float4(0.f, 0.f, 0.f, 0.f);
-        x32[i] = z; p32[i] = z; v32[i] = z;
+        x32[i] = z; p32[i] = P_IS_R ? f : z; v32[i] = z;
         s[0] += (double)f.x * f.x + (double)f.y * f.y + (double)f.z * f.z + (double)f.w * f.w;
     }
     s[2] = s[0];
@@ -257,9 +296,12 @@ int wd_inner_solve_f32(wd_ctx* c, int dag, int n, int recon, int max_inner, cons
     {
         // P32 (two sites per thread, packed fp32 instructions: wd_f2.cuh) wherever the z-march kernel serves it
         const bool paired = c->opt[WD_OPT_PAIRED] != 0 && c->opt[WD_OPT_HOP_IMPL] == 2 && n >= 3 && wd_hop_zm_serves(c, recon, n, 2);
+        // merged x,r,p update (WD_OPT_MERGE) wherever the z-march kernel, which has the seven-sum epilogue, serves the hop
+        const bool merged = c->opt[WD_OPT_MERGE] != 0 && !paired && c->opt[WD_OPT_HOP_IMPL] == 2 && n >= 3 && wd_hop_zm_serves(c, recon, n, 0);
         {
             wd_prof_scope pr__(c, WD_PROF_BLAS);
             if (paired) demote_kernel<true><<<L32.G, L32.B, 0, st>>>(Vh, (long)c->RB, n, rb, R64, r32, rt32, x32, p32, v32);
+            else if (merged) demote_kernel<false, true><<<L32.G, L32.B, 0, st>>>(Vh, (long)c->RB, n, rb, R64, r32, rt32, x32, p32, v32);
             else demote_kernel<false><<<L32.G, L32.B, 0, st>>>(Vh, (long)c->RB, n, rb, R64, r32, rt32, x32, p32, v32);
         }
         WD_LAUNCH_CHECK(c);
@@ -276,12 +318,12 @@ int wd_inner_solve_f32(wd_ctx* c, int dag, int n, int recon, int max_inner, cons
         o.storage = paired ? 2 : 0;
         // one BiCGStab iteration on c->stream (which is the capture stream while a graph is being recorded)
         auto enqueue_iteration = [&]() -> int {
-            {
+            if (!merged) {
                 wd_prof_scope pr__(c, WD_PROF_BLAS);
                 if (paired) p_update_kernel<float, true><<<L32.G, L32.B, 0, c->stream>>>(nv32, n, sweep(), c->d_scal, r32, p32, v32);
                 else p_update_kernel<float, false><<<L32.G, L32.B, 0, c->stream>>>(nv32, n, sweep(), c->d_scal, r32, p32, v32);
+                WD_LAUNCH_CHECK(c);
             }
-            WD_LAUNCH_CHECK(c);
             // v = Ahat p, sigma = <rt, v> -> alpha.  (wd_profile: one event pair brackets the two hop launches of an
             // application of Ahat, so that the per-launch average carries one kernel-to-kernel gap, not two.)
             int rc2;
@@ -309,14 +351,15 @@ int wd_inner_solve_f32(wd_ctx* c, int dag, int n, int recon, int max_inner, cons
                 o.rev = sweep();
                 rc2 = wd_hop_launch_ex(c, WD_F32, recon, dag, n, 1, o);
                 if (rc2) return rc2;
-                o.in = tmp32; o.out = t32; o.in2 = r32; o.in3 = nullptr; o.a = 1.0; o.b = -kap * kap; o.epi = 3;
+                o.in = tmp32; o.out = t32; o.in2 = r32; o.in3 = merged ? rt32 : nullptr; o.a = 1.0; o.b = -kap * kap; o.epi = merged ? 4 : 3;
                 o.rev = sweep();
                 rc2 = wd_hop_launch_ex(c, WD_F32, recon, dag, n, 0, o);
                 if (rc2) return rc2;
             }
             {
                 wd_prof_scope pr__(c, WD_PROF_BLAS);
-                if (paired) xr_update_kernel<float, true><<<L32.G, L32.B, 0, c->stream>>>(nv32, n, sweep(), rb, x32, p32, r32, t32, rt32);
+                if (merged) xrp_update_kernel<float, false><<<L32.G, L32.B, 0, c->stream>>>(nv32, n, sweep(), rb, x32, p32, r32, t32, v32);
+                else if (paired) xr_update_kernel<float, true><<<L32.G, L32.B, 0, c->stream>>>(nv32, n, sweep(), rb, x32, p32, r32, t32, rt32);
                 else xr_update_kernel<float, false><<<L32.G, L32.B, 0, c->stream>>>(nv32, n, sweep(), rb, x32, p32, r32, t32, rt32);
             }
             WD_LAUNCH_CHECK(c);
@@ -345,7 +388,7 @@ int wd_inner_solve_f32(wd_ctx* c, int dag, int n, int recon, int max_inner, cons
             if (use_graph && blk == poll_every) {
                 const unsigned long long key = graph_key = (unsigned long long)dag | ((unsigned long long)n << 1) | ((unsigned long long)recon << 8) |
                                                ((unsigned long long)start_dir << 9) | ((unsigned long long)(paired ? 1 : 0) << 10) |
-                                               ((unsigned long long)(c->prof_on ? 1 : 0) << 11);
+                                               ((unsigned long long)(c->prof_on ? 1 : 0) << 11) | ((unsigned long long)(merged ? 1 : 0) << 12);
                 wd_graph_entry* ge = nullptr;
                 for (wd_graph_entry& g : c->graphs)
                     if (g.key == key) ge = &g;
@@ -383,7 +426,7 @@ int wd_inner_solve_f32(wd_ctx* c, int dag, int n, int recon, int max_inner, cons
                     }
                     WD_CUDA_CHECK(c, cudaGraphLaunch(ge->exec, c->stream));
                     c->launches += ge->launches;
-                    if (c->opt[WD_OPT_ALTERNATE_SWEEP] && ((7 * blk) & 1)) sweep_dir ^= 1;   // 7 launches per iteration
+                    if (c->opt[WD_OPT_ALTERNATE_SWEEP] && (((merged ? 6 : 7) * blk) & 1)) sweep_dir ^= 1;   // launches per iteration
                     launched = true;
                 }
             }

@@ -29,7 +29,7 @@ ORDER_LINEAR, ORDER_TILED = 0, 1
 ACTION_FULL, ACTION_EO = 0, 1
 PARITY_EVEN, PARITY_ODD, PARITY_BOTH = 0, 1, 2
 MAX_RHS = 16
-OPT_HOP32_SITES, OPT_HOP64_SITES, OPT_HOP32_REGS, OPT_HOP64_REGS, OPT_POLL_EVERY, OPT_HOP_IMPL, OPT_ALTERNATE_SWEEP, OPT_HOP_ROWS, OPT_SOLVER, OPT_PAIRED, OPT_GRAPH = 0, 1, 2, 3, 4, 5, 6, 7, 8, 9, 10
+OPT_HOP32_SITES, OPT_HOP64_SITES, OPT_HOP32_REGS, OPT_HOP64_REGS, OPT_POLL_EVERY, OPT_HOP_IMPL, OPT_ALTERNATE_SWEEP, OPT_HOP_ROWS, OPT_SOLVER, OPT_PAIRED, OPT_GRAPH, OPT_MERGE = 0, 1, 2, 3, 4, 5, 6, 7, 8, 9, 10, 11
 SOLVER_DC_F32, SOLVER_RELIABLE_H16, SOLVER_GL_FLEX, SOLVER_GL_F64, SOLVER_BL_F64 = 0, 1, 2, 3, 4
 PROF_NAMES = ("hop32", "hop64", "blas", "force", "layout")
 PROF_N = len(PROF_NAMES)

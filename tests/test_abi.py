@@ -69,7 +69,7 @@ def test_option_and_enum_constants_match_header():
              "WD_OPT_HOP64_SITES": wd.OPT_HOP64_SITES, "WD_OPT_HOP32_REGS": wd.OPT_HOP32_REGS,
              "WD_OPT_HOP64_REGS": wd.OPT_HOP64_REGS, "WD_OPT_POLL_EVERY": wd.OPT_POLL_EVERY,
              "WD_OPT_HOP_IMPL": wd.OPT_HOP_IMPL, "WD_OPT_ALTERNATE_SWEEP": wd.OPT_ALTERNATE_SWEEP,
-             "WD_OPT_HOP_ROWS": wd.OPT_HOP_ROWS, "WD_OPT_SOLVER": wd.OPT_SOLVER, "WD_OPT_PAIRED": wd.OPT_PAIRED, "WD_OPT_GRAPH": wd.OPT_GRAPH, "WD_F32P": wd.F32P, "WD_SOLVER_DC_F32": wd.SOLVER_DC_F32,
+             "WD_OPT_HOP_ROWS": wd.OPT_HOP_ROWS, "WD_OPT_SOLVER": wd.OPT_SOLVER, "WD_OPT_PAIRED": wd.OPT_PAIRED, "WD_OPT_GRAPH": wd.OPT_GRAPH, "WD_OPT_MERGE": wd.OPT_MERGE, "WD_F32P": wd.F32P, "WD_SOLVER_DC_F32": wd.SOLVER_DC_F32,
              "WD_SOLVER_RELIABLE_H16": wd.SOLVER_RELIABLE_H16, "WD_SOLVER_GL_FLEX": wd.SOLVER_GL_FLEX,
              "WD_SOLVER_GL_F64": wd.SOLVER_GL_F64, "WD_SOLVER_BL_F64": wd.SOLVER_BL_F64, "WD_ACTION_FULL": wd.ACTION_FULL, "WD_ACTION_EO": wd.ACTION_EO,
              "WD_PARITY_EVEN": wd.PARITY_EVEN, "WD_PARITY_ODD": wd.PARITY_ODD, "WD_PARITY_BOTH": wd.PARITY_BOTH}

@@ -411,6 +411,35 @@ def test_launch_options_change_speed_only():
     ctx.close()
 
 
+@pytest.mark.parametrize("cfg_idx,n_rhs,recon", [(1, 5, 0), (1, 3, 1), (2, 5, 0)])
+def test_merged_update_schedule_matches_oracle_and_textbook_order(cfg_idx, n_rhs, recon):
+    """WD_OPT_MERGE: the p-update folded into the x,r-update (rho' = <rt,s> - omega <rt,t> from the hop epilogue) against
+    the textbook order of BiCGStab: both reach the tolerance, X agrees with the oracle to 1e-9 either way and between
+    the two to solver accuracy, iteration counts within a few of each other, one kernel fewer per iteration."""
+    pkg = _wd()
+    cfg, U, Phi = wi.make_config(cfg_idx, n_rhs)
+    dims, kappa, bc, n = cfg["dims"], cfg["kappa"], cfg["bc"], cfg["n_rhs"]
+    ctx = make_ctx(dims, kappa, bc, n, U)
+    assert ctx.get_option(pkg.OPT_MERGE) == 1
+    P = ctx.pack(dev(Phi))
+    for op in (pkg.OP_D, pkg.OP_DDAG):
+        Xr, rr, _, rc = orc.solve(dims, kappa, bc, op, U, Phi, tol=1e-14)
+        assert rc == 0 and rr.max() < 1e-13
+        res = {}
+        for merge in (0, 1):
+            ctx.set_option(pkg.OPT_MERGE, merge)
+            l0 = ctx.launch_count()
+            X, info = ctx.solve_block(op, P, n, tol=1e-12, recon=recon)
+            res[merge] = (ctx.unpack(X, n).cpu().numpy(), info, ctx.launch_count() - l0)
+            assert info["converged"] and max(info["relres"]) < 1e-12
+            assert rel_per_rhs(res[merge][0], Xr).max() < 1e-9, (op, merge)
+        assert rel_per_rhs(res[1][0], res[0][0]).max() < 1e-10
+        it0, it1 = res[0][1]["inner_iters_total"], res[1][1]["inner_iters_total"]
+        assert abs(it1 - it0) <= 4, (it0, it1)
+        assert res[1][2] < res[0][2]
+    ctx.close()
+
+
 @pytest.mark.parametrize("poll", [1, 3, 4])
 def test_graph_replay_of_iteration_blocks_changes_nothing(poll):
     """WD_OPT_GRAPH: blocks of WD_OPT_POLL_EVERY inner iterations replayed as a CUDA graph (captured at the second
