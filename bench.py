@@ -528,10 +528,14 @@ def run_ours(args):
     # enqueued between the last iteration and the next convergence poll; they must not dilute the average.)
     hop_cnt = 4 * (ix["inner_iters_total"] + iy["inner_iters_total"])
     tot_prof = sum(v[0] for v in prof.values())
-    # the four fp32 hop launches of one BiCGStab iteration: plain, xpay + <rt, v> (2 extra operands), plain,
-    # xpay + <t, s>, <t, t> (1 extra operand): 0.75 extra operands per launch on average
+    # the four fp32 hop launches of one BiCGStab iteration: plain, xpay + <rt, v> (2 extra operands), plain, and
+    # xpay + <t, s>, <t, t> (1 extra operand: 0.75 per launch on average) or, in the merged-update schedule the solver
+    # runs by default where the z-march kernel serves the hop, xpay + <t, s>, <t, t>, <rt, s>, <rt, t> (2 extra: 1.0)
     interior = (dims[3] - 1) / dims[3] if bc == wi.BC_SF else 1.0
-    hop_bytes = hop_bytes_per_launch(Vh, n, 4, R, extra_operands=0.75, interior=interior)
+    impl0 = ctx.get_option(pkg.OPT_HOP_IMPL)
+    merged = bool(ctx.get_option(pkg.OPT_MERGE)) and not ctx.get_option(pkg.OPT_PAIRED) and impl0 == 2 and \
+        (dims[0] // 2) % 2 == 0 and n >= 3
+    hop_bytes = hop_bytes_per_launch(Vh, n, 4, R, extra_operands=1.0 if merged else 0.75, interior=interior)
     hop_us = hop_ms * 1e3 / max(1, hop_cnt)
     achieved = hop_bytes / (hop_us * 1e-6) * 1e-9 if hop_cnt else 0.0
     # which kernel the library's dispatch picks (wd_hop.cu wd_hop_launch_ex): z-march (impl 2) or row-group ring (impl 1)
@@ -561,6 +565,8 @@ def run_ours(args):
                 "peak_source": peak_src, "traffic": traffic, "traffic_note": traffic_note, "bytes_per_launch": hop_bytes,
                 "bytes_counted": f"interior sites only for everything read ((T-1)/T = {interior:.4f}), all sites for the output",
                 "avg_launch_us": round(hop_us, 2), "launches_in_step": hop_cnt,
+                "schedule": "merged x,r,p update: 23 vector passes per iteration, 2 + 5 + 2 + 5 of them in the four hop launches" if merged
+                            else "textbook order: 25 vector passes per iteration, 2 + 4 + 2 + 3 of them in the four hop launches",
                 "timing": "CUDA event pairs on the library's stream around the two hop launches of every application of the "
                           "even/odd operator (one kernel-to-kernel gap inside each pair); in the graph-replayed blocks the pairs "
                           "are event-record nodes of the graph, read back after every replay",
