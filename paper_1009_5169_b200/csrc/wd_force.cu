@@ -64,7 +64,7 @@ __device__ __forceinline__ void force_dir(const ForceArgs& A, int p, long nb, in
 }
 
 __global__ void force_kernel(const ForceArgs A) {
-    extern __shared__ double sh[];  // [4][spb*n][18]
+    extern __shared__ double sh[];  // [4][18][spb*n]: component-major, so that the threads of a warp write consecutive words
     const int n = A.n, spb = A.spb;
     const int t = threadIdx.x;
     const int ls = t / n, r = t - ls * n;   // local site, column
@@ -78,13 +78,13 @@ __global__ void force_kernel(const ForceArgs A) {
         h = gsite - (long)p * A.Vh;
         const int4 n0 = __ldg(reinterpret_cast<const int4*>(A.nbr + gsite * WD_NDIR));
         const int4 n1 = __ldg(reinterpret_cast<const int4*>(A.nbr + gsite * WD_NDIR) + 1);
-        double* w = sh + (long)t * 18;
-        const int slab = spb * n * 18;
+        const int items = spb * n;
+        double* w = sh + t;               // element (mu, k) of this thread's item at w[(mu * 18 + k) * items]
         if ((uint32_t)n0.x & WD_SITE_FROZEN) {  // SF t=0: x(s) = y(s) = 0, so W = 0
 #pragma unroll
             for (int mu = 0; mu < 4; ++mu)
 #pragma unroll
-                for (int k = 0; k < 18; ++k) w[mu * slab + k] = 0.0;
+                for (int k = 0; k < 18; ++k) w[(mu * 18 + k) * items] = 0.0;
         } else {
             cx<double> x0[12], y0[12];
             const long hb = h / A.RB, ho = h - hb * A.RB, rbn = (long)A.RB * n;
@@ -93,16 +93,16 @@ __global__ void force_kernel(const ForceArgs A) {
             double wl[18];
             force_dir<0>(A, p, n0.x, r, x0, y0, wl);
 #pragma unroll
-            for (int k = 0; k < 18; ++k) w[0 * slab + k] = wl[k];
+            for (int k = 0; k < 18; ++k) w[(0 * 18 + k) * items] = wl[k];
             force_dir<1>(A, p, n0.z, r, x0, y0, wl);
 #pragma unroll
-            for (int k = 0; k < 18; ++k) w[1 * slab + k] = wl[k];
+            for (int k = 0; k < 18; ++k) w[(1 * 18 + k) * items] = wl[k];
             force_dir<2>(A, p, n1.x, r, x0, y0, wl);
 #pragma unroll
-            for (int k = 0; k < 18; ++k) w[2 * slab + k] = wl[k];
+            for (int k = 0; k < 18; ++k) w[(2 * 18 + k) * items] = wl[k];
             force_dir<3>(A, p, n1.z, r, x0, y0, wl);
 #pragma unroll
-            for (int k = 0; k < 18; ++k) w[3 * slab + k] = wl[k];
+            for (int k = 0; k < 18; ++k) w[(3 * 18 + k) * items] = wl[k];
         }
     }
     __syncthreads();
@@ -113,13 +113,14 @@ __global__ void force_kernel(const ForceArgs A) {
         if (g2 < 2 * A.Vh) {
             const int p2 = (int)(g2 / A.Vh);
             const long h2 = g2 - (long)p2 * A.Vh;
-            const double* w = sh + (long)mu * spb * n * 18 + (long)ls2 * n * 18;
+            const int items = spb * n;
+            const double* w = sh + (long)mu * 18 * items + (long)ls2 * n;
             cx<double> W[9];
 #pragma unroll
             for (int k = 0; k < 9; ++k) { W[k].re = 0.0; W[k].im = 0.0; }
             for (int rr = 0; rr < n; ++rr)
 #pragma unroll
-                for (int k = 0; k < 9; ++k) { W[k].re += w[rr * 18 + 2 * k]; W[k].im += w[rr * 18 + 2 * k + 1]; }
+                for (int k = 0; k < 9; ++k) { W[k].re += w[(2 * k) * items + rr]; W[k].im += w[(2 * k + 1) * items + rr]; }
             cx<double> u[9], M[9];
             const long hb2 = h2 / A.RB;
             load_link<18>(A.U + (long)(mu * 2 + p2) * 18 * A.Vh + hb2 * 18 * A.RB, (long)A.RB, h2 - hb2 * A.RB, u);
@@ -168,7 +169,8 @@ int wd_force_impl(wd_ctx* c, int n, const double* X, const double* Y, double* F)
     A.RB = c->RB;
     A.lg = c->rb_lg;
     A.n = n;
-    A.spb = 128 / n < 1 ? 1 : 128 / n;  // about 128 threads; at least 4*spb threads are needed for stage 2
+    // about 128 threads (255 registers each: 256 threads is all an SM holds); stage 2 needs 4 * spb of them
+    A.spb = 128 / n < 1 ? 1 : (128 / n > 32 ? 32 : 128 / n);
     int B = A.spb * n;
     if (B < 4 * A.spb) B = 4 * A.spb;
     B = (B + 31) / 32 * 32;

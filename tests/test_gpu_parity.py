@@ -208,6 +208,21 @@ def test_force_accumulates_and_matches_oracle_on_random_fields():
     ctx.close()
 
 
+@pytest.mark.parametrize("n_rhs", [1, 2, 3, 16])
+def test_force_for_every_block_shape(n_rhs):
+    """wd_force at the ends of the n_rhs range (the CTA shape depends on it; n_rhs = 1 once asked for 512 threads at 255
+    registers and failed to launch): parity with the oracle on random fields."""
+    pkg = _wd()
+    dims, bc, kappa = (8, 4, 6, 4), wi.BC_SF, 0.13
+    U = wi.gauge_field(dims, 0.4, 7, bc)
+    X = wi.spinor_field(dims, n_rhs, 21, bc)
+    Y = wi.spinor_field(dims, n_rhs, 22, bc)
+    ctx = make_ctx(dims, kappa, bc, n_rhs, U)
+    F = ctx.force(ctx.pack(dev(X)), ctx.pack(dev(Y)), n_rhs).cpu().numpy()
+    force_close(F, orc.force(dims, kappa, bc, U, X, Y), 1e-13)
+    ctx.close()
+
+
 def test_md_force_host_matches_device_path():
     pkg = _wd()
     cfg, U, Phi = wi.make_config(0)
