@@ -101,12 +101,15 @@ int wd_site_order(wd_ctx* ctx, int order, const int tile[4]);
  *       sites * n_rhs threads, halved until <= 1024).  0 (default) = chosen from n_rhs; else 1..1024.
  *   WD_OPT_HOP32_REGS / WD_OPT_HOP64_REGS    register budget per thread: picks among the compiled
  *       variants (fp32: 64, 128; fp64: 128, 168), clamped so that one CTA fits an SM.  0 (default) = chosen from n_rhs.
- *   WD_OPT_HOP_IMPL     1 (default): the hopping kernel that stages whole lattice rows through shared memory with
- *       bulk copies (cp.async.bulk + mbarrier ring, persistent CTAs, producer and consumer warps) wherever it
- *       applies (linear site order with Lx/2 even, i.e. the row-major native layout, and n_rhs >= 3), else the
- *       register kernel.
- *       0: always the register kernel (one thread per site and column, operands loaded straight into
- *       registers).  Same results bit for bit.
+ *   WD_OPT_HOP_IMPL     which hopping kernel serves a launch.  The two staged kernels (persistent CTAs, producer warps
+ *       feeding shared memory with cp.async.bulk + mbarrier, consumer warps) need the row-major native layout (linear
+ *       site order, Lx/2 even) and n_rhs >= 3; everything else goes to the register kernel.
+ *       2 (default): fp32: the z-march kernel (sliding window of three lattice planes) or, where its step would be
+ *          small and the rows long, the row-group ring kernel (csrc/wd_hop_zm.cu wd_hop_zm_preferred); fp64: the ring kernel.
+ *       3: the z-march kernel wherever it can run at all (fp32).
+ *       1: the ring kernel.
+ *       0: always the register kernel (one thread per site and column, operands loaded straight into registers).
+ *       The register and z-march kernels agree bit for bit; the ring kernel adds the eight directions in another order.
  *   WD_OPT_HOP_ROWS     staged kernel: upper bound on the lattice rows (consecutive in y) one CTA works on at a
  *       time; 0 (default) = as many as the thread and shared-memory budgets allow.  Fewer rows = smaller
  *       units, more ring slots (deeper prefetch), fewer consumer warps.

@@ -217,7 +217,7 @@ int wd_set_option(wd_ctx* ctx, int key, int value) {
             if (value != 0 && (value < 32 || value > 255)) return wd_fail(ctx, WD_EINVAL, "register budget out of range");
             break;
         case WD_OPT_HOP_IMPL:
-            if (value < 0 || value > 2) return wd_fail(ctx, WD_EINVAL, "hop implementation is 0, 1 or 2");
+            if (value < 0 || value > 3) return wd_fail(ctx, WD_EINVAL, "hop implementation is 0, 1, 2 or 3");
             break;
         case WD_OPT_ALTERNATE_SWEEP:
         case WD_OPT_PAIRED:

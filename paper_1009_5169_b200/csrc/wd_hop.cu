@@ -266,7 +266,8 @@ int wd_hop_launch_ex(wd_ctx* c, int prec, int recon, int dag, int n, int par, co
     }
     if (c->opt[WD_OPT_HOP_IMPL] >= 1 && n >= 3) {
         int rc = 1;
-        if (c->opt[WD_OPT_HOP_IMPL] == 2) rc = wd_hop_zm_launch(c, prec, recon, dag, n, par, o);
+        const int impl = c->opt[WD_OPT_HOP_IMPL];
+        if (impl == 3 || (impl == 2 && (prec != WD_F32 || wd_hop_zm_preferred(c, recon, n)))) rc = wd_hop_zm_launch(c, prec, recon, dag, n, par, o);
         if (rc > 0) rc = wd_hop_tma_launch(c, prec, recon, dag, n, par, o);
         if (rc <= 0) {
             if (rc == WD_OK) WD_LAUNCH_CHECK(c);

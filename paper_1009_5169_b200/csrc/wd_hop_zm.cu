@@ -817,6 +817,19 @@ bool wd_hop_zm_serves(const wd_ctx* c, int recon, int n, int storage) {
     return recon == WD_LINK18 ? pick_shape<float, 18, 0>(c, n, 512, &sh) : pick_shape<float, 12, 0>(c, n, 512, &sh);
 }
 
+// The dispatch rule of WD_OPT_HOP_IMPL = 2 for plain fp32 operands: the z-march kernel unless its step is small AND its
+// rows are long -- few consumer threads hide little latency, and long rows are what the row-group ring kernel copies well.
+// Measured at 24^4, fp32, 18-real links (us per launch, z-march / ring): n = 3: 46.8 / 55.6, 4: 57.9 / 56.2, 5: 59 / 71,
+// 6: 83.1 / 73.5, 8: 84.7 / 105.8, 10: 111.7 / 127.6, 12: 160.0 / 135.5, 16: 233.9 / 177.6; at 16^4 the z-march kernel is
+// ahead for every n up to 12.
+bool wd_hop_zm_preferred(const wd_ctx* c, int recon, int n) {
+    if (!wd_hop_zm_serves(c, recon, n, 0)) return false;
+    Shape sh;
+    if (recon == WD_LINK18) pick_shape<float, 18, 0>(c, n, 512, &sh); else pick_shape<float, 12, 0>(c, n, 512, &sh);
+    const size_t rowB = (size_t)(c->L[0] / 2) * n * 96;
+    return !(sh.threads - 128 < 320 && rowB >= 6000);
+}
+
 // Returns WD_OK if launched, a positive value if this lattice / option set is not served by this kernel (tiled site
 // order, fp64, nothing fits): the caller then tries wd_hop_tma.cu's kernel and then the register kernel.
 int wd_hop_zm_launch(wd_ctx* c, int prec, int recon, int dag, int n, int par, const wd_hop_ops& o) {

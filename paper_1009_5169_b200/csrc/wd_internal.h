@@ -198,6 +198,8 @@ int wd_hop_tma_launch(wd_ctx* c, int prec, int recon, int dag, int n, int par, c
 int wd_hop_zm_launch(wd_ctx* c, int prec, int recon, int dag, int n, int par, const wd_hop_ops& o);
 // does the z-march kernel serve this (n_rhs, link form, storage) on this context's lattice?
 bool wd_hop_zm_serves(const wd_ctx* c, int recon, int n, int storage);
+// ... and is it the faster of the two staged kernels there (plain fp32 operands)?
+bool wd_hop_zm_preferred(const wd_ctx* c, int recon, int n);
 int wd_hop_launch(wd_ctx* c, int prec, int recon, int dag, int n, int par, const void* in, void* out,
                   const void* in2, double a, double b);
 

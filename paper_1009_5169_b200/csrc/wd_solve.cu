@@ -295,9 +295,11 @@ int wd_inner_solve_f32(wd_ctx* c, int dag, int n, int recon, int max_inner, cons
     int rc;
     {
         // P32 (two sites per thread, packed fp32 instructions: wd_f2.cuh) wherever the z-march kernel serves it
-        const bool paired = c->opt[WD_OPT_PAIRED] != 0 && c->opt[WD_OPT_HOP_IMPL] == 2 && n >= 3 && wd_hop_zm_serves(c, recon, n, 2);
+        const int impl = c->opt[WD_OPT_HOP_IMPL];
+        const bool paired = c->opt[WD_OPT_PAIRED] != 0 && impl >= 2 && n >= 3 && wd_hop_zm_serves(c, recon, n, 2);
         // merged x,r,p update (WD_OPT_MERGE) wherever the z-march kernel, which has the seven-sum epilogue, serves the hop
-        const bool merged = c->opt[WD_OPT_MERGE] != 0 && !paired && c->opt[WD_OPT_HOP_IMPL] == 2 && n >= 3 && wd_hop_zm_serves(c, recon, n, 0);
+        const bool merged = c->opt[WD_OPT_MERGE] != 0 && !paired && n >= 3 &&
+                            ((impl == 2 && wd_hop_zm_preferred(c, recon, n)) || (impl == 3 && wd_hop_zm_serves(c, recon, n, 0)));
         {
             wd_prof_scope pr__(c, WD_PROF_BLAS);
             if (paired) demote_kernel<true><<<L32.G, L32.B, 0, st>>>(Vh, (long)c->RB, n, rb, R64, r32, rt32, x32, p32, v32);
