@@ -797,6 +797,10 @@ int launch_zm(wd_ctx* c, int dag, int n, int par, const wd_hop_ops& o, const T* 
     // shape runs the same kernel with run-time strides
 #define WD_ZM_GEOM(LXH, NR, RGT) if (A.Lxh == LXH && A.n == NR && A.RG == RGT) return launch_epi<T, RECON, MAXT, LXH, NR, RGT, ST>(c, A, sh, G, dag, o.epi)
     WD_ZM_GEOM(12, 5, 6);
+    if constexpr (ST == 0) {   // the other shapes of BASELINE.json's sweeps that this kernel serves: 24^4 at n_rhs = 8, 16^4 at n_rhs = 5
+        WD_ZM_GEOM(12, 8, 4);
+        WD_ZM_GEOM(8, 5, 8);
+    }
 #undef WD_ZM_GEOM
     return launch_epi<T, RECON, MAXT, 0, 0, 0, ST>(c, A, sh, G, dag, o.epi);
 }
