@@ -291,6 +291,14 @@ int wd_inner_solve_f32(wd_ctx* c, int dag, int n, int recon, int max_inner, cons
     RedBuf rb{c->d_scal, c->d_partials, c->d_ticket};
     const long nv32 = 6 * Vh * n;
     const Launch L32 = blas_cfg(c, nv32, n);
+    // Schroedinger functional, row-major layout: the rows of the frozen t = 0 slice open every half-lattice block and hold
+    // zeros in every vector of the solver (the demotion writes them, the hops keep them); the update kernels of the
+    // iteration skip them: 1/T of their bytes
+    const long skip = (c->bc == WD_BC_SF && c->order == WD_ORDER_LINEAR && c->RB == (uint32_t)(c->L[0] / 2))
+                          ? (long)c->L[1] * c->L[2] * 6 * (c->L[0] / 2) * n : 0;
+    const long nvu = nv32 - skip;
+    const Launch LU = blas_cfg(c, nvu, n);
+    float4 *xu = x32 + skip, *ru = r32 + skip, *pu = p32 + skip, *vu = v32 + skip, *tu = t32 + skip, *rtu = rt32 + skip;
     double* hp = c->h_pinned;
     int rc;
     {
@@ -322,8 +330,8 @@ int wd_inner_solve_f32(wd_ctx* c, int dag, int n, int recon, int max_inner, cons
         auto enqueue_iteration = [&]() -> int {
             if (!merged) {
                 wd_prof_scope pr__(c, WD_PROF_BLAS);
-                if (paired) p_update_kernel<float, true><<<L32.G, L32.B, 0, c->stream>>>(nv32, n, sweep(), c->d_scal, r32, p32, v32);
-                else p_update_kernel<float, false><<<L32.G, L32.B, 0, c->stream>>>(nv32, n, sweep(), c->d_scal, r32, p32, v32);
+                if (paired) p_update_kernel<float, true><<<LU.G, LU.B, 0, c->stream>>>(nvu, n, sweep(), c->d_scal, ru, pu, vu);
+                else p_update_kernel<float, false><<<LU.G, LU.B, 0, c->stream>>>(nvu, n, sweep(), c->d_scal, ru, pu, vu);
                 WD_LAUNCH_CHECK(c);
             }
             // v = Ahat p, sigma = <rt, v> -> alpha.  (wd_profile: one event pair brackets the two hop launches of an
@@ -342,8 +350,8 @@ int wd_inner_solve_f32(wd_ctx* c, int dag, int n, int recon, int max_inner, cons
             }
             {
                 wd_prof_scope pr__(c, WD_PROF_BLAS);
-                if (paired) s_update_kernel<float, true><<<L32.G, L32.B, 0, c->stream>>>(nv32, n, sweep(), c->d_scal, r32, v32);
-                else s_update_kernel<float, false><<<L32.G, L32.B, 0, c->stream>>>(nv32, n, sweep(), c->d_scal, r32, v32);
+                if (paired) s_update_kernel<float, true><<<LU.G, LU.B, 0, c->stream>>>(nvu, n, sweep(), c->d_scal, ru, vu);
+                else s_update_kernel<float, false><<<LU.G, LU.B, 0, c->stream>>>(nvu, n, sweep(), c->d_scal, ru, vu);
             }
             WD_LAUNCH_CHECK(c);
             // t = Ahat s, <t, s>, <t, t> -> omega
@@ -360,9 +368,9 @@ int wd_inner_solve_f32(wd_ctx* c, int dag, int n, int recon, int max_inner, cons
             }
             {
                 wd_prof_scope pr__(c, WD_PROF_BLAS);
-                if (merged) xrp_update_kernel<float, false><<<L32.G, L32.B, 0, c->stream>>>(nv32, n, sweep(), rb, x32, p32, r32, t32, v32);
-                else if (paired) xr_update_kernel<float, true><<<L32.G, L32.B, 0, c->stream>>>(nv32, n, sweep(), rb, x32, p32, r32, t32, rt32);
-                else xr_update_kernel<float, false><<<L32.G, L32.B, 0, c->stream>>>(nv32, n, sweep(), rb, x32, p32, r32, t32, rt32);
+                if (merged) xrp_update_kernel<float, false><<<LU.G, LU.B, 0, c->stream>>>(nvu, n, sweep(), rb, xu, pu, ru, tu, vu);
+                else if (paired) xr_update_kernel<float, true><<<LU.G, LU.B, 0, c->stream>>>(nvu, n, sweep(), rb, xu, pu, ru, tu, rtu);
+                else xr_update_kernel<float, false><<<LU.G, LU.B, 0, c->stream>>>(nvu, n, sweep(), rb, xu, pu, ru, tu, rtu);
             }
             WD_LAUNCH_CHECK(c);
             return WD_OK;
