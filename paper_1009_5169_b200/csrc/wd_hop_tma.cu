@@ -306,7 +306,9 @@ __global__ void __launch_bounds__(MAXT, 1) hop_tma_kernel(const TmaArgs<T> A) {
 #pragma unroll
             for (int u = 0; u < 4; ++u) {
                 const uint32_t m = 4 * q + u, slot = 1 + m % A.NS, use = m / A.NS;
-                if (EPI >= EPI_XPAY && u == 3 && active) load_spinor(A.in2 + own, rowV, e0, qv);
+                // (fp32 only: in fp64 the 24 extra doubles live across the last direction spill, 56-116 bytes of stack; there
+                // the operand, prefetched into L2 at the start of the group, is loaded in the epilogue)
+                if (EPI >= EPI_XPAY && u == 3 && active && sizeof(T) == 4) load_spinor(A.in2 + own, rowV, e0, qv);
                 mbar_wait(&full[slot], use & 1);
                 if (active) {
                     const vec* sp = reinterpret_cast<const vec*>(ring) + A.big_vecs + (size_t)(slot - 1) * A.small_vecs +
@@ -325,6 +327,7 @@ __global__ void __launch_bounds__(MAXT, 1) hop_tma_kernel(const TmaArgs<T> A) {
             // ---- epilogue and store
             if (active) {
                 if (EPI >= EPI_XPAY) {
+                    if (sizeof(T) == 8) load_spinor(A.in2 + own, rowV, e0, qv);
 #pragma unroll
                     for (int k = 0; k < 12; ++k) {
                         acc[k].re = fma(A.b, acc[k].re, A.a * qv[k].re);
