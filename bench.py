@@ -42,8 +42,9 @@ def parse_args():
     ap.add_argument("--n-rhs", type=int, default=5)
     ap.add_argument("--recon", type=int, default=18, choices=(12, 18), help="inner fp32 link form")
     ap.add_argument("--impl", default="ours", choices=("ours", "reference"))
-    ap.add_argument("--hop-impl", type=int, default=-1, choices=(-1, 0, 1),
-                    help="WD_OPT_HOP_IMPL: 0 register kernel, 1 shared-memory-staged kernel, -1 library default")
+    ap.add_argument("--hop-impl", type=int, default=-1, choices=(-1, 0, 1, 2, 3),
+                    help="WD_OPT_HOP_IMPL: 0 register kernel, 1 row-group ring kernel, 2 z-march or ring by shape (library default), "
+                         "3 z-march wherever it runs, -1 leave the default")
     ap.add_argument("--rhs-sweep", action="store_true", help="configs[4]: blocked solve at n_rhs = 1, 2, 5, 8, 12")
     ap.add_argument("--apply-sweep", action="store_true", help="configs[3]: D, D^dag apply on 16^4, fp32/fp64 x 18/12 reals")
     ap.add_argument("--shard-rhs", action="store_true",
@@ -542,7 +543,9 @@ def run_ours(args):
     # where the layout is row-major (linear site order, Lx/2 even, max_rhs >= 3) and n_rhs >= 3, else the register kernel
     impl = ctx.get_option(pkg.OPT_HOP_IMPL)
     staged = impl >= 1 and (dims[0] // 2) % 2 == 0 and n >= 3
-    kname = (f"hop_zm_kernel<float,{R}>" if impl == 2 else f"hop_tma_kernel<float,{R}>") if staged else f"hop_kernel<float,{R}>"
+    # (impl 2 hands shapes with a small step and long rows to the ring kernel: csrc/wd_hop_zm.cu wd_hop_zm_preferred; the
+    # bench workload, 24^4 at n_rhs = 5, is served by the z-march kernel, as profiles/r02_launches.md shows)
+    kname = (f"hop_zm_kernel<float,{R}>" if impl >= 2 else f"hop_tma_kernel<float,{R}>") if staged else f"hop_kernel<float,{R}>"
     # dram__bytes_read.sum + dram__bytes_write.sum per launch from an ncu --set full capture of THIS kernel source: the
     # committed record carries the sha256 of the kernel's source file and is ignored when the source has changed since
     traffic, traffic_note, ncu_us = None, "no capture on record for this kernel source", None
