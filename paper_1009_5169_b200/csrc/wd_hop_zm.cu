@@ -35,7 +35,7 @@ using namespace wdtma;
 
 namespace {
 #ifndef WD_ZM_ABLATE
-#define WD_ZM_ABLATE 0   // measurement builds only (_work/): 1 = consumers skip the arithmetic, 2 = no copies, no waits
+#define WD_ZM_ABLATE 0   // measurement builds only (build.py WD_NVCC_DEFINES, profiles/r02_hop_ablations.md): 1 = consumers skip the arithmetic, 2 = no copies, no waits
 #endif
 #if WD_ZM_ABLATE == 2
 #define mbar_wait(b, p) ((void)0)
@@ -287,7 +287,7 @@ __global__ void __launch_bounds__(MAXT, 1) hop_zm_kernel(const ZmArgs<T> A) {
         }
     } else if (warp >= ncw) {
         // ================= producer warps ================================================================
-        // One thread can start a bulk copy only every ~280 ns (measured: _work/ubench/tma_stream2.cu; the copy engine
+        // One thread can start a bulk copy only every ~280 ns (measured with a stand-alone streaming probe; the copy engine
         // itself takes 8 issuers in parallel at 85-92 GB/s per SM), and a step needs 13-14 copies, so the units are
         // dealt to FOUR producer warps, each walking the steps on its own and waiting only for its own buffers:
         //   P0: U1 {T+ rows, link t+}, U3 {link z-}      P1: U2 {T- rows, link t-}, window planes
