@@ -460,6 +460,30 @@ def test_merged_update_schedule_matches_oracle_and_textbook_order(cfg_idx, n_rhs
     ctx.close()
 
 
+@pytest.mark.parametrize("merge", [0, 1])
+def test_solver_that_cannot_converge_says_so(merge):
+    """An iteration budget that is too small, and a kappa far beyond the critical one (no convergence at all): wd_solve_block
+    returns WD_ENOCONV with converged = 0, finite residuals in info and a finite best iterate, in both update schedules;
+    given the budget back it converges on the first system."""
+    pkg = _wd()
+    cfg, U, Phi = wi.make_config(1)
+    dims, bc, n = cfg["dims"], cfg["bc"], cfg["n_rhs"]
+    for kappa, budget in ((cfg["kappa"], (1, 8)), (0.9, (4, 60))):
+        ctx = make_ctx(dims, kappa, bc, n, U)
+        ctx.set_option(pkg.OPT_MERGE, merge)
+        P = ctx.pack(dev(Phi))
+        X, info = ctx.solve_block(pkg.OP_D, P, n, tol=1e-12, max_outer=budget[0], max_inner=budget[1], raise_on_noconv=False)
+        assert not info["converged"]
+        assert all(np.isfinite(info["relres"])) and max(info["relres"]) > 1e-12
+        assert bool(torch.isfinite(X).all())
+        with pytest.raises(pkg.WdError):
+            ctx.solve_block(pkg.OP_D, P, n, tol=1e-12, max_outer=budget[0], max_inner=budget[1])
+        if kappa == cfg["kappa"]:
+            X, info = ctx.solve_block(pkg.OP_D, P, n, tol=1e-12)
+            assert info["converged"] and max(info["relres"]) < 1e-12
+        ctx.close()
+
+
 @pytest.mark.parametrize("poll", [1, 3, 4])
 def test_graph_replay_of_iteration_blocks_changes_nothing(poll):
     """WD_OPT_GRAPH: blocks of WD_OPT_POLL_EVERY inner iterations replayed as a CUDA graph (captured at the second
