@@ -484,6 +484,27 @@ def test_solver_that_cannot_converge_says_so(merge):
         ctx.close()
 
 
+def test_zero_and_duplicate_columns():
+    """Degenerate blocks: a zero right-hand side column (solution zero, the other columns unaffected) and two identical
+    columns (identical solutions): the per-column scalars keep the columns apart and a frozen column never spoils the rest."""
+    pkg = _wd()
+    cfg, U, Phi = wi.make_config(1)
+    dims, kappa, bc, n = cfg["dims"], cfg["kappa"], cfg["bc"], cfg["n_rhs"]
+    Phi = Phi.copy()
+    Phi[1] = 0.0
+    Phi[3] = Phi[0]
+    ctx = make_ctx(dims, kappa, bc, n, U)
+    X, info = ctx.solve_block(pkg.OP_D, ctx.pack(dev(Phi)), n, tol=1e-12)
+    assert info["converged"]
+    Xc = ctx.unpack(X, n).cpu().numpy()
+    assert np.all(Xc[1] == 0.0)
+    assert np.linalg.norm(Xc[3] - Xc[0]) <= 1e-12 * np.linalg.norm(Xc[0])
+    Xr, rr, _, rc = orc.solve(dims, kappa, bc, 0, U, Phi[[0, 2, 4]], tol=1e-14)
+    assert rc == 0 and rr.max() < 1e-13
+    assert rel_per_rhs(Xc[[0, 2, 4]], Xr).max() < 1e-9
+    ctx.close()
+
+
 @pytest.mark.parametrize("poll", [1, 3, 4])
 def test_graph_replay_of_iteration_blocks_changes_nothing(poll):
     """WD_OPT_GRAPH: blocks of WD_OPT_POLL_EVERY inner iterations replayed as a CUDA graph (captured at the second
