@@ -240,6 +240,40 @@ int wd_md_force(wd_ctx* ctx, int variant, int n_rhs, const double* Phi_native_de
                 double* Y_native_dev, double* F_canon_dev, double* S_host, double tol, int max_outer, int max_inner,
                 double inner_tol, int recon, wd_solve_info* info2);
 
+/* The action without a context, a workspace or any allocation: S_dev[i] = sum over the block of |x_i|^2, i.e. what
+ * wd_action computes (eq. 2.2; the number the Metropolis step of PAPER.md:60 needs), for callers that
+ * cannot allocate device memory -- a lattice code that has given the whole card to its own field arena, or code that
+ * must not stall other streams (cudaMalloc and cudaFree synchronise the device).  wd_action needs a context whose
+ * workspace the caller has to cudaMalloc; this call needs neither.  It calls no cudaMalloc, cudaFree, cudaMallocHost
+ * or any other allocating routine, creates no stream or event, and does not synchronise.
+ *   X_native_dev  DEVICE, read: n_complex consecutive complex numbers (double2) of a native fp64 block, RHS-minor,
+ *                 starting at a multiple of n_rhs complex numbers -- a whole block (wd_native_bytes / 16 numbers), or one
+ *                 parity half of it (the first half is the even sites, the second the odd ones).  16-byte aligned.
+ *   S_dev         DEVICE, written: n_rhs doubles, overwritten (not accumulated) by the kernel.  The result is there
+ *                 when the work enqueued on cuda_stream has finished; nothing is copied to the host.
+ *   cuda_stream   a cudaStream_t of the CURRENT device (NULL = legacy default stream).  X and S must be memory of
+ *                 that device too (checked).
+ * Scratch: the per-block partial sums and a ticket counter live in a fixed __device__ array inside the library,
+ * WD_STATIC_SCRATCH_BYTES (2 MiB + 256 B) that every GPU which loads libwd.so holds until the process exits.  Its size
+ * bounds the input: n_complex / n_rhs <= WD_STATIC_MAX_ROWS (2^25; a 24^4 block has 4.0e6 such rows for any n_rhs, a
+ * 40^4 block 3.1e7); beyond that the call returns WD_EINVAL and wd_action_static_error() says so -- use wd_action.
+ * Sharing: every call on a device uses the same array, which keeps what the previous call left in it; the call
+ * clears the one word that must start at zero (stream-ordered, before its kernel).  Calls enqueued on ONE stream are
+ * therefore safe back to back; two calls that can overlap on the GPU (different streams or threads, same device)
+ * race on the array and give wrong sums -- order them with an event.
+ * First call on a device: looks up the array's device address (cudaGetSymbolAddress, once per device, with that
+ * device current), which can make the driver load the library's kernels; make that first call at set-up time, before
+ * any stream capture is begun.
+ * The sum is fp64 and its order depends only on (n_rhs, n_complex), not on the GPU: the same input gives the same
+ * bits everywhere (wd_action's order depends on the SM count; the two agree to rounding, ~1e-15 relative).
+ * Errors: WD_EINVAL (n_rhs outside 1..WD_MAX_RHS, null or misaligned pointer, n_complex zero or not a multiple of
+ * n_rhs, input beyond the limit, memory not on the current device), WD_ECUDA.  wd_action_static_error() returns the
+ * text for the calling thread's last failure of this call ("" after a success); it never returns NULL. */
+#define WD_STATIC_MAX_ROWS 33554432        /* 2^25 = 16384 thread blocks x 2048 rows */
+#define WD_STATIC_SCRATCH_BYTES 2097408    /* 16384 x WD_MAX_RHS doubles + one 256-byte line for the counter */
+int wd_action_static(int n_rhs, size_t n_complex, const double* X_native_dev, double* S_dev, void* cuda_stream);
+const char* wd_action_static_error(void);
+
 /* Per-class device timing for measurement (bench.py's roofline line).  wd_profile(ctx, 1) makes every
  * later hop / BLAS1 / force launch record a CUDA event pair on the context's stream (a few
  * microseconds of host time each; leave it off when timing whole calls).  wd_profile_read

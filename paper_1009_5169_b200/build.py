@@ -16,7 +16,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libwd.so")
-SOURCES = ["wd_ctx.cu", "wd_layout.cu", "wd_hop.cu", "wd_hop_tma.cu", "wd_hop_zm.cu", "wd_solve.cu", "wd_solve_h16.cu", "wd_solve_gl.cu", "wd_force.cu", "wd_md.cu"]
+SOURCES = ["wd_ctx.cu", "wd_layout.cu", "wd_hop.cu", "wd_hop_tma.cu", "wd_hop_zm.cu", "wd_solve.cu", "wd_solve_h16.cu", "wd_solve_gl.cu", "wd_force.cu", "wd_md.cu", "wd_noalloc.cu"]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC", "--use_fast_math=false"]
 

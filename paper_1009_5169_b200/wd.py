@@ -39,7 +39,9 @@ SYMBOLS = ["wd_create", "wd_destroy", "wd_site_order", "wd_workspace_bytes", "wd
            "wd_set_option", "wd_get_option", "wd_set_gauge", "wd_native_bytes", "wd_pack", "wd_unpack", "wd_apply", "wd_hop",
            "wd_solve_block", "wd_force", "wd_md_force_host", "wd_md_force_host_gauge", "wd_refresh", "wd_action",
            "wd_project_parity", "wd_md_force", "wd_profile", "wd_profile_read", "wd_launch_count", "wd_strerror",
-           "wd_last_error", "wd_version"]
+           "wd_last_error", "wd_version", "wd_action_static", "wd_action_static_error"]
+STATIC_MAX_ROWS = 1 << 25          # WD_STATIC_MAX_ROWS
+STATIC_SCRATCH_BYTES = 2097408     # WD_STATIC_SCRATCH_BYTES
 
 
 class SolveInfo(ctypes.Structure):
@@ -107,6 +109,9 @@ def lib():
     L.wd_last_error.argtypes = [vp]
     L.wd_last_error.restype = ctypes.c_char_p
     L.wd_version.restype = ctypes.c_char_p
+    L.wd_action_static.argtypes = [ci, sz, vp, vp, vp]
+    L.wd_action_static.restype = ci
+    L.wd_action_static_error.restype = ctypes.c_char_p
     for name in ("wd_create", "wd_destroy", "wd_site_order", "wd_set_option", "wd_get_option", "wd_set_workspace", "wd_set_gauge", "wd_pack",
                  "wd_unpack", "wd_apply", "wd_hop", "wd_solve_block", "wd_force", "wd_md_force_host", "wd_md_force_host_gauge", "wd_refresh", "wd_action",
            "wd_project_parity", "wd_md_force", "wd_profile",
@@ -118,6 +123,33 @@ def lib():
 
 def _dims(dims):
     return (ctypes.c_int * 4)(*[int(d) for d in dims])
+
+
+def action_static(X_native, n_rhs, parity_sel=PARITY_BOTH, out=None, stream=None):
+    """wd_action_static: per-column |x_i|^2 of a native fp64 block WITHOUT a Context -- for callers that cannot
+    allocate device memory (all of it is in their own arena, or a cudaMalloc would stall their other streams).  The
+    library allocates nothing: its scratch is a fixed array inside libwd.so, which limits the input to
+    STATIC_MAX_ROWS * n_rhs complex numbers and means two calls that overlap on the GPU race (calls on one stream are
+    fine).  `out` is the caller's n_rhs-double CUDA tensor (made here with torch only if omitted); the result is
+    stream-ordered on `stream` (default: torch's current stream), nothing is synchronised or copied to the host.
+    parity_sel picks the even half, the odd half or the whole block, as in Context.action."""
+    assert X_native.is_cuda and X_native.dtype == torch.float64 and X_native.is_contiguous()
+    n = int(n_rhs)
+    total = X_native.numel() // 2   # complex numbers in the whole block
+    half = total // 2
+    offset, count = {PARITY_BOTH: (0, total), PARITY_EVEN: (0, half), PARITY_ODD: (half, half)}[int(parity_sel)]
+    if out is None:
+        out = torch.empty(n, dtype=torch.float64, device=X_native.device)
+    assert out.is_cuda and out.dtype == torch.float64 and out.is_contiguous() and out.numel() >= n
+    if stream is None:
+        stream = torch.cuda.current_stream(X_native.device)
+    L = lib()
+    with torch.cuda.device(X_native.device):   # the library uses the current device's copy of its scratch array
+        rc = L.wd_action_static(n, count, ctypes.c_void_p(X_native.data_ptr() + 16 * offset),
+                                ctypes.c_void_p(out.data_ptr()), ctypes.c_void_p(stream.cuda_stream))
+    if rc != OK:
+        raise WdError(rc, f"{L.wd_strerror(rc).decode()}: {L.wd_action_static_error().decode()}")
+    return out
 
 
 class Context:
