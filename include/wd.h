@@ -131,6 +131,9 @@ int wd_site_order(wd_ctx* ctx, int order, const int tile[4]);
  *       WD_SOLVER_GL_F64: case B, the same without preconditioner (all fp64; info.inner_iters_total = its iterations).
  *       WD_SOLVER_BL_F64: case C, fp64 Block BiCGStab (ref. [7] of the paper): n_rhs x n_rhs coefficient matrices from the
  *       Gram matrices of the block vectors, one Krylov space shared by the columns; max_inner bounds its iterations.
+ *       The n x n systems need a block of full rank: with a zero column, two equal columns, or on a breakdown of the
+ *       recurrence (pivot below 1e-13 of the largest Gram entry) the iteration freezes and the default solver
+ *       (WD_SOLVER_DC_F32) does the solve instead, with max_outer and max_inner as given.
  *   WD_OPT_PAIRED       1: the fp32 inner solver computes in the x-paired form WD_F32P (two sites per thread, packed
  *       fp32 instructions) wherever the z-march hop kernel serves the shape; 0 (default): plain WD_F32.  Same iterates
  *       up to the summation order of the inner products.  (Measured at 24^4, n_rhs = 5: 64 us against 59 us per hop --

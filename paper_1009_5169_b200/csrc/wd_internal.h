@@ -221,6 +221,9 @@ int wd_inner_solve_f32(wd_ctx* c, int dag, int n, int recon, int max_inner, cons
 // wd_solve_gl.cu
 int wd_solve_gl(wd_ctx* c, int flex, int dag, int n, const double* Phi, double* X, double tol, int max_outer, int max_inner,
                 double inner_tol, int recon, wd_solve_info* info);
+// returns WD_BL_BREAKDOWN (> 0, never seen by the caller of the C ABI) when the block recurrence lost rank: X is then
+// the last good iterate of the even sites only and wd_solve_impl runs the default route instead
+#define WD_BL_BREAKDOWN 1
 int wd_solve_bl(wd_ctx* c, int dag, int n, const double* Phi, double* X, double tol, int max_iters, wd_solve_info* info);
 // wd_solve_h16.cu
 bool wd_solve_h16_applies(const wd_ctx* c, int n);

@@ -477,7 +477,11 @@ int wd_solve_impl(wd_ctx* c, int dag, int n, const double* Phi, double* X, doubl
     if (solver == WD_SOLVER_GL_FLEX || solver == WD_SOLVER_GL_F64)
         return wd_solve_gl(c, solver == WD_SOLVER_GL_FLEX, dag, n, Phi, X, tol, max_outer, max_inner, inner_tol > 0.0 ? inner_tol : 1e-5,
                            recon, info);
-    if (solver == WD_SOLVER_BL_F64) return wd_solve_bl(c, dag, n, Phi, X, tol, max_inner, info);
+    if (solver == WD_SOLVER_BL_F64) {
+        const int rc = wd_solve_bl(c, dag, n, Phi, X, tol, max_inner, info);
+        if (rc != WD_BL_BREAKDOWN) return rc;
+        // rank-deficient block (zero or equal columns) or breakdown: the per-column default route solves it
+    }
     if (solver == WD_SOLVER_RELIABLE_H16 && wd_solve_h16_applies(c, n))
         return wd_solve_h16(c, dag, n, Phi, X, tol, max_outer, max_inner, inner_tol > 0.0 ? inner_tol : 0.01, recon, info);
     // default: the fp32 recurrence is run down to 3e-7, about what fp32 can deliver, so that TWO inner solves reach

@@ -255,14 +255,23 @@ namespace {
 enum { BL_MG = 0, BL_MR = 1, BL_MT = 2, BL_ALPHA = 3, BL_BETA = 4, BL_NMAT = 5 };
 constexpr int BL_LD = 2 * WD_MAX_RHS * WD_MAX_RHS;   // doubles per matrix
 
-// MA[i][j] += sum_g conj(Rt[g,i]) A[g,j]   (and MB with B when B != null); one thread per (g, i, j), stride % n^2 == 0
-__global__ void bl_gram(long ng, int n, const double2* __restrict__ Rt, const double2* __restrict__ A, const double2* B, double* MA, double* MB) {
-    extern __shared__ double shg[];   // [2][n*n][2]
-    const int nn = n * n;
-    for (int k = threadIdx.x; k < 4 * nn; k += blockDim.x) shg[k] = 0.0;
-    __syncthreads();
-    const long total = ng * nn, stride = (long)gridDim.x * blockDim.x;
-    const long i0 = (long)blockIdx.x * blockDim.x + threadIdx.x;
+// Every kernel of a Block BiCGStab iteration is a no-op once the recurrence has broken down or every column has converged:
+// iterations enqueued between two polls of the host then leave X and R at the last good iterate (wd.h: X holds the best
+// iterate on WD_ENOCONV).
+__device__ __forceinline__ bool bl_frozen(const double* scal) { return scal[G_GL_BREAK] != 0.0 || scal[G_OUT_DONE] != 0.0; }
+
+// MA[i][j] = sum_g conj(Rt[g,i]) A[g,j]   (and MB with B when B != null), written, not accumulated; one thread per
+// (g, i, j), stride % n^2 == 0.  The sums are added in a fixed order (threads of one entry within a block in index
+// order, then the block partials in block order by the last block to finish), so the result is the same run to run,
+// like every other reduction of the library.  partials: gridDim.x * (B ? 4 : 2) * n * n doubles.
+__global__ void bl_gram(long ng, int n, const double2* __restrict__ Rt, const double2* __restrict__ A, const double2* B, double* MA, double* MB,
+                        const double* __restrict__ scal, double* partials, unsigned int* ticket) {
+    if (bl_frozen(scal)) return;
+    extern __shared__ double shg[];   // [4][blockDim.x]
+    __shared__ bool is_last;
+    const int nn = n * n, t = threadIdx.x, Bd = blockDim.x;
+    const long total = ng * nn, stride = (long)gridDim.x * Bd;
+    const long i0 = (long)blockIdx.x * Bd + t;
     const int ij = (int)(i0 % nn), i = ij / n, j = ij - i * n;
     double ar = 0.0, ai = 0.0, br = 0.0, bi = 0.0;
     for (long idx = i0; idx < total; idx += stride) {
@@ -276,23 +285,46 @@ __global__ void bl_gram(long ng, int n, const double2* __restrict__ Rt, const do
             bi += q.x * b.y - q.y * b.x;
         }
     }
-    atomicAdd(&shg[2 * ij], ar); atomicAdd(&shg[2 * ij + 1], ai);
-    if (B) { atomicAdd(&shg[2 * nn + 2 * ij], br); atomicAdd(&shg[2 * nn + 2 * ij + 1], bi); }
+    shg[t] = ar; shg[Bd + t] = ai; shg[2 * Bd + t] = br; shg[3 * Bd + t] = bi;
     __syncthreads();
-    for (int k = threadIdx.x; k < 2 * nn; k += blockDim.x) {
-        atomicAdd(&MA[k], shg[k]);
-        if (B) atomicAdd(&MB[k], shg[2 * nn + k]);
+    // item k = ((matrix m) * nn + entry) * 2 + (re, im): the layout of MA followed by MB
+    const int items = (B ? 4 : 2) * nn;
+    for (int k = t; k < items; k += Bd) {
+        const int cpl = k & 1, e = k >> 1, m = e / nn, ent = e - m * nn;
+        double sum = 0.0;
+        for (int q = ent; q < Bd; q += nn) sum += shg[(2 * m + cpl) * Bd + q];
+        partials[(size_t)blockIdx.x * items + k] = sum;
     }
+    __threadfence();
+    __syncthreads();
+    if (t == 0) is_last = (atomicAdd(ticket, 1u) == gridDim.x - 1);
+    __syncthreads();
+    if (!is_last) return;
+    __threadfence();
+    for (int k = t; k < items; k += Bd) {
+        double sum = 0.0;
+        for (unsigned g = 0; g < gridDim.x; ++g) sum += __ldcg(partials + (size_t)g * items + k);
+        const int e = k >> 1, m = e / nn;
+        (m ? MB : MA)[k - 2 * m * nn] = sum;
+    }
+    if (t == 0) *ticket = 0u;
 }
 
-// OUT = sign * MG^-1 RHS  (n x n complex, row-major, Gaussian elimination with partial pivoting; one thread)
+// OUT = sign * MG^-1 RHS  (n x n complex, row-major, Gaussian elimination with partial pivoting; one thread).
+// A pivot below 1e-13 of the largest entry of MG means the block has lost rank (a zero column, two equal columns, or
+// the recurrence itself breaking down): OUT = 0 and the break flag is set, which freezes X and R (bl_frozen).
 __global__ void bl_small_solve(int n, const double* __restrict__ MG, const double* __restrict__ RHS, double* OUT, double sign, double* scal) {
+    if (bl_frozen(scal)) return;
     double2 a[WD_MAX_RHS][WD_MAX_RHS], b[WD_MAX_RHS][WD_MAX_RHS];
+    double amax2 = 0.0;
     for (int i = 0; i < n; ++i)
         for (int j = 0; j < n; ++j) {
             a[i][j] = make_double2(MG[2 * (i * n + j)], MG[2 * (i * n + j) + 1]);
             b[i][j] = make_double2(sign * RHS[2 * (i * n + j)], sign * RHS[2 * (i * n + j) + 1]);
+            const double m2 = a[i][j].x * a[i][j].x + a[i][j].y * a[i][j].y;
+            if (m2 > amax2) amax2 = m2;
         }
+    const double floor2 = 1e-26 * amax2;
     for (int k = 0; k < n; ++k) {
         int piv = k;
         double best = a[k][k].x * a[k][k].x + a[k][k].y * a[k][k].y;
@@ -300,7 +332,11 @@ __global__ void bl_small_solve(int n, const double* __restrict__ MG, const doubl
             const double m = a[i][k].x * a[i][k].x + a[i][k].y * a[i][k].y;
             if (m > best) { best = m; piv = i; }
         }
-        if (!(best > 0.0)) { scal[G_GL_BREAK] = 1.0; return; }
+        if (!(best > floor2)) {   // also catches NaN
+            for (int q = 0; q < 2 * n * n; ++q) OUT[q] = 0.0;
+            scal[G_GL_BREAK] = 1.0;
+            return;
+        }
         if (piv != k)
             for (int j = 0; j < n; ++j) { double2 t = a[k][j]; a[k][j] = a[piv][j]; a[piv][j] = t; t = b[k][j]; b[k][j] = b[piv][j]; b[piv][j] = t; }
         const double2 inv = make_double2(a[k][k].x / best, -a[k][k].y / best);
@@ -326,6 +362,7 @@ __global__ void bl_small_solve(int n, const double* __restrict__ MG, const doubl
 // out[g,i] = base[g,i] + csign * sum_j (A[g,j] - w B[g,j]) M[j][i]   (B nullable: w ignored); thread = (g, i)
 __global__ void bl_axpm(long nvec, int n, const double2* __restrict__ Base, const double2* __restrict__ A, const double2* B,
                         const double* __restrict__ scal, const double* __restrict__ M, double csign, double2* Out) {
+    if (bl_frozen(scal)) return;
     extern __shared__ double shm[];   // M: [n][n][2]
     for (int k = threadIdx.x; k < 2 * n * n; k += blockDim.x) shm[k] = M[k];
     __syncthreads();
@@ -350,6 +387,7 @@ __global__ void bl_axpm(long nvec, int n, const double2* __restrict__ Base, cons
 // X += P alpha + omega S;  R = S - omega T;  |R_i|^2 -> per-column convergence
 __global__ void bl_xr_update(long nvec, int n, RedBuf rb, double2* X, const double2* __restrict__ P, const double* __restrict__ ALPHA,
                              const double2* __restrict__ S, const double2* __restrict__ T, double2* R) {
+    if (bl_frozen(rb.scal)) return;
     extern __shared__ double shm[];
     for (int k = threadIdx.x; k < 2 * n * n; k += blockDim.x) shm[k] = ALPHA[k];
     __syncthreads();
@@ -411,8 +449,10 @@ int wd_solve_bl(wd_ctx* c, int dag, int n, const double* Phi, double* X, double 
     const GlLaunch L = gl_cfg(c, nv, n), Lf = gl_cfg(c, 2 * nv, n);
     const int nn = n * n;
     const int Bg = nn * (256 / nn > 0 ? 256 / nn : 1);
-    const unsigned Gg = (unsigned)c->n_sm * 4;
-    const size_t shM = sizeof(double) * 2 * nn, shG = sizeof(double) * 4 * nn;
+    // Gram kernel: its per-block partial sums (4 n^2 doubles a block) share d_partials with the matrices at its tail
+    const size_t gram_room = (c->partial_doubles - (size_t)BL_NMAT * BL_LD) / (size_t)(4 * nn);
+    const unsigned Gg = (unsigned)(gram_room < (size_t)c->n_sm * 4 ? gram_room : (size_t)c->n_sm * 4);
+    const size_t shM = sizeof(double) * 2 * nn, shG = sizeof(double) * 4 * Bg;
     double* hp = c->h_pinned;
     int rc;
 #define BL_K(call) { wd_prof_scope pr__(c, WD_PROF_BLAS); call; } WD_LAUNCH_CHECK(c)
@@ -422,6 +462,7 @@ int wd_solve_bl(wd_ctx* c, int dag, int n, const double* Phi, double* X, double 
     if (rc) return rc;
     WD_CUDA_CHECK(c, cudaMemsetAsync(XE, 0, hb64, st));
     BL_K((bl_init<<<L.G, L.B, 0, st>>>(nv, n, rb, phihat, R, Rt, P)));
+    WD_CUDA_CHECK(c, cudaMemsetAsync(mats, 0, sizeof(double) * BL_NMAT * BL_LD, st));   // alpha and beta too: nothing is ever read unset
     WD_CUDA_CHECK(c, cudaMemcpyAsync(hp, c->d_scal, sizeof(double) * G_COUNT, cudaMemcpyDeviceToHost, st));
     WD_CUDA_CHECK(c, cudaStreamSynchronize(st));
     int converged = hp[G_OUT_DONE] != 0.0 ? 1 : 0, it = 0;
@@ -430,15 +471,14 @@ int wd_solve_bl(wd_ctx* c, int dag, int n, const double* Phi, double* X, double 
         ++it;
         rc = gl_apply(c, dag, n, P, tmp64, V);
         if (rc) return rc;
-        WD_CUDA_CHECK(c, cudaMemsetAsync(mats, 0, sizeof(double) * 3 * BL_LD, st));
-        BL_K((bl_gram<<<Gg, Bg, shG, st>>>(ng, n, Rt, V, R, mats + BL_MG * BL_LD, mats + BL_MR * BL_LD)));
+        BL_K((bl_gram<<<Gg, Bg, shG, st>>>(ng, n, Rt, V, R, mats + BL_MG * BL_LD, mats + BL_MR * BL_LD, c->d_scal, c->d_partials, c->d_ticket)));
         BL_K((bl_small_solve<<<1, 1, 0, st>>>(n, mats + BL_MG * BL_LD, mats + BL_MR * BL_LD, mats + BL_ALPHA * BL_LD, 1.0, c->d_scal)));
         BL_K((bl_axpm<<<L.G, L.B, shM, st>>>(nv, n, R, V, nullptr, c->d_scal, mats + BL_ALPHA * BL_LD, -1.0, S)));   // S = R - V alpha
         rc = gl_apply(c, dag, n, S, tmp64, T);
         if (rc) return rc;
         BL_K((gl_omega<<<L.G, L.B, 0, st>>>(nv, n, rb, T, S)));
         BL_K((bl_xr_update<<<L.G, L.B, shM, st>>>(nv, n, rb, XE, P, mats + BL_ALPHA * BL_LD, S, T, R)));
-        BL_K((bl_gram<<<Gg, Bg, shG, st>>>(ng, n, Rt, T, nullptr, mats + BL_MT * BL_LD, nullptr)));
+        BL_K((bl_gram<<<Gg, Bg, shG, st>>>(ng, n, Rt, T, nullptr, mats + BL_MT * BL_LD, nullptr, c->d_scal, c->d_partials, c->d_ticket)));
         BL_K((bl_small_solve<<<1, 1, 0, st>>>(n, mats + BL_MG * BL_LD, mats + BL_MT * BL_LD, mats + BL_BETA * BL_LD, -1.0, c->d_scal)));
         BL_K((bl_axpm<<<L.G, L.B, shM, st>>>(nv, n, R, P, V, c->d_scal, mats + BL_BETA * BL_LD, 1.0, Pn)));           // P = R + (P - omega V) beta
         { double2* t = P; P = Pn; Pn = t; }
@@ -450,6 +490,9 @@ int wd_solve_bl(wd_ctx* c, int dag, int n, const double* Phi, double* X, double 
         }
     }
 #undef BL_K
+    // The block recurrence broke down (rank-deficient block: a zero column, two equal columns, or a true breakdown):
+    // X and R are frozen at the last good iterate, and the caller (wd_solve_impl) finishes the solve on the default route.
+    if (!converged && hp[G_GL_BREAK] != 0.0) return WD_BL_BREAKDOWN;
     rc = wd_hop_launch(c, WD_F64, WD_LINK18, dag, n, 1, XE, XO, PhiO, 1.0, c->kappa);
     if (rc) return rc;
     if (info) {

@@ -484,9 +484,12 @@ def test_solver_that_cannot_converge_says_so(merge):
         ctx.close()
 
 
-def test_zero_and_duplicate_columns():
+@pytest.mark.parametrize("solver", [0, 1, 2, 3, 4])
+def test_zero_and_duplicate_columns(solver):
     """Degenerate blocks: a zero right-hand side column (solution zero, the other columns unaffected) and two identical
-    columns (identical solutions): the per-column scalars keep the columns apart and a frozen column never spoils the rest."""
+    columns (identical solutions): the per-column scalars keep the columns apart and a frozen column never spoils the rest.
+    Every solver route (WD_OPT_SOLVER 0..4) at the default poll interval; the block solver's n x n systems are singular
+    here, so it has to notice and hand the solve to the default route (include/wd.h WD_SOLVER_BL_F64)."""
     pkg = _wd()
     cfg, U, Phi = wi.make_config(1)
     dims, kappa, bc, n = cfg["dims"], cfg["kappa"], cfg["bc"], cfg["n_rhs"]
@@ -494,7 +497,8 @@ def test_zero_and_duplicate_columns():
     Phi[1] = 0.0
     Phi[3] = Phi[0]
     ctx = make_ctx(dims, kappa, bc, n, U)
-    X, info = ctx.solve_block(pkg.OP_D, ctx.pack(dev(Phi)), n, tol=1e-12)
+    ctx.set_option(pkg.OPT_SOLVER, solver)
+    X, info = ctx.solve_block(pkg.OP_D, ctx.pack(dev(Phi)), n, tol=1e-12, max_outer=500)
     assert info["converged"]
     Xc = ctx.unpack(X, n).cpu().numpy()
     assert np.all(Xc[1] == 0.0)
@@ -502,6 +506,44 @@ def test_zero_and_duplicate_columns():
     Xr, rr, _, rc = orc.solve(dims, kappa, bc, 0, U, Phi[[0, 2, 4]], tol=1e-14)
     assert rc == 0 and rr.max() < 1e-13
     assert rel_per_rhs(Xc[[0, 2, 4]], Xr).max() < 1e-9
+    assert rel_per_rhs(orc.apply(dims, kappa, bc, 0, U, Xc[[0, 2, 3, 4]]), Phi[[0, 2, 3, 4]]).max() < 2e-12
+    ctx.close()
+
+
+@pytest.mark.parametrize("solver", [1, 2, 3, 4])
+def test_other_solver_routes_that_run_out_of_budget_say_so(solver):
+    """The alternative routes with an iteration budget that is too small, at the default poll interval: WD_ENOCONV,
+    converged = 0, and X a finite iterate (iterations enqueued after the last poll must not spoil it)."""
+    pkg = _wd()
+    cfg, U, Phi = wi.make_config(1)
+    dims, kappa, bc, n = cfg["dims"], cfg["kappa"], cfg["bc"], cfg["n_rhs"]
+    ctx = make_ctx(dims, kappa, bc, n, U)
+    ctx.set_option(pkg.OPT_SOLVER, solver)
+    P = ctx.pack(dev(Phi))
+    X, info = ctx.solve_block(pkg.OP_D, P, n, tol=1e-12, max_outer=1, max_inner=6, raise_on_noconv=False)
+    assert not info["converged"]
+    assert all(np.isfinite(info["relres"])) and max(info["relres"]) > 1e-12
+    assert bool(torch.isfinite(X).all())
+    X, info = ctx.solve_block(pkg.OP_D, P, n, tol=1e-12, max_outer=500)
+    assert info["converged"]
+    Xc = ctx.unpack(X, n).cpu().numpy()
+    assert rel_per_rhs(orc.apply(dims, kappa, bc, 0, U, Xc), Phi).max() < 2e-12
+    ctx.close()
+
+
+def test_block_solver_is_reproducible_run_to_run():
+    """The Gram matrices of the block solver are summed in a fixed order: two solves of the same system give the same bits."""
+    pkg = _wd()
+    cfg, U, Phi = wi.make_config(1)
+    dims, kappa, bc, n = cfg["dims"], cfg["kappa"], cfg["bc"], cfg["n_rhs"]
+    ctx = make_ctx(dims, kappa, bc, n, U)
+    ctx.set_option(pkg.OPT_SOLVER, pkg.SOLVER_BL_F64)
+    P = ctx.pack(dev(Phi))
+    X1, i1 = ctx.solve_block(pkg.OP_D, P, n, tol=1e-12)
+    X1 = X1.clone()
+    X2, i2 = ctx.solve_block(pkg.OP_D, P, n, tol=1e-12)
+    assert i1["converged"] and i2["converged"] and i1["inner_iters_total"] == i2["inner_iters_total"]
+    assert torch.equal(X1, X2)
     ctx.close()
 
 
