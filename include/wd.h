@@ -123,8 +123,10 @@ int wd_site_order(wd_ctx* ctx, int order, const int tile[4]);
  *       (fp16 mantissas + one fp32 scale per spinor, arithmetic in fp32) and fp64 reliable updates in place of
  *       restarts ("tuning techniques described in [4]"); inner_tol is then the
  *       reliable-update threshold delta (0 = default 0.01), max_outer bounds the number of updates and max_inner the
- *       total number of iterations.  Needs the z-march hop kernel (linear site order, Lx/2 even, n_rhs >= 3,
- *       Lx/2 * n_rhs a multiple of 4); elsewhere the default solver runs.
+ *       total number of iterations ENQUEUED (between the moment a column asks for an update and the next poll, up to
+ *       WD_OPT_POLL_EVERY - 1 enqueued iterations are no-ops; info.inner_iters_total counts the ones that did work).
+ *       Needs the z-march hop kernel with 16-bit operands (linear site order, Lx/2 even, n_rhs >= 3, Lx/2 * n_rhs a
+ *       multiple of 4 and at most 384, the consumer threads of one CTA); elsewhere the default solver runs.
  *       WD_SOLVER_GL_FLEX: the paper's case D1 (Table 1): fp64 Global BiCGStab (one alpha, beta, omega for the
  *       whole block, Frobenius inner products) in flexible form, preconditioned by the fp32 BiCGStab per column;
  *       max_outer bounds its iterations (two preconditioner calls each), info.outer_steps counts preconditioner calls.

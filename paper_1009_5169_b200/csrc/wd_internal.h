@@ -226,7 +226,7 @@ int wd_solve_gl(wd_ctx* c, int flex, int dag, int n, const double* Phi, double* 
 #define WD_BL_BREAKDOWN 1
 int wd_solve_bl(wd_ctx* c, int dag, int n, const double* Phi, double* X, double tol, int max_iters, wd_solve_info* info);
 // wd_solve_h16.cu
-bool wd_solve_h16_applies(const wd_ctx* c, int n);
+bool wd_solve_h16_applies(const wd_ctx* c, int recon, int n);
 int wd_solve_h16(wd_ctx* c, int dag, int n, const double* Phi, double* X, double tol, int max_updates, int max_iters,
                  double delta, int recon, wd_solve_info* info);
 

@@ -482,7 +482,7 @@ int wd_solve_impl(wd_ctx* c, int dag, int n, const double* Phi, double* X, doubl
         if (rc != WD_BL_BREAKDOWN) return rc;
         // rank-deficient block (zero or equal columns) or breakdown: the per-column default route solves it
     }
-    if (solver == WD_SOLVER_RELIABLE_H16 && wd_solve_h16_applies(c, n))
+    if (solver == WD_SOLVER_RELIABLE_H16 && wd_solve_h16_applies(c, recon, n))
         return wd_solve_h16(c, dag, n, Phi, X, tol, max_outer, max_inner, inner_tol > 0.0 ? inner_tol : 0.01, recon, info);
     // default: the fp32 recurrence is run down to 3e-7, about what fp32 can deliver, so that TWO inner solves reach
     // 1e-12 (at 1e-5 it takes three: an fp64 residual, a demotion and a promotion more per solve; reading R12)

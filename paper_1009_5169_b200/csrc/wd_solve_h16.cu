@@ -268,9 +268,11 @@ void shape(const wd_ctx* c, long work, int n, int* B, unsigned* G) {
 
 }  // namespace
 
-bool wd_solve_h16_applies(const wd_ctx* c, int n) {
-    const int Lxh = c->L[0] / 2;
-    return c->order == WD_ORDER_LINEAR && c->RB == (uint32_t)Lxh && n >= 3 && (Lxh * n) % 4 == 0;
+// The 16-bit route runs only where the z-march hop kernel takes H16 operands in this link form: row-major layout,
+// Lx/2 * n a multiple of 4, and a CTA shape that fits (Lx/2 * n consumer threads + the producer warps <= 512, so e.g.
+// not Lx = 64 at n = 16).  Elsewhere wd_solve_impl runs the default solver, as include/wd.h promises.
+bool wd_solve_h16_applies(const wd_ctx* c, int recon, int n) {
+    return n >= 3 && wd_hop_zm_serves(c, recon, n, 1);
 }
 
 size_t wd_h16_half_bytes(const wd_ctx* c, int n) { return (size_t)c->Vh * n * 52; }

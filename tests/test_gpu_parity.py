@@ -531,6 +531,22 @@ def test_other_solver_routes_that_run_out_of_budget_say_so(solver):
     ctx.close()
 
 
+def test_h16_route_falls_back_where_the_z_march_kernel_does_not_serve():
+    """WD_SOLVER_RELIABLE_H16 on a shape its hop kernel cannot take (Lx/2 * n_rhs = 512 consumer threads do not fit a CTA):
+    include/wd.h promises the default solver there, not an error."""
+    pkg = _wd()
+    dims, kappa, bc, n = (64, 4, 4, 4), 0.12, wi.BC_SF, 16
+    U = wi.gauge_field(dims, 0.3, 5, bc)
+    Phi = wi.spinor_field(dims, n, 6, bc)
+    ctx = make_ctx(dims, kappa, bc, n, U)
+    ctx.set_option(pkg.OPT_SOLVER, pkg.SOLVER_RELIABLE_H16)
+    X, info = ctx.solve_block(pkg.OP_D, ctx.pack(dev(Phi)), n, tol=1e-12)
+    assert info["converged"]
+    Xc = ctx.unpack(X, n).cpu().numpy()
+    assert rel_per_rhs(orc.apply(dims, kappa, bc, 0, U, Xc), Phi).max() < 2e-12
+    ctx.close()
+
+
 def test_block_solver_is_reproducible_run_to_run():
     """The Gram matrices of the block solver are summed in a fixed order: two solves of the same system give the same bits."""
     pkg = _wd()
