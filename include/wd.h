@@ -130,7 +130,10 @@ int wd_site_order(wd_ctx* ctx, int order, const int tile[4]);
  *       WD_SOLVER_GL_FLEX: the paper's case D1 (Table 1): fp64 Global BiCGStab (one alpha, beta, omega for the
  *       whole block, Frobenius inner products) in flexible form, preconditioned by the fp32 BiCGStab per column;
  *       max_outer bounds its iterations (two preconditioner calls each), info.outer_steps counts preconditioner calls.
- *       WD_SOLVER_GL_F64: case B, the same without preconditioner (all fp64; info.inner_iters_total = its iterations).
+ *       WD_SOLVER_GL_F64: case B, the same without preconditioner (all fp64; info.inner_iters_total = its iterations);
+ *       there being no inner solver, max_inner bounds its iterations (as for WD_SOLVER_BL_F64) and max_outer is unused.
+ *       These three blocked solvers stop on the recursive residual, then compute the true one (which info.relres
+ *       reports) and restart from it for as long as a column misses tol and iterations are left.
  *       WD_SOLVER_BL_F64: case C, fp64 Block BiCGStab (ref. [7] of the paper): n_rhs x n_rhs coefficient matrices from the
  *       Gram matrices of the block vectors, one Krylov space shared by the columns; max_inner bounds its iterations.
  *       The n x n systems need a block of full rank: with a zero column, two equal columns, or on a breakdown of the
