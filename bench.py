@@ -533,19 +533,15 @@ def run_ours(args):
     # xpay + <t, s>, <t, t> (1 extra operand: 0.75 per launch on average) or, in the merged-update schedule the solver
     # runs by default where the z-march kernel serves the hop, xpay + <t, s>, <t, t>, <rt, s>, <rt, t> (2 extra: 1.0)
     interior = (dims[3] - 1) / dims[3] if bc == wi.BC_SF else 1.0
-    impl0 = ctx.get_option(pkg.OPT_HOP_IMPL)
-    merged = bool(ctx.get_option(pkg.OPT_MERGE)) and not ctx.get_option(pkg.OPT_PAIRED) and impl0 == 2 and \
-        (dims[0] // 2) % 2 == 0 and n >= 3
+    # schedule and kernel from the library's own dispatch (wd_inner_plan), not a copy of its rules: at 24^4 the z-march
+    # kernel and the merged schedule serve n_rhs = 3, 5, 8, 10, while 4, 6, 12, 16 go to the ring kernel and the textbook order
+    plan = ctx.inner_plan(n, recon)
+    merged = plan["merged"]
     hop_bytes = hop_bytes_per_launch(Vh, n, 4, R, extra_operands=1.0 if merged else 0.75, interior=interior)
     hop_us = hop_ms * 1e3 / max(1, hop_cnt)
     achieved = hop_bytes / (hop_us * 1e-6) * 1e-9 if hop_cnt else 0.0
-    # which kernel the library's dispatch picks (wd_hop.cu wd_hop_launch_ex): z-march (impl 2) or row-group ring (impl 1)
-    # where the layout is row-major (linear site order, Lx/2 even, max_rhs >= 3) and n_rhs >= 3, else the register kernel
-    impl = ctx.get_option(pkg.OPT_HOP_IMPL)
-    staged = impl >= 1 and (dims[0] // 2) % 2 == 0 and n >= 3
-    # (impl 2 hands shapes with a small step and long rows to the ring kernel: csrc/wd_hop_zm.cu wd_hop_zm_preferred; the
-    # bench workload, 24^4 at n_rhs = 5, is served by the z-march kernel, as profiles/r02_launches.md shows)
-    kname = (f"hop_zm_kernel<float,{R}>" if impl >= 2 else f"hop_tma_kernel<float,{R}>") if staged else f"hop_kernel<float,{R}>"
+    kname = {"zmarch": f"hop_zm_kernel<float,{R}>", "ring": f"hop_tma_kernel<float,{R}>",
+             "register": f"hop_kernel<float,{R}>"}[plan["hop_kernel"]]
     # dram__bytes_read.sum + dram__bytes_write.sum per launch from an ncu --set full capture of THIS kernel source: the
     # committed record carries the sha256 of the kernel's source file and is ignored when the source has changed since
     traffic, traffic_note, ncu_us = None, "no capture on record for this kernel source", None
@@ -568,7 +564,7 @@ def run_ours(args):
                 "peak_source": peak_src, "traffic": traffic, "traffic_note": traffic_note, "bytes_per_launch": hop_bytes,
                 "bytes_counted": f"interior sites only for everything read ((T-1)/T = {interior:.4f}), all sites for the output",
                 "avg_launch_us": round(hop_us, 2), "launches_in_step": hop_cnt,
-                "schedule": "merged x,r,p update: 23 vector passes per iteration, 2 + 5 + 2 + 5 of them in the four hop launches" if merged
+                "schedule": "merged x,r,p update: 23 vector passes per iteration, 2 + 4 + 2 + 4 of them in the four hop launches" if merged
                             else "textbook order: 25 vector passes per iteration, 2 + 4 + 2 + 3 of them in the four hop launches",
                 "timing": "CUDA event pairs on the library's stream around the two hop launches of every application of the "
                           "even/odd operator (one kernel-to-kernel gap inside each pair); in the graph-replayed blocks the pairs "

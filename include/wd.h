@@ -292,6 +292,17 @@ enum { WD_PROF_HOP32 = 0, WD_PROF_HOP64 = 1, WD_PROF_BLAS = 2, WD_PROF_FORCE = 3
 int wd_profile(wd_ctx* ctx, int enable);
 int wd_profile_read(wd_ctx* ctx, double* ms_host, long long* count_host);
 
+/* What the fp32 inner solver of wd_solve_block will run for (n_rhs, recon) with the options as they are
+ * now, so that a measurement can count the right bytes without repeating the library's dispatch rules: plan_host is
+ * an array of WD_PLAN_N ints, [WD_PLAN_HOP_KERNEL] = the kernel that serves the four hop launches of an iteration
+ * (WD_HOP_KERNEL_*), [WD_PLAN_MERGED] = 1 for the merged x,r,p update schedule (WD_OPT_MERGE: 23 vector passes per
+ * iteration, seven-sum epilogue in the second hop pair), 0 for the textbook order (25), [WD_PLAN_PAIRED] = 1 for the
+ * x-paired form, [WD_PLAN_KERNELS_PER_ITER] = kernel launches per BiCGStab iteration (6 or 7).  Host only, launches
+ * nothing.  Errors: WD_EINVAL (null, n_rhs out of range, bad recon). */
+enum { WD_HOP_KERNEL_REGISTER = 0, WD_HOP_KERNEL_RING = 1, WD_HOP_KERNEL_ZMARCH = 2 };
+enum { WD_PLAN_HOP_KERNEL = 0, WD_PLAN_MERGED = 1, WD_PLAN_PAIRED = 2, WD_PLAN_KERNELS_PER_ITER = 3, WD_PLAN_N = 4 };
+int wd_inner_plan(const wd_ctx* ctx, int n_rhs, int recon, int* plan_host);
+
 /* Number of kernel launches this context has enqueued since creation (for bench.py's count). */
 long long wd_launch_count(const wd_ctx* ctx);
 

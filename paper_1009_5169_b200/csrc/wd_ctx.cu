@@ -490,6 +490,18 @@ int wd_action(wd_ctx* ctx, int n_rhs, int parity_sel, const double* X, double* S
     return wd_action_impl(ctx, n_rhs, parity_sel, X, S_host);
 }
 
+int wd_inner_plan(const wd_ctx* ctx, int n_rhs, int recon, int* plan_host) {
+    if (!ctx || !plan_host) return WD_EINVAL;
+    if (bad_n(ctx, n_rhs) || (recon != WD_LINK18 && recon != WD_LINK12)) return WD_EINVAL;
+    bool paired, merged;
+    wd_inner_forms(ctx, recon, n_rhs, &paired, &merged);
+    plan_host[WD_PLAN_HOP_KERNEL] = paired ? WD_HOP_KERNEL_ZMARCH : wd_hop_kernel_for(ctx, WD_F32, recon, n_rhs);
+    plan_host[WD_PLAN_MERGED] = merged ? 1 : 0;
+    plan_host[WD_PLAN_PAIRED] = paired ? 1 : 0;
+    plan_host[WD_PLAN_KERNELS_PER_ITER] = merged ? 6 : 7;
+    return WD_OK;
+}
+
 int wd_project_parity(wd_ctx* ctx, int prec, int n_rhs, int parity, void* native) {
     if (!ctx) return WD_EINVAL;
     if (!native || bad_n(ctx, n_rhs) || (prec != WD_F64 && prec != WD_F32) || (parity != 0 && parity != 1))

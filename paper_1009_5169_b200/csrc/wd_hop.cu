@@ -287,6 +287,18 @@ int wd_hop_launch_ex(wd_ctx* c, int prec, int recon, int dag, int n, int par, co
     return WD_OK;
 }
 
+// The kernel the dispatch above picks for plain operands (storage 0, epilogues 0-3): keep the two in step.
+int wd_hop_kernel_for(const wd_ctx* c, int prec, int recon, int n) {
+    const int impl = c->opt[WD_OPT_HOP_IMPL];
+    if (impl >= 1 && n >= 3) {
+        if ((impl == 3 || (impl == 2 && (prec != WD_F32 || wd_hop_zm_preferred(c, recon, n)))) && prec == WD_F32 &&
+            wd_hop_zm_serves(c, recon, n, 0))
+            return WD_HOP_KERNEL_ZMARCH;
+        if (wd_hop_tma_serves(c, prec, recon, n)) return WD_HOP_KERNEL_RING;
+    }
+    return WD_HOP_KERNEL_REGISTER;
+}
+
 int wd_hop_launch(wd_ctx* c, int prec, int recon, int dag, int n, int par, const void* in, void* out,
                   const void* in2, double a, double b) {
     wd_hop_ops o;

@@ -489,6 +489,14 @@ int launch_tma(wd_ctx* c, int dag, int n, int par, const wd_hop_ops& o, const T*
 
 }  // namespace
 
+// Would wd_hop_tma_launch serve plain operands of this precision and link form? (same conditions, nothing launched)
+bool wd_hop_tma_serves(const wd_ctx* c, int prec, int recon, int n) {
+    if (c->order != WD_ORDER_LINEAR || c->RB != (uint32_t)(c->L[0] / 2)) return false;
+    Shape sh;
+    if (prec == WD_F64) return recon == WD_LINK18 ? pick_shape<double, 18>(c, n, 384, &sh) : pick_shape<double, 12>(c, n, 384, &sh);
+    return recon == WD_LINK18 ? pick_shape<float, 18>(c, n, 512, &sh) : pick_shape<float, 12>(c, n, 512, &sh);
+}
+
 // Returns WD_OK if launched, a positive value if this lattice / option set is not served by the staged kernel
 // (tiled site order, odd Lx/2 with 18-real fp32 links, nothing fits): the caller then uses wd_hop.cu's kernel.
 int wd_hop_tma_launch(wd_ctx* c, int prec, int recon, int dag, int n, int par, const wd_hop_ops& o) {

@@ -194,6 +194,11 @@ struct wd_hop_ops {
 int wd_hop_launch_ex(wd_ctx* c, int prec, int recon, int dag, int n, int par, const wd_hop_ops& o);
 // wd_hop_tma.cu: the shared-memory-staged (bulk copy + mbarrier) form; > 0 = not applicable, use the plain kernel
 int wd_hop_tma_launch(wd_ctx* c, int prec, int recon, int dag, int n, int par, const wd_hop_ops& o);
+bool wd_hop_tma_serves(const wd_ctx* c, int prec, int recon, int n);
+// wd_hop.cu: which kernel wd_hop_launch_ex picks for plain operands (WD_HOP_KERNEL_*), without launching anything
+int wd_hop_kernel_for(const wd_ctx* c, int prec, int recon, int n);
+// wd_solve.cu: the forms the fp32 inner solver takes for (recon, n) under the current options
+void wd_inner_forms(const wd_ctx* c, int recon, int n, bool* paired, bool* merged);
 // wd_hop_zm.cu: the z-marching sliding-window form (fp32); > 0 = not applicable
 int wd_hop_zm_launch(wd_ctx* c, int prec, int recon, int dag, int n, int par, const wd_hop_ops& o);
 // does the z-march kernel serve this (n_rhs, link form, storage) on this context's lattice?

@@ -275,6 +275,15 @@ size_t wd_solver_scratch_bytes(const wd_ctx* c) {
 // The fp32 inner solver on its own: E_i = BiCGStab_fp32(R_i / scale_i) for the columns whose S_FLAG is 0, to a recursive
 // residual of S_THR2 (relative to the unit-norm right-hand side), then Xacc_i += scale_i E_i.  S_SCALE, S_FLAG, S_THR2 and
 // S_OUT_CONV are set on the device by the caller's preceding reduction.  Uses the seven fp32 slots of the solver scratch.
+void wd_inner_forms(const wd_ctx* c, int recon, int n, bool* paired, bool* merged) {
+    const int impl = c->opt[WD_OPT_HOP_IMPL];
+    // P32 (two sites per thread, packed fp32 instructions: wd_f2.cuh) wherever the z-march kernel serves it
+    *paired = c->opt[WD_OPT_PAIRED] != 0 && impl >= 2 && n >= 3 && wd_hop_zm_serves(c, recon, n, 2);
+    // merged x,r,p update (WD_OPT_MERGE) wherever the z-march kernel, which has the seven-sum epilogue, serves the hop
+    *merged = c->opt[WD_OPT_MERGE] != 0 && !*paired && n >= 3 &&
+              ((impl == 2 && wd_hop_zm_preferred(c, recon, n)) || (impl == 3 && wd_hop_zm_serves(c, recon, n, 0)));
+}
+
 int wd_inner_solve_f32(wd_ctx* c, int dag, int n, int recon, int max_inner, const double2* R64, double2* Xacc) {
     cudaStream_t st = c->stream;
     const long Vh = c->Vh;
@@ -303,11 +312,8 @@ int wd_inner_solve_f32(wd_ctx* c, int dag, int n, int recon, int max_inner, cons
     int rc;
     {
         // P32 (two sites per thread, packed fp32 instructions: wd_f2.cuh) wherever the z-march kernel serves it
-        const int impl = c->opt[WD_OPT_HOP_IMPL];
-        const bool paired = c->opt[WD_OPT_PAIRED] != 0 && impl >= 2 && n >= 3 && wd_hop_zm_serves(c, recon, n, 2);
-        // merged x,r,p update (WD_OPT_MERGE) wherever the z-march kernel, which has the seven-sum epilogue, serves the hop
-        const bool merged = c->opt[WD_OPT_MERGE] != 0 && !paired && n >= 3 &&
-                            ((impl == 2 && wd_hop_zm_preferred(c, recon, n)) || (impl == 3 && wd_hop_zm_serves(c, recon, n, 0)));
+        bool paired, merged;
+        wd_inner_forms(c, recon, n, &paired, &merged);
         {
             wd_prof_scope pr__(c, WD_PROF_BLAS);
             if (paired) demote_kernel<true><<<L32.G, L32.B, 0, st>>>(Vh, (long)c->RB, n, rb, R64, r32, rt32, x32, p32, v32);

@@ -39,7 +39,8 @@ SYMBOLS = ["wd_create", "wd_destroy", "wd_site_order", "wd_workspace_bytes", "wd
            "wd_set_option", "wd_get_option", "wd_set_gauge", "wd_native_bytes", "wd_pack", "wd_unpack", "wd_apply", "wd_hop",
            "wd_solve_block", "wd_force", "wd_md_force_host", "wd_md_force_host_gauge", "wd_refresh", "wd_action",
            "wd_project_parity", "wd_md_force", "wd_profile", "wd_profile_read", "wd_launch_count", "wd_strerror",
-           "wd_last_error", "wd_version", "wd_action_static", "wd_action_static_error"]
+           "wd_last_error", "wd_version", "wd_action_static", "wd_action_static_error", "wd_inner_plan"]
+HOP_KERNEL_NAMES = ("register", "ring", "zmarch")   # WD_HOP_KERNEL_*
 STATIC_MAX_ROWS = 1 << 25          # WD_STATIC_MAX_ROWS
 STATIC_SCRATCH_BYTES = 2097408     # WD_STATIC_SCRATCH_BYTES
 
@@ -109,6 +110,8 @@ def lib():
     L.wd_last_error.argtypes = [vp]
     L.wd_last_error.restype = ctypes.c_char_p
     L.wd_version.restype = ctypes.c_char_p
+    L.wd_inner_plan.argtypes = [vp, ci, ci, ip]
+    L.wd_inner_plan.restype = ci
     L.wd_action_static.argtypes = [ci, sz, vp, vp, vp]
     L.wd_action_static.restype = ci
     L.wd_action_static_error.restype = ctypes.c_char_p
@@ -349,6 +352,13 @@ class Context:
         v = ctypes.c_int()
         self._check(self.L.wd_get_option(self._h, int(key), ctypes.byref(v)))
         return v.value
+
+    def inner_plan(self, n_rhs, recon=LINK18):
+        """What the fp32 inner solver will run for (n_rhs, recon) under the current options (wd_inner_plan)."""
+        plan = (ctypes.c_int * 4)()
+        self._check(self.L.wd_inner_plan(self._h, int(n_rhs), int(recon), plan))
+        return dict(hop_kernel=HOP_KERNEL_NAMES[plan[0]], merged=bool(plan[1]), paired=bool(plan[2]),
+                    kernels_per_iter=int(plan[3]))
 
     def launch_count(self):
         return int(self.L.wd_launch_count(self._h))

@@ -547,6 +547,35 @@ def test_h16_route_falls_back_where_the_z_march_kernel_does_not_serve():
     ctx.close()
 
 
+def test_inner_plan_agrees_with_what_the_solver_launches():
+    """wd_inner_plan (what bench.py counts bytes by): its kernels-per-iteration figure is checked against the launch
+    counter.  With polls after every iteration nothing is enqueued in vain, so a solve launches a + b * outer_steps +
+    k * iterations kernels; the same system solved with WD_OPT_MERGE on and off differs by exactly the change of k
+    the plan announces -- one kernel per iteration where the merged schedule applies (n_rhs >= 3 on a lattice the
+    z-march kernel serves), none where it does not (n_rhs = 2: register kernel, textbook order)."""
+    pkg = _wd()
+    cfg, U, Phi = wi.make_config(1)
+    dims, kappa, bc = cfg["dims"], cfg["kappa"], cfg["bc"]
+    for n, want_merged, want_kernel in ((5, True, "zmarch"), (2, False, "register")):
+        ctx = make_ctx(dims, kappa, bc, n, U)
+        ctx.set_option(pkg.OPT_POLL_EVERY, 1)
+        ctx.set_option(pkg.OPT_GRAPH, 0)
+        P = ctx.pack(dev(Phi[:n]))
+        counts = {}
+        for merge in (1, 0):
+            ctx.set_option(pkg.OPT_MERGE, merge)
+            plan = ctx.inner_plan(n)
+            assert plan["merged"] == (want_merged and merge == 1) and plan["hop_kernel"] == want_kernel, plan
+            assert plan["kernels_per_iter"] == (6 if plan["merged"] else 7)
+            l0 = ctx.launch_count()
+            _, info = ctx.solve_block(pkg.OP_D, P, n, tol=1e-12)
+            counts[merge] = (ctx.launch_count() - l0, info["inner_iters_total"], info["outer_steps"], plan["kernels_per_iter"])
+        (l1, i1, o1, k1), (l0_, i0, o0, k0) = counts[1], counts[0]
+        assert o1 == o0
+        assert l1 - k1 * i1 == l0_ - k0 * i0, counts
+    ctx.close()
+
+
 def test_block_solver_is_reproducible_run_to_run():
     """The Gram matrices of the block solver are summed in a fixed order: two solves of the same system give the same bits."""
     pkg = _wd()
