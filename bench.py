@@ -45,8 +45,11 @@ def parse_args():
     ap.add_argument("--hop-impl", type=int, default=-1, choices=(-1, 0, 1, 2, 3),
                     help="WD_OPT_HOP_IMPL: 0 register kernel, 1 row-group ring kernel, 2 z-march or ring by shape (library default), "
                          "3 z-march wherever it runs, -1 leave the default")
-    ap.add_argument("--rhs-sweep", action="store_true", help="configs[4]: blocked solve at n_rhs = 1, 2, 5, 8, 12")
-    ap.add_argument("--apply-sweep", action="store_true", help="configs[3]: D, D^dag apply on 16^4, fp32/fp64 x 18/12 reals")
+    # the two tables BASELINE.json's configs[3] and configs[4] ask for are part of the default line (about 20 s); --quick
+    # leaves them out.  --rhs-sweep / --apply-sweep are still accepted (they were the opt-in switches of earlier rounds).
+    ap.add_argument("--quick", action="store_true", help="skip the configs[4] n_rhs sweep and the configs[3] 16^4 apply table")
+    ap.add_argument("--rhs-sweep", action="store_true", help="(default on) configs[4]: blocked solve at n_rhs = 1, 2, 5, 8, 12")
+    ap.add_argument("--apply-sweep", action="store_true", help="(default on) configs[3]: D, D^dag apply on 16^4, fp32/fp64 x 18/12 reals")
     ap.add_argument("--shard-rhs", action="store_true",
                     help="N > 1: deal the n_rhs columns of ONE problem to the ranks (gauge replicated, allReduce of F): strong scaling")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -603,9 +606,10 @@ def run_ours(args):
         line["hop"] = hop_sweep(pkg, ctx, torch, n, peak_gbs, interior=interior)
     ctx.close()
     del ctx, P, X, Y, F
-    if rank == 0 and args.rhs_sweep:
+    sweeps = (world == 1 and not args.quick)
+    if rank == 0 and (args.rhs_sweep or sweeps):
         line["rhs_sweep"] = rhs_sweep(pkg, wi, torch, peak_gbs, R, recon)
-    if rank == 0 and args.apply_sweep:
+    if rank == 0 and (args.apply_sweep or sweeps):
         line["apply_16"] = apply_sweep(pkg, wi, torch, peak_gbs)
     if rank == 0 and not args.no_config2:
         line["config2_12x12x12x12"] = config2_time(pkg, wi, torch, recon)
