@@ -181,13 +181,15 @@ size_t wd_native_bytes(const wd_ctx* ctx, int prec, int n_rhs);
 int wd_pack(wd_ctx* ctx, int prec, int n_rhs, const double* canon_dev, void* native_dev);
 int wd_unpack(wd_ctx* ctx, int prec, int n_rhs, const void* native_dev, double* canon_dev);
 
-/* out = D in (op = WD_OP_D) or D^dag in (WD_OP_DDAG) on a native full-lattice block, all n_rhs
+/* The operator of the linear systems of Algorithm 2 ("solve D X = Phi", "solve D^dag Y = X"; Wilson
+ * quarks; the form of D is DESIGN.md reading R4, D^dag R5): out = D in (op = WD_OP_D) or D^dag in (WD_OP_DDAG) on a native full-lattice block, all n_rhs
  * columns in one pass per output parity (two launches of the hopping kernel with the diagonal
  * term fused).  prec picks fp64 or fp32 arithmetic and storage, recon the link form.  in and out
  * must not overlap.  Errors: WD_ESTATE (no gauge), WD_EINVAL (n_rhs, enums, null). */
 int wd_apply(wd_ctx* ctx, int op, int prec, int recon, int n_rhs, const void* in_native_dev, void* out_native_dev);
 
-/* The bare hopping term on one output parity (hot-path step a2), exposed for measurement:
+/* The bare hopping term on one output parity (hot-path step a2; the kernel inside the paper's single-precision GPU
+ * solver, whose even/odd form PAPER.md:74 names: D = 1 - kappa H), exposed for measurement:
  * out[out_parity] = H in[1-out_parity] ("dslash").  in/out are native HALF-lattice blocks, i.e.
  * [k or c][V/2][n_rhs] (half of wd_native_bytes).  Same errors as wd_apply. */
 int wd_hop(wd_ctx* ctx, int op, int prec, int recon, int n_rhs, int out_parity, const void* in_half_dev, void* out_half_dev);

@@ -1,8 +1,10 @@
 """ctypes loader for the fp64 CPU oracle (oracle/wd_oracle.cpp).  TEST INFRASTRUCTURE ONLY.
 
 Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may import
-this module.  The product (paper_1009_5169_b200) never does.  Argument marshalling only: all
-arithmetic is in wd_oracle.cpp, which cites the passages it follows.
+this module.  The product (paper_1009_5169_b200) never does.  Argument marshalling for everything in
+wd_oracle.cpp, which cites the passages it follows; two functions hold arithmetic of their own in numpy, both pinned
+in tests/test_oracle_pins.py: action() (a sum of squares, eq. 2.2) and eo_md_force() (a composition of the pinned
+solve, project_parity and force for the even/odd-preconditioned action).
 """
 from __future__ import annotations
 

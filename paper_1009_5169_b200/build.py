@@ -4,6 +4,9 @@
 
 WD_NVCC_DEFINES (environment) adds -D flags for measurement builds, e.g. the ablation switches of csrc/wd_hop_zm.cu:
     WD_NVCC_DEFINES="-DWD_ZM_ABLATE=1" python -m paper_1009_5169_b200.build --force     (and --force again without it afterwards)
+Such a library computes wrong results on purpose; wd_version() then ends in "MEASUREMENT BUILD: <the defines>", the Python
+binding refuses to load it unless WD_ALLOW_MEASUREMENT_BUILD=1 is set (bench.py --hop-only timing runs), and
+tests/test_abi.py fails on it.
 
 The .so is git-ignored but travels to the GPU box with the gpurun snapshot.
 """
@@ -39,7 +42,10 @@ def build(force: bool = False, verbose: bool = False) -> str:
     for s in SOURCES:
         o = os.path.join(HERE, "build", s.replace(".cu", ".o"))
         objs.append(o)
-        cmd = [nvcc] + [f for f in NVCC_FLAGS if not f.startswith("--use_fast_math")] + os.environ.get("WD_NVCC_DEFINES", "").split() + \
+        defines = os.environ.get("WD_NVCC_DEFINES", "").split()
+        if defines:   # a measurement build says so in wd_version(); tests/test_abi.py and wd.lib() refuse to go on with one
+            defines = defines + ['-DWD_BUILD_DEFINES="' + " ".join(defines).replace('"', "") + '"']
+        cmd = [nvcc] + [f for f in NVCC_FLAGS if not f.startswith("--use_fast_math")] + defines + \
               (["-Xptxas", "-v"] if verbose else []) + ["-c", os.path.join(CSRC, s), "-o", o]
         procs.append((s, subprocess.Popen(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)))
     failed = False

@@ -110,7 +110,13 @@ void wd_graphs_clear(wd_ctx* c) {
 
 extern "C" {
 
+// A library built with extra -D switches (build.py WD_NVCC_DEFINES: the ablation switches of wd_hop_zm.cu) says so here,
+// because such a build computes wrong results on purpose.
+#ifdef WD_BUILD_DEFINES
+const char* wd_version(void) { return "wd 0.1 (sm_100a) MEASUREMENT BUILD: " WD_BUILD_DEFINES; }
+#else
 const char* wd_version(void) { return "wd 0.1 (sm_100a)"; }
+#endif
 
 const char* wd_strerror(int code) {
     switch (code) {

@@ -110,6 +110,10 @@ def lib():
     L.wd_last_error.argtypes = [vp]
     L.wd_last_error.restype = ctypes.c_char_p
     L.wd_version.restype = ctypes.c_char_p
+    if b"MEASUREMENT BUILD" in L.wd_version() and os.environ.get("WD_ALLOW_MEASUREMENT_BUILD") != "1":
+        raise RuntimeError(f"{LIB_PATH} is a measurement build ({L.wd_version().decode()}): its results are wrong on purpose. "
+                           "Rebuild with `python -m paper_1009_5169_b200.build --force` (WD_NVCC_DEFINES unset), or set "
+                           "WD_ALLOW_MEASUREMENT_BUILD=1 for a timing run")
     L.wd_inner_plan.argtypes = [vp, ci, ci, ip]
     L.wd_inner_plan.restype = ci
     L.wd_action_static.argtypes = [ci, sz, vp, vp, vp]

@@ -19,6 +19,8 @@ def test_library_builds_loads_and_exports_every_declared_symbol():
         assert hasattr(L, name), name
     L.wd_version.restype = ctypes.c_char_p
     assert b"sm_100a" in L.wd_version()
+    # a library built with the ablation switches of csrc/wd_hop_zm.cu (build.py WD_NVCC_DEFINES) must never be tested or shipped
+    assert b"MEASUREMENT BUILD" not in L.wd_version(), L.wd_version()
     L.wd_strerror.restype = ctypes.c_char_p
     L.wd_strerror.argtypes = [ctypes.c_int]
     assert L.wd_strerror(-4) and L.wd_strerror(0) == b"ok"
