@@ -294,6 +294,18 @@ enum { WD_PROF_HOP32 = 0, WD_PROF_HOP64 = 1, WD_PROF_BLAS = 2, WD_PROF_FORCE = 3
 int wd_profile(wd_ctx* ctx, int enable);
 int wd_profile_read(wd_ctx* ctx, double* ms_host, long long* count_host);
 
+/* Residual history: what the paper plots in Fig. 1-5, |D x - b| / |b| against the iteration number,
+ * one curve per pseudo-fermion.  hist_dev is the caller's DEVICE buffer of capacity rows of WD_MAX_RHS doubles (NULL or
+ * capacity 0 switches the record off; it is off by default and costs nothing then).  While it is set, every
+ * wd_solve_block (and the calls built on it) writes row k, column i = the estimate of |phi_i - A x_i| / |phi_i| after
+ * its k-th low-precision BiCGStab iteration, k counted from 0 over the whole solve (across the restarts of the outer
+ * loop), for k < capacity; info.inner_iters_total rows are valid after the call.  The estimate is the RECURSIVE residual of
+ * the fp32 (or 16-bit) even/odd system scaled back to the fp64 one, i.e. what the iteration itself sees; the true
+ * residual at the end is info.relres.  A column that has converged keeps its last value.  Routes: the default solver and
+ * WD_SOLVER_RELIABLE_H16 (for WD_SOLVER_GL_FLEX the rows are the preconditioner's inner iterations; the fp64 blocked
+ * solvers write nothing).  The buffer must stay valid while it is set.  Errors: WD_EINVAL. */
+int wd_set_residual_history(wd_ctx* ctx, double* hist_dev, int capacity);
+
 /* What the fp32 inner solver of wd_solve_block will run for (n_rhs, recon) with the options as they are
  * now, so that a measurement can count the right bytes without repeating the library's dispatch rules: plan_host is
  * an array of WD_PLAN_N ints, [WD_PLAN_HOP_KERNEL] = the kernel that serves the four hop launches of an iteration

@@ -45,6 +45,10 @@ struct RedBuf {
     double* scal;
     double* partials;
     unsigned int* ticket;
+    // optional residual history (wd_set_residual_history): row k = after inner iteration k, WD_MAX_RHS doubles a row.
+    // Aggregate initialisation with three members leaves it off.
+    double* hist = nullptr;
+    int hist_cap = 0;
 };
 
 template <typename T> struct V;
@@ -338,6 +342,15 @@ __device__ void reduce_finalize(double (&v)[K], int n, RedBuf rb) {
     }
     __syncthreads();
     if (t < n) finalize_column<KIND>(rb.scal, t, &sh[1536 + t * K]);
+    // the kernels that close a BiCGStab iteration (they own the recursive |r_i|^2) append a row to the residual history:
+    // |r_i| of the normalised low-precision system x its scale / |phi_i| = an estimate of |phi - A x| / |phi| per column
+    if ((KIND == K_RHO || KIND == K_RNORM || KIND == K_RHO_REL) && rb.hist != nullptr && t < n) {
+        const int it = (int)rb.scal[G_ITERS];   // iterations finished before this one, since the solve began
+        if (it < rb.hist_cap) {
+            const double phi2 = SC(rb.scal, S_PHI2, t);
+            rb.hist[(size_t)it * WD_MAX_RHS + t] = phi2 > 0.0 ? sqrt(SC(rb.scal, S_RNORM2, t) / phi2) * SC(rb.scal, S_SCALE, t) : 0.0;
+        }
+    }
     __syncthreads();
     if (t == 0) {
         finalize_global<KIND>(rb.scal, n);

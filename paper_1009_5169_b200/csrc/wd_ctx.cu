@@ -170,6 +170,8 @@ int wd_create(wd_ctx** out, const int dims[4], double kappa, int time_bc, int ma
     c->ws_bytes = 0;
     c->have_ws = c->have_gauge = false;
     c->launches = 0;
+    c->d_hist = nullptr;
+    c->hist_cap = 0;
     for (int k = 0; k < WD_OPT_N; ++k) c->opt[k] = 0;
     // hop CTA shape and register budget: 0 = chosen per launch from n_rhs (wd_hop.cu)
     c->opt[WD_OPT_POLL_EVERY] = 4;
@@ -494,6 +496,16 @@ int wd_action(wd_ctx* ctx, int n_rhs, int parity_sel, const double* X, double* S
     if (parity_sel < WD_PARITY_EVEN || parity_sel > WD_PARITY_BOTH) return wd_fail(ctx, WD_EINVAL, "bad parity selection");
     if (!ctx->have_ws) return wd_fail(ctx, WD_ESTATE, "wd_set_workspace first");
     return wd_action_impl(ctx, n_rhs, parity_sel, X, S_host);
+}
+
+int wd_set_residual_history(wd_ctx* ctx, double* hist_dev, int capacity) {
+    if (!ctx) return WD_EINVAL;
+    if (capacity < 0 || (hist_dev && capacity == 0) || ((size_t)hist_dev & 7) != 0)
+        return wd_fail(ctx, WD_EINVAL, "wd_set_residual_history: bad capacity or misaligned buffer");
+    ctx->d_hist = capacity > 0 ? hist_dev : nullptr;
+    ctx->hist_cap = ctx->d_hist ? capacity : 0;
+    wd_graphs_clear(ctx);   // the captured iteration blocks carry the pointer
+    return WD_OK;
 }
 
 int wd_inner_plan(const wd_ctx* ctx, int n_rhs, int recon, int* plan_host) {

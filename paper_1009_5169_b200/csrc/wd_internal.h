@@ -71,6 +71,9 @@ struct wd_ctx {
     char* d_solver;        // remaining scratch for solver vectors and host-path staging
     size_t solver_bytes;
 
+    double* d_hist;        // caller's residual-history buffer (wd_set_residual_history), null = off
+    int hist_cap;          // its capacity in rows of WD_MAX_RHS doubles
+
     int opt[WD_OPT_N];  // tunables (wd_set_option)
 
     // CUDA graphs of the inner solver's iteration blocks; dropped whenever an option or the workspace changes

@@ -297,7 +297,7 @@ int wd_inner_solve_f32(wd_ctx* c, int dag, int n, int recon, int max_inner, cons
     float4* rt32 = (float4*)w;  w += sb32;
     float4* tmp32 = (float4*)w; w += sb32;
     const double kap = c->kappa;
-    RedBuf rb{c->d_scal, c->d_partials, c->d_ticket};
+    RedBuf rb{c->d_scal, c->d_partials, c->d_ticket, c->d_hist, c->hist_cap};
     const long nv32 = 6 * Vh * n;
     const Launch L32 = blas_cfg(c, nv32, n);
     // Schroedinger functional, row-major layout: the rows of the frozen t = 0 slice open every half-lattice block and hold

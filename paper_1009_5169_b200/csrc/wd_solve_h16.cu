@@ -303,7 +303,7 @@ int wd_solve_h16(wd_ctx* c, int dag, int n, const double* Phi, double* X, double
     char* XE = (char*)X;
     char* XO = XE + hb64;
     const double kap = c->kappa;
-    RedBuf rb{c->d_scal, c->d_partials, c->d_ticket};
+    RedBuf rb{c->d_scal, c->d_partials, c->d_ticket, c->d_hist, c->hist_cap};
     int rc;
     Geo G;
     G.items = Vh * n; G.RB = c->RB; G.n = (uint32_t)n; G.rbn = c->RB * (uint32_t)n; G.rowH = h16_row_vecs(G.rbn);

@@ -39,7 +39,7 @@ SYMBOLS = ["wd_create", "wd_destroy", "wd_site_order", "wd_workspace_bytes", "wd
            "wd_set_option", "wd_get_option", "wd_set_gauge", "wd_native_bytes", "wd_pack", "wd_unpack", "wd_apply", "wd_hop",
            "wd_solve_block", "wd_force", "wd_md_force_host", "wd_md_force_host_gauge", "wd_refresh", "wd_action",
            "wd_project_parity", "wd_md_force", "wd_profile", "wd_profile_read", "wd_launch_count", "wd_strerror",
-           "wd_last_error", "wd_version", "wd_action_static", "wd_action_static_error", "wd_inner_plan"]
+           "wd_last_error", "wd_version", "wd_action_static", "wd_action_static_error", "wd_inner_plan", "wd_set_residual_history"]
 HOP_KERNEL_NAMES = ("register", "ring", "zmarch")   # WD_HOP_KERNEL_*
 STATIC_MAX_ROWS = 1 << 25          # WD_STATIC_MAX_ROWS
 STATIC_SCRATCH_BYTES = 2097408     # WD_STATIC_SCRATCH_BYTES
@@ -114,6 +114,8 @@ def lib():
         raise RuntimeError(f"{LIB_PATH} is a measurement build ({L.wd_version().decode()}): its results are wrong on purpose. "
                            "Rebuild with `python -m paper_1009_5169_b200.build --force` (WD_NVCC_DEFINES unset), or set "
                            "WD_ALLOW_MEASUREMENT_BUILD=1 for a timing run")
+    L.wd_set_residual_history.argtypes = [vp, vp, ci]
+    L.wd_set_residual_history.restype = ci
     L.wd_inner_plan.argtypes = [vp, ci, ci, ip]
     L.wd_inner_plan.restype = ci
     L.wd_action_static.argtypes = [ci, sz, vp, vp, vp]
@@ -356,6 +358,16 @@ class Context:
         v = ctypes.c_int()
         self._check(self.L.wd_get_option(self._h, int(key), ctypes.byref(v)))
         return v.value
+
+    def set_residual_history(self, hist):
+        """wd_set_residual_history: `hist` is a CUDA float64 tensor [capacity, MAX_RHS] (kept alive here), or None to
+        switch the record off.  After a solve, hist[:info['inner_iters_total'], :n_rhs] is the residual curve per column."""
+        if hist is None:
+            self._check(self.L.wd_set_residual_history(self._h, None, 0))
+        else:
+            assert hist.is_cuda and hist.dtype == torch.float64 and hist.is_contiguous() and hist.shape[1] == MAX_RHS
+            self._check(self.L.wd_set_residual_history(self._h, self._ptr(hist), int(hist.shape[0])))
+        self._hist = hist
 
     def inner_plan(self, n_rhs, recon=LINK18):
         """What the fp32 inner solver will run for (n_rhs, recon) under the current options (wd_inner_plan)."""

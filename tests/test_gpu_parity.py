@@ -576,6 +576,57 @@ def test_inner_plan_agrees_with_what_the_solver_launches():
     ctx.close()
 
 
+@pytest.mark.parametrize("solver", [0, 1])
+def test_residual_history_is_the_curve_of_the_solve(solver):
+    """wd_set_residual_history (the per-iteration |Dx - b| / |b| of the paper's Fig. 1-5): as many rows
+    as the solve took iterations, nothing written past them or past the capacity, curves that start at O(1) and end below
+    the tolerance the solve met, a zero column recorded as zeros, and the same bits with and without CUDA-graph replay."""
+    pkg = _wd()
+    cfg, U, Phi = wi.make_config(1)
+    dims, kappa, bc, n = cfg["dims"], cfg["kappa"], cfg["bc"], cfg["n_rhs"]
+    Phi = Phi.copy()
+    Phi[2] = 0.0
+    ctx = make_ctx(dims, kappa, bc, n, U)
+    ctx.set_option(pkg.OPT_SOLVER, solver)
+    P = ctx.pack(dev(Phi))
+    cap = 400
+    hist = torch.full((cap, pkg.wd.MAX_RHS), -7.0, dtype=torch.float64, device="cuda")
+    ctx.set_residual_history(hist)
+    X, info = ctx.solve_block(pkg.OP_D, P, n, tol=1e-12)
+    iters = info["inner_iters_total"]
+    assert info["converged"] and 10 < iters < cap
+    H = hist.cpu().numpy()
+    assert np.all(H[iters:] == -7.0) and np.all(H[:iters, n:] == -7.0)         # nothing outside rows < iters, columns < n
+    C = H[:iters, :n]
+    assert np.all(np.isfinite(C)) and np.all(C >= 0.0)
+    assert np.all(C[:, 2] == 0.0)                                              # the zero column
+    live = [0, 1, 3, 4]
+    assert np.all(C[0, live] > 1e-2) and np.all(C[0, live] < 10.0)             # one iteration in: still O(1)
+    assert np.all(C[-1, live] <= 1e-12)                                        # the recursive estimate at the end
+    assert np.all(C[-1, live] <= 10 * np.maximum(np.array(info["relres"])[live], 1e-13))   # and it is of the size of the true one
+    assert np.all(C[iters // 2, live] < 1e-2 * C[0, live])                     # a falling curve, not a constant
+    if solver == 0:
+        ctx.set_option(pkg.OPT_GRAPH, 0)
+        hist2 = torch.full_like(hist, -7.0)
+        ctx.set_residual_history(hist2)
+        ctx.solve_block(pkg.OP_D, P, n, tol=1e-12)
+        assert torch.equal(hist, hist2)
+        ctx.set_option(pkg.OPT_GRAPH, 1)
+    # a capacity smaller than the solve: the first rows only
+    small = torch.full((8, pkg.wd.MAX_RHS), -7.0, dtype=torch.float64, device="cuda")
+    ctx.set_residual_history(small)
+    ctx.solve_block(pkg.OP_D, P, n, tol=1e-12)
+    if solver == 0:
+        assert torch.equal(small[:, :n], hist[:8, :n])
+    assert bool((small[:, :n] >= 0).all())
+    # switched off again: the old buffer is left alone
+    ctx.set_residual_history(None)
+    before = small.clone()
+    ctx.solve_block(pkg.OP_D, P, n, tol=1e-12)
+    assert torch.equal(small, before)
+    ctx.close()
+
+
 def test_block_solver_is_reproducible_run_to_run():
     """The Gram matrices of the block solver are summed in a fixed order: two solves of the same system give the same bits."""
     pkg = _wd()
