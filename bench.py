@@ -372,10 +372,10 @@ def apply_sweep(pkg, wi, torch, peak_gbs, reps=50):
     return res
 
 
-def config2_time(pkg, wi, torch, recon):
-    """BASELINE.json configs[2]: full MD force evaluation (two blocked solves + force) on the 12^4 SF lattice, 5 RHS.
-    L2-resident and launch-bound: an absolute time only, no roofline claim."""
-    cfg, U, Phi = wi.make_config(2)
+def config2_time(pkg, wi, torch, recon, idx=2):
+    """BASELINE.json configs[idx] (2: the 12^4 SF lattice; 1: 8^4; 0: 4^4), 5 RHS: full MD force evaluation (two blocked
+    solves + force).  L2-resident and launch-bound: an absolute time only, no roofline claim."""
+    cfg, U, Phi = wi.make_config(idx)
     dims, kappa, bc, n = cfg["dims"], cfg["kappa"], cfg["bc"], cfg["n_rhs"]
     ctx = pkg.Context(dims, kappa, bc=bc, max_rhs=n)
     ctx.set_gauge(torch.from_numpy(U).cuda())
@@ -613,6 +613,9 @@ def run_ours(args):
         line["apply_16"] = apply_sweep(pkg, wi, torch, peak_gbs)
     if rank == 0 and not args.no_config2:
         line["config2_12x12x12x12"] = config2_time(pkg, wi, torch, recon)
+        # the two smaller parity configurations beside it (launch-bound: what a persistent small-lattice mode would have to beat)
+        line["config1_8x8x8x8"] = config2_time(pkg, wi, torch, recon, 1)
+        line["config0_4x4x4x4"] = config2_time(pkg, wi, torch, recon, 0)
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         line["cpu_baseline"] = cpu_baseline(dict(wi.CONFIGS[args.config]), n, full=args.cpu_baseline_full)
     if world > 1:
