@@ -86,3 +86,15 @@ def test_set_option_rejects_null_context():
     assert L.wd_set_option(None, 0, 1) == wd.EINVAL
     v = ctypes.c_int()
     assert L.wd_get_option(None, 0, ctypes.byref(v)) == wd.EINVAL
+
+
+def test_round3_entry_points_reject_null_context():
+    """wd_inner_plan and wd_set_residual_history are host-only calls on a context: without one they return WD_EINVAL
+    (checked here on the CPU box; their behaviour on a context is in tests/test_gpu_parity.py)."""
+    from paper_1009_5169_b200 import wd
+    L = wd.lib()
+    plan = (ctypes.c_int * 4)()
+    assert L.wd_inner_plan(None, 5, wd.LINK18, plan) == wd.EINVAL
+    assert L.wd_set_residual_history(None, None, 0) == wd.EINVAL
+    hdr = open(os.path.join(ROOT, "include", "wd.h")).read()
+    assert "WD_PLAN_N = 4" in hdr and len(wd.HOP_KERNEL_NAMES) == 3
